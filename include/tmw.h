@@ -1,0 +1,157 @@
+/*
+ * tmw.h — C ABI of libtmw.so: the twisted-mass Wilson(-clover) Dirac operator of arXiv:2201.09004 on one B200
+ * (sm_100a), and an even-odd preconditioned mixed-precision BiCGStab that inverts it.
+ *
+ * What the calls compute (citations: /root/reference/PAPER.md line, section; readings Cn = DESIGN.md "Readings"):
+ *
+ *   (D psi)(x) = 1/2 sum_mu [ (1+g_mu) U_mu(x) psi(x+mu) s+ + (1-g_mu) U_mu(x-mu)^dag psi(x-mu) s- ]   PAPER.md:62 Eq. (2)
+ *                - (4 + Re m) psi(x) - i (Im m) g5 psi(x)                   PAPER.md:62 "-(4+m) delta_xy", m = m_cri+omega
+ *                                                                           complex (Eq. (1), :65), reading C4
+ *                + (c_sw/2) sum_{mu<nu} sigma_mu_nu F_mu_nu(x) psi(x)       PAPER.md:67 Eq. (3), reading C7
+ *
+ *   s+- = -1 on a hop that wraps around the time direction (antiperiodic in t, periodic in x,y,z; C6); lattice
+ *   units a = 1; gamma matrices in the DeGrand-Rossi basis (C5; g5 = diag(+1,+1,-1,-1)); F_mu_nu is the clover-leaf
+ *   field strength built from the same links (clover term and its inverse are computed on the GPU).
+ *   tmw_solve returns x with D x = b by BiCGStab (the solver of PAPER.md:73, Table 2 row 1) on the even-odd Schur
+ *   complement, fp32 inner recurrences with fp64 reliable updates; the stopping rule is the relative residual of
+ *   the FULL system, |b - D x|_2 / |b|_2 <= tol ("residual").
+ *
+ * Every step runs in CUDA kernels of this library. There is no CPU fallback.
+ *
+ * Canonical (user-facing) layouts, fp64, x fastest (same as the oracle's; the spin basis is part of the boundary):
+ *   gauge   double[4][T][L][L][L][3][3][2]   = [mu (x,y,z,t)][t][z][y][x][row][col][re,im],  U_mu(x)_{row,col}
+ *   spinor  double[T][L][L][L][4][3][2]      = [t][z][y][x][spin][colour][re,im]
+ *
+ * Internal ("packed") layout, used only by the raw parity path (tmw_pack / tmw_unpack / tmw_apply EVEN|ODD /
+ * tmw_apply_schur): one parity (x+y+z+t mod 2) of the lattice, checkerboard index cb = lex/2 with
+ * lex = x + L (y + L (z + L t)), stored as planes of 16-byte vectors: plane k of a spinor holds reals
+ * [k*n, k*n+n) of the site's 24 reals (spin, colour, re/im order), n = 4 (fp32, float4) or 2 (fp64, double2);
+ * element (k, cb) is at vector index k*V_h + cb, V_h = L^3 T / 2. tmw_spinor_bytes gives the size.
+ *
+ * Pointers: `location` in tmw_options says whether the gauge/in/out/b/x pointers of the canonical-layout calls are
+ * HOST or DEVICE pointers. Packed-layout pointers are always DEVICE pointers. All pointers must be 16-byte aligned;
+ * in and out must not alias. The context owns every internal buffer and frees it in tmw_destroy; the caller owns
+ * gauge (read only during tmw_create; may be freed afterwards), in, out, b, x.
+ *
+ * Errors: every int function returns TMW_OK (0) or a negative code; tmw_last_error gives a text. Nothing aborts
+ * or throws across this boundary.
+ */
+#ifndef TMW_H
+#define TMW_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tmw_ctx tmw_ctx; /* opaque */
+
+typedef struct { double re, im; } tmw_complex;
+
+/* error codes */
+#define TMW_OK 0
+#define TMW_EINVAL (-1)     /* null pointer, odd or too small L/T, tol <= 0, bad enum */
+#define TMW_ENOMEM (-2)     /* a device or host allocation failed */
+#define TMW_ECUDA (-3)      /* a CUDA call failed; text in tmw_last_error */
+#define TMW_ESINGULAR (-4)  /* a clover block (or the twisted-mass diagonal) is not invertible */
+#define TMW_ENOCONV (-5)    /* max_iter reached: x holds the best iterate, info is filled */
+#define TMW_EBREAKDOWN (-6) /* BiCGStab breakdown (rho or <t,t> vanished / NaN) that restarts did not cure */
+
+/* enums */
+#define TMW_DEVICE 0
+#define TMW_HOST 1
+
+#define TMW_MIXED 0  /* fp32 inner BiCGStab, fp64 reliable updates (default) */
+#define TMW_DOUBLE 1 /* everything in fp64 */
+
+#define TMW_TWIST_GAMMA5 0 /* mass term -(4+Re m) - i Im m g5  (default, reading C4) */
+#define TMW_MASS_SCALAR 1  /* mass term -(4+m) with a complex scalar m (the literal alternative) */
+
+#define TMW_D 0
+#define TMW_DDAG 1
+
+#define TMW_FULL 0
+#define TMW_EVEN 1
+#define TMW_ODD 2
+
+#define TMW_F32 0
+#define TMW_F64 1
+
+typedef struct {
+  int location;     /* TMW_DEVICE (default) | TMW_HOST: where canonical-layout pointers live */
+  int precision;    /* TMW_MIXED (default) | TMW_DOUBLE: solver arithmetic */
+  int reconstruct;  /* fp32 gauge storage: 12 (default; third row rebuilt in-kernel, links must be SU(3)) | 18 */
+  int mass_reading; /* TMW_TWIST_GAMMA5 (default) | TMW_MASS_SCALAR */
+  int max_iter;     /* BiCGStab iterations; 0 -> 10000 */
+  double delta;     /* reliable-update threshold; 0 -> 0.1 */
+  void* stream;     /* cudaStream_t all work is queued on; NULL = the legacy default stream */
+} tmw_options;
+
+typedef struct {
+  int iters;            /* BiCGStab iterations (each = 2 Schur-operator applications) */
+  int reliable_updates; /* fp64 true-residual recomputations */
+  int restarts;         /* breakdown restarts (rhat := r) */
+  double iter_resid;    /* last iterated |r| / |b| */
+  double true_resid;    /* |b - D x| / |b| on the full lattice, fp64, recomputed after reconstruction */
+  double device_ms;     /* CUDA-event time of the whole solve on the context stream */
+} tmw_solve_info;
+
+/*
+ * Build a context for an L^3 x T lattice (L, T even, >= 4): copies the gauge field and re-lays it out
+ * (checkerboarded SoA, fp64 18-real and fp32 12/18-real copies), and, if c_sw != 0, computes the clover-leaf
+ * F_mu_nu (Eq. (3), C7), the two Hermitian 6x6 chiral blocks per site and the inverses on the even sites
+ * (PAPER.md:80). gauge: canonical layout, HOST or DEVICE per opt->location. opt may be NULL (all defaults).
+ */
+int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, double c_sw, const tmw_options* opt);
+
+/*
+ * out = D in (op = TMW_D) or D^dag in (TMW_DDAG), Eq. (2)+(3).
+ *   parity = TMW_FULL: in, out are canonical fp64 full-lattice spinors (HOST or DEVICE per location); fp64 arithmetic.
+ *   parity = TMW_EVEN | TMW_ODD: the raw benchmark path. out (packed, parity p) = H_{p pbar} in (packed, the other
+ *     parity) = only the hopping part of Eq. (2) (the 1/2 sum over mu), in precision `prec` (TMW_F32 | TMW_F64).
+ *     DEVICE pointers. Asynchronous on the context stream.
+ */
+int tmw_apply(tmw_ctx* ctx, int op, int parity, int prec, const void* in, void* out);
+
+/*
+ * Even-odd Schur complement on the odd sites (packed DEVICE spinors, precision prec):
+ *   out_o = A_oo in_o - H_oe A_ee^{-1} H_eo in_o,  A = the site-diagonal part of D (mass, twist, clover).
+ * op = TMW_DDAG applies its conjugate transpose. Asynchronous on the context stream.
+ */
+int tmw_apply_schur(tmw_ctx* ctx, int op, int prec, const void* in_odd, void* out_odd);
+
+/*
+ * Solve D x = b to |b - D x| / |b| <= tol. b, x: canonical fp64 spinors (HOST or DEVICE per location).
+ * b = 0 gives x = 0. Returns after the final fp64 true residual is known. info may be NULL.
+ */
+int tmw_solve(tmw_ctx* ctx, const double* b, double* x, double tol, tmw_solve_info* info);
+
+/* bytes of one packed parity spinor in precision prec (TMW_F32 | TMW_F64); 0 on bad arguments */
+long long tmw_spinor_bytes(const tmw_ctx* ctx, int prec);
+
+/*
+ * Layout conversion between a canonical fp64 full-lattice spinor and a packed parity spinor (both DEVICE
+ * pointers regardless of `location`). parity = TMW_EVEN | TMW_ODD. tmw_unpack writes only the sites of that parity.
+ */
+int tmw_pack(tmw_ctx* ctx, int prec, int parity, const double* canonical, void* packed);
+int tmw_unpack(tmw_ctx* ctx, int prec, int parity, const void* packed, double* canonical);
+
+/*
+ * Copy the packed clover blocks out for inspection (tests): for the given parity, 72 doubles per site
+ * [cb][chirality 0..1][36], each block = 6 real diagonal entries then the 15 strictly-lower entries (row-major:
+ * (1,0),(2,0),(2,1),(3,0),...) as re,im; block index i = 3*(spin mod 2) + colour; the diagonal includes
+ * -(4 + Re m). inverse != 0 returns the stored inverse (even parity only). dst: DEVICE pointer.
+ */
+int tmw_get_clover(tmw_ctx* ctx, int parity, int inverse, double* dst);
+
+/* number of kernel launches this context has issued since creation (bench.py's gpu_launches) */
+long long tmw_launch_count(const tmw_ctx* ctx);
+
+void tmw_destroy(tmw_ctx* ctx);
+
+/* text of the last error of this context (ctx-owned, valid until the next call); ctx may be NULL for create errors */
+const char* tmw_last_error(const tmw_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TMW_H */

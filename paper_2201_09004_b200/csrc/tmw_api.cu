@@ -1,0 +1,558 @@
+// tmw_api.cu — the C ABI of include/tmw.h: context, layout conversion, operator application, and the even-odd
+// mixed-precision BiCGStab driver (the solver named at PAPER.md:73). Host code only
+// sequences kernel launches and reads a few reduction scalars per iteration; all arithmetic on fields runs in
+// the CUDA kernels of this directory.
+#include <math.h>
+#include <stddef.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/tmw.h"
+#include "tmw_internal.h"
+
+using namespace tmw;
+
+struct tmw_ctx {
+  Geom g;
+  int64_t V;
+  double m_re, m_im, c_sw;
+  tmw_options opt;
+  cudaStream_t stream;
+  bool clover;
+  int ng32;
+  void* g64[2];
+  void* g32[2];
+  void* c64[2];
+  void* c32[2];
+  void* ci64;  // inverse blocks, even parity
+  void* ci32;
+  std::vector<void*> owned;  // every device allocation
+  // lazily allocated workspaces
+  void* w64[10];  // packed fp64 parity spinors
+  void* w32[8];   // packed inner-precision parity spinors (fp32 for TMW_MIXED, fp64 for TMW_DOUBLE)
+  void* canon[2]; // canonical fp64 full-lattice staging (HOST location only)
+  Scalars* sc;
+  Scalars* sc_host;  // pinned
+  double* red;       // 4 device doubles
+  double* red_host;  // pinned
+  cudaEvent_t ev0, ev1;
+  long long launches;
+  std::string err;
+};
+
+static thread_local std::string g_create_err;
+
+static int fail(tmw_ctx* c, int code, const char* msg) {
+  if (c) c->err = msg; else g_create_err = msg;
+  return code;
+}
+static int fail_cuda(tmw_ctx* c, cudaError_t e, const char* where) {
+  char buf[512];
+  snprintf(buf, sizeof(buf), "CUDA error in %s: %s", where, cudaGetErrorString(e));
+  cudaGetLastError();
+  return fail(c, e == cudaErrorMemoryAllocation ? TMW_ENOMEM : TMW_ECUDA, buf);
+}
+#define CK(call)                                               \
+  do {                                                         \
+    cudaError_t e_ = (call);                                   \
+    if (e_ != cudaSuccess) return fail_cuda(ctx, e_, #call);   \
+  } while (0)
+#define LAUNCH(call)                                           \
+  do {                                                         \
+    cudaError_t e_ = (call);                                   \
+    ctx->launches++;                                           \
+    if (e_ != cudaSuccess) return fail_cuda(ctx, e_, #call);   \
+  } while (0)
+
+static int dev_alloc(tmw_ctx* ctx, void** p, size_t bytes) {
+  cudaError_t e = cudaMalloc(p, bytes);
+  if (e != cudaSuccess) { *p = nullptr; return fail_cuda(ctx, e, "cudaMalloc"); }
+  ctx->owned.push_back(*p);
+  return TMW_OK;
+}
+static void dev_free(tmw_ctx* ctx, void* p) {
+  for (size_t i = 0; i < ctx->owned.size(); i++)
+    if (ctx->owned[i] == p) { ctx->owned.erase(ctx->owned.begin() + i); break; }
+  cudaFree(p);
+}
+
+static size_t spinor_bytes(const tmw_ctx* c, int prec) { return (size_t)c->g.Vh * 24 * (prec == TMW_F32 ? 4 : 8); }
+
+// ---- the diagonal part for D (dagger = 0) or D^dagger ----
+template <typename R> static Diag<R> make_diag(const tmw_ctx* c, int dagger) {
+  Diag<R> d;
+  const double dg = -(4.0 + c->m_re);
+  double tu, tl;
+  if (c->opt.mass_reading == TMW_TWIST_GAMMA5) { tu = -c->m_im; tl = c->m_im; }
+  else { tu = -c->m_im; tl = -c->m_im; }
+  if (dagger) { tu = -tu; tl = -tl; }
+  d.diag = (R)dg;
+  d.tw_up = (R)tu;
+  d.tw_lo = (R)tl;
+  const double den = dg * dg + tu * tu;
+  d.inv_re = (R)(dg / den);
+  d.inv_im_up = (R)(-tu / den);
+  d.inv_im_lo = (R)(-tl / den);
+  d.twisted_clover = (c->clover && c->m_im != 0.0) ? 1 : 0;
+  const bool f = sizeof(R) == 4;
+  d.c[0] = f ? c->c32[0] : c->c64[0];
+  d.c[1] = f ? c->c32[1] : c->c64[1];
+  d.cinv[0] = f ? c->ci32 : c->ci64;
+  d.cinv[1] = nullptr;
+  return d;
+}
+
+template <typename R>
+static DslashArgs<R> make_args(const tmw_ctx* c, int par, int dagger, const void* in, void* out, const void* aux, double sgn) {
+  DslashArgs<R> a;
+  a.in = in;
+  a.out = out;
+  a.aux = aux;
+  const bool f = sizeof(R) == 4;
+  a.U[0] = f ? c->g32[0] : c->g64[0];
+  a.U[1] = f ? c->g32[1] : c->g64[1];
+  a.g = c->g;
+  a.par = par;
+  a.sig = dagger ? (R)-1 : (R)1;
+  a.coef = (R)(0.5 * sgn);
+  a.d = make_diag<R>(c, dagger);
+  a.red_mode = 0;
+  a.dotv = nullptr;
+  a.red = nullptr;
+  return a;
+}
+template <typename R> static int ng_of(const tmw_ctx* c) { return sizeof(R) == 4 ? c->ng32 : 18; }
+
+// out(par) = epilogue(H in)
+template <typename R>
+static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, void* out, const void* aux, double sgn, int red_mode = 0, const void* dotv = nullptr, double* red = nullptr) {
+  DslashArgs<R> a = make_args<R>(ctx, par, dagger, in, out, aux, sgn);
+  a.red_mode = red_mode;
+  a.dotv = dotv;
+  a.red = red;
+  LAUNCH(launch_dslash(a, ng_of<R>(ctx), epi, ctx->clover, ctx->stream));
+  return TMW_OK;
+}
+// Schur operator on the odd sites: out = A_oo in - H_oe A_ee^{-1} H_eo in  (tmp: even-parity scratch)
+// The conjugate transpose is A_oo^dag in - H_eo^dag (A_ee^dag)^{-1} H_oe^dag in: the same two kernels with the
+// daggered projectors / twist, because (H_oe)^dag = the daggered hopping block from odd to even.
+template <typename R>
+static int schur(tmw_ctx* ctx, int dagger, const void* in, void* out, void* tmp, int red_mode = 0, const void* dotv = nullptr, double* red = nullptr) {
+  int rc = dslash<R>(ctx, EPI_AINV_HOP, 0, dagger, in, tmp, nullptr, 1.0);
+  if (rc) return rc;
+  return dslash<R>(ctx, EPI_A_XPAY, 1, dagger, tmp, out, in, -1.0, red_mode, dotv, red);
+}
+
+extern "C" {
+
+const char* tmw_last_error(const tmw_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
+
+void tmw_destroy(tmw_ctx* ctx) {
+  if (!ctx) return;
+  cudaStreamSynchronize(ctx->stream);
+  for (void* p : ctx->owned) cudaFree(p);
+  if (ctx->sc_host) cudaFreeHost(ctx->sc_host);
+  if (ctx->red_host) cudaFreeHost(ctx->red_host);
+  if (ctx->ev0) cudaEventDestroy(ctx->ev0);
+  if (ctx->ev1) cudaEventDestroy(ctx->ev1);
+  delete ctx;
+}
+
+int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, double c_sw, const tmw_options* opt) {
+  if (!out) return fail(nullptr, TMW_EINVAL, "tmw_create: out is null");
+  *out = nullptr;
+  if (!gauge) return fail(nullptr, TMW_EINVAL, "tmw_create: gauge is null");
+  if (L < 4 || T < 4 || (L & 1) || (T & 1)) return fail(nullptr, TMW_EINVAL, "tmw_create: L and T must be even and >= 4");
+  const int64_t V = (int64_t)L * L * L * T;
+  if (V / 2 >= (int64_t)1 << 31) return fail(nullptr, TMW_EINVAL, "tmw_create: lattice too large");
+  tmw_options o;
+  memset(&o, 0, sizeof(o));
+  if (opt) o = *opt;
+  if (o.reconstruct == 0) o.reconstruct = 12;
+  if (o.max_iter == 0) o.max_iter = 10000;
+  if (o.delta == 0.0) o.delta = 0.1;
+  if ((o.location != TMW_DEVICE && o.location != TMW_HOST) || (o.precision != TMW_MIXED && o.precision != TMW_DOUBLE) ||
+      (o.reconstruct != 12 && o.reconstruct != 18) || (o.mass_reading != TMW_TWIST_GAMMA5 && o.mass_reading != TMW_MASS_SCALAR) ||
+      o.max_iter < 0 || !(o.delta > 0.0) || !(o.delta < 1.0))
+    return fail(nullptr, TMW_EINVAL, "tmw_create: bad option value");
+  if (!isfinite(m.re) || !isfinite(m.im) || !isfinite(c_sw)) return fail(nullptr, TMW_EINVAL, "tmw_create: non-finite parameter");
+  tmw_ctx* ctx = new (std::nothrow) tmw_ctx();
+  if (!ctx) return fail(nullptr, TMW_ENOMEM, "tmw_create: host allocation failed");
+  ctx->g.L = L; ctx->g.T = T; ctx->g.Lh = L / 2; ctx->g.Vh = (int)(V / 2);
+  ctx->g.sy = L / 2; ctx->g.sz = (L / 2) * L; ctx->g.st = (L / 2) * L * L;
+  ctx->V = V;
+  ctx->m_re = m.re; ctx->m_im = m.im; ctx->c_sw = c_sw;
+  ctx->opt = o;
+  ctx->stream = (cudaStream_t)o.stream;
+  ctx->clover = (c_sw != 0.0);
+  ctx->ng32 = o.reconstruct;
+  ctx->launches = 0;
+  int rc = TMW_OK;
+  // from here on errors must free ctx
+#define CKC(call)                                                       \
+  do {                                                                  \
+    cudaError_t e_ = (call);                                            \
+    if (e_ != cudaSuccess) {                                            \
+      rc = fail_cuda(nullptr, e_, #call);                               \
+      tmw_destroy(ctx);                                                 \
+      return rc;                                                        \
+    }                                                                   \
+  } while (0)
+#define CKA(p, bytes)                                                   \
+  do {                                                                  \
+    rc = dev_alloc(ctx, (void**)(p), (bytes));                          \
+    if (rc) { g_create_err = ctx->err; tmw_destroy(ctx); return rc; }   \
+  } while (0)
+  if (!ctx->clover) {
+    const double dg = -(4.0 + m.re);
+    if (dg * dg + m.im * m.im == 0.0) { tmw_destroy(ctx); return fail(nullptr, TMW_ESINGULAR, "tmw_create: 4 + m = 0, the diagonal part is singular"); }
+  }
+  CKC(cudaMallocHost((void**)&ctx->sc_host, sizeof(Scalars)));
+  CKC(cudaMallocHost((void**)&ctx->red_host, 4 * sizeof(double)));
+  CKC(cudaEventCreate(&ctx->ev0));
+  CKC(cudaEventCreate(&ctx->ev1));
+  CKA(&ctx->sc, sizeof(Scalars));
+  CKA(&ctx->red, 4 * sizeof(double));
+  const size_t Vh = (size_t)ctx->g.Vh;
+  const int np32 = (ctx->ng32 == 12) ? 3 : 5;
+  for (int p = 0; p < 2; p++) {
+    CKA(&ctx->g64[p], Vh * 4 * 9 * 16);
+    CKA(&ctx->g32[p], Vh * 4 * np32 * 16);
+  }
+  const double* gdev = gauge;
+  void* staging = nullptr;
+  if (o.location == TMW_HOST) {
+    CKA(&staging, (size_t)V * 4 * 18 * 8);
+    CKC(cudaMemcpyAsync(staging, gauge, (size_t)V * 4 * 18 * 8, cudaMemcpyHostToDevice, ctx->stream));
+    gdev = (const double*)staging;
+  }
+  CKC(launch_pack_gauge(ctx->g, gdev, ctx->g64[0], ctx->g64[1], ctx->g32[0], ctx->g32[1], ctx->ng32, ctx->stream));
+  ctx->launches++;
+  if (ctx->clover) {
+    for (int p = 0; p < 2; p++) {
+      CKA(&ctx->c64[p], Vh * 36 * 16);
+      CKA(&ctx->c32[p], Vh * 18 * 16);
+    }
+    CKA(&ctx->ci64, Vh * 36 * 16);
+    CKA(&ctx->ci32, Vh * 18 * 16);
+    CKC(launch_clover_build(ctx->g, gdev, c_sw, -(4.0 + m.re), ctx->c64[0], ctx->c64[1], ctx->c32[0], ctx->c32[1], ctx->stream));
+    ctx->launches++;
+    int* flag = (int*)ctx->red;
+    CKC(cudaMemsetAsync(flag, 0, sizeof(int), ctx->stream));
+    const double tw2 = m.im * m.im;
+    CKC(launch_clover_invert(ctx->g, ctx->c64[0], tw2, ctx->ci64, ctx->ci32, flag, ctx->stream));
+    ctx->launches++;
+    int hflag = 0;
+    CKC(cudaMemcpyAsync(&hflag, flag, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+    CKC(cudaStreamSynchronize(ctx->stream));
+    if (hflag) { tmw_destroy(ctx); return fail(nullptr, TMW_ESINGULAR, "tmw_create: a clover block on an even site is singular"); }
+  }
+  CKC(cudaStreamSynchronize(ctx->stream));
+  if (staging) dev_free(ctx, staging);
+  *out = ctx;
+  return TMW_OK;
+#undef CKC
+#undef CKA
+}
+
+long long tmw_spinor_bytes(const tmw_ctx* ctx, int prec) {
+  if (!ctx || (prec != TMW_F32 && prec != TMW_F64)) return 0;
+  return (long long)spinor_bytes(ctx, prec);
+}
+long long tmw_launch_count(const tmw_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int tmw_pack(tmw_ctx* ctx, int prec, int parity, const double* canonical, void* packed) {
+  if (!ctx) return TMW_EINVAL;
+  if (!canonical || !packed || (prec != TMW_F32 && prec != TMW_F64) || (parity != TMW_EVEN && parity != TMW_ODD)) return fail(ctx, TMW_EINVAL, "tmw_pack: bad argument");
+  LAUNCH(launch_pack_spinor(ctx->g, parity == TMW_ODD, prec, canonical, packed, ctx->stream));
+  return TMW_OK;
+}
+int tmw_unpack(tmw_ctx* ctx, int prec, int parity, const void* packed, double* canonical) {
+  if (!ctx) return TMW_EINVAL;
+  if (!canonical || !packed || (prec != TMW_F32 && prec != TMW_F64) || (parity != TMW_EVEN && parity != TMW_ODD)) return fail(ctx, TMW_EINVAL, "tmw_unpack: bad argument");
+  LAUNCH(launch_unpack_spinor(ctx->g, parity == TMW_ODD, prec, packed, canonical, ctx->stream));
+  return TMW_OK;
+}
+
+int tmw_get_clover(tmw_ctx* ctx, int parity, int inverse, double* dst) {
+  if (!ctx) return TMW_EINVAL;
+  if (!dst || (parity != TMW_EVEN && parity != TMW_ODD)) return fail(ctx, TMW_EINVAL, "tmw_get_clover: bad argument");
+  if (!ctx->clover) return fail(ctx, TMW_EINVAL, "tmw_get_clover: context has no clover term (c_sw = 0)");
+  if (inverse && parity != TMW_EVEN) return fail(ctx, TMW_EINVAL, "tmw_get_clover: the inverse is stored on the even parity only");
+  const void* src = inverse ? ctx->ci64 : ctx->c64[parity == TMW_ODD];
+  LAUNCH(launch_clover_export(ctx->g, src, dst, ctx->stream));
+  return TMW_OK;
+}
+
+}  // extern "C"
+
+// ---- workspaces ----
+static int need_w64(tmw_ctx* ctx, int n) {
+  for (int i = 0; i < n; i++)
+    if (!ctx->w64[i]) { int rc = dev_alloc(ctx, &ctx->w64[i], spinor_bytes(ctx, TMW_F64)); if (rc) return rc; }
+  return TMW_OK;
+}
+static int need_w32(tmw_ctx* ctx, int n, int prec) {
+  for (int i = 0; i < n; i++)
+    if (!ctx->w32[i]) { int rc = dev_alloc(ctx, &ctx->w32[i], spinor_bytes(ctx, prec)); if (rc) return rc; }
+  return TMW_OK;
+}
+static int need_canon(tmw_ctx* ctx) {
+  for (int i = 0; i < 2; i++)
+    if (!ctx->canon[i]) { int rc = dev_alloc(ctx, &ctx->canon[i], (size_t)ctx->V * 24 * 8); if (rc) return rc; }
+  return TMW_OK;
+}
+
+// out_p = A in_p + H in_pbar for both parities, fp64 packed
+static int full_apply64(tmw_ctx* ctx, int dagger, const void* in_e, const void* in_o, void* out_e, void* out_o) {
+  int rc = dslash<double>(ctx, EPI_A_XPAY, 0, dagger, in_o, out_e, in_e, 1.0);
+  if (rc) return rc;
+  return dslash<double>(ctx, EPI_A_XPAY, 1, dagger, in_e, out_o, in_o, 1.0);
+}
+
+extern "C" int tmw_apply(tmw_ctx* ctx, int op, int parity, int prec, const void* in, void* out) {
+  if (!ctx) return TMW_EINVAL;
+  if (!in || !out || in == out) return fail(ctx, TMW_EINVAL, "tmw_apply: null or aliased pointers");
+  if ((op != TMW_D && op != TMW_DDAG) || (parity != TMW_FULL && parity != TMW_EVEN && parity != TMW_ODD)) return fail(ctx, TMW_EINVAL, "tmw_apply: bad op or parity");
+  const int dagger = (op == TMW_DDAG);
+  if (parity != TMW_FULL) {
+    if (prec != TMW_F32 && prec != TMW_F64) return fail(ctx, TMW_EINVAL, "tmw_apply: bad precision");
+    const int par = (parity == TMW_ODD);
+    if (prec == TMW_F32) return dslash<float>(ctx, EPI_HOP, par, dagger, in, out, nullptr, 1.0);
+    return dslash<double>(ctx, EPI_HOP, par, dagger, in, out, nullptr, 1.0);
+  }
+  int rc = need_w64(ctx, 4);
+  if (rc) return rc;
+  const double* cin = (const double*)in;
+  double* cout = (double*)out;
+  const size_t cbytes = (size_t)ctx->V * 24 * 8;
+  if (ctx->opt.location == TMW_HOST) {
+    rc = need_canon(ctx);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(ctx->canon[0], in, cbytes, cudaMemcpyHostToDevice, ctx->stream));
+    cin = (const double*)ctx->canon[0];
+    cout = (double*)ctx->canon[1];
+  }
+  LAUNCH(launch_pack_spinor(ctx->g, 0, 1, cin, ctx->w64[0], ctx->stream));
+  LAUNCH(launch_pack_spinor(ctx->g, 1, 1, cin, ctx->w64[1], ctx->stream));
+  rc = full_apply64(ctx, dagger, ctx->w64[0], ctx->w64[1], ctx->w64[2], ctx->w64[3]);
+  if (rc) return rc;
+  LAUNCH(launch_unpack_spinor(ctx->g, 0, 1, ctx->w64[2], cout, ctx->stream));
+  LAUNCH(launch_unpack_spinor(ctx->g, 1, 1, ctx->w64[3], cout, ctx->stream));
+  if (ctx->opt.location == TMW_HOST) {
+    CK(cudaMemcpyAsync(out, cout, cbytes, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaStreamSynchronize(ctx->stream));
+  }
+  return TMW_OK;
+}
+
+extern "C" int tmw_apply_schur(tmw_ctx* ctx, int op, int prec, const void* in_odd, void* out_odd) {
+  if (!ctx) return TMW_EINVAL;
+  if (!in_odd || !out_odd || in_odd == out_odd) return fail(ctx, TMW_EINVAL, "tmw_apply_schur: null or aliased pointers");
+  if ((op != TMW_D && op != TMW_DDAG) || (prec != TMW_F32 && prec != TMW_F64)) return fail(ctx, TMW_EINVAL, "tmw_apply_schur: bad op or precision");
+  const int dagger = (op == TMW_DDAG);
+  int rc;
+  if (prec == TMW_F64) {
+    if ((rc = need_w64(ctx, 1))) return rc;
+    return schur<double>(ctx, dagger, in_odd, out_odd, ctx->w64[0]);
+  }
+  // an fp32 even-parity scratch: reuse the head of an fp64 workspace
+  if ((rc = need_w64(ctx, 1))) return rc;
+  return schur<float>(ctx, dagger, in_odd, out_odd, ctx->w64[0]);
+}
+
+// ---- the solver ----
+namespace {
+
+struct SolveState {
+  int iters, updates, restarts;
+  double iter_resid, true_resid;
+};
+
+// download the scalar block and wait
+int fetch_scalars(tmw_ctx* ctx) {
+  CK(cudaMemcpyAsync(ctx->sc_host, ctx->sc, sizeof(Scalars), cudaMemcpyDeviceToHost, ctx->stream));
+  CK(cudaStreamSynchronize(ctx->stream));
+  return TMW_OK;
+}
+int push_scalars(tmw_ctx* ctx) {
+  CK(cudaMemcpyAsync(ctx->sc, ctx->sc_host, sizeof(Scalars), cudaMemcpyHostToDevice, ctx->stream));
+  // the pinned block is rewritten by the host right after some pushes: wait for the copy
+  CK(cudaStreamSynchronize(ctx->stream));
+  return TMW_OK;
+}
+int fetch_red(tmw_ctx* ctx) {
+  CK(cudaMemcpyAsync(ctx->red_host, ctx->red, 4 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+  CK(cudaStreamSynchronize(ctx->stream));
+  return TMW_OK;
+}
+
+// BiCGStab (van der Vorst) on the odd-site Schur system Mhat y = bhat, inner precision R, fp64 reliable updates.
+//   w64: 0 b_e, 1 b_o, 2 bhat_o, 3 y, 4 r64, 5 tmp_e64, 6 w (Mhat y), 7 x_e
+//   w32: 0 r, 1 rhat, 2 p, 3 v, 4 s, 5 t, 6 x, 7 tmp_e
+template <typename R>
+int solve_schur(tmw_ctx* ctx, double tol, double bnorm, SolveState* st) {
+  cudaStream_t s = ctx->stream;
+  const int64_t n64 = (int64_t)ctx->g.Vh * 12;                           // double2 vectors per fp64 parity spinor
+  const int64_t nR = (int64_t)ctx->g.Vh * 24 * (int64_t)sizeof(R) / 16;  // 16-byte vectors per inner spinor
+  const size_t bytesR = (size_t)nR * 16;
+  void** W = ctx->w64;
+  void** X = ctx->w32;
+  void *r = X[0], *rhat = X[1], *p = X[2], *v = X[3], *sv = X[4], *t = X[5], *x = X[6], *tmp = X[7];
+  Scalars* h = ctx->sc_host;
+  const double eps_break = sizeof(R) == 4 ? 1e-6 : 1e-12;
+  int rc;
+  // y = 0, r64 = bhat, r = (R) r64, rhat = r, x = p = v = 0
+  CK(cudaMemsetAsync(W[3], 0, (size_t)n64 * 16, s));
+  CK(cudaMemsetAsync(W[6], 0, (size_t)n64 * 16, s));
+  CK(cudaMemsetAsync(x, 0, bytesR, s));
+  CK(cudaMemsetAsync(p, 0, bytesR, s));
+  CK(cudaMemsetAsync(v, 0, bytesR, s));
+  LAUNCH(launch_convert<R>(n64, W[2], rhat, s));
+  memset(h, 0, sizeof(Scalars));
+  if ((rc = push_scalars(ctx))) return rc;
+  LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], r, rhat, ctx->sc, s));  // r64 = bhat - 0; rho = <rhat,r>; rr = |r64|^2
+  if ((rc = fetch_scalars(ctx))) return rc;
+  h->rho_old[0] = h->alpha[0] = h->omega[0] = 1.0;
+  h->rho_old[1] = h->alpha[1] = h->omega[1] = 0.0;
+  if ((rc = push_scalars(ctx))) return rc;
+  double rnorm = sqrt(h->rr), maxr = rnorm, rhat_norm = rnorm;
+  st->iter_resid = rnorm / bnorm;
+  if (rnorm <= tol * bnorm) return TMW_OK;
+  const int max_iter = ctx->opt.max_iter;
+  for (int k = 1; k <= max_iter; k++) {
+    st->iters = k;
+    LAUNCH(launch_sc_begin_iter(ctx->sc, s));
+    LAUNCH(launch_update_p<R>(nR, p, r, v, ctx->sc, s));
+    if ((rc = schur<R>(ctx, 0, p, v, tmp, 1, rhat, (double*)((char*)ctx->sc + offsetof(Scalars, rhat_v))))) return rc;
+    LAUNCH(launch_sc_alpha(ctx->sc, s));
+    LAUNCH(launch_update_s<R>(nR, sv, r, v, ctx->sc, s));
+    if ((rc = schur<R>(ctx, 0, sv, t, tmp, 2, nullptr, (double*)((char*)ctx->sc + offsetof(Scalars, ts))))) return rc;
+    LAUNCH(launch_sc_omega(ctx->sc, s));
+    LAUNCH(launch_update_xr<R>(nR, x, r, p, sv, t, rhat, ctx->sc, s));
+    if ((rc = fetch_scalars(ctx))) return rc;
+    bool broken = !isfinite(h->rr) || !isfinite(h->rho[0]) || !isfinite(h->rho[1]);
+    rnorm = broken ? maxr : sqrt(h->rr);
+    if (!broken) st->iter_resid = rnorm / bnorm;
+    const bool conv = !broken && rnorm <= tol * bnorm;
+    if (broken || conv || rnorm < ctx->opt.delta * maxr || k == max_iter) {
+      // reliable update: y += x (skipped if the iterate is corrupted), true residual in fp64
+      if (!broken) LAUNCH(launch_acc_y<R>(n64, W[3], x, s));
+      else CK(cudaMemsetAsync(x, 0, bytesR, s));
+      if ((rc = schur<double>(ctx, 0, W[3], W[6], W[5]))) return rc;
+      h->rho[0] = h->rho[1] = 0.0;
+      h->rr = 0.0;
+      if (broken) { h->rho_old[0] = h->alpha[0] = h->omega[0] = 1.0; h->rho_old[1] = h->alpha[1] = h->omega[1] = 0.0; }
+      if ((rc = push_scalars(ctx))) return rc;
+      LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], r, rhat, ctx->sc, s));
+      if ((rc = fetch_scalars(ctx))) return rc;
+      st->updates++;
+      rnorm = sqrt(h->rr);
+      maxr = rnorm;
+      st->iter_resid = rnorm / bnorm;
+      if (!isfinite(rnorm)) return fail(ctx, TMW_EBREAKDOWN, "tmw_solve: non-finite true residual");
+      if (rnorm <= tol * bnorm) return TMW_OK;
+      if (k == max_iter) break;
+    } else if (rnorm > maxr) {
+      maxr = rnorm;
+    }
+    const double rho_abs = hypot(h->rho[0], h->rho[1]);
+    if (broken || !(rho_abs > eps_break * rhat_norm * rnorm)) {
+      // breakdown: restart the recurrence with rhat = r (C11)
+      if (++st->restarts > 5) return fail(ctx, TMW_EBREAKDOWN, "tmw_solve: BiCGStab breakdown persists after 5 restarts");
+      // fold the current iterate into y first so that r is the residual of y
+      LAUNCH(launch_acc_y<R>(n64, W[3], x, s));
+      if ((rc = schur<double>(ctx, 0, W[3], W[6], W[5]))) return rc;
+      CK(cudaMemsetAsync(p, 0, bytesR, s));
+      CK(cudaMemsetAsync(v, 0, bytesR, s));
+      memset(h, 0, sizeof(Scalars));
+      h->rho_old[0] = h->alpha[0] = h->omega[0] = 1.0;
+      if ((rc = push_scalars(ctx))) return rc;
+      LAUNCH(launch_sub_norm(n64, W[2], W[6], W[4], ctx->red, s));  // r64 = bhat - Mhat y (norm discarded)
+      LAUNCH(launch_convert<R>(n64, W[4], rhat, s));
+      LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], r, rhat, ctx->sc, s));
+      if ((rc = fetch_scalars(ctx))) return rc;
+      rnorm = sqrt(h->rr);
+      maxr = rhat_norm = rnorm;
+      st->updates++;
+      if (rnorm <= tol * bnorm) return TMW_OK;
+    }
+  }
+  return fail(ctx, TMW_ENOCONV, "tmw_solve: max_iter reached");
+}
+
+}  // namespace
+
+extern "C" int tmw_solve(tmw_ctx* ctx, const double* b, double* x, double tol, tmw_solve_info* info) {
+  if (!ctx) return TMW_EINVAL;
+  if (!b || !x || b == x) return fail(ctx, TMW_EINVAL, "tmw_solve: null or aliased pointers");
+  if (!(tol > 0.0) || !isfinite(tol)) return fail(ctx, TMW_EINVAL, "tmw_solve: tol must be > 0");
+  if (info) memset(info, 0, sizeof(*info));
+  const bool dbl = ctx->opt.precision == TMW_DOUBLE;
+  int rc;
+  if ((rc = need_w64(ctx, 8))) return rc;
+  if ((rc = need_w32(ctx, 8, dbl ? TMW_F64 : TMW_F32))) return rc;
+  cudaStream_t s = ctx->stream;
+  const size_t cbytes = (size_t)ctx->V * 24 * 8;
+  const double* cb = b;
+  double* cx_ = x;
+  if (ctx->opt.location == TMW_HOST) {
+    if ((rc = need_canon(ctx))) return rc;
+    cb = (const double*)ctx->canon[0];
+    cx_ = (double*)ctx->canon[1];
+  }
+  CK(cudaEventRecord(ctx->ev0, s));
+  if (ctx->opt.location == TMW_HOST) CK(cudaMemcpyAsync(ctx->canon[0], b, cbytes, cudaMemcpyHostToDevice, s));
+  void** W = ctx->w64;
+  const int64_t n64 = (int64_t)ctx->g.Vh * 12;
+  SolveState st;
+  memset(&st, 0, sizeof(st));
+  // A0/A7: split b, |b|, bhat_o = b_o - H_oe A_ee^{-1} b_e
+  LAUNCH(launch_pack_spinor(ctx->g, 0, 1, cb, W[0], s));
+  LAUNCH(launch_pack_spinor(ctx->g, 1, 1, cb, W[1], s));
+  CK(cudaMemsetAsync(ctx->red, 0, 4 * sizeof(double), s));
+  LAUNCH(launch_dot_norm<double>(n64, nullptr, W[0], ctx->red, s));
+  LAUNCH(launch_dot_norm<double>(n64, nullptr, W[1], ctx->red, s));
+  if ((rc = fetch_red(ctx))) return rc;
+  const double bnorm = sqrt(ctx->red_host[2]);
+  if (!isfinite(bnorm)) return fail(ctx, TMW_EINVAL, "tmw_solve: b has non-finite entries");
+  int status = TMW_OK;
+  if (bnorm == 0.0) {
+    CK(cudaMemsetAsync(cx_, 0, cbytes, s));
+  } else {
+    Diag<double> d = make_diag<double>(ctx, 0);
+    LAUNCH(launch_diag(d, ctx->g, 0, ctx->clover, 1, W[0], W[5], s));
+    if ((rc = dslash<double>(ctx, EPI_XPAY, 1, 0, W[5], W[2], W[1], -1.0))) return rc;
+    status = dbl ? solve_schur<double>(ctx, tol, bnorm, &st) : solve_schur<float>(ctx, tol, bnorm, &st);
+    if (status != TMW_OK && status != TMW_ENOCONV) return status;
+    // A7: x_o = y, x_e = A_ee^{-1} (b_e - H_eo x_o)
+    if ((rc = dslash<double>(ctx, EPI_AINV_XPAY, 0, 0, W[3], W[7], W[0], -1.0))) return rc;
+    LAUNCH(launch_unpack_spinor(ctx->g, 0, 1, W[7], cx_, s));
+    LAUNCH(launch_unpack_spinor(ctx->g, 1, 1, W[3], cx_, s));
+    // true residual of the full system in fp64: |b - D x|
+    if ((rc = full_apply64(ctx, 0, W[7], W[3], W[5], W[6]))) return rc;
+    CK(cudaMemsetAsync(ctx->red, 0, 4 * sizeof(double), s));
+    LAUNCH(launch_sub_norm(n64, W[0], W[5], W[5], ctx->red, s));
+    LAUNCH(launch_sub_norm(n64, W[1], W[6], W[6], ctx->red, s));
+    if ((rc = fetch_red(ctx))) return rc;
+    st.true_resid = sqrt(ctx->red_host[2]) / bnorm;
+  }
+  if (ctx->opt.location == TMW_HOST) CK(cudaMemcpyAsync(x, cx_, cbytes, cudaMemcpyDeviceToHost, s));
+  CK(cudaEventRecord(ctx->ev1, s));
+  CK(cudaStreamSynchronize(s));
+  float ms = 0;
+  CK(cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
+  if (info) {
+    info->iters = st.iters;
+    info->reliable_updates = st.updates;
+    info->restarts = st.restarts;
+    info->iter_resid = st.iter_resid;
+    info->true_resid = st.true_resid;
+    info->device_ms = ms;
+  }
+  return status;
+}

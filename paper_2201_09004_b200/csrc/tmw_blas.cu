@@ -1,0 +1,259 @@
+// tmw_blas.cu — fused BLAS-1 kernels of the BiCGStab recurrences (the "vector operations" of
+// PAPER.md:315). Complex scalars (alpha, beta, omega, rho) live on the device in a Scalars block; reductions are
+// accumulated in fp64 (per-thread -> warp shuffle -> block -> one atomicAdd per block and value).
+// All vectors are packed parity spinors viewed as flat arrays of complex numbers; a work item is a PAIR of
+// complex numbers = 4 reals (one float4, or two double2).
+#include "tmw_internal.h"
+
+namespace tmw {
+
+__device__ __forceinline__ void ldp(const float* base, int64_t i, float* v) {
+  const float4 q = *((const float4*)base + i);
+  v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
+}
+__device__ __forceinline__ void ldp(const double* base, int64_t i, double* v) {
+  const double2 a = *((const double2*)base + 2 * i), b = *((const double2*)base + 2 * i + 1);
+  v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
+}
+__device__ __forceinline__ void stp(float* base, int64_t i, const float* v) { *((float4*)base + i) = make_float4(v[0], v[1], v[2], v[3]); }
+__device__ __forceinline__ void stp(double* base, int64_t i, const double* v) {
+  *((double2*)base + 2 * i) = make_double2(v[0], v[1]);
+  *((double2*)base + 2 * i + 1) = make_double2(v[2], v[3]);
+}
+
+enum { BB = 256 };
+static inline int blas_grid(int64_t n) {
+  int64_t g = (n + BB - 1) / BB;
+  const int64_t cap = 148 * 8;
+  return (int)(g < cap ? (g > 0 ? g : 1) : cap);
+}
+
+template <int NV> __device__ __forceinline__ void reduce_atomic(double (&v)[NV], double* const* dst) {
+  __shared__ double sm[NV][BB / 32];
+#pragma unroll
+  for (int k = 0; k < NV; k++)
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v[k] += __shfl_down_sync(0xffffffffu, v[k], off);
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  if (lane == 0)
+#pragma unroll
+    for (int k = 0; k < NV; k++) sm[k][w] = v[k];
+  __syncthreads();
+  if (threadIdx.x < NV) {
+    double s = 0;
+#pragma unroll
+    for (int i = 0; i < BB / 32; i++) s += sm[threadIdx.x][i];
+    atomicAdd(dst[threadIdx.x], s);
+  }
+}
+
+// ---- scalar phase kernels (one thread) ----
+__device__ __forceinline__ void cdiv(const double* a, const double* b, double* q) {  // q = a / b
+  const double d = b[0] * b[0] + b[1] * b[1];
+  const double re = (a[0] * b[0] + a[1] * b[1]) / d, im = (a[1] * b[0] - a[0] * b[1]) / d;
+  q[0] = re; q[1] = im;
+}
+__global__ void sc_begin_iter_kernel(Scalars* sc) {  // beta = (rho/rho_old)(alpha/omega)
+  double a[2], b[2];
+  cdiv(sc->rho, sc->rho_old, a);
+  cdiv(sc->alpha, sc->omega, b);
+  sc->beta[0] = a[0] * b[0] - a[1] * b[1];
+  sc->beta[1] = a[0] * b[1] + a[1] * b[0];
+  sc->rhat_v[0] = sc->rhat_v[1] = 0.0;
+  sc->ts[0] = sc->ts[1] = 0.0;
+  sc->tt = 0.0;
+}
+__global__ void sc_alpha_kernel(Scalars* sc) { cdiv(sc->rho, sc->rhat_v, sc->alpha); }
+__global__ void sc_omega_kernel(Scalars* sc) {
+  sc->omega[0] = sc->ts[0] / sc->tt;
+  sc->omega[1] = sc->ts[1] / sc->tt;
+  sc->rho_old[0] = sc->rho[0];
+  sc->rho_old[1] = sc->rho[1];
+  sc->rho[0] = sc->rho[1] = 0.0;
+  sc->rr = 0.0;
+}
+cudaError_t launch_sc_begin_iter(Scalars* sc, cudaStream_t s) { sc_begin_iter_kernel<<<1, 1, 0, s>>>(sc); return cudaGetLastError(); }
+cudaError_t launch_sc_alpha(Scalars* sc, cudaStream_t s) { sc_alpha_kernel<<<1, 1, 0, s>>>(sc); return cudaGetLastError(); }
+cudaError_t launch_sc_omega(Scalars* sc, cudaStream_t s) { sc_omega_kernel<<<1, 1, 0, s>>>(sc); return cudaGetLastError(); }
+
+// ---- vector updates ----
+template <typename R> __global__ void __launch_bounds__(BB) update_p_kernel(int64_t n, R* p, const R* r, const R* v, const Scalars* sc) {
+  const R br = (R)sc->beta[0], bi = (R)sc->beta[1], wr = (R)sc->omega[0], wi = (R)sc->omega[1];
+  for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
+    R pp[4], rr[4], vv[4];
+    ldp(p, i, pp); ldp(r, i, rr); ldp(v, i, vv);
+#pragma unroll
+    for (int c = 0; c < 2; c++) {
+      const R ur = pp[2 * c] - (wr * vv[2 * c] - wi * vv[2 * c + 1]);
+      const R ui = pp[2 * c + 1] - (wr * vv[2 * c + 1] + wi * vv[2 * c]);
+      pp[2 * c] = rr[2 * c] + (br * ur - bi * ui);
+      pp[2 * c + 1] = rr[2 * c + 1] + (br * ui + bi * ur);
+    }
+    stp(p, i, pp);
+  }
+}
+template <typename R> __global__ void __launch_bounds__(BB) update_s_kernel(int64_t n, R* s, const R* r, const R* v, const Scalars* sc) {
+  const R ar = (R)sc->alpha[0], ai = (R)sc->alpha[1];
+  for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
+    R rr[4], vv[4], ss[4];
+    ldp(r, i, rr); ldp(v, i, vv);
+#pragma unroll
+    for (int c = 0; c < 2; c++) {
+      ss[2 * c] = rr[2 * c] - (ar * vv[2 * c] - ai * vv[2 * c + 1]);
+      ss[2 * c + 1] = rr[2 * c + 1] - (ar * vv[2 * c + 1] + ai * vv[2 * c]);
+    }
+    stp(s, i, ss);
+  }
+}
+template <typename R> __global__ void __launch_bounds__(BB) update_xr_kernel(int64_t n, R* x, R* r, const R* p, const R* s, const R* t, const R* rhat, Scalars* sc) {
+  const R ar = (R)sc->alpha[0], ai = (R)sc->alpha[1], wr = (R)sc->omega[0], wi = (R)sc->omega[1];
+  double acc[3] = {0, 0, 0};
+  for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
+    R xx[4], pp[4], ss[4], tt[4], hh[4], rr[4];
+    ldp(x, i, xx); ldp(p, i, pp); ldp(s, i, ss); ldp(t, i, tt); ldp(rhat, i, hh);
+    R re = 0, im = 0, nn = 0;
+#pragma unroll
+    for (int c = 0; c < 2; c++) {
+      xx[2 * c] += (ar * pp[2 * c] - ai * pp[2 * c + 1]) + (wr * ss[2 * c] - wi * ss[2 * c + 1]);
+      xx[2 * c + 1] += (ar * pp[2 * c + 1] + ai * pp[2 * c]) + (wr * ss[2 * c + 1] + wi * ss[2 * c]);
+      rr[2 * c] = ss[2 * c] - (wr * tt[2 * c] - wi * tt[2 * c + 1]);
+      rr[2 * c + 1] = ss[2 * c + 1] - (wr * tt[2 * c + 1] + wi * tt[2 * c]);
+      re += hh[2 * c] * rr[2 * c] + hh[2 * c + 1] * rr[2 * c + 1];
+      im += hh[2 * c] * rr[2 * c + 1] - hh[2 * c + 1] * rr[2 * c];
+      nn += rr[2 * c] * rr[2 * c] + rr[2 * c + 1] * rr[2 * c + 1];
+    }
+    stp(x, i, xx);
+    stp(r, i, rr);
+    acc[0] += re; acc[1] += im; acc[2] += nn;
+  }
+  double* dst[3] = {&sc->rho[0], &sc->rho[1], &sc->rr};
+  reduce_atomic<3>(acc, dst);
+}
+template <typename R> __global__ void __launch_bounds__(BB) dot_norm_kernel(int64_t n, const R* a, const R* b, double* out) {
+  double acc[3] = {0, 0, 0};
+  for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
+    R aa[4] = {0, 0, 0, 0}, bb[4];
+    if (a) ldp(a, i, aa);
+    ldp(b, i, bb);
+    R re = 0, im = 0, nn = 0;
+#pragma unroll
+    for (int c = 0; c < 2; c++) {
+      re += aa[2 * c] * bb[2 * c] + aa[2 * c + 1] * bb[2 * c + 1];
+      im += aa[2 * c] * bb[2 * c + 1] - aa[2 * c + 1] * bb[2 * c];
+      nn += bb[2 * c] * bb[2 * c] + bb[2 * c + 1] * bb[2 * c + 1];
+    }
+    acc[0] += re; acc[1] += im; acc[2] += nn;
+  }
+  double* dst[3] = {out, out + 1, out + 2};
+  reduce_atomic<3>(acc, dst);
+}
+template <typename R> __global__ void __launch_bounds__(BB) acc_y_kernel(int64_t n, double* y, R* x) {
+  for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
+    R xx[4];
+    double yy[4];
+    ldp(x, i, xx); ldp(y, i, yy);
+#pragma unroll
+    for (int c = 0; c < 4; c++) { yy[c] += (double)xx[c]; xx[c] = (R)0; }
+    stp(y, i, yy);
+    stp(x, i, xx);
+  }
+}
+template <typename R> __global__ void __launch_bounds__(BB) resid_convert_kernel(int64_t n, const double* b, const double* w, double* r64, R* r, const R* rhat, Scalars* sc) {
+  double acc[3] = {0, 0, 0};
+  for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
+    double bb[4], ww[4], dd[4];
+    R hh[4], rr[4];
+    ldp(b, i, bb); ldp(w, i, ww); ldp(rhat, i, hh);
+#pragma unroll
+    for (int c = 0; c < 4; c++) { dd[c] = bb[c] - ww[c]; rr[c] = (R)dd[c]; }
+    stp(r64, i, dd);
+    stp(r, i, rr);
+#pragma unroll
+    for (int c = 0; c < 2; c++) {
+      acc[0] += (double)hh[2 * c] * dd[2 * c] + (double)hh[2 * c + 1] * dd[2 * c + 1];
+      acc[1] += (double)hh[2 * c] * dd[2 * c + 1] - (double)hh[2 * c + 1] * dd[2 * c];
+      acc[2] += dd[2 * c] * dd[2 * c] + dd[2 * c + 1] * dd[2 * c + 1];
+    }
+  }
+  double* dst[3] = {&sc->rho[0], &sc->rho[1], &sc->rr};
+  reduce_atomic<3>(acc, dst);
+}
+template <typename R> __global__ void __launch_bounds__(BB) convert_kernel(int64_t n, const double* src, R* dst) {
+  for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
+    double ss[4];
+    R dd[4];
+    ldp(src, i, ss);
+#pragma unroll
+    for (int c = 0; c < 4; c++) dd[c] = (R)ss[c];
+    stp(dst, i, dd);
+  }
+}
+__global__ void __launch_bounds__(BB) sub_norm_kernel(int64_t n, const double* a, const double* b, double* d, double* out) {
+  double acc[1] = {0};
+  for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
+    double aa[4], bb[4], dd[4];
+    ldp(a, i, aa); ldp(b, i, bb);
+#pragma unroll
+    for (int c = 0; c < 4; c++) { dd[c] = aa[c] - bb[c]; acc[0] += dd[c] * dd[c]; }
+    stp(d, i, dd);
+  }
+  double* dst[1] = {out + 2};
+  reduce_atomic<1>(acc, dst);
+}
+
+// n16 = number of 16-byte vectors of R; pairs = n16 (float) or n16/2 (double)
+template <typename R> static inline int64_t pairs_of(int64_t n16) { return sizeof(R) == 4 ? n16 : n16 / 2; }
+
+template <typename R> cudaError_t launch_update_p(int64_t n, void* p, const void* r, const void* v, const Scalars* sc, cudaStream_t s) {
+  const int64_t np = pairs_of<R>(n);
+  update_p_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, (R*)p, (const R*)r, (const R*)v, sc);
+  return cudaGetLastError();
+}
+template <typename R> cudaError_t launch_update_s(int64_t n, void* sv, const void* r, const void* v, const Scalars* sc, cudaStream_t s) {
+  const int64_t np = pairs_of<R>(n);
+  update_s_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, (R*)sv, (const R*)r, (const R*)v, sc);
+  return cudaGetLastError();
+}
+template <typename R> cudaError_t launch_update_xr(int64_t n, void* x, void* r, const void* p, const void* sv, const void* t, const void* rhat, Scalars* sc, cudaStream_t s) {
+  const int64_t np = pairs_of<R>(n);
+  update_xr_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, (R*)x, (R*)r, (const R*)p, (const R*)sv, (const R*)t, (const R*)rhat, sc);
+  return cudaGetLastError();
+}
+template <typename R> cudaError_t launch_dot_norm(int64_t n, const void* a, const void* b, double* out, cudaStream_t s) {
+  const int64_t np = pairs_of<R>(n);
+  dot_norm_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, (const R*)a, (const R*)b, out);
+  return cudaGetLastError();
+}
+template <typename R> cudaError_t launch_acc_y(int64_t n64, void* y64, void* x, cudaStream_t s) {
+  const int64_t np = n64 / 2;
+  acc_y_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, (double*)y64, (R*)x);
+  return cudaGetLastError();
+}
+template <typename R> cudaError_t launch_resid_convert(int64_t n64, const void* b64, const void* w64, void* r64, void* r, const void* rhat, Scalars* sc, cudaStream_t s) {
+  const int64_t np = n64 / 2;
+  resid_convert_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, (const double*)b64, (const double*)w64, (double*)r64, (R*)r, (const R*)rhat, sc);
+  return cudaGetLastError();
+}
+template <typename R> cudaError_t launch_convert(int64_t n64, const void* src64, void* dst, cudaStream_t s) {
+  const int64_t np = n64 / 2;
+  convert_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, (const double*)src64, (R*)dst);
+  return cudaGetLastError();
+}
+cudaError_t launch_sub_norm(int64_t n64, const void* a, const void* b, void* d, double* out, cudaStream_t s) {
+  const int64_t np = n64 / 2;
+  sub_norm_kernel<<<blas_grid(np), BB, 0, s>>>(np, (const double*)a, (const double*)b, (double*)d, out);
+  return cudaGetLastError();
+}
+
+#define TMW_INST(R)                                                                                                          \
+  template cudaError_t launch_update_p<R>(int64_t, void*, const void*, const void*, const Scalars*, cudaStream_t);           \
+  template cudaError_t launch_update_s<R>(int64_t, void*, const void*, const void*, const Scalars*, cudaStream_t);           \
+  template cudaError_t launch_update_xr<R>(int64_t, void*, void*, const void*, const void*, const void*, const void*, Scalars*, cudaStream_t); \
+  template cudaError_t launch_dot_norm<R>(int64_t, const void*, const void*, double*, cudaStream_t);                         \
+  template cudaError_t launch_acc_y<R>(int64_t, void*, void*, cudaStream_t);                                                 \
+  template cudaError_t launch_resid_convert<R>(int64_t, const void*, const void*, void*, void*, const void*, Scalars*, cudaStream_t); \
+  template cudaError_t launch_convert<R>(int64_t, const void*, void*, cudaStream_t);
+TMW_INST(float)
+TMW_INST(double)
+
+}  // namespace tmw

@@ -1,0 +1,426 @@
+// tmw_core.cuh — per-site arithmetic of the twisted-mass Wilson(-clover) operator (arXiv:2201.09004 Eqs. (1)-(3),
+// PAPER.md:58-67) for the CUDA kernels of libtmw.so: packed-layout loads/stores, spin projection to half
+// spinors, SU(3) multiply with 12-real reconstruction, packed Hermitian 6x6 clover blocks, fused epilogues.
+// This header is private to csrc/ and shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define TMW_HD __host__ __device__ __forceinline__
+
+namespace tmw {
+
+// ---------------------------------------------------------------------------------------------------------
+// geometry of one parity of an L^3 x T lattice; cb = (x/2) + Lh*(y + L*(z + L*t))
+// ---------------------------------------------------------------------------------------------------------
+struct Geom {
+  int L, T, Lh;
+  int Vh;          // sites per parity (< 2^31)
+  int sy, sz, st;  // cb strides of +1 in y, z, t
+};
+
+// ---------------------------------------------------------------------------------------------------------
+// 16-byte vector access. A packed field of NREAL reals per site is stored as planes of 16-byte vectors:
+// vector (k, cb) at index k*stride + cb holds reals [k*N, k*N+N) of the site, N = 4 (float) or 2 (double).
+// ---------------------------------------------------------------------------------------------------------
+template <typename R> struct Vec16;
+template <> struct Vec16<float> { typedef float4 T; enum { N = 4 }; };
+template <> struct Vec16<double> { typedef double2 T; enum { N = 2 }; };
+
+template <typename R, int NREAL> struct Planes { enum { N = (NREAL + Vec16<R>::N - 1) / Vec16<R>::N }; };
+
+TMW_HD float4 ldv(const float4* p) {
+#ifdef __CUDA_ARCH__
+  return __ldg(p);
+#else
+  return *p;
+#endif
+}
+TMW_HD double2 ldv(const double2* p) {
+#ifdef __CUDA_ARCH__
+  return __ldg(p);
+#else
+  return *p;
+#endif
+}
+
+template <int NREAL> TMW_HD void load_reals(const void* base, int64_t stride, int64_t idx, float* v) {
+  const float4* p = (const float4*)base + idx;
+#pragma unroll
+  for (int k = 0; k < (NREAL + 3) / 4; k++) {
+    float4 q = ldv(p + k * stride);
+    v[4 * k] = q.x;
+    v[4 * k + 1] = q.y;
+    if (4 * k + 2 < NREAL) v[4 * k + 2] = q.z;
+    if (4 * k + 3 < NREAL) v[4 * k + 3] = q.w;
+  }
+}
+template <int NREAL> TMW_HD void load_reals(const void* base, int64_t stride, int64_t idx, double* v) {
+  const double2* p = (const double2*)base + idx;
+#pragma unroll
+  for (int k = 0; k < NREAL / 2; k++) {
+    double2 q = ldv(p + k * stride);
+    v[2 * k] = q.x;
+    v[2 * k + 1] = q.y;
+  }
+}
+template <int NREAL> TMW_HD void store_reals(void* base, int64_t stride, int64_t idx, const float* v) {
+  float4* p = (float4*)base + idx;
+#pragma unroll
+  for (int k = 0; k < (NREAL + 3) / 4; k++) {
+    float4 q;
+    q.x = v[4 * k];
+    q.y = v[4 * k + 1];
+    q.z = (4 * k + 2 < NREAL) ? v[4 * k + 2] : 0.f;
+    q.w = (4 * k + 3 < NREAL) ? v[4 * k + 3] : 0.f;
+    p[k * stride] = q;
+  }
+}
+template <int NREAL> TMW_HD void store_reals(void* base, int64_t stride, int64_t idx, const double* v) {
+  double2* p = (double2*)base + idx;
+#pragma unroll
+  for (int k = 0; k < NREAL / 2; k++) {
+    double2 q;
+    q.x = v[2 * k];
+    q.y = v[2 * k + 1];
+    p[k * stride] = q;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// complex helpers on (re, im) pairs held in plain arrays: z[2*i] = re, z[2*i+1] = im
+// ---------------------------------------------------------------------------------------------------------
+template <typename R> struct cx {
+  R re, im;
+};
+template <typename R> TMW_HD cx<R> mk(R re, R im) { cx<R> z; z.re = re; z.im = im; return z; }
+template <typename R> TMW_HD cx<R> operator+(cx<R> a, cx<R> b) { return mk<R>(a.re + b.re, a.im + b.im); }
+template <typename R> TMW_HD cx<R> operator-(cx<R> a, cx<R> b) { return mk<R>(a.re - b.re, a.im - b.im); }
+template <typename R> TMW_HD cx<R> operator*(cx<R> a, cx<R> b) {
+  return mk<R>(a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re);
+}
+template <typename R> TMW_HD cx<R> conj(cx<R> a) { return mk<R>(a.re, -a.im); }
+// acc += a*b
+template <typename R> TMW_HD void cmad(cx<R>& acc, cx<R> a, cx<R> b) {
+  acc.re += a.re * b.re;
+  acc.re -= a.im * b.im;
+  acc.im += a.re * b.im;
+  acc.im += a.im * b.re;
+}
+// acc += conj(a)*b
+template <typename R> TMW_HD void cmadc(cx<R>& acc, cx<R> a, cx<R> b) {
+  acc.re += a.re * b.re;
+  acc.re += a.im * b.im;
+  acc.im += a.re * b.im;
+  acc.im -= a.im * b.re;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// SU(3) link from NG stored reals (rows 0,1 [+ row 2]); NG = 12 rebuilds row 2 = conj(row0 x row1)
+// ---------------------------------------------------------------------------------------------------------
+template <typename R, int NG> TMW_HD void load_link(const void* base, int64_t stride, int64_t idx, cx<R> (&U)[9]) {
+  R g[(NG == 12) ? 12 : 20];
+  load_reals<NG>(base, stride, idx, g);
+#pragma unroll
+  for (int i = 0; i < NG / 2; i++) U[i] = mk<R>(g[2 * i], g[2 * i + 1]);
+  if (NG == 12) {
+    U[6] = conj(U[1] * U[5] - U[2] * U[4]);
+    U[7] = conj(U[2] * U[3] - U[0] * U[5]);
+    U[8] = conj(U[0] * U[4] - U[1] * U[3]);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// One hop of Eq. (2): acc += P(U h), with the spin projector 1 + sig*gamma_MU of rank 2 (DeGrand-Rossi basis):
+// only rows h0, h1 go through the colour multiply; rows 2, 3 of the result are +-1/+-i multiples of them.
+//   MU = x: h0 = p0 + sig*i*p3, h1 = p1 + sig*i*p2, row2 = -sig*i*h1, row3 = -sig*i*h0
+//   MU = y: h0 = p0 - sig*p3,   h1 = p1 + sig*p2,   row2 = +sig*h1,   row3 = -sig*h0
+//   MU = z: h0 = p0 + sig*i*p2, h1 = p1 - sig*i*p3, row2 = -sig*i*h0, row3 = +sig*i*h1
+//   MU = t: h0 = p0 + sig*p2,   h1 = p1 + sig*p3,   row2 = +sig*h0,   row3 = +sig*h1
+// FWD: colour matrix U (forward hop, U_mu(x)); else U^dagger (backward hop, U_mu(x-mu)^dagger).
+// bc multiplies the whole hop (antiperiodic time boundary: -1 when the hop wraps).
+// psi: 24 reals of the neighbour spinor, index 2*(3*spin+colour)+ri. acc: 24 reals.
+// ---------------------------------------------------------------------------------------------------------
+template <typename R, int MU, bool FWD> TMW_HD void hop(const R* psi, const cx<R> (&U)[9], R sig, R bc, R* acc) {
+  cx<R> h[6];  // h[3*s + c], s = 0,1
+#pragma unroll
+  for (int c = 0; c < 3; c++) {
+    const cx<R> p0 = mk<R>(psi[2 * c], psi[2 * c + 1]);
+    const cx<R> p1 = mk<R>(psi[6 + 2 * c], psi[6 + 2 * c + 1]);
+    const cx<R> p2 = mk<R>(psi[12 + 2 * c], psi[12 + 2 * c + 1]);
+    const cx<R> p3 = mk<R>(psi[18 + 2 * c], psi[18 + 2 * c + 1]);
+    if (MU == 0) {
+      h[c] = mk<R>(p0.re - sig * p3.im, p0.im + sig * p3.re);
+      h[3 + c] = mk<R>(p1.re - sig * p2.im, p1.im + sig * p2.re);
+    } else if (MU == 1) {
+      h[c] = mk<R>(p0.re - sig * p3.re, p0.im - sig * p3.im);
+      h[3 + c] = mk<R>(p1.re + sig * p2.re, p1.im + sig * p2.im);
+    } else if (MU == 2) {
+      h[c] = mk<R>(p0.re - sig * p2.im, p0.im + sig * p2.re);
+      h[3 + c] = mk<R>(p1.re + sig * p3.im, p1.im - sig * p3.re);
+    } else {
+      h[c] = mk<R>(p0.re + sig * p2.re, p0.im + sig * p2.im);
+      h[3 + c] = mk<R>(p1.re + sig * p3.re, p1.im + sig * p3.im);
+    }
+  }
+  if (MU == 3) {
+#pragma unroll
+    for (int i = 0; i < 6; i++) { h[i].re *= bc; h[i].im *= bc; }
+  }
+#pragma unroll
+  for (int s = 0; s < 2; s++) {
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+      cx<R> w = mk<R>((R)0, (R)0);
+#pragma unroll
+      for (int b = 0; b < 3; b++) {
+        if (FWD) cmad(w, U[3 * a + b], h[3 * s + b]);
+        else cmadc(w, U[3 * b + a], h[3 * s + b]);
+      }
+      // rows 0,1
+      acc[2 * (3 * s + a)] += w.re;
+      acc[2 * (3 * s + a) + 1] += w.im;
+      // rows 2,3
+      if (MU == 0) {  // row2 = -sig*i*h1, row3 = -sig*i*h0 : -i*w = (w.im, -w.re)
+        const int r = (s == 0) ? 3 : 2;
+        acc[2 * (3 * r + a)] += sig * w.im;
+        acc[2 * (3 * r + a) + 1] -= sig * w.re;
+      } else if (MU == 1) {  // row2 = +sig*h1, row3 = -sig*h0
+        if (s == 0) {
+          acc[2 * (9 + a)] -= sig * w.re;
+          acc[2 * (9 + a) + 1] -= sig * w.im;
+        } else {
+          acc[2 * (6 + a)] += sig * w.re;
+          acc[2 * (6 + a) + 1] += sig * w.im;
+        }
+      } else if (MU == 2) {  // row2 = -sig*i*h0, row3 = +sig*i*h1
+        if (s == 0) {
+          acc[2 * (6 + a)] += sig * w.im;
+          acc[2 * (6 + a) + 1] -= sig * w.re;
+        } else {
+          acc[2 * (9 + a)] -= sig * w.im;
+          acc[2 * (9 + a) + 1] += sig * w.re;
+        }
+      } else {  // row2 = +sig*h0, row3 = +sig*h1
+        acc[2 * (3 * (s + 2) + a)] += sig * w.re;
+        acc[2 * (3 * (s + 2) + a) + 1] += sig * w.im;
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Packed Hermitian 6x6 block (36 reals: 6 real diagonal, then 15 strictly-lower complex entries row-major,
+// entry (i,j), i>j, at 6 + 2*(i*(i-1)/2 + j)) times a 6-vector: out = B v.
+// v, out: 12 reals = 6 complex, index i = 3*(spin mod 2) + colour of one chirality.
+// ---------------------------------------------------------------------------------------------------------
+template <typename R> TMW_HD void herm6_mul(const R* B, const R* v, R* out) {
+#pragma unroll
+  for (int i = 0; i < 6; i++) {
+    R re = B[i] * v[2 * i], im = B[i] * v[2 * i + 1];
+#pragma unroll
+    for (int j = 0; j < 6; j++) {
+      if (j < i) {
+        const int k = 6 + 2 * (i * (i - 1) / 2 + j);
+        re += B[k] * v[2 * j] - B[k + 1] * v[2 * j + 1];
+        im += B[k] * v[2 * j + 1] + B[k + 1] * v[2 * j];
+      } else if (j > i) {
+        const int k = 6 + 2 * (j * (j - 1) / 2 + i);
+        re += B[k] * v[2 * j] + B[k + 1] * v[2 * j + 1];
+        im += B[k] * v[2 * j + 1] - B[k + 1] * v[2 * j];
+      }
+    }
+    out[2 * i] = re;
+    out[2 * i + 1] = im;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// The site-diagonal part A of D and its inverse.
+//   A v = C v + i*tw_chi*v   per chirality chi (upper = spins 0,1; lower = spins 2,3)
+//   no clover: C = diag (= -(4 + Re m)); clover: C = packed Hermitian block that includes the diagonal.
+//   tw_up = -Im m, tw_lo = +Im m for D with the gamma5 twist (C4); signs flip for D^dagger; both = -Im m (D) for
+//   the complex-scalar reading.
+//   A^{-1}: no clover: complex scalar (inv_re, inv_im_chi) per chirality. Clover, tw = 0: packed C^{-1}.
+//   Clover with twist ("complex diagonal part"): (C + i tw)^{-1} = (C - i tw) (C^2 + tw^2)^{-1};
+//   the Hermitian (C^2 + tw^2)^{-1} is what `cinv` holds then, and C is read as well.
+// ---------------------------------------------------------------------------------------------------------
+template <typename R> struct Diag {
+  R diag;                 // -(4 + Re m), no-clover case
+  R tw_up, tw_lo;         // i*tw added per chirality
+  R inv_re, inv_im_up, inv_im_lo;  // no-clover inverse scalars
+  int twisted_clover;     // clover && tw != 0
+  const void* c[2];       // packed C blocks, per parity: [18 or 36 planes][Vh]
+  const void* cinv[2];    // packed inverse blocks (even parity only in practice)
+};
+
+// out = A v at site cb of parity par (v, out: 24 reals; may not alias)
+template <typename R, bool CLOVER> TMW_HD void apply_A(const Diag<R>& d, int par, int64_t Vh, int64_t cb, const R* v, R* out) {
+  if (CLOVER) {
+    const int NPB = Planes<R, 36>::N;  // planes per block
+#pragma unroll
+    for (int b = 0; b < 2; b++) {
+      R B[36];
+      load_reals<36>((const typename Vec16<R>::T*)d.c[par] + (int64_t)b * NPB * Vh, Vh, cb, B);
+      herm6_mul(B, v + 12 * b, out + 12 * b);
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < 24; i++) out[i] = d.diag * v[i];
+  }
+#pragma unroll
+  for (int i = 0; i < 6; i++) {
+    out[2 * i] -= d.tw_up * v[2 * i + 1];
+    out[2 * i + 1] += d.tw_up * v[2 * i];
+    out[12 + 2 * i] -= d.tw_lo * v[12 + 2 * i + 1];
+    out[12 + 2 * i + 1] += d.tw_lo * v[12 + 2 * i];
+  }
+}
+
+// out = A^{-1} v
+template <typename R, bool CLOVER> TMW_HD void apply_Ainv(const Diag<R>& d, int par, int64_t Vh, int64_t cb, const R* v, R* out) {
+  if (CLOVER) {
+    const int NPB = Planes<R, 36>::N;
+#pragma unroll
+    for (int b = 0; b < 2; b++) {
+      R B[36];
+      load_reals<36>((const typename Vec16<R>::T*)d.cinv[par] + (int64_t)b * NPB * Vh, Vh, cb, B);
+      if (!d.twisted_clover) {
+        herm6_mul(B, v + 12 * b, out + 12 * b);
+      } else {
+        R w[12];
+        herm6_mul(B, v + 12 * b, w);
+        load_reals<36>((const typename Vec16<R>::T*)d.c[par] + (int64_t)b * NPB * Vh, Vh, cb, B);
+        herm6_mul(B, w, out + 12 * b);
+        const R tw = b ? d.tw_lo : d.tw_up;  // (C - i tw) w
+#pragma unroll
+        for (int i = 0; i < 6; i++) {
+          out[12 * b + 2 * i] += tw * w[2 * i + 1];
+          out[12 * b + 2 * i + 1] -= tw * w[2 * i];
+        }
+      }
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < 6; i++) {
+      out[2 * i] = d.inv_re * v[2 * i] - d.inv_im_up * v[2 * i + 1];
+      out[2 * i + 1] = d.inv_re * v[2 * i + 1] + d.inv_im_up * v[2 * i];
+      out[12 + 2 * i] = d.inv_re * v[12 + 2 * i] - d.inv_im_lo * v[12 + 2 * i + 1];
+      out[12 + 2 * i + 1] = d.inv_re * v[12 + 2 * i + 1] + d.inv_im_lo * v[12 + 2 * i];
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// The stencil. Epilogues (h = 1/2 sum of the 8 hops = the hopping block H_{p pbar} applied to `in`):
+// ---------------------------------------------------------------------------------------------------------
+enum { EPI_HOP = 0,        // out = h
+       EPI_AINV_HOP = 1,   // out = A^{-1} h                      (K1 of the Schur operator)
+       EPI_A_XPAY = 2,     // out = A aux + sgn*h                 (K2: sgn = -1; full apply: sgn = +1)
+       EPI_XPAY = 3,       // out = aux + sgn*h                   (source preparation)
+       EPI_AINV_XPAY = 4   // out = A^{-1} (aux + sgn*h)          (solution reconstruction)
+};
+
+template <typename R> struct DslashArgs {
+  const void* in;    // packed spinor, parity 1-par
+  void* out;         // packed spinor, parity par
+  const void* aux;   // packed spinor, parity par (EPI >= 2)
+  const void* U[2];  // packed gauge per parity: [mu][planes][Vh]
+  Geom g;
+  int par;           // parity of the output sites
+  R sig;             // +1 for D, -1 for D^dagger (sign of gamma_mu in the projectors)
+  R coef;            // 1/2 * sgn
+  Diag<R> d;
+  // fused reductions (kernel wrapper): red_mode 0 none; 1: red[0..1] += <dotv, out>; 2: red[0..1] += <out, aux>, red[2] += <out,out>
+  int red_mode;
+  const void* dotv;
+  double* red;
+};
+
+// neighbour checkerboard indices and the time-boundary sign
+struct Nbr {
+  int fwd[4], bwd[4];
+  bool wrap_tf, wrap_tb;
+};
+TMW_HD Nbr neighbours(const Geom& g, int par, int cb) {
+  Nbr n;
+  const int xh = cb % g.Lh;
+  int q = cb / g.Lh;
+  const int y = q % g.L;
+  q /= g.L;
+  const int z = q % g.L;
+  const int t = q / g.L;
+  const int o = (y + z + t + par) & 1;  // x = 2*xh + o
+  // x+1 -> xh + o (wrap to 0), x-1 -> xh + o - 1 (wrap to Lh-1)
+  const int xf = xh + o, xb = xh + o - 1;
+  n.fwd[0] = cb - xh + (xf == g.Lh ? 0 : xf);
+  n.bwd[0] = cb - xh + (xb < 0 ? g.Lh - 1 : xb);
+  n.fwd[1] = (y == g.L - 1) ? cb - (g.L - 1) * g.sy : cb + g.sy;
+  n.bwd[1] = (y == 0) ? cb + (g.L - 1) * g.sy : cb - g.sy;
+  n.fwd[2] = (z == g.L - 1) ? cb - (g.L - 1) * g.sz : cb + g.sz;
+  n.bwd[2] = (z == 0) ? cb + (g.L - 1) * g.sz : cb - g.sz;
+  n.wrap_tf = (t == g.T - 1);
+  n.wrap_tb = (t == 0);
+  n.fwd[3] = n.wrap_tf ? cb - (g.T - 1) * g.st : cb + g.st;
+  n.bwd[3] = n.wrap_tb ? cb + (g.T - 1) * g.st : cb - g.st;
+  return n;
+}
+
+template <typename R, int NG, int MU>
+TMW_HD void hop_pair(const DslashArgs<R>& a, const Nbr& n, int cb, R* acc) {
+  const int NPG = Planes<R, NG>::N;
+  const int64_t Vh = a.g.Vh;
+  typedef typename Vec16<R>::T V;
+  {  // forward: (1 + sig g_mu) U_mu(x) psi(x+mu)
+    R psi[24];
+    cx<R> U[9];
+    load_reals<24>(a.in, Vh, n.fwd[MU], psi);
+    load_link<R, NG>((const V*)a.U[a.par] + (int64_t)MU * NPG * Vh, Vh, cb, U);
+    hop<R, MU, true>(psi, U, a.sig, (MU == 3 && n.wrap_tf) ? (R)-1 : (R)1, acc);
+  }
+  {  // backward: (1 - sig g_mu) U_mu(x-mu)^dag psi(x-mu)
+    R psi[24];
+    cx<R> U[9];
+    load_reals<24>(a.in, Vh, n.bwd[MU], psi);
+    load_link<R, NG>((const V*)a.U[1 - a.par] + (int64_t)MU * NPG * Vh, Vh, n.bwd[MU], U);
+    hop<R, MU, false>(psi, U, -a.sig, (MU == 3 && n.wrap_tb) ? (R)-1 : (R)1, acc);
+  }
+}
+
+// computes the output spinor o[24] of site cb; ax[24] receives aux(cb) when EPI >= 2
+template <typename R, int NG, int EPI, bool CLOVER>
+TMW_HD void dslash_site(const DslashArgs<R>& a, int cb, R* o, R* ax) {
+  const Nbr n = neighbours(a.g, a.par, cb);
+  R acc[24];
+#pragma unroll
+  for (int i = 0; i < 24; i++) acc[i] = (R)0;
+  hop_pair<R, NG, 0>(a, n, cb, acc);
+  hop_pair<R, NG, 1>(a, n, cb, acc);
+  hop_pair<R, NG, 2>(a, n, cb, acc);
+  hop_pair<R, NG, 3>(a, n, cb, acc);
+  const int64_t Vh = a.g.Vh;
+  if (EPI == EPI_HOP) {
+#pragma unroll
+    for (int i = 0; i < 24; i++) o[i] = a.coef * acc[i];
+  } else if (EPI == EPI_AINV_HOP) {
+#pragma unroll
+    for (int i = 0; i < 24; i++) acc[i] *= a.coef;
+    apply_Ainv<R, CLOVER>(a.d, a.par, Vh, cb, acc, o);
+  } else if (EPI == EPI_A_XPAY) {
+    load_reals<24>(a.aux, Vh, cb, ax);
+    apply_A<R, CLOVER>(a.d, a.par, Vh, cb, ax, o);
+#pragma unroll
+    for (int i = 0; i < 24; i++) o[i] += a.coef * acc[i];
+  } else if (EPI == EPI_XPAY) {
+    load_reals<24>(a.aux, Vh, cb, ax);
+#pragma unroll
+    for (int i = 0; i < 24; i++) o[i] = ax[i] + a.coef * acc[i];
+  } else {
+    load_reals<24>(a.aux, Vh, cb, ax);
+#pragma unroll
+    for (int i = 0; i < 24; i++) acc[i] = ax[i] + a.coef * acc[i];
+    apply_Ainv<R, CLOVER>(a.d, a.par, Vh, cb, acc, o);
+  }
+}
+
+}  // namespace tmw

@@ -1,0 +1,66 @@
+// tmw_internal.h — launcher declarations shared by the .cu files of libtmw.so (private to csrc/).
+#pragma once
+#include "tmw_core.cuh"
+
+namespace tmw {
+
+// ---- stencil (tmw_dslash_f32.cu / tmw_dslash_f64.cu) ----
+// ng = stored reals per link (12 | 18), epi = EPI_*, clover = the diagonal part has clover blocks
+cudaError_t launch_dslash(const DslashArgs<float>& a, int ng, int epi, bool clover, cudaStream_t s);
+cudaError_t launch_dslash(const DslashArgs<double>& a, int ng, int epi, bool clover, cudaStream_t s);
+// out = A in (inverse = 0) or A^{-1} in (inverse = 1) on parity par, site-local
+cudaError_t launch_diag(const Diag<float>& d, const Geom& g, int par, bool clover, int inverse, const void* in, void* out, cudaStream_t s);
+cudaError_t launch_diag(const Diag<double>& d, const Geom& g, int par, bool clover, int inverse, const void* in, void* out, cudaStream_t s);
+
+// ---- layout (tmw_pack.cu) ----
+// canonical gauge [mu][lex][3][3][2] fp64 -> packed per parity: g64 [par][mu][9 planes][Vh] double2,
+// g32 [par][mu][NP planes][Vh] float4 with ng32 reals (12 | 18)
+cudaError_t launch_pack_gauge(const Geom& g, const double* canon, void* g64_even, void* g64_odd, void* g32_even, void* g32_odd, int ng32, cudaStream_t s);
+// canonical spinor fp64 <-> packed parity spinor (prec 0: float4 planes, 1: double2 planes)
+cudaError_t launch_pack_spinor(const Geom& g, int par, int prec, const double* canon, void* packed, cudaStream_t s);
+cudaError_t launch_unpack_spinor(const Geom& g, int par, int prec, const void* packed, double* canon, cudaStream_t s);
+
+// ---- clover (tmw_clover.cu) ----
+// From the canonical fp64 gauge: packed Hermitian blocks C = (c_sw/2) sum sigma F + diag, both parities,
+// fp64 [36 planes][Vh] double2 and fp32 [18 planes][Vh] float4.
+cudaError_t launch_clover_build(const Geom& g, const double* canon_gauge, double c_sw, double diag, void* c64_even, void* c64_odd, void* c32_even, void* c32_odd, cudaStream_t s);
+// inverse blocks of one parity: (C^2 + tw2)^{-1} if tw2 != 0 else C^{-1}; *singular (device int) is set on failure
+cudaError_t launch_clover_invert(const Geom& g, const void* c64, double tw2, void* inv64, void* inv32, int* singular, cudaStream_t s);
+// packed [planes][Vh] double2 blocks -> [cb][2][36] doubles
+cudaError_t launch_clover_export(const Geom& g, const void* c64, double* dst, cudaStream_t s);
+
+// ---- BLAS-1 with fused reductions (tmw_blas.cu) ----
+// Device scalar block of the BiCGStab recurrences (all complex as re,im doubles).
+struct Scalars {
+  double rho[2];      // <rhat, r>           (accumulated by blas_update_xr / blas_convert)
+  double rho_old[2];
+  double alpha[2];
+  double omega[2];
+  double beta[2];
+  double rhat_v[2];   // <rhat, v>           (accumulated by the first K2)
+  double ts[2];       // <t, s>              (accumulated by the second K2)
+  double tt;          // <t, t>
+  double rr;          // <r, r>              (accumulated by blas_update_xr / blas_convert)
+  double nrm;         // generic norm^2 accumulator
+  double pad;
+};
+// sc phase kernels (single thread): see tmw_blas.cu
+cudaError_t launch_sc_begin_iter(Scalars* sc, cudaStream_t s);  // beta = (rho/rho_old)(alpha/omega); zero rhat_v, ts, tt
+cudaError_t launch_sc_alpha(Scalars* sc, cudaStream_t s);       // alpha = rho / rhat_v
+cudaError_t launch_sc_omega(Scalars* sc, cudaStream_t s);       // omega = ts/tt; rho_old = rho; zero rho, rr
+// n = number of 16-byte vectors in each array
+template <typename R> cudaError_t launch_update_p(int64_t n, void* p, const void* r, const void* v, const Scalars* sc, cudaStream_t s);      // p = r + beta (p - omega v)
+template <typename R> cudaError_t launch_update_s(int64_t n, void* sv, const void* r, const void* v, const Scalars* sc, cudaStream_t s);     // s = r - alpha v
+template <typename R> cudaError_t launch_update_xr(int64_t n, void* x, void* r, const void* p, const void* sv, const void* t, const void* rhat, Scalars* sc, cudaStream_t s);  // x += alpha p + omega s; r = s - omega t; rho += <rhat,r>; rr += <r,r>
+// out[0..1] += <a,b>, out[2] += <b,b> (a may be null: only the norm)
+template <typename R> cudaError_t launch_dot_norm(int64_t n, const void* a, const void* b, double* out, cudaStream_t s);
+// fp64 helpers for the reliable update
+template <typename R> cudaError_t launch_acc_y(int64_t n64, void* y64, void* x, cudaStream_t s);  // y += x; x = 0   (n64 = number of double2 vectors)
+// r64 = b64 - w64; r = (R) r64; rho += <rhat, r>; rr += <r64, r64>
+template <typename R> cudaError_t launch_resid_convert(int64_t n64, const void* b64, const void* w64, void* r64, void* r, const void* rhat, Scalars* sc, cudaStream_t s);
+// dst(R) = src(double), n64 double2 vectors
+template <typename R> cudaError_t launch_convert(int64_t n64, const void* src64, void* dst, cudaStream_t s);
+// d = a - b (fp64, n64 double2 vectors), out[2] += <d,d>
+cudaError_t launch_sub_norm(int64_t n64, const void* a, const void* b, void* d, double* out, cudaStream_t s);
+
+}  // namespace tmw

@@ -1,0 +1,81 @@
+// tmw_pack.cu — layout conversion: canonical fp64 arrays (include/tmw.h) <-> even-odd
+// checkerboarded planes of 16-byte vectors. The gauge field gets an fp64 18-real copy and an fp32 copy with
+// 12 reals (rows 0,1; row 2 is rebuilt in the stencil) or 18 reals.
+#include "tmw_internal.h"
+
+namespace tmw {
+
+// lexicographic site of checkerboard index cb on parity par
+__device__ __forceinline__ int64_t lex_of_cb(const Geom& g, int par, int cb) {
+  const int xh = cb % g.Lh;
+  int q = cb / g.Lh;
+  const int y = q % g.L;
+  q /= g.L;
+  const int z = q % g.L;
+  const int t = q / g.L;
+  const int x = 2 * xh + ((y + z + t + par) & 1);
+  return x + (int64_t)g.L * (y + (int64_t)g.L * (z + (int64_t)g.L * t));
+}
+
+template <int NG32> __global__ void __launch_bounds__(128) pack_gauge_kernel(const Geom g, const double* __restrict__ canon, double2* g64e, double2* g64o, float4* g32e, float4* g32o) {
+  // one thread per (cb, mu, parity)
+  const int cb = blockIdx.x * 128 + threadIdx.x;
+  if (cb >= g.Vh) return;
+  const int mu = blockIdx.y, par = blockIdx.z;
+  const int64_t V = 2 * (int64_t)g.Vh;
+  const int64_t lex = lex_of_cb(g, par, cb);
+  const double* u = canon + 18 * ((int64_t)mu * V + lex);
+  double r[18];
+#pragma unroll
+  for (int i = 0; i < 18; i++) r[i] = u[i];
+  double2* d64 = (par ? g64o : g64e) + (int64_t)mu * 9 * g.Vh;
+  store_reals<18>(d64, g.Vh, cb, r);
+  const int NP = Planes<float, NG32>::N;
+  float4* d32 = (par ? g32o : g32e) + (int64_t)mu * NP * g.Vh;
+  float f[20];
+#pragma unroll
+  for (int i = 0; i < 18; i++) f[i] = (float)r[i];
+  f[18] = f[19] = 0.f;
+  store_reals<NG32>(d32, g.Vh, cb, f);
+}
+
+cudaError_t launch_pack_gauge(const Geom& g, const double* canon, void* g64_even, void* g64_odd, void* g32_even, void* g32_odd, int ng32, cudaStream_t s) {
+  dim3 grid((g.Vh + 127) / 128, 4, 2);
+  if (ng32 == 12) pack_gauge_kernel<12><<<grid, 128, 0, s>>>(g, canon, (double2*)g64_even, (double2*)g64_odd, (float4*)g32_even, (float4*)g32_odd);
+  else pack_gauge_kernel<18><<<grid, 128, 0, s>>>(g, canon, (double2*)g64_even, (double2*)g64_odd, (float4*)g32_even, (float4*)g32_odd);
+  return cudaGetLastError();
+}
+
+template <typename R> __global__ void __launch_bounds__(128) pack_spinor_kernel(const Geom g, int par, const double* __restrict__ canon, void* packed) {
+  const int cb = blockIdx.x * 128 + threadIdx.x;
+  if (cb >= g.Vh) return;
+  const double* p = canon + 24 * lex_of_cb(g, par, cb);
+  R v[24];
+#pragma unroll
+  for (int i = 0; i < 24; i++) v[i] = (R)p[i];
+  store_reals<24>(packed, g.Vh, cb, v);
+}
+template <typename R> __global__ void __launch_bounds__(128) unpack_spinor_kernel(const Geom g, int par, const void* packed, double* __restrict__ canon) {
+  const int cb = blockIdx.x * 128 + threadIdx.x;
+  if (cb >= g.Vh) return;
+  double* p = canon + 24 * lex_of_cb(g, par, cb);
+  R v[24];
+  load_reals<24>(packed, g.Vh, cb, v);
+#pragma unroll
+  for (int i = 0; i < 24; i++) p[i] = (double)v[i];
+}
+
+cudaError_t launch_pack_spinor(const Geom& g, int par, int prec, const double* canon, void* packed, cudaStream_t s) {
+  const int grid = (g.Vh + 127) / 128;
+  if (prec == 0) pack_spinor_kernel<float><<<grid, 128, 0, s>>>(g, par, canon, packed);
+  else pack_spinor_kernel<double><<<grid, 128, 0, s>>>(g, par, canon, packed);
+  return cudaGetLastError();
+}
+cudaError_t launch_unpack_spinor(const Geom& g, int par, int prec, const void* packed, double* canon, cudaStream_t s) {
+  const int grid = (g.Vh + 127) / 128;
+  if (prec == 0) unpack_spinor_kernel<float><<<grid, 128, 0, s>>>(g, par, packed, canon);
+  else unpack_spinor_kernel<double><<<grid, 128, 0, s>>>(g, par, packed, canon);
+  return cudaGetLastError();
+}
+
+}  // namespace tmw
