@@ -143,6 +143,9 @@ int tmw_unpack(tmw_ctx* ctx, int prec, int parity, const void* packed, double* c
  */
 int tmw_get_clover(tmw_ctx* ctx, int parity, int inverse, double* dst);
 
+/* change where the canonical-layout pointers of subsequent calls live (TMW_DEVICE | TMW_HOST) */
+int tmw_set_location(tmw_ctx* ctx, int location);
+
 /* number of kernel launches this context has issued since creation (bench.py's gpu_launches) */
 long long tmw_launch_count(const tmw_ctx* ctx);
 

@@ -5,6 +5,7 @@
 #include <math.h>
 #include <stddef.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -264,6 +265,12 @@ long long tmw_spinor_bytes(const tmw_ctx* ctx, int prec) {
   return (long long)spinor_bytes(ctx, prec);
 }
 long long tmw_launch_count(const tmw_ctx* ctx) { return ctx ? ctx->launches : 0; }
+int tmw_set_location(tmw_ctx* ctx, int location) {
+  if (!ctx) return TMW_EINVAL;
+  if (location != TMW_DEVICE && location != TMW_HOST) return fail(ctx, TMW_EINVAL, "tmw_set_location: bad location");
+  ctx->opt.location = location;
+  return TMW_OK;
+}
 
 int tmw_pack(tmw_ctx* ctx, int prec, int parity, const double* canonical, void* packed) {
   if (!ctx) return TMW_EINVAL;
@@ -405,6 +412,7 @@ int solve_schur(tmw_ctx* ctx, double tol, double bnorm, SolveState* st) {
   void *r = X[0], *rhat = X[1], *p = X[2], *v = X[3], *sv = X[4], *t = X[5], *x = X[6], *tmp = X[7];
   Scalars* h = ctx->sc_host;
   const double eps_break = sizeof(R) == 4 ? 1e-6 : 1e-12;
+  const bool verbose = getenv("TMW_VERBOSE") != nullptr;  // per-iteration residual log on stderr
   int rc;
   // y = 0, r64 = bhat, r = (R) r64, rhat = r, x = p = v = 0
   CK(cudaMemsetAsync(W[3], 0, (size_t)n64 * 16, s));
@@ -437,6 +445,9 @@ int solve_schur(tmw_ctx* ctx, double tol, double bnorm, SolveState* st) {
     if ((rc = fetch_scalars(ctx))) return rc;
     bool broken = !isfinite(h->rr) || !isfinite(h->rho[0]) || !isfinite(h->rho[1]);
     rnorm = broken ? maxr : sqrt(h->rr);
+    if (verbose)
+      fprintf(stderr, "[tmw] it %d |r|/|b| %.3e rho (%.3e,%.3e) alpha (%.3e,%.3e) omega (%.3e,%.3e) <rhat,v> (%.3e,%.3e) tt %.3e\n", k, sqrt(h->rr) / bnorm,
+              h->rho[0], h->rho[1], h->alpha[0], h->alpha[1], h->omega[0], h->omega[1], h->rhat_v[0], h->rhat_v[1], h->tt);
     if (!broken) st->iter_resid = rnorm / bnorm;
     const bool conv = !broken && rnorm <= tol * bnorm;
     if (broken || conv || rnorm < ctx->opt.delta * maxr || k == max_iter) {
@@ -454,6 +465,7 @@ int solve_schur(tmw_ctx* ctx, double tol, double bnorm, SolveState* st) {
       rnorm = sqrt(h->rr);
       maxr = rnorm;
       st->iter_resid = rnorm / bnorm;
+      if (verbose) fprintf(stderr, "[tmw]   reliable update %d: true |r|/|b| %.3e rho (%.3e,%.3e)\n", st->updates, rnorm / bnorm, h->rho[0], h->rho[1]);
       if (!isfinite(rnorm)) return fail(ctx, TMW_EBREAKDOWN, "tmw_solve: non-finite true residual");
       if (rnorm <= tol * bnorm) return TMW_OK;
       if (k == max_iter) break;
@@ -463,6 +475,7 @@ int solve_schur(tmw_ctx* ctx, double tol, double bnorm, SolveState* st) {
     const double rho_abs = hypot(h->rho[0], h->rho[1]);
     if (broken || !(rho_abs > eps_break * rhat_norm * rnorm)) {
       // breakdown: restart the recurrence with rhat = r (C11)
+      if (verbose) fprintf(stderr, "[tmw]   breakdown: |rho| %.3e vs %.3e * %.3e * %.3e -> restart\n", rho_abs, eps_break, rhat_norm, rnorm);
       if (++st->restarts > 5) return fail(ctx, TMW_EBREAKDOWN, "tmw_solve: BiCGStab breakdown persists after 5 restarts");
       // fold the current iterate into y first so that r is the residual of y
       LAUNCH(launch_acc_y<R>(n64, W[3], x, s));

@@ -21,6 +21,22 @@ __device__ __forceinline__ void stp(double* base, int64_t i, const double* v) {
   *((double2*)base + 2 * i + 1) = make_double2(v[2], v[3]);
 }
 
+// Mixed-precision kernels pair an fp32 packed spinor with an fp64 packed spinor. The plane layouts differ: the
+// float4 vector (k, cb) holds reals 4k..4k+3 of site cb, which are the double2 vectors (2k, cb) and (2k+1, cb).
+// Work item i = k*Vh + cb (a float4 index); the "m" accessors address either precision by that item.
+__device__ __forceinline__ void ldm(const float* base, int64_t i, int64_t, float* v) { ldp(base, i, v); }
+__device__ __forceinline__ void stm(float* base, int64_t i, int64_t, const float* v) { stp(base, i, v); }
+__device__ __forceinline__ void ldm(const double* base, int64_t i, int64_t Vh, double* v) {
+  const int64_t k = i / Vh, cb = i - k * Vh;
+  const double2 a = *((const double2*)base + (2 * k) * Vh + cb), b = *((const double2*)base + (2 * k + 1) * Vh + cb);
+  v[0] = a.x; v[1] = a.y; v[2] = b.x; v[3] = b.y;
+}
+__device__ __forceinline__ void stm(double* base, int64_t i, int64_t Vh, const double* v) {
+  const int64_t k = i / Vh, cb = i - k * Vh;
+  *((double2*)base + (2 * k) * Vh + cb) = make_double2(v[0], v[1]);
+  *((double2*)base + (2 * k + 1) * Vh + cb) = make_double2(v[2], v[3]);
+}
+
 enum { BB = 256 };
 static inline int blas_grid(int64_t n) {
   int64_t g = (n + BB - 1) / BB;
@@ -147,27 +163,27 @@ template <typename R> __global__ void __launch_bounds__(BB) dot_norm_kernel(int6
   double* dst[3] = {out, out + 1, out + 2};
   reduce_atomic<3>(acc, dst);
 }
-template <typename R> __global__ void __launch_bounds__(BB) acc_y_kernel(int64_t n, double* y, R* x) {
+template <typename R> __global__ void __launch_bounds__(BB) acc_y_kernel(int64_t n, int64_t Vh, double* y, R* x) {
   for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
     R xx[4];
     double yy[4];
-    ldp(x, i, xx); ldp(y, i, yy);
+    ldm(x, i, Vh, xx); ldm(y, i, Vh, yy);
 #pragma unroll
     for (int c = 0; c < 4; c++) { yy[c] += (double)xx[c]; xx[c] = (R)0; }
-    stp(y, i, yy);
-    stp(x, i, xx);
+    stm(y, i, Vh, yy);
+    stm(x, i, Vh, xx);
   }
 }
-template <typename R> __global__ void __launch_bounds__(BB) resid_convert_kernel(int64_t n, const double* b, const double* w, double* r64, R* r, const R* rhat, Scalars* sc) {
+template <typename R> __global__ void __launch_bounds__(BB) resid_convert_kernel(int64_t n, int64_t Vh, const double* b, const double* w, double* r64, R* r, const R* rhat, Scalars* sc) {
   double acc[3] = {0, 0, 0};
   for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
     double bb[4], ww[4], dd[4];
     R hh[4], rr[4];
-    ldp(b, i, bb); ldp(w, i, ww); ldp(rhat, i, hh);
+    ldm(b, i, Vh, bb); ldm(w, i, Vh, ww); ldm(rhat, i, Vh, hh);
 #pragma unroll
     for (int c = 0; c < 4; c++) { dd[c] = bb[c] - ww[c]; rr[c] = (R)dd[c]; }
-    stp(r64, i, dd);
-    stp(r, i, rr);
+    stm(r64, i, Vh, dd);
+    stm(r, i, Vh, rr);
 #pragma unroll
     for (int c = 0; c < 2; c++) {
       acc[0] += (double)hh[2 * c] * dd[2 * c] + (double)hh[2 * c + 1] * dd[2 * c + 1];
@@ -178,14 +194,14 @@ template <typename R> __global__ void __launch_bounds__(BB) resid_convert_kernel
   double* dst[3] = {&sc->rho[0], &sc->rho[1], &sc->rr};
   reduce_atomic<3>(acc, dst);
 }
-template <typename R> __global__ void __launch_bounds__(BB) convert_kernel(int64_t n, const double* src, R* dst) {
+template <typename R> __global__ void __launch_bounds__(BB) convert_kernel(int64_t n, int64_t Vh, const double* src, R* dst) {
   for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
     double ss[4];
     R dd[4];
-    ldp(src, i, ss);
+    ldm(src, i, Vh, ss);
 #pragma unroll
     for (int c = 0; c < 4; c++) dd[c] = (R)ss[c];
-    stp(dst, i, dd);
+    stm(dst, i, Vh, dd);
   }
 }
 __global__ void __launch_bounds__(BB) sub_norm_kernel(int64_t n, const double* a, const double* b, double* d, double* out) {
@@ -226,17 +242,17 @@ template <typename R> cudaError_t launch_dot_norm(int64_t n, const void* a, cons
 }
 template <typename R> cudaError_t launch_acc_y(int64_t n64, void* y64, void* x, cudaStream_t s) {
   const int64_t np = n64 / 2;
-  acc_y_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, (double*)y64, (R*)x);
+  acc_y_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, np / 6, (double*)y64, (R*)x);
   return cudaGetLastError();
 }
 template <typename R> cudaError_t launch_resid_convert(int64_t n64, const void* b64, const void* w64, void* r64, void* r, const void* rhat, Scalars* sc, cudaStream_t s) {
   const int64_t np = n64 / 2;
-  resid_convert_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, (const double*)b64, (const double*)w64, (double*)r64, (R*)r, (const R*)rhat, sc);
+  resid_convert_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, np / 6, (const double*)b64, (const double*)w64, (double*)r64, (R*)r, (const R*)rhat, sc);
   return cudaGetLastError();
 }
 template <typename R> cudaError_t launch_convert(int64_t n64, const void* src64, void* dst, cudaStream_t s) {
   const int64_t np = n64 / 2;
-  convert_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, (const double*)src64, (R*)dst);
+  convert_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, np / 6, (const double*)src64, (R*)dst);
   return cudaGetLastError();
 }
 cudaError_t launch_sub_norm(int64_t n64, const void* a, const void* b, void* d, double* out, cudaStream_t s) {

@@ -25,7 +25,7 @@ FULL, EVEN, ODD = 0, 1, 2
 F32, F64 = 0, 1
 
 EXPORTS = ["tmw_create", "tmw_apply", "tmw_apply_schur", "tmw_solve", "tmw_spinor_bytes", "tmw_pack", "tmw_unpack",
-           "tmw_get_clover", "tmw_launch_count", "tmw_destroy", "tmw_last_error"]
+           "tmw_get_clover", "tmw_set_location", "tmw_launch_count", "tmw_destroy", "tmw_last_error"]
 
 
 class tmw_complex(ctypes.Structure):
@@ -78,6 +78,8 @@ def load():
     lib.tmw_unpack.restype = I
     lib.tmw_get_clover.argtypes = [P, I, I, P]
     lib.tmw_get_clover.restype = I
+    lib.tmw_set_location.argtypes = [P, I]
+    lib.tmw_set_location.restype = I
     lib.tmw_launch_count.argtypes = [P]
     lib.tmw_launch_count.restype = LL
     lib.tmw_destroy.argtypes = [P]
@@ -150,6 +152,10 @@ class Context:
 
     def get_clover(self, parity: int, inverse: int, dst):
         self._check(self._lib.tmw_get_clover(self._h, parity, inverse, _ptr(dst)))
+
+    def set_location(self, location: int):
+        self._check(self._lib.tmw_set_location(self._h, location))
+        self.location = location
 
     def launch_count(self) -> int:
         return int(self._lib.tmw_launch_count(self._h))
