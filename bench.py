@@ -1,0 +1,370 @@
+"""bench.py — the hot path of arXiv:2201.09004 Eqs. (1)-(3) on B200, through the C ABI of include/tmw.h.
+
+    python bench.py --gpus N --steps K --warmup W            (N > 1: launched by torch.distributed.run, one rank per GPU)
+    python bench.py --impl reference ...                      (the fp64 CPU oracle as it stands, on the host cores)
+
+Workload (BASELINE.json configs[4], the configuration its metric is quoted on): 48^3 x 144 twisted-mass clover,
+m_cri+omega = -0.0398, c_sw = 1.0349, eps = 0.3 seeded random SU(3) links (stand-in for the MILC06 ensemble of
+PAPER.md:41 Table 1, which is not available), fp32 12-real gauge. One STEP is one pass of the per-source hot path:
+  (i)  tmw_solve of a point source at the origin (mixed-precision even-odd BiCGStab to 1e-10),
+  (ii) the Dslash-only run: --napply back-to-back applications of the fp32 hopping block H_{p pbar} (A3),
+       ping-ponging even -> odd -> even between two packed parity spinors.
+The once-per-gauge-field rows A0-A2 (layout, clover-leaf F, block inverses = tmw_create) are timed separately
+and reported as setup_ms. `value` is the Dslash throughput in GFLOP/s at the conventional 1320 flop/site;
+`solve_ms` is the BiCGStab time-to-solution. N > 1: replicas only — every rank owns a full context
+and takes its own right-hand-side columns (colour/spin index = rank mod 12); no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+FLOP_PER_SITE = 1320          # 8 x (12 + 2 x 66) + 7 x 24, the conventional Wilson Dslash count
+BYTES_COMPULSORY = 576        # fp32, 12-real: 96 (in, each site once) + 8 x 48 (links) + 96 (out) per output site
+BYTES_STREAMING = 1248        # 8 x 96 + 8 x 48 + 96: no neighbour reuse (the QUDA-style "effective bandwidth" model)
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="tmw", choices=["tmw", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="index into BASELINE.json configs (default 4: 48^3 x 144)")
+    ap.add_argument("--napply", type=int, default=200, help="Dslash applications per step")
+    ap.add_argument("--e2e-steps", type=int, default=2, help="timed host-buffer steps for the e2e figure")
+    ap.add_argument("--tol", type=float, default=1e-10)
+    ap.add_argument("--cpu-sites", type=int, default=0, help="oracle sample size in sites (0: sized for ~15 s)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and clock-event reasons of one GPU through NVML while the timed region runs."""
+
+    REASONS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+               0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+
+    def __init__(self, index: int, period: float = 0.05):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reason_bits, self.power = [], 0, []
+        self.stop_flag = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception as e:  # NVML missing: the clocks key says so
+            self.err = str(e)
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        while not self.stop_flag.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                self.reason_bits |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+            except Exception:
+                pass
+            self.stop_flag.wait(self.period)
+
+    def summary(self):
+        if not self.ok:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml unavailable: " + getattr(self, "err", "")]}
+        reasons = [name for bit, name in self.REASONS.items() if self.reason_bits & bit and name != "gpu_idle"]
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None, "sm_max_mhz": float(self.max_mhz),
+                "reasons": reasons, "samples": len(self.samples),
+                "power_w_max": float(max(self.power)) if self.power else None}
+
+
+def shared_gauge(cfg, rank: int, world: int, barrier):
+    """The seeded gauge field of the config as a canonical complex128 array. With several ranks on one node rank 0
+    generates it once into /dev/shm and the others map it read-only (replicas share one field)."""
+    from paper_2201_09004_b200 import synth
+    L, T = cfg["L"], cfg["T"]
+    if world == 1:
+        return synth.gauge_field(L, T, cfg["eps"], seed=1), None
+    path = f"/dev/shm/tmw_bench_gauge_{os.environ.get('MASTER_PORT', '0')}_{L}x{T}.bin"
+    shape = (4, T, L, L, L, 3, 3)
+    if rank == 0:
+        U = synth.gauge_field(L, T, cfg["eps"], seed=1)
+        mm = np.memmap(path, dtype=np.complex128, mode="w+", shape=shape)
+        mm[...] = U
+        mm.flush()
+        del mm
+        barrier()
+        return U, path
+    barrier()
+    return np.memmap(path, dtype=np.complex128, mode="r", shape=shape), path
+
+
+def time_oracle_sample(U, psi, cfg, n_sites: int):
+    """The oracle as it stands on a bounded sample of the workload: (D psi)(x) with the hopping + mass terms of Eq. (2)
+    at n_sites sites spread evenly over the lattice (its per-site routine; c_sw = 0 so that one site = the 8 hops
+    the GPU metric counts). Returns (seconds, sites, threads)."""
+    import oracle
+    L, T = cfg["L"], cfg["T"]
+    V = L ** 3 * T
+    stride = max(1, V // n_sites)
+    sites = np.arange(0, V, stride, dtype=np.int64)[:n_sites]
+    m = complex(*cfg["m"])
+    oracle.apply_sites(U, psi, sites[:1024], m, 0.0)  # page in
+    t0 = time.perf_counter()
+    oracle.apply_sites(U, psi, sites, m, 0.0)
+    return time.perf_counter() - t0, int(sites.size), oracle.num_threads()
+
+
+def run_reference(args, cfg, rank: int):
+    """--impl reference: the oracle timed on the host cores, same metric / unit / config; rank 0 only."""
+    if rank != 0:
+        return
+    from paper_2201_09004_b200 import synth
+    import oracle
+    L, T = cfg["L"], cfg["T"]
+    U = synth.gauge_field(L, T, cfg["eps"], seed=1)
+    psi = synth.gaussian_spinor(L, T, seed=3)
+    n = min(args.cpu_sites or 1_000_000, L ** 3 * T)
+    for _ in range(args.warmup):
+        time_oracle_sample(U, psi, cfg, max(1024, n // 8))
+    secs, sites = 0.0, 0
+    for _ in range(args.steps):
+        dt, ns, threads = time_oracle_sample(U, psi, cfg, n)
+        secs += dt
+        sites += ns
+    gflops = FLOP_PER_SITE * sites / secs / 1e9
+    sample = (f"oracle.apply_sites (fp64, hopping + mass of Eq. (2)) at {n} evenly spaced sites of the "
+              f"{L}^3x{T} field per step")
+    line = {"impl": "reference", "metric": "dslash_gflops", "value": gflops, "unit": "GFLOP/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg["name"], "L": L, "T": T, "m": list(cfg["m"]), "c_sw": cfg["c_sw"],
+                       "eps": cfg["eps"], "sample_sites_per_step": n},
+            "cpu_baseline": {"value": gflops, "unit": "GFLOP/s", "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": gflops, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
+    import torch
+    from paper_2201_09004_b200 import synth, tmw
+
+    tmw.load()  # raises when libtmw.so is missing: there is no fallback path
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (use --impl reference for the CPU oracle)"
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(v: float) -> float:
+        if dist is None:
+            return v
+        t = torch.tensor([v], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    L, T, m, c_sw = cfg["L"], cfg["T"], complex(*cfg["m"]), cfg["c_sw"]
+    V = L ** 3 * T
+    Vh = V // 2
+    U, shm_path = shared_gauge(cfg, rank, world, barrier)
+    stream = torch.cuda.current_stream().cuda_stream
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    # ---- setup rows A0-A2 (once per gauge field): tmw_create from a device-resident canonical gauge field ----
+    dU = torch.from_numpy(np.asarray(U)).cuda() if U.flags.writeable else torch.from_numpy(np.array(U)).cuda()
+    torch.cuda.synchronize()
+    e0, e1 = ev(), ev()
+    e0.record()
+    ctx = tmw.Context(L, T, dU, m, c_sw, stream=stream)
+    e1.record()
+    torch.cuda.synchronize()
+    setup_ms = e0.elapsed_time(e1)
+    del dU
+    torch.cuda.empty_cache()
+    barrier()
+    if shm_path and rank == 0:
+        os.unlink(shm_path)
+
+    # ---- inputs resident in HBM: a point source for the solve, a Gaussian spinor for the Dslash-only run ----
+    col = rank % 12
+    spin, colour = divmod(col, 3)
+    b = torch.zeros((T, L, L, L, 4, 3), dtype=torch.complex128, device="cuda")
+    b[0, 0, 0, 0, spin, colour] = 1.0
+    x = torch.empty_like(b)
+    psi_host = synth.gaussian_spinor(L, T, seed=3)
+    nb = ctx.spinor_bytes(tmw.F32)
+    pe, po, pe2 = (torch.empty(nb, dtype=torch.uint8, device="cuda") for _ in range(3))
+    x.copy_(torch.from_numpy(psi_host))
+    ctx.pack(tmw.F32, tmw.EVEN, x, pe)
+    torch.cuda.synchronize()
+
+    def dslash_run(n):
+        # even -> odd -> even: pe is never overwritten, so the values stay bounded however long the run is
+        for i in range(n // 2):
+            ctx.apply(tmw.D, tmw.ODD, tmw.F32, pe, po)
+            ctx.apply(tmw.D, tmw.EVEN, tmw.F32, po, pe2)
+
+    napply = max(2, args.napply // 2 * 2)
+    infos = []
+
+    def step(timers):
+        s0, s1, d0, d1 = ev(), ev(), ev(), ev()
+        s0.record()
+        info = ctx.solve(b, x, args.tol)
+        s1.record()
+        d0.record()
+        dslash_run(napply)
+        d1.record()
+        timers.append((s0, s1, d0, d1))
+        infos.append(info)
+
+    for _ in range(max(3, args.warmup)):
+        step([])
+    sampler = ClockSampler(local_rank)
+    timers = []
+    barrier()
+    sampler.start()
+    launches0 = ctx.launch_count()
+    t0, t1 = ev(), ev()
+    t0.record()
+    for _ in range(args.steps):
+        step(timers)
+    t1.record()
+    barrier()
+    sampler.stop_flag.set()
+    launches = ctx.launch_count() - launches0
+    total_ms = max_over_ranks(t0.elapsed_time(t1))
+    solve_ms = [a.elapsed_time(bb) for a, bb, _, _ in timers]
+    dsl_ms = [c.elapsed_time(d) for _, _, c, d in timers]
+    dsl_total_ms = max_over_ranks(sum(dsl_ms))
+    solve_mean_ms = max_over_ranks(sum(solve_ms) / len(solve_ms))
+    info = infos[-1]
+    sites = float(Vh) * napply * args.steps * world
+    gflops = FLOP_PER_SITE * sites / (dsl_total_ms * 1e-3) / 1e9
+    t_launch_s = sum(dsl_ms) * 1e-3 / (napply * args.steps)  # this rank's mean launch duration, events on `stream`
+    peak, peak_src = load_peaks()
+    achieved = BYTES_COMPULSORY * Vh / t_launch_s / 1e9
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "dslash_traffic.json")
+    if os.path.exists(tp):
+        with open(tp) as f:
+            traffic = json.load(f).get(cfg["name"], {}).get("dram_bytes_per_launch")
+    roofline = {"bound": "hbm", "kernel": "dslash_kernel<float,12,EPI_HOP> (fp32 hopping block, A3)",
+                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
+                "peak_source": peak_src, "bytes_per_site": BYTES_COMPULSORY, "sites_per_launch": Vh,
+                "launch_ms": 1e3 * t_launch_s, "streaming_model_gbs": BYTES_STREAMING * Vh / t_launch_s / 1e9,
+                "frac_of_8TBs_nominal": achieved / 8000.0}
+
+    # ---- e2e: the same two calls with HOST buffers (pinned), host<->device copies inside the timed region ----
+    e2e = None
+    if not args.no_e2e:
+        cbytes = V * 24 * 8
+        hb = torch.zeros((T, L, L, L, 4, 3), dtype=torch.complex128).pin_memory()
+        hb[0, 0, 0, 0, spin, colour] = 1.0
+        hx = torch.empty((T, L, L, L, 4, 3), dtype=torch.complex128).pin_memory()
+        hpsi = torch.from_numpy(psi_host).pin_memory()
+        ctx.set_location(tmw.HOST)
+        es, ea = [], []
+        n_e2e = max(1, args.e2e_steps)
+        for i in range(1 + n_e2e):  # one untimed pass first (allocates the staging buffers)
+            a0, a1, a2 = ev(), ev(), ev()
+            barrier()
+            a0.record()
+            ctx.solve(hb.data_ptr(), hx.data_ptr(), args.tol)
+            a1.record()
+            ctx.apply(tmw.D, tmw.FULL, tmw.F64, hpsi.data_ptr(), hx.data_ptr())
+            a2.record()
+            torch.cuda.synchronize()
+            if i > 0:
+                es.append(a0.elapsed_time(a1))
+                ea.append(a1.elapsed_time(a2))
+        ctx.set_location(tmw.DEVICE)
+        apply_ms = max_over_ranks(sum(ea) / len(ea))
+        e2e = {"value": FLOP_PER_SITE * float(V) * world / (apply_ms * 1e-3) / 1e9, "unit": "GFLOP/s",
+               "h2d_bytes_per_step": 2 * cbytes, "d2h_bytes_per_step": 2 * cbytes,
+               "call": "tmw_apply(TMW_D, TMW_FULL) with HOST pointers: canonical fp64 spinor in (H2D), D psi out (D2H)",
+               "apply_ms": apply_ms, "solve_ms": max_over_ranks(sum(es) / len(es)),
+               "solve_call": "tmw_solve with HOST pointers: b in (H2D), x out (D2H)", "steps": n_e2e}
+        del hb, hx, hpsi
+
+    # ---- the oracle beside it: rank 0, N = 1 only, a bounded sample of the same workload ----
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        n = args.cpu_sites
+        if not n:
+            dt, ns, _ = time_oracle_sample(U, psi_host, cfg, 100_000)
+            n = int(min(V, max(100_000, 12.0 * ns / dt)))
+        dt, ns, threads = time_oracle_sample(U, psi_host, cfg, n)
+        cpu = {"value": FLOP_PER_SITE * ns / dt / 1e9, "unit": "GFLOP/s", "cores": threads, "kind": "oracle",
+               "sample": f"oracle.apply_sites (fp64, hopping + mass of Eq. (2), explicit 4x4 gamma matrices) at {ns} "
+                         f"evenly spaced sites of the same {L}^3x{T} field, {dt:.1f} s", "msites_per_s": ns / dt / 1e6}
+
+    ctx.destroy()
+    if rank == 0:
+        line = {"metric": "dslash_gflops", "value": gflops, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
+                "warmup": max(3, args.warmup), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": cfg["name"], "L": L, "T": T, "m": list(cfg["m"]), "c_sw": c_sw, "eps": cfg["eps"],
+                           "gauge": "fp32 12-real (fp64 18-real for the outer residual)", "source": "point, origin",
+                           "step": f"1 tmw_solve(tol={args.tol:g}) + {napply} fp32 Dslash applications",
+                           "parallelism": "replicas" if world > 1 else "single",
+                           "l2": "inputs larger than L2 (a parity spinor is %.0f MB, gauge %.0f MB)" % (nb / 1e6, Vh * 8 * 48 / 1e6)},
+                "dslash_gsites_per_s": sites / (dsl_total_ms * 1e-3) / 1e9, "dslash_ms": dsl_total_ms / (napply * args.steps),
+                "solve_ms": solve_mean_ms, "solve_iters": info["iters"], "solve_reliable_updates": info["reliable_updates"],
+                "solve_true_resid": info["true_resid"], "setup_ms": setup_ms,
+                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
+                "clocks": sampler.summary()}
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    from paper_2201_09004_b200 import synth
+    cfg = synth.CONFIGS[args.config]
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, cfg, rank)
+        return
+    if world != args.gpus:
+        raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={world}: launch with torch.distributed.run --nproc-per-node {args.gpus}")
+    run_tmw(args, cfg, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()
