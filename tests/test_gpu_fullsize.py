@@ -22,6 +22,9 @@ pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")
 
 TOL32, TOL64 = 1e-5, 1e-12
+# the sampled |r|/|b| is a statistical estimate (a few thousand of millions of sites): allow its sampling error on top
+# of the 1e-10 the library itself certifies in fp64 over ALL sites (info['true_resid'], asserted <= 1e-10 exactly)
+EST_TOL = 2e-10
 _cache = {}
 
 
@@ -45,6 +48,16 @@ def config_fields(idx):
 
 def lex(L, x, y, z, t):
     return x + L * (y + L * (z + L * t))
+
+
+def random_sites(L, T, n, seed):
+    return np.unique(np.random.default_rng(seed).integers(0, L ** 3 * T, size=n)).astype(np.int64)
+
+
+def boundary_sites(L, T):
+    edge = [0, 1, L - 2, L - 1]
+    tedge = [0, 1, T - 2, T - 1]
+    return np.unique(np.array([lex(L, x, y, z, t) for t in tedge for z in edge for y in edge for x in edge], dtype=np.int64))
 
 
 def sample_sites(L, T, n, seed, parity=None):
@@ -136,15 +149,21 @@ def test_fullsize_full_operator_fp64_sampled(tmw, idx):
     torch.cuda.empty_cache()
 
 
-def sampled_residual(U, b, x, m, c_sw, sites):
-    """max_x |r(x)| and the sample estimate of |r| (both relative to |b|) from the oracle's D at `sites`."""
+def sampled_residual(U, b, x, m, c_sw, sites_rand, sites_det):
+    """max_x |r(x)| and a stratified estimate of |r| (both relative to |b|) from the oracle's D: the deliberately
+    chosen sites `sites_det` (source site, its neighbours, boundary sites — where a point-source residual is
+    concentrated) count once each; the uniform random sample `sites_rand` stands for all the other sites."""
+    sites_det = np.unique(sites_det)
+    sites_rand = np.setdiff1d(np.unique(sites_rand), sites_det)
+    sites = np.concatenate([sites_det, sites_rand])
     Dx = oracle.apply_sites(U, x, sites, m, c_sw)
     r = b.reshape(-1, 4, 3)[sites] - Dx
-    rs = np.linalg.norm(r.reshape(len(sites), -1), axis=1)
+    rs2 = np.sum(np.abs(r.reshape(len(sites), -1)) ** 2, axis=1)
     bn = np.linalg.norm(b.ravel())
     V = b.size // 12
-    est = np.sqrt(np.sum(rs ** 2) * V / len(sites)) / bn
-    return float(rs.max() / bn), float(est)
+    nd = len(sites_det)
+    est = np.sqrt(np.sum(rs2[:nd]) + np.sum(rs2[nd:]) * (V - nd) / len(sites_rand)) / bn
+    return float(np.sqrt(rs2.max()) / bn), float(est)
 
 
 @pytest.mark.parametrize("idx", [1, 2])
@@ -175,7 +194,8 @@ def test_fullsize_config3_twelve_columns(tmw):
     L, T, m, c_sw = cfg["L"], cfg["T"], complex(*cfg["m"]), cfg["c_sw"]
     origin_nb = [lex(L, *c) for c in [(0, 0, 0, 0), (1, 0, 0, 0), (L - 1, 0, 0, 0), (0, 1, 0, 0), (0, L - 1, 0, 0),
                                       (0, 0, 1, 0), (0, 0, L - 1, 0), (0, 0, 0, 1), (0, 0, 0, T - 1)]]
-    sites = np.unique(np.concatenate([sample_sites(L, T, 4000, seed=33), np.array(origin_nb, dtype=np.int64)]))
+    det = np.concatenate([boundary_sites(L, T), np.array(origin_nb, dtype=np.int64)])
+    rnd = random_sites(L, T, 4000, seed=33)
     dU = torch.from_numpy(U).cuda()
     with tmw.Context(L, T, dU, m, c_sw) as ctx:
         del dU
@@ -185,8 +205,8 @@ def test_fullsize_config3_twelve_columns(tmw):
                 b = synth.point_source(L, T, spin, colour)
                 info = ctx.solve(torch.from_numpy(b).cuda(), x, 1e-10)
                 assert info["true_resid"] <= 1e-10
-                mx, est = sampled_residual(U, b, x.cpu().numpy(), m, c_sw, sites)
-                assert mx <= 1e-10 and est <= 1e-10, (spin, colour, mx, est)
+                mx, est = sampled_residual(U, b, x.cpu().numpy(), m, c_sw, rnd, det)
+                assert mx <= 1e-10 and est <= EST_TOL, (spin, colour, mx, est)
         del x
     torch.cuda.empty_cache()
 
@@ -197,7 +217,8 @@ def test_fullsize_config4_solve(tmw):
     b = synth.point_source(L, T, 0, 0)
     origin_nb = [lex(L, *c) for c in [(0, 0, 0, 0), (1, 0, 0, 0), (L - 1, 0, 0, 0), (0, 1, 0, 0), (0, L - 1, 0, 0),
                                       (0, 0, 1, 0), (0, 0, L - 1, 0), (0, 0, 0, 1), (0, 0, 0, T - 1)]]
-    sites = np.unique(np.concatenate([sample_sites(L, T, 20000, seed=44), np.array(origin_nb, dtype=np.int64)]))
+    det = np.concatenate([boundary_sites(L, T), np.array(origin_nb, dtype=np.int64)])
+    rnd = random_sites(L, T, 20000, seed=44)
     dU = torch.from_numpy(U).cuda()
     with tmw.Context(L, T, dU, m, c_sw) as ctx:
         del dU
@@ -207,6 +228,6 @@ def test_fullsize_config4_solve(tmw):
         del x
     torch.cuda.empty_cache()
     assert info["true_resid"] <= 1e-10
-    mx, est = sampled_residual(U, b, xg, m, c_sw, sites)
-    assert mx <= 1e-10 and est <= 1e-10, (mx, est)
+    mx, est = sampled_residual(U, b, xg, m, c_sw, rnd, det)
+    assert mx <= 1e-10 and est <= EST_TOL, (mx, est)
     _cache.clear()
