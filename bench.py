@@ -12,7 +12,7 @@ PAPER.md:41 Table 1, which is not available), fp32 12-real gauge. One STEP is on
 The once-per-gauge-field rows A0-A2 (layout, clover-leaf F, block inverses = tmw_create) are timed separately
 and reported as setup_ms. `value` is the Dslash throughput in GFLOP/s at the conventional 1320 flop/site;
 `solve_ms` is the BiCGStab time-to-solution. N > 1: replicas only — every rank owns a full context
-and takes its own right-hand-side columns (colour/spin index = rank mod 12); no data-path collective.
+and takes its own right-hand-side columns (paper_2201_09004_b200/columns.py, round-robin); no data-path collective.
 """
 from __future__ import annotations
 
@@ -220,8 +220,8 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
         os.unlink(shm_path)
 
     # ---- inputs resident in HBM: a point source for the solve, a Gaussian spinor for the Dslash-only run ----
-    col = rank % 12
-    spin, colour = divmod(col, 3)
+    from paper_2201_09004_b200 import columns
+    spin, colour = columns.spin_colour(columns.columns_for_rank(rank, world)[0])
     b = torch.zeros((T, L, L, L, 4, 3), dtype=torch.complex128, device="cuda")
     b[0, 0, 0, 0, spin, colour] = 1.0
     x = torch.empty_like(b)
