@@ -278,11 +278,14 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
     t_launch_s = sum(dsl_ms) * 1e-3 / (napply * args.steps)  # this rank's mean launch duration, events on `stream`
     peak, peak_src = load_peaks()
     achieved = BYTES_COMPULSORY * Vh / t_launch_s / 1e9
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "dslash_traffic.json")
+    traffic = None  # ncu dram__bytes_read.sum + dram__bytes_write.sum per launch of the hop kernel (profiles/dslash_traffic.csv)
+    tp = os.path.join(ROOT, "profiles", "dslash_traffic.csv")
     if os.path.exists(tp):
+        import csv
         with open(tp) as f:
-            traffic = json.load(f).get(cfg["name"], {}).get("dram_bytes_per_launch")
+            for row in csv.DictReader(f):
+                if row["workload"] == cfg["name"] and row["kernel"] == "hop_f32_12":
+                    traffic = float(row["dram_bytes_per_launch"])
     roofline = {"bound": "hbm", "kernel": "dslash_kernel<float,12,EPI_HOP> (fp32 hopping block, A3)",
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
                 "peak_source": peak_src, "bytes_per_site": BYTES_COMPULSORY, "sites_per_launch": Vh,

@@ -82,7 +82,7 @@ typedef struct {
   int reconstruct;  /* fp32 gauge storage: 12 (default; third row rebuilt in-kernel, links must be SU(3)) | 18 */
   int mass_reading; /* TMW_TWIST_GAMMA5 (default) | TMW_MASS_SCALAR */
   int max_iter;     /* BiCGStab iterations; 0 -> 10000 */
-  double delta;     /* reliable-update threshold; 0 -> 0.1 */
+  double delta;     /* reliable-update threshold: fp64 true residual when |r| < delta * max|r|; 0 -> 1e-3 */
   void* stream;     /* cudaStream_t all work is queued on; NULL = the legacy default stream */
 } tmw_options;
 

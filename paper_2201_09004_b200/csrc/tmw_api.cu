@@ -175,7 +175,7 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
   if (opt) o = *opt;
   if (o.reconstruct == 0) o.reconstruct = 12;
   if (o.max_iter == 0) o.max_iter = 10000;
-  if (o.delta == 0.0) o.delta = 0.1;
+  if (o.delta == 0.0) o.delta = 1e-3;
   if ((o.location != TMW_DEVICE && o.location != TMW_HOST) || (o.precision != TMW_MIXED && o.precision != TMW_DOUBLE) ||
       (o.reconstruct != 12 && o.reconstruct != 18) || (o.mass_reading != TMW_TWIST_GAMMA5 && o.mass_reading != TMW_MASS_SCALAR) ||
       o.max_iter < 0 || !(o.delta > 0.0) || !(o.delta < 1.0))

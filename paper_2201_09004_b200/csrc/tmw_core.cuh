@@ -44,6 +44,95 @@ TMW_HD double2 ldv(const double2* p) {
 #endif
 }
 
+// Loads of data that a kernel touches exactly once (links, clover blocks): TMW_LD_STREAM selects the cache policy
+//   0: ld.global.nc (same as the spinor loads)   1: ld.global.cs (evict-first)   2: ld.global.nc.L1::no_allocate
+#ifndef TMW_LD_STREAM
+#define TMW_LD_STREAM 1  // measured on B200 (profiles/r1_tuning.md): -0.7 % hop, -2 % K2 vs ld.global.nc
+#endif
+// Stores of the stencil output: TMW_ST_STREAM 0: st.global   1: st.global.cs (evict-first)
+#ifndef TMW_ST_STREAM
+#define TMW_ST_STREAM 0
+#endif
+TMW_HD float4 ldv_s(const float4* p) {
+#if defined(__CUDA_ARCH__) && TMW_LD_STREAM == 1
+  return __ldcs(p);
+#elif defined(__CUDA_ARCH__) && TMW_LD_STREAM == 2
+  float4 q;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(q.x), "=f"(q.y), "=f"(q.z), "=f"(q.w) : "l"(p));
+  return q;
+#else
+  return ldv(p);
+#endif
+}
+TMW_HD double2 ldv_s(const double2* p) {
+#if defined(__CUDA_ARCH__) && TMW_LD_STREAM == 1
+  return __ldcs(p);
+#elif defined(__CUDA_ARCH__) && TMW_LD_STREAM == 2
+  double2 q;
+  asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0,%1}, [%2];" : "=d"(q.x), "=d"(q.y) : "l"(p));
+  return q;
+#else
+  return ldv(p);
+#endif
+}
+TMW_HD void stv_s(float4* p, float4 q) {
+#if defined(__CUDA_ARCH__) && TMW_ST_STREAM == 1
+  __stcs(p, q);
+#else
+  *p = q;
+#endif
+}
+TMW_HD void stv_s(double2* p, double2 q) {
+#if defined(__CUDA_ARCH__) && TMW_ST_STREAM == 1
+  __stcs(p, q);
+#else
+  *p = q;
+#endif
+}
+
+template <int NREAL> TMW_HD void load_reals_s(const void* base, int64_t stride, int64_t idx, float* v) {
+  const float4* p = (const float4*)base + idx;
+#pragma unroll
+  for (int k = 0; k < (NREAL + 3) / 4; k++) {
+    float4 q = ldv_s(p + k * stride);
+    v[4 * k] = q.x;
+    v[4 * k + 1] = q.y;
+    if (4 * k + 2 < NREAL) v[4 * k + 2] = q.z;
+    if (4 * k + 3 < NREAL) v[4 * k + 3] = q.w;
+  }
+}
+template <int NREAL> TMW_HD void load_reals_s(const void* base, int64_t stride, int64_t idx, double* v) {
+  const double2* p = (const double2*)base + idx;
+#pragma unroll
+  for (int k = 0; k < NREAL / 2; k++) {
+    double2 q = ldv_s(p + k * stride);
+    v[2 * k] = q.x;
+    v[2 * k + 1] = q.y;
+  }
+}
+template <int NREAL> TMW_HD void store_reals_s(void* base, int64_t stride, int64_t idx, const float* v) {
+  float4* p = (float4*)base + idx;
+#pragma unroll
+  for (int k = 0; k < (NREAL + 3) / 4; k++) {
+    float4 q;
+    q.x = v[4 * k];
+    q.y = v[4 * k + 1];
+    q.z = (4 * k + 2 < NREAL) ? v[4 * k + 2] : 0.f;
+    q.w = (4 * k + 3 < NREAL) ? v[4 * k + 3] : 0.f;
+    stv_s(p + k * stride, q);
+  }
+}
+template <int NREAL> TMW_HD void store_reals_s(void* base, int64_t stride, int64_t idx, const double* v) {
+  double2* p = (double2*)base + idx;
+#pragma unroll
+  for (int k = 0; k < NREAL / 2; k++) {
+    double2 q;
+    q.x = v[2 * k];
+    q.y = v[2 * k + 1];
+    stv_s(p + k * stride, q);
+  }
+}
+
 template <int NREAL> TMW_HD void load_reals(const void* base, int64_t stride, int64_t idx, float* v) {
   const float4* p = (const float4*)base + idx;
 #pragma unroll
@@ -120,7 +209,7 @@ template <typename R> TMW_HD void cmadc(cx<R>& acc, cx<R> a, cx<R> b) {
 // ---------------------------------------------------------------------------------------------------------
 template <typename R, int NG> TMW_HD void load_link(const void* base, int64_t stride, int64_t idx, cx<R> (&U)[9]) {
   R g[(NG == 12) ? 12 : 20];
-  load_reals<NG>(base, stride, idx, g);
+  load_reals_s<NG>(base, stride, idx, g);
 #pragma unroll
   for (int i = 0; i < NG / 2; i++) U[i] = mk<R>(g[2 * i], g[2 * i + 1]);
   if (NG == 12) {
@@ -261,7 +350,7 @@ template <typename R, bool CLOVER> TMW_HD void apply_A(const Diag<R>& d, int par
 #pragma unroll
     for (int b = 0; b < 2; b++) {
       R B[36];
-      load_reals<36>((const typename Vec16<R>::T*)d.c[par] + (int64_t)b * NPB * Vh, Vh, cb, B);
+      load_reals_s<36>((const typename Vec16<R>::T*)d.c[par] + (int64_t)b * NPB * Vh, Vh, cb, B);
       herm6_mul(B, v + 12 * b, out + 12 * b);
     }
   } else {
@@ -284,13 +373,13 @@ template <typename R, bool CLOVER> TMW_HD void apply_Ainv(const Diag<R>& d, int 
 #pragma unroll
     for (int b = 0; b < 2; b++) {
       R B[36];
-      load_reals<36>((const typename Vec16<R>::T*)d.cinv[par] + (int64_t)b * NPB * Vh, Vh, cb, B);
+      load_reals_s<36>((const typename Vec16<R>::T*)d.cinv[par] + (int64_t)b * NPB * Vh, Vh, cb, B);
       if (!d.twisted_clover) {
         herm6_mul(B, v + 12 * b, out + 12 * b);
       } else {
         R w[12];
         herm6_mul(B, v + 12 * b, w);
-        load_reals<36>((const typename Vec16<R>::T*)d.c[par] + (int64_t)b * NPB * Vh, Vh, cb, B);
+        load_reals_s<36>((const typename Vec16<R>::T*)d.c[par] + (int64_t)b * NPB * Vh, Vh, cb, B);
         herm6_mul(B, w, out + 12 * b);
         const R tw = b ? d.tw_lo : d.tw_up;  // (C - i tw) w
 #pragma unroll

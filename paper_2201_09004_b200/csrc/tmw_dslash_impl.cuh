@@ -35,7 +35,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<R>
   R o[24], ax[24];
   if (active) {
     dslash_site<R, NG, EPI, CLOVER>(a, cb, o, ax);
-    store_reals<24>(a.out, a.g.Vh, cb, o);
+    store_reals_s<24>(a.out, a.g.Vh, cb, o);
   }
   if (a.red_mode != 0) {  // uniform across the grid
     double v[3] = {0, 0, 0};
