@@ -47,7 +47,7 @@ TMW_HD double2 ldv(const double2* p) {
 // Loads of data that a kernel touches exactly once (links, clover blocks): TMW_LD_STREAM selects the cache policy
 //   0: ld.global.nc (same as the spinor loads)   1: ld.global.cs (evict-first)   2: ld.global.nc.L1::no_allocate
 #ifndef TMW_LD_STREAM
-#define TMW_LD_STREAM 1  // measured on B200 (profiles/r1_tuning.md): -0.7 % hop, -2 % K2 vs ld.global.nc
+#define TMW_LD_STREAM 1  // measured on B200: -0.7 % hop, -2 % K2 vs ld.global.nc
 #endif
 // Stores of the stencil output: TMW_ST_STREAM 0: st.global   1: st.global.cs (evict-first)
 #ifndef TMW_ST_STREAM
