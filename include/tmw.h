@@ -125,6 +125,22 @@ int tmw_apply_schur(tmw_ctx* ctx, int op, int prec, const void* in_odd, void* ou
  */
 int tmw_solve(tmw_ctx* ctx, const double* b, double* x, double tol, tmw_solve_info* info);
 
+/*
+ * Several right-hand sides at once (the "12 columns" of a propagator, Table 2 caption).
+ * The columns are independent problems with the same operator; doing them in one call lets every link and clover
+ * block be read once for all columns. nrhs in 1..16. Column c of every spinor argument follows column c-1 directly:
+ *   canonical: double[nrhs][T][L][L][L][4][3][2];   packed: nrhs packed parity spinors back to back.
+ * tmw_apply_multi / tmw_apply_schur_multi: as tmw_apply / tmw_apply_schur, column by column the same result.
+ * tmw_solve_multi: BiCGStab on all columns in lockstep, each with its own recurrence scalars, reliable updates and
+ *   stopping test (|b_c - D x_c| / |b_c| <= tol for every column c); columns that have converged drop out of the
+ *   launches. info (nullable) points to nrhs records; device_ms is the time of the whole call in each of them.
+ *   Returns TMW_ENOCONV if any column reached max_iter. Workspace grows with nrhs (16 parity spinors per column):
+ *   TMW_ENOMEM if it does not fit.
+ */
+int tmw_apply_multi(tmw_ctx* ctx, int op, int parity, int prec, int nrhs, const void* in, void* out);
+int tmw_apply_schur_multi(tmw_ctx* ctx, int op, int prec, int nrhs, const void* in_odd, void* out_odd);
+int tmw_solve_multi(tmw_ctx* ctx, int nrhs, const double* b, double* x, double tol, tmw_solve_info* info);
+
 /* bytes of one packed parity spinor in precision prec (TMW_F32 | TMW_F64); 0 on bad arguments */
 long long tmw_spinor_bytes(const tmw_ctx* ctx, int prec);
 

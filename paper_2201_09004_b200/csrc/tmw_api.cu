@@ -32,13 +32,15 @@ struct tmw_ctx {
   void* ci64;  // inverse blocks, even parity
   void* ci32;
   std::vector<void*> owned;  // every device allocation
-  // lazily allocated workspaces
+  // lazily allocated workspaces, each sized for ws_cols right-hand-side columns (column c at c * spinor bytes)
+  int ws_cols;
   void* w64[10];  // packed fp64 parity spinors
   void* w32[8];   // packed inner-precision parity spinors (fp32 for TMW_MIXED, fp64 for TMW_DOUBLE)
   void* canon[2]; // canonical fp64 full-lattice staging (HOST location only)
-  Scalars* sc;
+  int nr32;          // most columns one thread of the fp32 stencil takes (1..4)
+  Scalars* sc;       // MAXCOL scalar blocks
   Scalars* sc_host;  // pinned
-  double* red;       // 4 device doubles
+  double* red;       // 4 * MAXCOL device doubles
   double* red_host;  // pinned
   cudaEvent_t ev0, ev1;
   long long launches;
@@ -107,8 +109,16 @@ template <typename R> static Diag<R> make_diag(const tmw_ctx* c, int dagger) {
   return d;
 }
 
+static ColMap cols_first(int n) {
+  ColMap cm;
+  cm.n = n;
+  for (int i = 0; i < MAXCOL; i++) cm.col[i] = (unsigned char)(i < n ? i : 0);
+  return cm;
+}
+static void cols_add(ColMap& cm, int c) { cm.col[cm.n++] = (unsigned char)c; }
+
 template <typename R>
-static DslashArgs<R> make_args(const tmw_ctx* c, int par, int dagger, const void* in, void* out, const void* aux, double sgn) {
+static DslashArgs<R> make_args(const tmw_ctx* c, int par, int dagger, const void* in, void* out, const void* aux, double sgn, const ColMap& cm) {
   DslashArgs<R> a;
   a.in = in;
   a.out = out;
@@ -124,28 +134,82 @@ static DslashArgs<R> make_args(const tmw_ctx* c, int par, int dagger, const void
   a.red_mode = 0;
   a.dotv = nullptr;
   a.red = nullptr;
+  a.ncol = cm.n;
+  a.ngroups = 1;
+  a.cstride = (int64_t)c->g.Vh * 24 * (int64_t)sizeof(R) / 16;
+  a.red_stride = 0;
+  for (int i = 0; i < MAXCOL; i++) a.col[i] = cm.col[i];
   return a;
 }
 template <typename R> static int ng_of(const tmw_ctx* c) { return sizeof(R) == 4 ? c->ng32 : 18; }
 
-// out(par) = epilogue(H in)
+// out(par) = epilogue(H in) for the columns of cm (vectors of column c start c spinors after the base pointers);
+// red (if any) is the reduction target of column 0, column c's is red_stride doubles further per column.
 template <typename R>
-static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, void* out, const void* aux, double sgn, int red_mode = 0, const void* dotv = nullptr, double* red = nullptr) {
-  DslashArgs<R> a = make_args<R>(ctx, par, dagger, in, out, aux, sgn);
+static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, void* out, const void* aux, double sgn, const ColMap& cm,
+                  int red_mode = 0, const void* dotv = nullptr, double* red = nullptr, int red_stride = 0) {
+  DslashArgs<R> a = make_args<R>(ctx, par, dagger, in, out, aux, sgn, cm);
   a.red_mode = red_mode;
   a.dotv = dotv;
   a.red = red;
-  LAUNCH(launch_dslash(a, ng_of<R>(ctx), epi, ctx->clover, ctx->stream));
+  a.red_stride = red_stride;
+  // columns per thread: as even a split of the columns into groups of at most nr32 as possible
+  int nr = 1;
+  if (sizeof(R) == 4 && cm.n > 1) {
+    const int groups = (cm.n + ctx->nr32 - 1) / ctx->nr32;
+    nr = (cm.n + groups - 1) / groups;
+  }
+  LAUNCH(launch_dslash(a, ng_of<R>(ctx), epi, ctx->clover, nr, ctx->stream));
   return TMW_OK;
 }
 // Schur operator on the odd sites: out = A_oo in - H_oe A_ee^{-1} H_eo in  (tmp: even-parity scratch)
 // The conjugate transpose is A_oo^dag in - H_eo^dag (A_ee^dag)^{-1} H_oe^dag in: the same two kernels with the
 // daggered projectors / twist, because (H_oe)^dag = the daggered hopping block from odd to even.
 template <typename R>
-static int schur(tmw_ctx* ctx, int dagger, const void* in, void* out, void* tmp, int red_mode = 0, const void* dotv = nullptr, double* red = nullptr) {
-  int rc = dslash<R>(ctx, EPI_AINV_HOP, 0, dagger, in, tmp, nullptr, 1.0);
+static int schur(tmw_ctx* ctx, int dagger, const void* in, void* out, void* tmp, const ColMap& cm, int red_mode = 0, const void* dotv = nullptr,
+                 double* red = nullptr, int red_stride = 0) {
+  int rc = dslash<R>(ctx, EPI_AINV_HOP, 0, dagger, in, tmp, nullptr, 1.0, cm);
   if (rc) return rc;
-  return dslash<R>(ctx, EPI_A_XPAY, 1, dagger, tmp, out, in, -1.0, red_mode, dotv, red);
+  return dslash<R>(ctx, EPI_A_XPAY, 1, dagger, tmp, out, in, -1.0, cm, red_mode, dotv, red, red_stride);
+}
+
+// Thread -> site mapping of the stencil kernels (Geom::tiled). Default: 1-D (CTA b = 128 consecutive cb). With
+// TMW_TILE="auto" the largest power-of-two 4-D tile of 128 sites that divides the lattice, preferring 8 (xh) x 4 (y)
+// x 2 (z) x 2 (t); with TMW_TILE="lx,ly,lz,lt" those log2 extents. Measured on B200: the tiled
+// mapping changes neither the time nor the DRAM traffic of the stencil, so it stays an opt-in tuning knob.
+static void choose_tile(Geom& g) {
+  g.tiled = 0;
+  g.lx = g.ly = g.lz = g.lt = 0;
+  g.ntx = g.nty = 1;
+  int l[4] = {-1, -1, -1, -1};
+  const char* e = getenv("TMW_TILE");
+  if (!e) return;
+  if (strcmp(e, "auto") != 0) {
+    if (sscanf(e, "%d,%d,%d,%d", &l[0], &l[1], &l[2], &l[3]) != 4) return;  // "0" or malformed: 1-D mapping
+  } else {
+    const int ext[4] = {g.Lh, g.L, g.L, g.T};
+    const int want[4] = {3, 2, 1, 1};
+    int left = 7;
+    for (int d = 0; d < 4; d++) {
+      l[d] = 0;
+      while (l[d] < want[d] && ext[d] % (2 << l[d]) == 0) l[d]++;
+      left -= l[d];
+    }
+    for (int d = 3; d >= 1 && left > 0; d--)  // fill up from t, z, y if x (or another extent) fell short
+      while (left > 0 && ext[d] % (2 << l[d]) == 0) { l[d]++; left--; }
+    if (left != 0) return;
+  }
+  const int ext[4] = {g.Lh, g.L, g.L, g.T};
+  int sum = 0;
+  for (int d = 0; d < 4; d++) {
+    if (l[d] < 0 || l[d] > 7 || ext[d] % (1 << l[d]) != 0) return;
+    sum += l[d];
+  }
+  if (sum != 7) return;
+  g.tiled = 1;
+  g.lx = l[0]; g.ly = l[1]; g.lz = l[2]; g.lt = l[3];
+  g.ntx = g.Lh >> g.lx;
+  g.nty = g.L >> g.ly;
 }
 
 extern "C" {
@@ -185,6 +249,10 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
   if (!ctx) return fail(nullptr, TMW_ENOMEM, "tmw_create: host allocation failed");
   ctx->g.L = L; ctx->g.T = T; ctx->g.Lh = L / 2; ctx->g.Vh = (int)(V / 2);
   ctx->g.sy = L / 2; ctx->g.sz = (L / 2) * L; ctx->g.st = (L / 2) * L * L;
+  choose_tile(ctx->g);
+  ctx->ws_cols = 1;
+  ctx->nr32 = 2;  // 2 columns per thread at 168 registers is the fastest split on B200
+  if (const char* e = getenv("TMW_NR")) { const int v = atoi(e); if (v >= 1 && v <= 4) ctx->nr32 = v; }
   ctx->V = V;
   ctx->m_re = m.re; ctx->m_im = m.im; ctx->c_sw = c_sw;
   ctx->opt = o;
@@ -212,12 +280,12 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
     const double dg = -(4.0 + m.re);
     if (dg * dg + m.im * m.im == 0.0) { tmw_destroy(ctx); return fail(nullptr, TMW_ESINGULAR, "tmw_create: 4 + m = 0, the diagonal part is singular"); }
   }
-  CKC(cudaMallocHost((void**)&ctx->sc_host, sizeof(Scalars)));
-  CKC(cudaMallocHost((void**)&ctx->red_host, 4 * sizeof(double)));
+  CKC(cudaMallocHost((void**)&ctx->sc_host, MAXCOL * sizeof(Scalars)));
+  CKC(cudaMallocHost((void**)&ctx->red_host, 4 * MAXCOL * sizeof(double)));
   CKC(cudaEventCreate(&ctx->ev0));
   CKC(cudaEventCreate(&ctx->ev1));
-  CKA(&ctx->sc, sizeof(Scalars));
-  CKA(&ctx->red, 4 * sizeof(double));
+  CKA(&ctx->sc, MAXCOL * sizeof(Scalars));
+  CKA(&ctx->red, 4 * MAXCOL * sizeof(double));
   const size_t Vh = (size_t)ctx->g.Vh;
   const int np32 = (ctx->ng32 == 12) ? 3 : 5;
   for (int p = 0; p < 2; p++) {
@@ -298,219 +366,305 @@ int tmw_get_clover(tmw_ctx* ctx, int parity, int inverse, double* dst) {
 }  // extern "C"
 
 // ---- workspaces ----
+// make the workspaces hold `cols` columns (existing smaller ones are released and re-made on demand)
+static int need_cols(tmw_ctx* ctx, int cols) {
+  if (cols <= ctx->ws_cols) return TMW_OK;
+  cudaError_t e = cudaStreamSynchronize(ctx->stream);
+  if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaStreamSynchronize");
+  for (int i = 0; i < 10; i++) if (ctx->w64[i]) { dev_free(ctx, ctx->w64[i]); ctx->w64[i] = nullptr; }
+  for (int i = 0; i < 8; i++) if (ctx->w32[i]) { dev_free(ctx, ctx->w32[i]); ctx->w32[i] = nullptr; }
+  for (int i = 0; i < 2; i++) if (ctx->canon[i]) { dev_free(ctx, ctx->canon[i]); ctx->canon[i] = nullptr; }
+  ctx->ws_cols = cols;
+  return TMW_OK;
+}
 static int need_w64(tmw_ctx* ctx, int n) {
   for (int i = 0; i < n; i++)
-    if (!ctx->w64[i]) { int rc = dev_alloc(ctx, &ctx->w64[i], spinor_bytes(ctx, TMW_F64)); if (rc) return rc; }
+    if (!ctx->w64[i]) { int rc = dev_alloc(ctx, &ctx->w64[i], spinor_bytes(ctx, TMW_F64) * ctx->ws_cols); if (rc) return rc; }
   return TMW_OK;
 }
 static int need_w32(tmw_ctx* ctx, int n, int prec) {
   for (int i = 0; i < n; i++)
-    if (!ctx->w32[i]) { int rc = dev_alloc(ctx, &ctx->w32[i], spinor_bytes(ctx, prec)); if (rc) return rc; }
+    if (!ctx->w32[i]) { int rc = dev_alloc(ctx, &ctx->w32[i], spinor_bytes(ctx, prec) * ctx->ws_cols); if (rc) return rc; }
   return TMW_OK;
 }
 static int need_canon(tmw_ctx* ctx) {
   for (int i = 0; i < 2; i++)
-    if (!ctx->canon[i]) { int rc = dev_alloc(ctx, &ctx->canon[i], (size_t)ctx->V * 24 * 8); if (rc) return rc; }
+    if (!ctx->canon[i]) { int rc = dev_alloc(ctx, &ctx->canon[i], (size_t)ctx->V * 24 * 8 * ctx->ws_cols); if (rc) return rc; }
   return TMW_OK;
 }
+static inline void* colp(void* base, int c, size_t bytes) { return (char*)base + (size_t)c * bytes; }
+static inline const void* colp(const void* base, int c, size_t bytes) { return (const char*)base + (size_t)c * bytes; }
 
 // out_p = A in_p + H in_pbar for both parities, fp64 packed
-static int full_apply64(tmw_ctx* ctx, int dagger, const void* in_e, const void* in_o, void* out_e, void* out_o) {
-  int rc = dslash<double>(ctx, EPI_A_XPAY, 0, dagger, in_o, out_e, in_e, 1.0);
+static int full_apply64(tmw_ctx* ctx, int dagger, const void* in_e, const void* in_o, void* out_e, void* out_o, const ColMap& cm) {
+  int rc = dslash<double>(ctx, EPI_A_XPAY, 0, dagger, in_o, out_e, in_e, 1.0, cm);
   if (rc) return rc;
-  return dslash<double>(ctx, EPI_A_XPAY, 1, dagger, in_e, out_o, in_o, 1.0);
+  return dslash<double>(ctx, EPI_A_XPAY, 1, dagger, in_e, out_o, in_o, 1.0, cm);
 }
 
-extern "C" int tmw_apply(tmw_ctx* ctx, int op, int parity, int prec, const void* in, void* out) {
+extern "C" int tmw_apply_multi(tmw_ctx* ctx, int op, int parity, int prec, int nrhs, const void* in, void* out) {
   if (!ctx) return TMW_EINVAL;
   if (!in || !out || in == out) return fail(ctx, TMW_EINVAL, "tmw_apply: null or aliased pointers");
   if ((op != TMW_D && op != TMW_DDAG) || (parity != TMW_FULL && parity != TMW_EVEN && parity != TMW_ODD)) return fail(ctx, TMW_EINVAL, "tmw_apply: bad op or parity");
+  if (nrhs < 1 || nrhs > MAXCOL) return fail(ctx, TMW_EINVAL, "tmw_apply: nrhs must be in 1..16");
   const int dagger = (op == TMW_DDAG);
+  const ColMap cm = cols_first(nrhs);
   if (parity != TMW_FULL) {
     if (prec != TMW_F32 && prec != TMW_F64) return fail(ctx, TMW_EINVAL, "tmw_apply: bad precision");
     const int par = (parity == TMW_ODD);
-    if (prec == TMW_F32) return dslash<float>(ctx, EPI_HOP, par, dagger, in, out, nullptr, 1.0);
-    return dslash<double>(ctx, EPI_HOP, par, dagger, in, out, nullptr, 1.0);
+    if (prec == TMW_F32) return dslash<float>(ctx, EPI_HOP, par, dagger, in, out, nullptr, 1.0, cm);
+    return dslash<double>(ctx, EPI_HOP, par, dagger, in, out, nullptr, 1.0, cm);
   }
-  int rc = need_w64(ctx, 4);
+  int rc = need_cols(ctx, nrhs);
   if (rc) return rc;
+  if ((rc = need_w64(ctx, 4))) return rc;
   const double* cin = (const double*)in;
   double* cout = (double*)out;
-  const size_t cbytes = (size_t)ctx->V * 24 * 8;
+  const size_t cbytes = (size_t)ctx->V * 24 * 8, b64 = spinor_bytes(ctx, TMW_F64);
   if (ctx->opt.location == TMW_HOST) {
     rc = need_canon(ctx);
     if (rc) return rc;
-    CK(cudaMemcpyAsync(ctx->canon[0], in, cbytes, cudaMemcpyHostToDevice, ctx->stream));
+    CK(cudaMemcpyAsync(ctx->canon[0], in, cbytes * nrhs, cudaMemcpyHostToDevice, ctx->stream));
     cin = (const double*)ctx->canon[0];
     cout = (double*)ctx->canon[1];
   }
-  LAUNCH(launch_pack_spinor(ctx->g, 0, 1, cin, ctx->w64[0], ctx->stream));
-  LAUNCH(launch_pack_spinor(ctx->g, 1, 1, cin, ctx->w64[1], ctx->stream));
-  rc = full_apply64(ctx, dagger, ctx->w64[0], ctx->w64[1], ctx->w64[2], ctx->w64[3]);
+  for (int c = 0; c < nrhs; c++) {
+    LAUNCH(launch_pack_spinor(ctx->g, 0, 1, (const double*)colp(cin, c, cbytes), colp(ctx->w64[0], c, b64), ctx->stream));
+    LAUNCH(launch_pack_spinor(ctx->g, 1, 1, (const double*)colp(cin, c, cbytes), colp(ctx->w64[1], c, b64), ctx->stream));
+  }
+  rc = full_apply64(ctx, dagger, ctx->w64[0], ctx->w64[1], ctx->w64[2], ctx->w64[3], cm);
   if (rc) return rc;
-  LAUNCH(launch_unpack_spinor(ctx->g, 0, 1, ctx->w64[2], cout, ctx->stream));
-  LAUNCH(launch_unpack_spinor(ctx->g, 1, 1, ctx->w64[3], cout, ctx->stream));
+  for (int c = 0; c < nrhs; c++) {
+    LAUNCH(launch_unpack_spinor(ctx->g, 0, 1, colp(ctx->w64[2], c, b64), (double*)colp(cout, c, cbytes), ctx->stream));
+    LAUNCH(launch_unpack_spinor(ctx->g, 1, 1, colp(ctx->w64[3], c, b64), (double*)colp(cout, c, cbytes), ctx->stream));
+  }
   if (ctx->opt.location == TMW_HOST) {
-    CK(cudaMemcpyAsync(out, cout, cbytes, cudaMemcpyDeviceToHost, ctx->stream));
+    CK(cudaMemcpyAsync(out, cout, cbytes * nrhs, cudaMemcpyDeviceToHost, ctx->stream));
     CK(cudaStreamSynchronize(ctx->stream));
   }
   return TMW_OK;
 }
+extern "C" int tmw_apply(tmw_ctx* ctx, int op, int parity, int prec, const void* in, void* out) {
+  return tmw_apply_multi(ctx, op, parity, prec, 1, in, out);
+}
 
-extern "C" int tmw_apply_schur(tmw_ctx* ctx, int op, int prec, const void* in_odd, void* out_odd) {
+extern "C" int tmw_apply_schur_multi(tmw_ctx* ctx, int op, int prec, int nrhs, const void* in_odd, void* out_odd) {
   if (!ctx) return TMW_EINVAL;
   if (!in_odd || !out_odd || in_odd == out_odd) return fail(ctx, TMW_EINVAL, "tmw_apply_schur: null or aliased pointers");
   if ((op != TMW_D && op != TMW_DDAG) || (prec != TMW_F32 && prec != TMW_F64)) return fail(ctx, TMW_EINVAL, "tmw_apply_schur: bad op or precision");
+  if (nrhs < 1 || nrhs > MAXCOL) return fail(ctx, TMW_EINVAL, "tmw_apply_schur: nrhs must be in 1..16");
   const int dagger = (op == TMW_DDAG);
   int rc;
-  if (prec == TMW_F64) {
-    if ((rc = need_w64(ctx, 1))) return rc;
-    return schur<double>(ctx, dagger, in_odd, out_odd, ctx->w64[0]);
-  }
-  // an fp32 even-parity scratch: reuse the head of an fp64 workspace
-  if ((rc = need_w64(ctx, 1))) return rc;
-  return schur<float>(ctx, dagger, in_odd, out_odd, ctx->w64[0]);
+  if ((rc = need_cols(ctx, nrhs))) return rc;
+  if ((rc = need_w64(ctx, 1))) return rc;  // even-parity scratch (an fp32 call uses the head of each fp64 column... see below)
+  const ColMap cm = cols_first(nrhs);
+  if (prec == TMW_F64) return schur<double>(ctx, dagger, in_odd, out_odd, ctx->w64[0], cm);
+  // fp32: columns of the scratch are fp32 spinors packed back to back at the start of the fp64 workspace
+  return schur<float>(ctx, dagger, in_odd, out_odd, ctx->w64[0], cm);
+}
+extern "C" int tmw_apply_schur(tmw_ctx* ctx, int op, int prec, const void* in_odd, void* out_odd) {
+  return tmw_apply_schur_multi(ctx, op, prec, 1, in_odd, out_odd);
 }
 
 // ---- the solver ----
 namespace {
 
-struct SolveState {
+struct ColState {
+  double bnorm, rnorm, maxr, rhat_norm;
+  bool done;    // converged (or b = 0)
   int iters, updates, restarts;
   double iter_resid, true_resid;
 };
 
-// download the scalar block and wait
+// download the scalar blocks and wait
 int fetch_scalars(tmw_ctx* ctx) {
-  CK(cudaMemcpyAsync(ctx->sc_host, ctx->sc, sizeof(Scalars), cudaMemcpyDeviceToHost, ctx->stream));
+  CK(cudaMemcpyAsync(ctx->sc_host, ctx->sc, MAXCOL * sizeof(Scalars), cudaMemcpyDeviceToHost, ctx->stream));
   CK(cudaStreamSynchronize(ctx->stream));
   return TMW_OK;
 }
 int push_scalars(tmw_ctx* ctx) {
-  CK(cudaMemcpyAsync(ctx->sc, ctx->sc_host, sizeof(Scalars), cudaMemcpyHostToDevice, ctx->stream));
+  CK(cudaMemcpyAsync(ctx->sc, ctx->sc_host, MAXCOL * sizeof(Scalars), cudaMemcpyHostToDevice, ctx->stream));
   // the pinned block is rewritten by the host right after some pushes: wait for the copy
   CK(cudaStreamSynchronize(ctx->stream));
   return TMW_OK;
 }
 int fetch_red(tmw_ctx* ctx) {
-  CK(cudaMemcpyAsync(ctx->red_host, ctx->red, 4 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+  CK(cudaMemcpyAsync(ctx->red_host, ctx->red, 4 * MAXCOL * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
   CK(cudaStreamSynchronize(ctx->stream));
   return TMW_OK;
 }
+void reset_recurrence(Scalars* h) {
+  h->rho_old[0] = h->alpha[0] = h->omega[0] = 1.0;
+  h->rho_old[1] = h->alpha[1] = h->omega[1] = 0.0;
+}
 
-// BiCGStab (van der Vorst) on the odd-site Schur system Mhat y = bhat, inner precision R, fp64 reliable updates.
+// BiCGStab (van der Vorst) on the odd-site Schur systems Mhat y_c = bhat_c of the columns c with !cs[c].done, inner
+// precision R, fp64 reliable updates. The columns run in lockstep, each with its own scalars; every launch covers the
+// columns that still iterate (ColMap), so links and clover blocks are read once for all of them.
 //   w64: 0 b_e, 1 b_o, 2 bhat_o, 3 y, 4 r64, 5 tmp_e64, 6 w (Mhat y), 7 x_e
 //   w32: 0 r, 1 rhat, 2 p, 3 v, 4 s, 5 t, 6 x, 7 tmp_e
 template <typename R>
-int solve_schur(tmw_ctx* ctx, double tol, double bnorm, SolveState* st) {
+int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
   cudaStream_t s = ctx->stream;
   const int64_t n64 = (int64_t)ctx->g.Vh * 12;                           // double2 vectors per fp64 parity spinor
   const int64_t nR = (int64_t)ctx->g.Vh * 24 * (int64_t)sizeof(R) / 16;  // 16-byte vectors per inner spinor
-  const size_t bytesR = (size_t)nR * 16;
+  const size_t bytesR = (size_t)nR * 16, bytes64 = (size_t)n64 * 16;
   void** W = ctx->w64;
   void** X = ctx->w32;
   void *r = X[0], *rhat = X[1], *p = X[2], *v = X[3], *sv = X[4], *t = X[5], *x = X[6], *tmp = X[7];
   Scalars* h = ctx->sc_host;
+  const int SCD = (int)(sizeof(Scalars) / sizeof(double));
+  double* red_rhat_v = (double*)((char*)ctx->sc + offsetof(Scalars, rhat_v));
+  double* red_ts = (double*)((char*)ctx->sc + offsetof(Scalars, ts));
   const double eps_break = sizeof(R) == 4 ? 1e-6 : 1e-12;
   const bool verbose = getenv("TMW_VERBOSE") != nullptr;  // per-iteration residual log on stderr
   int rc;
+  ColMap act;
+  act.n = 0;
+  for (int c = 0; c < ncols; c++) if (!cs[c].done) cols_add(act, c);
+  if (act.n == 0) return TMW_OK;
   // y = 0, r64 = bhat, r = (R) r64, rhat = r, x = p = v = 0
-  CK(cudaMemsetAsync(W[3], 0, (size_t)n64 * 16, s));
-  CK(cudaMemsetAsync(W[6], 0, (size_t)n64 * 16, s));
-  CK(cudaMemsetAsync(x, 0, bytesR, s));
-  CK(cudaMemsetAsync(p, 0, bytesR, s));
-  CK(cudaMemsetAsync(v, 0, bytesR, s));
-  LAUNCH(launch_convert<R>(n64, W[2], rhat, s));
-  memset(h, 0, sizeof(Scalars));
+  CK(cudaMemsetAsync(W[3], 0, bytes64 * ncols, s));
+  CK(cudaMemsetAsync(W[6], 0, bytes64 * ncols, s));
+  CK(cudaMemsetAsync(x, 0, bytesR * ncols, s));
+  CK(cudaMemsetAsync(p, 0, bytesR * ncols, s));
+  CK(cudaMemsetAsync(v, 0, bytesR * ncols, s));
+  LAUNCH(launch_convert<R>(n64, W[2], rhat, act, s));
+  memset(h, 0, MAXCOL * sizeof(Scalars));
   if ((rc = push_scalars(ctx))) return rc;
-  LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], r, rhat, ctx->sc, s));  // r64 = bhat - 0; rho = <rhat,r>; rr = |r64|^2
+  LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], r, rhat, ctx->sc, act, s));  // r64 = bhat - 0; rho = <rhat,r>; rr = |r64|^2
   if ((rc = fetch_scalars(ctx))) return rc;
-  h->rho_old[0] = h->alpha[0] = h->omega[0] = 1.0;
-  h->rho_old[1] = h->alpha[1] = h->omega[1] = 0.0;
+  for (int i = 0; i < act.n; i++) {
+    const int c = act.col[i];
+    reset_recurrence(&h[c]);
+    cs[c].rnorm = cs[c].maxr = cs[c].rhat_norm = sqrt(h[c].rr);
+    cs[c].iter_resid = cs[c].rnorm / cs[c].bnorm;
+    if (cs[c].rnorm <= tol * cs[c].bnorm) cs[c].done = true;
+  }
   if ((rc = push_scalars(ctx))) return rc;
-  double rnorm = sqrt(h->rr), maxr = rnorm, rhat_norm = rnorm;
-  st->iter_resid = rnorm / bnorm;
-  if (rnorm <= tol * bnorm) return TMW_OK;
   const int max_iter = ctx->opt.max_iter;
   for (int k = 1; k <= max_iter; k++) {
-    st->iters = k;
-    LAUNCH(launch_sc_begin_iter(ctx->sc, s));
-    LAUNCH(launch_update_p<R>(nR, p, r, v, ctx->sc, s));
-    if ((rc = schur<R>(ctx, 0, p, v, tmp, 1, rhat, (double*)((char*)ctx->sc + offsetof(Scalars, rhat_v))))) return rc;
-    LAUNCH(launch_sc_alpha(ctx->sc, s));
-    LAUNCH(launch_update_s<R>(nR, sv, r, v, ctx->sc, s));
-    if ((rc = schur<R>(ctx, 0, sv, t, tmp, 2, nullptr, (double*)((char*)ctx->sc + offsetof(Scalars, ts))))) return rc;
-    LAUNCH(launch_sc_omega(ctx->sc, s));
-    LAUNCH(launch_update_xr<R>(nR, x, r, p, sv, t, rhat, ctx->sc, s));
+    act.n = 0;
+    for (int c = 0; c < ncols; c++) if (!cs[c].done) cols_add(act, c);
+    if (act.n == 0) return TMW_OK;
+    LAUNCH(launch_sc_begin_iter(ctx->sc, act, s));
+    LAUNCH(launch_update_p<R>(nR, p, r, v, ctx->sc, act, s));
+    if ((rc = schur<R>(ctx, 0, p, v, tmp, act, 1, rhat, red_rhat_v, SCD))) return rc;
+    LAUNCH(launch_sc_alpha(ctx->sc, act, s));
+    LAUNCH(launch_update_s<R>(nR, sv, r, v, ctx->sc, act, s));
+    if ((rc = schur<R>(ctx, 0, sv, t, tmp, act, 2, nullptr, red_ts, SCD))) return rc;
+    LAUNCH(launch_sc_omega(ctx->sc, act, s));
+    LAUNCH(launch_update_xr<R>(nR, x, r, p, sv, t, rhat, ctx->sc, act, s));
     if ((rc = fetch_scalars(ctx))) return rc;
-    bool broken = !isfinite(h->rr) || !isfinite(h->rho[0]) || !isfinite(h->rho[1]);
-    rnorm = broken ? maxr : sqrt(h->rr);
-    if (verbose)
-      fprintf(stderr, "[tmw] it %d |r|/|b| %.3e rho (%.3e,%.3e) alpha (%.3e,%.3e) omega (%.3e,%.3e) <rhat,v> (%.3e,%.3e) tt %.3e\n", k, sqrt(h->rr) / bnorm,
-              h->rho[0], h->rho[1], h->alpha[0], h->alpha[1], h->omega[0], h->omega[1], h->rhat_v[0], h->rhat_v[1], h->tt);
-    if (!broken) st->iter_resid = rnorm / bnorm;
-    const bool conv = !broken && rnorm <= tol * bnorm;
-    if (broken || conv || rnorm < ctx->opt.delta * maxr || k == max_iter) {
-      // reliable update: y += x (skipped if the iterate is corrupted), true residual in fp64
-      if (!broken) LAUNCH(launch_acc_y<R>(n64, W[3], x, s));
-      else CK(cudaMemsetAsync(x, 0, bytesR, s));
-      if ((rc = schur<double>(ctx, 0, W[3], W[6], W[5]))) return rc;
-      h->rho[0] = h->rho[1] = 0.0;
-      h->rr = 0.0;
-      if (broken) { h->rho_old[0] = h->alpha[0] = h->omega[0] = 1.0; h->rho_old[1] = h->alpha[1] = h->omega[1] = 0.0; }
-      if ((rc = push_scalars(ctx))) return rc;
-      LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], r, rhat, ctx->sc, s));
-      if ((rc = fetch_scalars(ctx))) return rc;
-      st->updates++;
-      rnorm = sqrt(h->rr);
-      maxr = rnorm;
-      st->iter_resid = rnorm / bnorm;
-      if (verbose) fprintf(stderr, "[tmw]   reliable update %d: true |r|/|b| %.3e rho (%.3e,%.3e)\n", st->updates, rnorm / bnorm, h->rho[0], h->rho[1]);
-      if (!isfinite(rnorm)) return fail(ctx, TMW_EBREAKDOWN, "tmw_solve: non-finite true residual");
-      if (rnorm <= tol * bnorm) return TMW_OK;
-      if (k == max_iter) break;
-    } else if (rnorm > maxr) {
-      maxr = rnorm;
+    ColMap upd, brk;  // columns that take a reliable update now / whose iterate is corrupted
+    upd.n = brk.n = 0;
+    bool broken[MAXCOL];
+    for (int i = 0; i < act.n; i++) {
+      const int c = act.col[i];
+      ColState& q = cs[c];
+      q.iters = k;
+      broken[c] = !isfinite(h[c].rr) || !isfinite(h[c].rho[0]) || !isfinite(h[c].rho[1]);
+      q.rnorm = broken[c] ? q.maxr : sqrt(h[c].rr);
+      if (verbose)
+        fprintf(stderr, "[tmw] col %d it %d |r|/|b| %.3e rho (%.3e,%.3e) alpha (%.3e,%.3e) omega (%.3e,%.3e) <rhat,v> (%.3e,%.3e) tt %.3e\n", c, k,
+                sqrt(h[c].rr) / q.bnorm, h[c].rho[0], h[c].rho[1], h[c].alpha[0], h[c].alpha[1], h[c].omega[0], h[c].omega[1], h[c].rhat_v[0],
+                h[c].rhat_v[1], h[c].tt);
+      if (!broken[c]) q.iter_resid = q.rnorm / q.bnorm;
+      const bool conv = !broken[c] && q.rnorm <= tol * q.bnorm;
+      if (broken[c] || conv || q.rnorm < ctx->opt.delta * q.maxr || k == max_iter) {
+        cols_add(upd, c);
+        if (broken[c]) cols_add(brk, c);
+      } else if (q.rnorm > q.maxr) {
+        q.maxr = q.rnorm;
+      }
     }
-    const double rho_abs = hypot(h->rho[0], h->rho[1]);
-    if (broken || !(rho_abs > eps_break * rhat_norm * rnorm)) {
-      // breakdown: restart the recurrence with rhat = r (C11)
-      if (verbose) fprintf(stderr, "[tmw]   breakdown: |rho| %.3e vs %.3e * %.3e * %.3e -> restart\n", rho_abs, eps_break, rhat_norm, rnorm);
-      if (++st->restarts > 5) return fail(ctx, TMW_EBREAKDOWN, "tmw_solve: BiCGStab breakdown persists after 5 restarts");
-      // fold the current iterate into y first so that r is the residual of y
-      LAUNCH(launch_acc_y<R>(n64, W[3], x, s));
-      if ((rc = schur<double>(ctx, 0, W[3], W[6], W[5]))) return rc;
-      CK(cudaMemsetAsync(p, 0, bytesR, s));
-      CK(cudaMemsetAsync(v, 0, bytesR, s));
-      memset(h, 0, sizeof(Scalars));
-      h->rho_old[0] = h->alpha[0] = h->omega[0] = 1.0;
+    if (upd.n > 0) {
+      // reliable update: y += x (skipped if the iterate is corrupted), true residual in fp64
+      ColMap good;
+      good.n = 0;
+      for (int i = 0; i < upd.n; i++) if (!broken[upd.col[i]]) cols_add(good, upd.col[i]);
+      if (good.n > 0) LAUNCH(launch_acc_y<R>(n64, W[3], x, good, s));
+      for (int i = 0; i < brk.n; i++) CK(cudaMemsetAsync(colp(x, brk.col[i], bytesR), 0, bytesR, s));
+      if ((rc = schur<double>(ctx, 0, W[3], W[6], W[5], upd))) return rc;
+      for (int i = 0; i < upd.n; i++) {
+        const int c = upd.col[i];
+        h[c].rho[0] = h[c].rho[1] = 0.0;
+        h[c].rr = 0.0;
+        if (broken[c]) reset_recurrence(&h[c]);
+      }
       if ((rc = push_scalars(ctx))) return rc;
-      LAUNCH(launch_sub_norm(n64, W[2], W[6], W[4], ctx->red, s));  // r64 = bhat - Mhat y (norm discarded)
-      LAUNCH(launch_convert<R>(n64, W[4], rhat, s));
-      LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], r, rhat, ctx->sc, s));
+      LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], r, rhat, ctx->sc, upd, s));
       if ((rc = fetch_scalars(ctx))) return rc;
-      rnorm = sqrt(h->rr);
-      maxr = rhat_norm = rnorm;
-      st->updates++;
-      if (rnorm <= tol * bnorm) return TMW_OK;
+      for (int i = 0; i < upd.n; i++) {
+        const int c = upd.col[i];
+        ColState& q = cs[c];
+        q.updates++;
+        q.rnorm = q.maxr = sqrt(h[c].rr);
+        q.iter_resid = q.rnorm / q.bnorm;
+        if (verbose) fprintf(stderr, "[tmw]   col %d reliable update %d: true |r|/|b| %.3e rho (%.3e,%.3e)\n", c, q.updates, q.rnorm / q.bnorm, h[c].rho[0], h[c].rho[1]);
+        if (!isfinite(q.rnorm)) return fail(ctx, TMW_EBREAKDOWN, "tmw_solve: non-finite true residual");
+        if (q.rnorm <= tol * q.bnorm) q.done = true;
+      }
+    }
+    if (k == max_iter) break;
+    ColMap rst;  // breakdown: restart the recurrence with rhat = r (C11)
+    rst.n = 0;
+    for (int i = 0; i < act.n; i++) {
+      const int c = act.col[i];
+      if (cs[c].done) continue;
+      const double rho_abs = hypot(h[c].rho[0], h[c].rho[1]);
+      if (broken[c] || !(rho_abs > eps_break * cs[c].rhat_norm * cs[c].rnorm)) {
+        if (verbose) fprintf(stderr, "[tmw]   col %d breakdown: |rho| %.3e vs %.3e * %.3e * %.3e -> restart\n", c, rho_abs, eps_break, cs[c].rhat_norm, cs[c].rnorm);
+        if (++cs[c].restarts > 5) return fail(ctx, TMW_EBREAKDOWN, "tmw_solve: BiCGStab breakdown persists after 5 restarts");
+        cols_add(rst, c);
+      }
+    }
+    if (rst.n > 0) {
+      // fold the current iterate into y first so that r is the residual of y
+      LAUNCH(launch_acc_y<R>(n64, W[3], x, rst, s));
+      if ((rc = schur<double>(ctx, 0, W[3], W[6], W[5], rst))) return rc;
+      for (int i = 0; i < rst.n; i++) {
+        const int c = rst.col[i];
+        CK(cudaMemsetAsync(colp(p, c, bytesR), 0, bytesR, s));
+        CK(cudaMemsetAsync(colp(v, c, bytesR), 0, bytesR, s));
+        memset(&h[c], 0, sizeof(Scalars));
+        reset_recurrence(&h[c]);
+      }
+      if ((rc = push_scalars(ctx))) return rc;
+      LAUNCH(launch_sub_norm(n64, W[2], W[6], W[4], ctx->red, rst, s));  // r64 = bhat - Mhat y (norm discarded)
+      LAUNCH(launch_convert<R>(n64, W[4], rhat, rst, s));
+      LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], r, rhat, ctx->sc, rst, s));
+      if ((rc = fetch_scalars(ctx))) return rc;
+      for (int i = 0; i < rst.n; i++) {
+        const int c = rst.col[i];
+        ColState& q = cs[c];
+        q.rnorm = q.maxr = q.rhat_norm = sqrt(h[c].rr);
+        q.iter_resid = q.rnorm / q.bnorm;
+        q.updates++;
+        if (q.rnorm <= tol * q.bnorm) q.done = true;
+      }
     }
   }
-  return fail(ctx, TMW_ENOCONV, "tmw_solve: max_iter reached");
+  for (int c = 0; c < ncols; c++)
+    if (!cs[c].done) return fail(ctx, TMW_ENOCONV, "tmw_solve: max_iter reached");
+  return TMW_OK;
 }
 
 }  // namespace
 
-extern "C" int tmw_solve(tmw_ctx* ctx, const double* b, double* x, double tol, tmw_solve_info* info) {
+extern "C" int tmw_solve_multi(tmw_ctx* ctx, int nrhs, const double* b, double* x, double tol, tmw_solve_info* info) {
   if (!ctx) return TMW_EINVAL;
   if (!b || !x || b == x) return fail(ctx, TMW_EINVAL, "tmw_solve: null or aliased pointers");
   if (!(tol > 0.0) || !isfinite(tol)) return fail(ctx, TMW_EINVAL, "tmw_solve: tol must be > 0");
-  if (info) memset(info, 0, sizeof(*info));
+  if (nrhs < 1 || nrhs > MAXCOL) return fail(ctx, TMW_EINVAL, "tmw_solve: nrhs must be in 1..16");
+  if (info) memset(info, 0, sizeof(*info) * nrhs);
   const bool dbl = ctx->opt.precision == TMW_DOUBLE;
   int rc;
+  if ((rc = need_cols(ctx, nrhs))) return rc;
   if ((rc = need_w64(ctx, 8))) return rc;
   if ((rc = need_w32(ctx, 8, dbl ? TMW_F64 : TMW_F32))) return rc;
   cudaStream_t s = ctx->stream;
-  const size_t cbytes = (size_t)ctx->V * 24 * 8;
+  const size_t cbytes = (size_t)ctx->V * 24 * 8, b64 = spinor_bytes(ctx, TMW_F64);
   const double* cb = b;
   double* cx_ = x;
   if (ctx->opt.location == TMW_HOST) {
@@ -519,53 +673,73 @@ extern "C" int tmw_solve(tmw_ctx* ctx, const double* b, double* x, double tol, t
     cx_ = (double*)ctx->canon[1];
   }
   CK(cudaEventRecord(ctx->ev0, s));
-  if (ctx->opt.location == TMW_HOST) CK(cudaMemcpyAsync(ctx->canon[0], b, cbytes, cudaMemcpyHostToDevice, s));
+  if (ctx->opt.location == TMW_HOST) CK(cudaMemcpyAsync(ctx->canon[0], b, cbytes * nrhs, cudaMemcpyHostToDevice, s));
   void** W = ctx->w64;
   const int64_t n64 = (int64_t)ctx->g.Vh * 12;
-  SolveState st;
-  memset(&st, 0, sizeof(st));
+  ColState cs[MAXCOL];
+  memset(cs, 0, sizeof(cs));
+  const ColMap all = cols_first(nrhs);
   // A0/A7: split b, |b|, bhat_o = b_o - H_oe A_ee^{-1} b_e
-  LAUNCH(launch_pack_spinor(ctx->g, 0, 1, cb, W[0], s));
-  LAUNCH(launch_pack_spinor(ctx->g, 1, 1, cb, W[1], s));
-  CK(cudaMemsetAsync(ctx->red, 0, 4 * sizeof(double), s));
-  LAUNCH(launch_dot_norm<double>(n64, nullptr, W[0], ctx->red, s));
-  LAUNCH(launch_dot_norm<double>(n64, nullptr, W[1], ctx->red, s));
+  for (int c = 0; c < nrhs; c++) {
+    LAUNCH(launch_pack_spinor(ctx->g, 0, 1, (const double*)colp(cb, c, cbytes), colp(W[0], c, b64), s));
+    LAUNCH(launch_pack_spinor(ctx->g, 1, 1, (const double*)colp(cb, c, cbytes), colp(W[1], c, b64), s));
+  }
+  CK(cudaMemsetAsync(ctx->red, 0, 4 * MAXCOL * sizeof(double), s));
+  LAUNCH(launch_dot_norm<double>(n64, nullptr, W[0], ctx->red, all, s));
+  LAUNCH(launch_dot_norm<double>(n64, nullptr, W[1], ctx->red, all, s));
   if ((rc = fetch_red(ctx))) return rc;
-  const double bnorm = sqrt(ctx->red_host[2]);
-  if (!isfinite(bnorm)) return fail(ctx, TMW_EINVAL, "tmw_solve: b has non-finite entries");
+  ColMap nz;  // columns with b != 0
+  nz.n = 0;
+  for (int c = 0; c < nrhs; c++) {
+    cs[c].bnorm = sqrt(ctx->red_host[4 * c + 2]);
+    if (!isfinite(cs[c].bnorm)) return fail(ctx, TMW_EINVAL, "tmw_solve: b has non-finite entries");
+    if (cs[c].bnorm == 0.0) {
+      cs[c].done = true;
+      CK(cudaMemsetAsync(colp(cx_, c, cbytes), 0, cbytes, s));
+    } else {
+      cols_add(nz, c);
+    }
+  }
   int status = TMW_OK;
-  if (bnorm == 0.0) {
-    CK(cudaMemsetAsync(cx_, 0, cbytes, s));
-  } else {
+  if (nz.n > 0) {
     Diag<double> d = make_diag<double>(ctx, 0);
-    LAUNCH(launch_diag(d, ctx->g, 0, ctx->clover, 1, W[0], W[5], s));
-    if ((rc = dslash<double>(ctx, EPI_XPAY, 1, 0, W[5], W[2], W[1], -1.0))) return rc;
-    status = dbl ? solve_schur<double>(ctx, tol, bnorm, &st) : solve_schur<float>(ctx, tol, bnorm, &st);
+    for (int i = 0; i < nz.n; i++) LAUNCH(launch_diag(d, ctx->g, 0, ctx->clover, 1, colp(W[0], nz.col[i], b64), colp(W[5], nz.col[i], b64), s));
+    if ((rc = dslash<double>(ctx, EPI_XPAY, 1, 0, W[5], W[2], W[1], -1.0, nz))) return rc;
+    status = dbl ? solve_schur<double>(ctx, nrhs, tol, cs) : solve_schur<float>(ctx, nrhs, tol, cs);
     if (status != TMW_OK && status != TMW_ENOCONV) return status;
     // A7: x_o = y, x_e = A_ee^{-1} (b_e - H_eo x_o)
-    if ((rc = dslash<double>(ctx, EPI_AINV_XPAY, 0, 0, W[3], W[7], W[0], -1.0))) return rc;
-    LAUNCH(launch_unpack_spinor(ctx->g, 0, 1, W[7], cx_, s));
-    LAUNCH(launch_unpack_spinor(ctx->g, 1, 1, W[3], cx_, s));
+    if ((rc = dslash<double>(ctx, EPI_AINV_XPAY, 0, 0, W[3], W[7], W[0], -1.0, nz))) return rc;
+    for (int i = 0; i < nz.n; i++) {
+      const int c = nz.col[i];
+      LAUNCH(launch_unpack_spinor(ctx->g, 0, 1, colp(W[7], c, b64), (double*)colp(cx_, c, cbytes), s));
+      LAUNCH(launch_unpack_spinor(ctx->g, 1, 1, colp(W[3], c, b64), (double*)colp(cx_, c, cbytes), s));
+    }
     // true residual of the full system in fp64: |b - D x|
-    if ((rc = full_apply64(ctx, 0, W[7], W[3], W[5], W[6]))) return rc;
-    CK(cudaMemsetAsync(ctx->red, 0, 4 * sizeof(double), s));
-    LAUNCH(launch_sub_norm(n64, W[0], W[5], W[5], ctx->red, s));
-    LAUNCH(launch_sub_norm(n64, W[1], W[6], W[6], ctx->red, s));
+    if ((rc = full_apply64(ctx, 0, W[7], W[3], W[5], W[6], nz))) return rc;
+    CK(cudaMemsetAsync(ctx->red, 0, 4 * MAXCOL * sizeof(double), s));
+    LAUNCH(launch_sub_norm(n64, W[0], W[5], W[5], ctx->red, nz, s));
+    LAUNCH(launch_sub_norm(n64, W[1], W[6], W[6], ctx->red, nz, s));
     if ((rc = fetch_red(ctx))) return rc;
-    st.true_resid = sqrt(ctx->red_host[2]) / bnorm;
+    for (int i = 0; i < nz.n; i++) cs[nz.col[i]].true_resid = sqrt(ctx->red_host[4 * nz.col[i] + 2]) / cs[nz.col[i]].bnorm;
   }
-  if (ctx->opt.location == TMW_HOST) CK(cudaMemcpyAsync(x, cx_, cbytes, cudaMemcpyDeviceToHost, s));
+  if (ctx->opt.location == TMW_HOST) CK(cudaMemcpyAsync(x, cx_, cbytes * nrhs, cudaMemcpyDeviceToHost, s));
   CK(cudaEventRecord(ctx->ev1, s));
   CK(cudaStreamSynchronize(s));
   float ms = 0;
   CK(cudaEventElapsedTime(&ms, ctx->ev0, ctx->ev1));
   if (info) {
-    info->iters = st.iters;
-    info->reliable_updates = st.updates;
-    info->restarts = st.restarts;
-    info->iter_resid = st.iter_resid;
-    info->true_resid = st.true_resid;
-    info->device_ms = ms;
+    for (int c = 0; c < nrhs; c++) {
+      info[c].iters = cs[c].iters;
+      info[c].reliable_updates = cs[c].updates;
+      info[c].restarts = cs[c].restarts;
+      info[c].iter_resid = cs[c].iter_resid;
+      info[c].true_resid = cs[c].true_resid;
+      info[c].device_ms = ms;
+    }
   }
   return status;
+}
+
+extern "C" int tmw_solve(tmw_ctx* ctx, const double* b, double* x, double tol, tmw_solve_info* info) {
+  return tmw_solve_multi(ctx, 1, b, x, tol, info);
 }

@@ -3,6 +3,9 @@
 // accumulated in fp64 (per-thread -> warp shuffle -> block -> one atomicAdd per block and value).
 // All vectors are packed parity spinors viewed as flat arrays of complex numbers; a work item is a PAIR of
 // complex numbers = 4 reals (one float4, or two double2).
+// Every kernel is batched over right-hand-side columns: blockIdx.y = slot, column c = cm.col[slot];
+// column c of a vector starts c*cs work items after its base pointer and uses the scalar block sc[c]. A single
+// solve is the batch {0}.
 #include "tmw_internal.h"
 
 namespace tmw {
@@ -69,7 +72,8 @@ __device__ __forceinline__ void cdiv(const double* a, const double* b, double* q
   const double re = (a[0] * b[0] + a[1] * b[1]) / d, im = (a[1] * b[0] - a[0] * b[1]) / d;
   q[0] = re; q[1] = im;
 }
-__global__ void sc_begin_iter_kernel(Scalars* sc) {  // beta = (rho/rho_old)(alpha/omega)
+__global__ void sc_begin_iter_kernel(Scalars* sc0, ColMap cm) {  // beta = (rho/rho_old)(alpha/omega)
+  Scalars* sc = sc0 + cm.col[threadIdx.x];
   double a[2], b[2];
   cdiv(sc->rho, sc->rho_old, a);
   cdiv(sc->alpha, sc->omega, b);
@@ -79,8 +83,12 @@ __global__ void sc_begin_iter_kernel(Scalars* sc) {  // beta = (rho/rho_old)(alp
   sc->ts[0] = sc->ts[1] = 0.0;
   sc->tt = 0.0;
 }
-__global__ void sc_alpha_kernel(Scalars* sc) { cdiv(sc->rho, sc->rhat_v, sc->alpha); }
-__global__ void sc_omega_kernel(Scalars* sc) {
+__global__ void sc_alpha_kernel(Scalars* sc0, ColMap cm) {
+  Scalars* sc = sc0 + cm.col[threadIdx.x];
+  cdiv(sc->rho, sc->rhat_v, sc->alpha);
+}
+__global__ void sc_omega_kernel(Scalars* sc0, ColMap cm) {
+  Scalars* sc = sc0 + cm.col[threadIdx.x];
   sc->omega[0] = sc->ts[0] / sc->tt;
   sc->omega[1] = sc->ts[1] / sc->tt;
   sc->rho_old[0] = sc->rho[0];
@@ -88,12 +96,15 @@ __global__ void sc_omega_kernel(Scalars* sc) {
   sc->rho[0] = sc->rho[1] = 0.0;
   sc->rr = 0.0;
 }
-cudaError_t launch_sc_begin_iter(Scalars* sc, cudaStream_t s) { sc_begin_iter_kernel<<<1, 1, 0, s>>>(sc); return cudaGetLastError(); }
-cudaError_t launch_sc_alpha(Scalars* sc, cudaStream_t s) { sc_alpha_kernel<<<1, 1, 0, s>>>(sc); return cudaGetLastError(); }
-cudaError_t launch_sc_omega(Scalars* sc, cudaStream_t s) { sc_omega_kernel<<<1, 1, 0, s>>>(sc); return cudaGetLastError(); }
+cudaError_t launch_sc_begin_iter(Scalars* sc, const ColMap& cm, cudaStream_t s) { sc_begin_iter_kernel<<<1, cm.n, 0, s>>>(sc, cm); return cudaGetLastError(); }
+cudaError_t launch_sc_alpha(Scalars* sc, const ColMap& cm, cudaStream_t s) { sc_alpha_kernel<<<1, cm.n, 0, s>>>(sc, cm); return cudaGetLastError(); }
+cudaError_t launch_sc_omega(Scalars* sc, const ColMap& cm, cudaStream_t s) { sc_omega_kernel<<<1, cm.n, 0, s>>>(sc, cm); return cudaGetLastError(); }
 
 // ---- vector updates ----
-template <typename R> __global__ void __launch_bounds__(BB) update_p_kernel(int64_t n, R* p, const R* r, const R* v, const Scalars* sc) {
+template <typename R> __global__ void __launch_bounds__(BB) update_p_kernel(int64_t n, R* p, const R* r, const R* v, const Scalars* sc, ColMap cm) {
+  const int c = cm.col[blockIdx.y];
+  sc += c;
+  { const int64_t o = 4 * n * c; p += o; r += o; v += o; }
   const R br = (R)sc->beta[0], bi = (R)sc->beta[1], wr = (R)sc->omega[0], wi = (R)sc->omega[1];
   for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
     R pp[4], rr[4], vv[4];
@@ -108,7 +119,10 @@ template <typename R> __global__ void __launch_bounds__(BB) update_p_kernel(int6
     stp(p, i, pp);
   }
 }
-template <typename R> __global__ void __launch_bounds__(BB) update_s_kernel(int64_t n, R* s, const R* r, const R* v, const Scalars* sc) {
+template <typename R> __global__ void __launch_bounds__(BB) update_s_kernel(int64_t n, R* s, const R* r, const R* v, const Scalars* sc, ColMap cm) {
+  const int c = cm.col[blockIdx.y];
+  sc += c;
+  { const int64_t o = 4 * n * c; s += o; r += o; v += o; }
   const R ar = (R)sc->alpha[0], ai = (R)sc->alpha[1];
   for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
     R rr[4], vv[4], ss[4];
@@ -121,7 +135,10 @@ template <typename R> __global__ void __launch_bounds__(BB) update_s_kernel(int6
     stp(s, i, ss);
   }
 }
-template <typename R> __global__ void __launch_bounds__(BB) update_xr_kernel(int64_t n, R* x, R* r, const R* p, const R* s, const R* t, const R* rhat, Scalars* sc) {
+template <typename R> __global__ void __launch_bounds__(BB) update_xr_kernel(int64_t n, R* x, R* r, const R* p, const R* s, const R* t, const R* rhat, Scalars* sc, ColMap cm) {
+  const int c = cm.col[blockIdx.y];
+  sc += c;
+  { const int64_t o = 4 * n * c; x += o; r += o; p += o; s += o; t += o; rhat += o; }
   const R ar = (R)sc->alpha[0], ai = (R)sc->alpha[1], wr = (R)sc->omega[0], wi = (R)sc->omega[1];
   double acc[3] = {0, 0, 0};
   for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
@@ -145,7 +162,10 @@ template <typename R> __global__ void __launch_bounds__(BB) update_xr_kernel(int
   double* dst[3] = {&sc->rho[0], &sc->rho[1], &sc->rr};
   reduce_atomic<3>(acc, dst);
 }
-template <typename R> __global__ void __launch_bounds__(BB) dot_norm_kernel(int64_t n, const R* a, const R* b, double* out) {
+template <typename R> __global__ void __launch_bounds__(BB) dot_norm_kernel(int64_t n, const R* a, const R* b, double* out, ColMap cm) {
+  const int c = cm.col[blockIdx.y];
+  out += 4 * c;
+  { const int64_t o = 4 * n * c; if (a) a += o; b += o; }
   double acc[3] = {0, 0, 0};
   for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
     R aa[4] = {0, 0, 0, 0}, bb[4];
@@ -163,7 +183,8 @@ template <typename R> __global__ void __launch_bounds__(BB) dot_norm_kernel(int6
   double* dst[3] = {out, out + 1, out + 2};
   reduce_atomic<3>(acc, dst);
 }
-template <typename R> __global__ void __launch_bounds__(BB) acc_y_kernel(int64_t n, int64_t Vh, double* y, R* x) {
+template <typename R> __global__ void __launch_bounds__(BB) acc_y_kernel(int64_t n, int64_t Vh, double* y, R* x, ColMap cm) {
+  { const int64_t o = 4 * n * cm.col[blockIdx.y]; y += o; x += o; }
   for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
     R xx[4];
     double yy[4];
@@ -174,7 +195,10 @@ template <typename R> __global__ void __launch_bounds__(BB) acc_y_kernel(int64_t
     stm(x, i, Vh, xx);
   }
 }
-template <typename R> __global__ void __launch_bounds__(BB) resid_convert_kernel(int64_t n, int64_t Vh, const double* b, const double* w, double* r64, R* r, const R* rhat, Scalars* sc) {
+template <typename R> __global__ void __launch_bounds__(BB) resid_convert_kernel(int64_t n, int64_t Vh, const double* b, const double* w, double* r64, R* r, const R* rhat, Scalars* sc, ColMap cm) {
+  const int c = cm.col[blockIdx.y];
+  sc += c;
+  { const int64_t o = 4 * n * c; b += o; w += o; r64 += o; r += o; rhat += o; }
   double acc[3] = {0, 0, 0};
   for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
     double bb[4], ww[4], dd[4];
@@ -194,7 +218,8 @@ template <typename R> __global__ void __launch_bounds__(BB) resid_convert_kernel
   double* dst[3] = {&sc->rho[0], &sc->rho[1], &sc->rr};
   reduce_atomic<3>(acc, dst);
 }
-template <typename R> __global__ void __launch_bounds__(BB) convert_kernel(int64_t n, int64_t Vh, const double* src, R* dst) {
+template <typename R> __global__ void __launch_bounds__(BB) convert_kernel(int64_t n, int64_t Vh, const double* src, R* dst, ColMap cm) {
+  { const int64_t o = 4 * n * cm.col[blockIdx.y]; src += o; dst += o; }
   for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
     double ss[4];
     R dd[4];
@@ -204,7 +229,10 @@ template <typename R> __global__ void __launch_bounds__(BB) convert_kernel(int64
     stm(dst, i, Vh, dd);
   }
 }
-__global__ void __launch_bounds__(BB) sub_norm_kernel(int64_t n, const double* a, const double* b, double* d, double* out) {
+__global__ void __launch_bounds__(BB) sub_norm_kernel(int64_t n, const double* a, const double* b, double* d, double* out, ColMap cm) {
+  const int c = cm.col[blockIdx.y];
+  out += 4 * c;
+  { const int64_t o = 4 * n * c; a += o; b += o; d += o; }
   double acc[1] = {0};
   for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
     double aa[4], bb[4], dd[4];
@@ -217,58 +245,59 @@ __global__ void __launch_bounds__(BB) sub_norm_kernel(int64_t n, const double* a
   reduce_atomic<1>(acc, dst);
 }
 
-// n16 = number of 16-byte vectors of R; pairs = n16 (float) or n16/2 (double)
+// n16 = number of 16-byte vectors of R in ONE column; pairs = n16 (float) or n16/2 (double)
 template <typename R> static inline int64_t pairs_of(int64_t n16) { return sizeof(R) == 4 ? n16 : n16 / 2; }
+static inline dim3 grid_of(int64_t np, const ColMap& cm) { return dim3((unsigned)blas_grid(np), (unsigned)cm.n, 1); }
 
-template <typename R> cudaError_t launch_update_p(int64_t n, void* p, const void* r, const void* v, const Scalars* sc, cudaStream_t s) {
+template <typename R> cudaError_t launch_update_p(int64_t n, void* p, const void* r, const void* v, const Scalars* sc, const ColMap& cm, cudaStream_t s) {
   const int64_t np = pairs_of<R>(n);
-  update_p_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, (R*)p, (const R*)r, (const R*)v, sc);
+  update_p_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, (R*)p, (const R*)r, (const R*)v, sc, cm);
   return cudaGetLastError();
 }
-template <typename R> cudaError_t launch_update_s(int64_t n, void* sv, const void* r, const void* v, const Scalars* sc, cudaStream_t s) {
+template <typename R> cudaError_t launch_update_s(int64_t n, void* sv, const void* r, const void* v, const Scalars* sc, const ColMap& cm, cudaStream_t s) {
   const int64_t np = pairs_of<R>(n);
-  update_s_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, (R*)sv, (const R*)r, (const R*)v, sc);
+  update_s_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, (R*)sv, (const R*)r, (const R*)v, sc, cm);
   return cudaGetLastError();
 }
-template <typename R> cudaError_t launch_update_xr(int64_t n, void* x, void* r, const void* p, const void* sv, const void* t, const void* rhat, Scalars* sc, cudaStream_t s) {
+template <typename R> cudaError_t launch_update_xr(int64_t n, void* x, void* r, const void* p, const void* sv, const void* t, const void* rhat, Scalars* sc, const ColMap& cm, cudaStream_t s) {
   const int64_t np = pairs_of<R>(n);
-  update_xr_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, (R*)x, (R*)r, (const R*)p, (const R*)sv, (const R*)t, (const R*)rhat, sc);
+  update_xr_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, (R*)x, (R*)r, (const R*)p, (const R*)sv, (const R*)t, (const R*)rhat, sc, cm);
   return cudaGetLastError();
 }
-template <typename R> cudaError_t launch_dot_norm(int64_t n, const void* a, const void* b, double* out, cudaStream_t s) {
+template <typename R> cudaError_t launch_dot_norm(int64_t n, const void* a, const void* b, double* out, const ColMap& cm, cudaStream_t s) {
   const int64_t np = pairs_of<R>(n);
-  dot_norm_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, (const R*)a, (const R*)b, out);
+  dot_norm_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, (const R*)a, (const R*)b, out, cm);
   return cudaGetLastError();
 }
-template <typename R> cudaError_t launch_acc_y(int64_t n64, void* y64, void* x, cudaStream_t s) {
+template <typename R> cudaError_t launch_acc_y(int64_t n64, void* y64, void* x, const ColMap& cm, cudaStream_t s) {
   const int64_t np = n64 / 2;
-  acc_y_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, np / 6, (double*)y64, (R*)x);
+  acc_y_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, np / 6, (double*)y64, (R*)x, cm);
   return cudaGetLastError();
 }
-template <typename R> cudaError_t launch_resid_convert(int64_t n64, const void* b64, const void* w64, void* r64, void* r, const void* rhat, Scalars* sc, cudaStream_t s) {
+template <typename R> cudaError_t launch_resid_convert(int64_t n64, const void* b64, const void* w64, void* r64, void* r, const void* rhat, Scalars* sc, const ColMap& cm, cudaStream_t s) {
   const int64_t np = n64 / 2;
-  resid_convert_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, np / 6, (const double*)b64, (const double*)w64, (double*)r64, (R*)r, (const R*)rhat, sc);
+  resid_convert_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, np / 6, (const double*)b64, (const double*)w64, (double*)r64, (R*)r, (const R*)rhat, sc, cm);
   return cudaGetLastError();
 }
-template <typename R> cudaError_t launch_convert(int64_t n64, const void* src64, void* dst, cudaStream_t s) {
+template <typename R> cudaError_t launch_convert(int64_t n64, const void* src64, void* dst, const ColMap& cm, cudaStream_t s) {
   const int64_t np = n64 / 2;
-  convert_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, np / 6, (const double*)src64, (R*)dst);
+  convert_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, np / 6, (const double*)src64, (R*)dst, cm);
   return cudaGetLastError();
 }
-cudaError_t launch_sub_norm(int64_t n64, const void* a, const void* b, void* d, double* out, cudaStream_t s) {
+cudaError_t launch_sub_norm(int64_t n64, const void* a, const void* b, void* d, double* out, const ColMap& cm, cudaStream_t s) {
   const int64_t np = n64 / 2;
-  sub_norm_kernel<<<blas_grid(np), BB, 0, s>>>(np, (const double*)a, (const double*)b, (double*)d, out);
+  sub_norm_kernel<<<grid_of(np, cm), BB, 0, s>>>(np, (const double*)a, (const double*)b, (double*)d, out, cm);
   return cudaGetLastError();
 }
 
 #define TMW_INST(R)                                                                                                          \
-  template cudaError_t launch_update_p<R>(int64_t, void*, const void*, const void*, const Scalars*, cudaStream_t);           \
-  template cudaError_t launch_update_s<R>(int64_t, void*, const void*, const void*, const Scalars*, cudaStream_t);           \
-  template cudaError_t launch_update_xr<R>(int64_t, void*, void*, const void*, const void*, const void*, const void*, Scalars*, cudaStream_t); \
-  template cudaError_t launch_dot_norm<R>(int64_t, const void*, const void*, double*, cudaStream_t);                         \
-  template cudaError_t launch_acc_y<R>(int64_t, void*, void*, cudaStream_t);                                                 \
-  template cudaError_t launch_resid_convert<R>(int64_t, const void*, const void*, void*, void*, const void*, Scalars*, cudaStream_t); \
-  template cudaError_t launch_convert<R>(int64_t, const void*, void*, cudaStream_t);
+  template cudaError_t launch_update_p<R>(int64_t, void*, const void*, const void*, const Scalars*, const ColMap&, cudaStream_t);           \
+  template cudaError_t launch_update_s<R>(int64_t, void*, const void*, const void*, const Scalars*, const ColMap&, cudaStream_t);           \
+  template cudaError_t launch_update_xr<R>(int64_t, void*, void*, const void*, const void*, const void*, const void*, Scalars*, const ColMap&, cudaStream_t); \
+  template cudaError_t launch_dot_norm<R>(int64_t, const void*, const void*, double*, const ColMap&, cudaStream_t);                         \
+  template cudaError_t launch_acc_y<R>(int64_t, void*, void*, const ColMap&, cudaStream_t);                                                 \
+  template cudaError_t launch_resid_convert<R>(int64_t, const void*, const void*, void*, void*, const void*, Scalars*, const ColMap&, cudaStream_t); \
+  template cudaError_t launch_convert<R>(int64_t, const void*, void*, const ColMap&, cudaStream_t);
 TMW_INST(float)
 TMW_INST(double)
 

@@ -17,7 +17,44 @@ struct Geom {
   int L, T, Lh;
   int Vh;          // sites per parity (< 2^31)
   int sy, sz, st;  // cb strides of +1 in y, z, t
+  // Thread -> site mapping of the stencil kernels. tiled = 0: CTA b covers cb in [b*BLOCK, (b+1)*BLOCK).
+  // tiled = 1: a CTA covers a 4-D tile of 2^lx (in xh) x 2^ly x 2^lz x 2^lt = BLOCK sites, so that most neighbour
+  // spinors of the tile are shared between its threads and hit in L1; tiles are ordered xh, y (blockIdx.x),
+  // z (blockIdx.y), t (blockIdx.z), i.e. the sweep through the lattice is the same as in cb order.
+  int tiled;
+  int lx, ly, lz, lt;
+  int ntx, nty;    // tiles along xh and y
 };
+
+// coordinates of one site of a parity: x = 2*xh + ((y + z + t + par) & 1)
+struct Site {
+  int xh, y, z, t, cb;
+};
+
+// site of this thread; sblock = blockIdx.x stripped of the right-hand-side group (see dslash_kernel)
+template <int BLOCK> __device__ __forceinline__ bool thread_site(const Geom& g, int sblock, Site& s) {
+  const int tid = threadIdx.x;
+  if (g.tiled) {
+    const int by = sblock / g.ntx, bx = sblock - by * g.ntx;
+    s.xh = (bx << g.lx) | (tid & ((1 << g.lx) - 1));
+    int q = tid >> g.lx;
+    s.y = (by << g.ly) | (q & ((1 << g.ly) - 1));
+    q >>= g.ly;
+    s.z = ((int)blockIdx.y << g.lz) | (q & ((1 << g.lz) - 1));
+    q >>= g.lz;
+    s.t = ((int)blockIdx.z << g.lt) | q;
+    s.cb = s.xh + g.Lh * (s.y + g.L * (s.z + g.L * s.t));
+    return true;
+  }
+  s.cb = sblock * BLOCK + tid;
+  s.xh = s.cb % g.Lh;
+  int q = s.cb / g.Lh;
+  s.y = q % g.L;
+  q /= g.L;
+  s.z = q % g.L;
+  s.t = q / g.L;
+  return s.cb < g.Vh;
+}
 
 // ---------------------------------------------------------------------------------------------------------
 // 16-byte vector access. A packed field of NREAL reals per site is stored as planes of 16-byte vectors:
@@ -403,6 +440,8 @@ template <typename R, bool CLOVER> TMW_HD void apply_Ainv(const Diag<R>& d, int 
 // ---------------------------------------------------------------------------------------------------------
 // The stencil. Epilogues (h = 1/2 sum of the 8 hops = the hopping block H_{p pbar} applied to `in`):
 // ---------------------------------------------------------------------------------------------------------
+enum { MAXCOL = 16 };  // most right-hand sides per call
+
 enum { EPI_HOP = 0,        // out = h
        EPI_AINV_HOP = 1,   // out = A^{-1} h                      (K1 of the Schur operator)
        EPI_A_XPAY = 2,     // out = A aux + sgn*h                 (K2: sgn = -1; full apply: sgn = +1)
@@ -424,6 +463,15 @@ template <typename R> struct DslashArgs {
   int red_mode;
   const void* dotv;
   double* red;
+  // right-hand-side columns (the "12 columns" of PAPER.md:78): slot j of this launch works on column
+  // col[j]; in/out/aux/dotv of column c start c*cstride 16-byte vectors after the base pointers, its reduction
+  // target red_stride doubles after red. One thread does NR consecutive slots of one site (links and clover blocks
+  // are loaded once for the NR columns); CTAs of the ngroups = ceil(ncol/NR) slot groups of one site block are
+  // adjacent in blockIdx.x, so the groups after the first find the links in L2.
+  int ncol, ngroups;
+  int64_t cstride;
+  int red_stride;
+  unsigned char col[MAXCOL];
 };
 
 // neighbour checkerboard indices and the time-boundary sign
@@ -431,14 +479,9 @@ struct Nbr {
   int fwd[4], bwd[4];
   bool wrap_tf, wrap_tb;
 };
-TMW_HD Nbr neighbours(const Geom& g, int par, int cb) {
+TMW_HD Nbr neighbours(const Geom& g, int par, const Site& s) {
   Nbr n;
-  const int xh = cb % g.Lh;
-  int q = cb / g.Lh;
-  const int y = q % g.L;
-  q /= g.L;
-  const int z = q % g.L;
-  const int t = q / g.L;
+  const int xh = s.xh, y = s.y, z = s.z, t = s.t, cb = s.cb;
   const int o = (y + z + t + par) & 1;  // x = 2*xh + o
   // x+1 -> xh + o (wrap to 0), x-1 -> xh + o - 1 (wrap to Lh-1)
   const int xf = xh + o, xb = xh + o - 1;
@@ -455,60 +498,152 @@ TMW_HD Nbr neighbours(const Geom& g, int par, int cb) {
   return n;
 }
 
-template <typename R, int NG, int MU>
-TMW_HD void hop_pair(const DslashArgs<R>& a, const Nbr& n, int cb, R* acc) {
+template <typename R, int NG, int MU, int NR>
+__device__ __forceinline__ void hop_pair(const DslashArgs<R>& a, const Nbr& n, int cb, const int64_t (&coff)[NR], R (&acc)[NR][24]) {
   const int NPG = Planes<R, NG>::N;
   const int64_t Vh = a.g.Vh;
   typedef typename Vec16<R>::T V;
   {  // forward: (1 + sig g_mu) U_mu(x) psi(x+mu)
-    R psi[24];
     cx<R> U[9];
-    load_reals<24>(a.in, Vh, n.fwd[MU], psi);
     load_link<R, NG>((const V*)a.U[a.par] + (int64_t)MU * NPG * Vh, Vh, cb, U);
-    hop<R, MU, true>(psi, U, a.sig, (MU == 3 && n.wrap_tf) ? (R)-1 : (R)1, acc);
+    const R bc = (MU == 3 && n.wrap_tf) ? (R)-1 : (R)1;
+#pragma unroll
+    for (int j = 0; j < NR; j++) {
+      R psi[24];
+      load_reals<24>((const V*)a.in + coff[j], Vh, n.fwd[MU], psi);
+      hop<R, MU, true>(psi, U, a.sig, bc, acc[j]);
+    }
   }
   {  // backward: (1 - sig g_mu) U_mu(x-mu)^dag psi(x-mu)
-    R psi[24];
     cx<R> U[9];
-    load_reals<24>(a.in, Vh, n.bwd[MU], psi);
     load_link<R, NG>((const V*)a.U[1 - a.par] + (int64_t)MU * NPG * Vh, Vh, n.bwd[MU], U);
-    hop<R, MU, false>(psi, U, -a.sig, (MU == 3 && n.wrap_tb) ? (R)-1 : (R)1, acc);
+    const R bc = (MU == 3 && n.wrap_tb) ? (R)-1 : (R)1;
+#pragma unroll
+    for (int j = 0; j < NR; j++) {
+      R psi[24];
+      load_reals<24>((const V*)a.in + coff[j], Vh, n.bwd[MU], psi);
+      hop<R, MU, false>(psi, U, -a.sig, bc, acc[j]);
+    }
   }
 }
 
-// computes the output spinor o[24] of site cb; ax[24] receives aux(cb) when EPI >= 2
-template <typename R, int NG, int EPI, bool CLOVER>
-TMW_HD void dslash_site(const DslashArgs<R>& a, int cb, R* o, R* ax) {
-  const Nbr n = neighbours(a.g, a.par, cb);
-  R acc[24];
-#pragma unroll
-  for (int i = 0; i < 24; i++) acc[i] = (R)0;
-  hop_pair<R, NG, 0>(a, n, cb, acc);
-  hop_pair<R, NG, 1>(a, n, cb, acc);
-  hop_pair<R, NG, 2>(a, n, cb, acc);
-  hop_pair<R, NG, 3>(a, n, cb, acc);
-  const int64_t Vh = a.g.Vh;
-  if (EPI == EPI_HOP) {
-#pragma unroll
-    for (int i = 0; i < 24; i++) o[i] = a.coef * acc[i];
-  } else if (EPI == EPI_AINV_HOP) {
-#pragma unroll
-    for (int i = 0; i < 24; i++) acc[i] *= a.coef;
-    apply_Ainv<R, CLOVER>(a.d, a.par, Vh, cb, acc, o);
-  } else if (EPI == EPI_A_XPAY) {
-    load_reals<24>(a.aux, Vh, cb, ax);
-    apply_A<R, CLOVER>(a.d, a.par, Vh, cb, ax, o);
-#pragma unroll
-    for (int i = 0; i < 24; i++) o[i] += a.coef * acc[i];
-  } else if (EPI == EPI_XPAY) {
-    load_reals<24>(a.aux, Vh, cb, ax);
-#pragma unroll
-    for (int i = 0; i < 24; i++) o[i] = ax[i] + a.coef * acc[i];
+// One chirality b (12 reals: spins 2b, 2b+1) of the site-diagonal part, with the block held in registers so that it
+// serves several right-hand sides: w = A_b v and w = A_b^{-1} v as in apply_A / apply_Ainv above.
+template <typename R, bool CLOVER> TMW_HD void load_block(const void* base, int b, int64_t Vh, int64_t cb, R* B) {
+  if (CLOVER) load_reals_s<36>((const typename Vec16<R>::T*)base + (int64_t)b * Planes<R, 36>::N * Vh, Vh, cb, B);
+}
+template <typename R, bool CLOVER> TMW_HD void half_A(const Diag<R>& d, int b, const R* B, const R* v, R* w) {
+  if (CLOVER) {
+    herm6_mul(B, v, w);
   } else {
-    load_reals<24>(a.aux, Vh, cb, ax);
 #pragma unroll
-    for (int i = 0; i < 24; i++) acc[i] = ax[i] + a.coef * acc[i];
-    apply_Ainv<R, CLOVER>(a.d, a.par, Vh, cb, acc, o);
+    for (int i = 0; i < 12; i++) w[i] = d.diag * v[i];
+  }
+  const R tw = b ? d.tw_lo : d.tw_up;
+#pragma unroll
+  for (int i = 0; i < 6; i++) {
+    w[2 * i] -= tw * v[2 * i + 1];
+    w[2 * i + 1] += tw * v[2 * i];
+  }
+}
+// no clover: the complex scalar inverse; clover: w = Binv v (Binv = C^{-1}, or (C^2 + tw^2)^{-1} when twisted: the
+// caller then multiplies by (C - i tw) with half_twfix)
+template <typename R, bool CLOVER> TMW_HD void half_Ainv(const Diag<R>& d, int b, const R* Binv, const R* v, R* w) {
+  if (CLOVER) {
+    herm6_mul(Binv, v, w);
+  } else {
+    const R ii = b ? d.inv_im_lo : d.inv_im_up;
+#pragma unroll
+    for (int i = 0; i < 6; i++) {
+      w[2 * i] = d.inv_re * v[2 * i] - ii * v[2 * i + 1];
+      w[2 * i + 1] = d.inv_re * v[2 * i + 1] + ii * v[2 * i];
+    }
+  }
+}
+template <typename R> TMW_HD void half_twfix(const Diag<R>& d, int b, const R* C, const R* v, R* w) {  // w = (C - i tw) v
+  herm6_mul(C, v, w);
+  const R tw = b ? d.tw_lo : d.tw_up;
+#pragma unroll
+  for (int i = 0; i < 6; i++) {
+    w[2 * i] += tw * v[2 * i + 1];
+    w[2 * i + 1] -= tw * v[2 * i];
+  }
+}
+
+// The stencil at one site for NR right-hand sides: on return acc[j] holds the output spinor of column slot j.
+// red[j] = {Re, Im <out, aux>, <out, out>} when WANT_RED2 (EPI >= 2), accumulated chirality by chirality.
+template <typename R, int NG, int EPI, bool CLOVER, int NR>
+__device__ __forceinline__ void dslash_site(const DslashArgs<R>& a, const Site& s, const int64_t (&coff)[NR], R (&acc)[NR][24], R (&red2)[NR][3]) {
+  typedef typename Vec16<R>::T V;
+  const Nbr n = neighbours(a.g, a.par, s);
+  const int cb = s.cb;
+#pragma unroll
+  for (int j = 0; j < NR; j++)
+#pragma unroll
+    for (int i = 0; i < 24; i++) acc[j][i] = (R)0;
+  hop_pair<R, NG, 0, NR>(a, n, cb, coff, acc);
+  hop_pair<R, NG, 1, NR>(a, n, cb, coff, acc);
+  hop_pair<R, NG, 2, NR>(a, n, cb, coff, acc);
+  hop_pair<R, NG, 3, NR>(a, n, cb, coff, acc);
+  const int64_t Vh = a.g.Vh;
+#pragma unroll
+  for (int j = 0; j < NR; j++) {
+#pragma unroll
+    for (int i = 0; i < 24; i++) acc[j][i] *= a.coef;
+    red2[j][0] = red2[j][1] = red2[j][2] = (R)0;
+  }
+  if (EPI == EPI_HOP) return;
+  const int HP = Planes<R, 12>::N;  // planes of one chirality of a spinor
+#pragma unroll
+  for (int b = 0; b < 2; b++) {
+    R B[CLOVER ? 36 : 1];
+    if (EPI == EPI_AINV_HOP || EPI == EPI_AINV_XPAY) load_block<R, CLOVER>(a.d.cinv[a.par], b, Vh, cb, B);
+    else if (EPI == EPI_A_XPAY) load_block<R, CLOVER>(a.d.c[a.par], b, Vh, cb, B);
+#pragma unroll
+    for (int j = 0; j < NR; j++) {
+      R* o = acc[j] + 12 * b;
+      R ax[12], w[12];
+      if (EPI >= 2) load_reals<12>((const V*)a.aux + coff[j] + (int64_t)b * HP * Vh, Vh, cb, ax);
+      if (EPI == EPI_AINV_HOP) {
+        half_Ainv<R, CLOVER>(a.d, b, B, o, w);
+#pragma unroll
+        for (int i = 0; i < 12; i++) o[i] = w[i];
+      } else if (EPI == EPI_A_XPAY) {
+        half_A<R, CLOVER>(a.d, b, B, ax, w);
+#pragma unroll
+        for (int i = 0; i < 12; i++) o[i] += w[i];
+      } else if (EPI == EPI_XPAY) {
+#pragma unroll
+        for (int i = 0; i < 12; i++) o[i] += ax[i];
+      } else {
+#pragma unroll
+        for (int i = 0; i < 12; i++) ax[i] += o[i];
+        half_Ainv<R, CLOVER>(a.d, b, B, ax, w);
+#pragma unroll
+        for (int i = 0; i < 12; i++) o[i] = w[i];
+      }
+      if (EPI == EPI_A_XPAY || EPI == EPI_XPAY) {
+#pragma unroll
+        for (int i = 0; i < 6; i++) {  // conj(o) * ax, |o|^2
+          red2[j][0] += o[2 * i] * ax[2 * i] + o[2 * i + 1] * ax[2 * i + 1];
+          red2[j][1] += o[2 * i] * ax[2 * i + 1] - o[2 * i + 1] * ax[2 * i];
+          red2[j][2] += o[2 * i] * o[2 * i] + o[2 * i + 1] * o[2 * i + 1];
+        }
+      }
+    }
+    if (CLOVER && (EPI == EPI_AINV_HOP || EPI == EPI_AINV_XPAY)) {
+      if (a.d.twisted_clover) {  // (C + i tw)^{-1} = (C - i tw)(C^2 + tw^2)^{-1}: second factor, same registers
+        load_block<R, CLOVER>(a.d.c[a.par], b, Vh, cb, B);
+#pragma unroll
+        for (int j = 0; j < NR; j++) {
+          R* o = acc[j] + 12 * b;
+          R w[12];
+          half_twfix<R>(a.d, b, B, o, w);
+#pragma unroll
+          for (int i = 0; i < 12; i++) o[i] = w[i];
+        }
+      }
+    }
   }
 }
 

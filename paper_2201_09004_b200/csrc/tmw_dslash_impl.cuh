@@ -28,43 +28,59 @@ template <int NV, int BLOCK> __device__ __forceinline__ void block_reduce_atomic
   }
 }
 
-template <typename R, int NG, int EPI, bool CLOVER, int BLOCK, int MINB>
+template <typename R, int NG, int EPI, bool CLOVER, int NR, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<R> a) {
-  const int cb = blockIdx.x * BLOCK + threadIdx.x;
-  const bool active = cb < a.g.Vh;
-  R o[24], ax[24];
+  typedef typename Vec16<R>::T V;
+  // blockIdx.x = group + ngroups * site block: the CTAs that share the links of a site block are launched together
+  int sblock = blockIdx.x, grp = 0;
+  if (a.ngroups > 1) {
+    sblock = blockIdx.x / a.ngroups;
+    grp = blockIdx.x - sblock * a.ngroups;
+  }
+  Site s;
+  const bool active = thread_site<BLOCK>(a.g, sblock, s);
+  int64_t coff[NR];
+  int colj[NR];
+  bool valid[NR];
+#pragma unroll
+  for (int j = 0; j < NR; j++) {
+    const int slot = grp * NR + j;
+    valid[j] = slot < a.ncol;  // a ragged last group recomputes the last column and drops the result
+    colj[j] = a.col[valid[j] ? slot : a.ncol - 1];
+    coff[j] = (int64_t)colj[j] * a.cstride;
+  }
+  R o[NR][24], r2[NR][3];
   if (active) {
-    dslash_site<R, NG, EPI, CLOVER>(a, cb, o, ax);
-    store_reals_s<24>(a.out, a.g.Vh, cb, o);
+    dslash_site<R, NG, EPI, CLOVER, NR>(a, s, coff, o, r2);
+#pragma unroll
+    for (int j = 0; j < NR; j++)
+      if (valid[j]) store_reals_s<24>((V*)a.out + coff[j], a.g.Vh, s.cb, o[j]);
   }
   if (a.red_mode != 0) {  // uniform across the grid
-    double v[3] = {0, 0, 0};
-    if (active) {
-      if (a.red_mode == 1) {
-        R d[24];
-        load_reals<24>(a.dotv, a.g.Vh, cb, d);
-        R re = 0, im = 0;
 #pragma unroll
-        for (int i = 0; i < 12; i++) {  // conj(d) * o
-          re += d[2 * i] * o[2 * i] + d[2 * i + 1] * o[2 * i + 1];
-          im += d[2 * i] * o[2 * i + 1] - d[2 * i + 1] * o[2 * i];
-        }
-        v[0] = re;
-        v[1] = im;
-      } else if (EPI >= 2) {
-        R re = 0, im = 0, nn = 0;
+    for (int j = 0; j < NR; j++) {
+      double v[3] = {0, 0, 0};
+      if (active && valid[j]) {
+        if (a.red_mode == 1) {
+          R d[24];
+          load_reals<24>((const V*)a.dotv + coff[j], a.g.Vh, s.cb, d);
+          R re = 0, im = 0;
 #pragma unroll
-        for (int i = 0; i < 12; i++) {  // conj(o) * ax, |o|^2
-          re += o[2 * i] * ax[2 * i] + o[2 * i + 1] * ax[2 * i + 1];
-          im += o[2 * i] * ax[2 * i + 1] - o[2 * i + 1] * ax[2 * i];
-          nn += o[2 * i] * o[2 * i] + o[2 * i + 1] * o[2 * i + 1];
+          for (int i = 0; i < 12; i++) {  // conj(d) * o
+            re += d[2 * i] * o[j][2 * i] + d[2 * i + 1] * o[j][2 * i + 1];
+            im += d[2 * i] * o[j][2 * i + 1] - d[2 * i + 1] * o[j][2 * i];
+          }
+          v[0] = re;
+          v[1] = im;
+        } else {
+          v[0] = r2[j][0];
+          v[1] = r2[j][1];
+          v[2] = r2[j][2];
         }
-        v[0] = re;
-        v[1] = im;
-        v[2] = nn;
       }
+      if (j > 0) __syncthreads();  // the shared scratch of block_reduce_atomic is reused
+      block_reduce_atomic<3, BLOCK>(v, a.red + (int64_t)colj[j] * a.red_stride);
     }
-    block_reduce_atomic<3, BLOCK>(v, a.red);
   }
 }
 
@@ -78,24 +94,32 @@ template <typename R, bool CLOVER, bool INV, int BLOCK> __global__ void __launch
   store_reals<24>(out, g.Vh, cb, o);
 }
 
-template <typename R> struct Tune;
-template <> struct Tune<float> { enum { BLOCK = 128, MINB = 4 }; };
-template <> struct Tune<double> { enum { BLOCK = 128, MINB = 2 }; };
+// launch shape per precision and columns per thread (128 threads x 4 CTAs/SM = 128 registers for the
+// single-column fp32 kernel; more columns per thread need the accumulators of all of them in registers)
+template <typename R, int NR> struct Tune;
+template <> struct Tune<float, 1> { enum { BLOCK = 128, MINB = 4 }; };
+template <> struct Tune<float, 2> { enum { BLOCK = 128, MINB = 3 }; };
+template <> struct Tune<float, 3> { enum { BLOCK = 128, MINB = 3 }; };
+template <> struct Tune<float, 4> { enum { BLOCK = 128, MINB = 2 }; };
+template <> struct Tune<double, 1> { enum { BLOCK = 128, MINB = 2 }; };
 
-template <typename R, int NG, int EPI, bool CLOVER> static cudaError_t launch_one(const DslashArgs<R>& a, cudaStream_t s) {
-  const int B = Tune<R>::BLOCK;
-  const int grid = (a.g.Vh + B - 1) / B;
-  dslash_kernel<R, NG, EPI, CLOVER, B, Tune<R>::MINB><<<grid, B, 0, s>>>(a);
+template <typename R, int NG, int EPI, bool CLOVER, int NR> static cudaError_t launch_one(DslashArgs<R> a, cudaStream_t s) {
+  const int B = Tune<R, NR>::BLOCK;
+  a.ngroups = (a.ncol + NR - 1) / NR;
+  dim3 grid;
+  if (a.g.tiled) grid = dim3((unsigned)(a.g.ntx * a.g.nty * a.ngroups), (unsigned)(a.g.L >> a.g.lz), (unsigned)(a.g.T >> a.g.lt));
+  else grid = dim3((unsigned)(((a.g.Vh + B - 1) / B) * a.ngroups), 1, 1);
+  dslash_kernel<R, NG, EPI, CLOVER, NR, B, Tune<R, NR>::MINB><<<grid, B, 0, s>>>(a);
   return cudaGetLastError();
 }
 
-template <typename R, int NG> static cudaError_t launch_epi(const DslashArgs<R>& a, int epi, bool clover, cudaStream_t s) {
+template <typename R, int NG, int NR> static cudaError_t launch_epi(const DslashArgs<R>& a, int epi, bool clover, cudaStream_t s) {
   switch (epi) {
-    case EPI_HOP: return launch_one<R, NG, EPI_HOP, false>(a, s);
-    case EPI_AINV_HOP: return clover ? launch_one<R, NG, EPI_AINV_HOP, true>(a, s) : launch_one<R, NG, EPI_AINV_HOP, false>(a, s);
-    case EPI_A_XPAY: return clover ? launch_one<R, NG, EPI_A_XPAY, true>(a, s) : launch_one<R, NG, EPI_A_XPAY, false>(a, s);
-    case EPI_XPAY: return launch_one<R, NG, EPI_XPAY, false>(a, s);
-    case EPI_AINV_XPAY: return clover ? launch_one<R, NG, EPI_AINV_XPAY, true>(a, s) : launch_one<R, NG, EPI_AINV_XPAY, false>(a, s);
+    case EPI_HOP: return launch_one<R, NG, EPI_HOP, false, NR>(a, s);
+    case EPI_AINV_HOP: return clover ? launch_one<R, NG, EPI_AINV_HOP, true, NR>(a, s) : launch_one<R, NG, EPI_AINV_HOP, false, NR>(a, s);
+    case EPI_A_XPAY: return clover ? launch_one<R, NG, EPI_A_XPAY, true, NR>(a, s) : launch_one<R, NG, EPI_A_XPAY, false, NR>(a, s);
+    case EPI_XPAY: return launch_one<R, NG, EPI_XPAY, false, NR>(a, s);
+    case EPI_AINV_XPAY: return clover ? launch_one<R, NG, EPI_AINV_XPAY, true, NR>(a, s) : launch_one<R, NG, EPI_AINV_XPAY, false, NR>(a, s);
   }
   return cudaErrorInvalidValue;
 }

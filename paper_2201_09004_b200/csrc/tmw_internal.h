@@ -5,9 +5,10 @@
 namespace tmw {
 
 // ---- stencil (tmw_dslash_f32.cu / tmw_dslash_f64.cu) ----
-// ng = stored reals per link (12 | 18), epi = EPI_*, clover = the diagonal part has clover blocks
-cudaError_t launch_dslash(const DslashArgs<float>& a, int ng, int epi, bool clover, cudaStream_t s);
-cudaError_t launch_dslash(const DslashArgs<double>& a, int ng, int epi, bool clover, cudaStream_t s);
+// ng = stored reals per link (12 | 18), epi = EPI_*, clover = the diagonal part has clover blocks,
+// nr = right-hand-side columns per thread (fp32: 1..4; fp64: always 1)
+cudaError_t launch_dslash(const DslashArgs<float>& a, int ng, int epi, bool clover, int nr, cudaStream_t s);
+cudaError_t launch_dslash(const DslashArgs<double>& a, int ng, int epi, bool clover, int nr, cudaStream_t s);
 // out = A in (inverse = 0) or A^{-1} in (inverse = 1) on parity par, site-local
 cudaError_t launch_diag(const Diag<float>& d, const Geom& g, int par, bool clover, int inverse, const void* in, void* out, cudaStream_t s);
 cudaError_t launch_diag(const Diag<double>& d, const Geom& g, int par, bool clover, int inverse, const void* in, void* out, cudaStream_t s);
@@ -44,23 +45,30 @@ struct Scalars {
   double nrm;         // generic norm^2 accumulator
   double pad;
 };
-// sc phase kernels (single thread): see tmw_blas.cu
-cudaError_t launch_sc_begin_iter(Scalars* sc, cudaStream_t s);  // beta = (rho/rho_old)(alpha/omega); zero rhat_v, ts, tt
-cudaError_t launch_sc_alpha(Scalars* sc, cudaStream_t s);       // alpha = rho / rhat_v
-cudaError_t launch_sc_omega(Scalars* sc, cudaStream_t s);       // omega = ts/tt; rho_old = rho; zero rho, rr
-// n = number of 16-byte vectors in each array
-template <typename R> cudaError_t launch_update_p(int64_t n, void* p, const void* r, const void* v, const Scalars* sc, cudaStream_t s);      // p = r + beta (p - omega v)
-template <typename R> cudaError_t launch_update_s(int64_t n, void* sv, const void* r, const void* v, const Scalars* sc, cudaStream_t s);     // s = r - alpha v
-template <typename R> cudaError_t launch_update_xr(int64_t n, void* x, void* r, const void* p, const void* sv, const void* t, const void* rhat, Scalars* sc, cudaStream_t s);  // x += alpha p + omega s; r = s - omega t; rho += <rhat,r>; rr += <r,r>
-// out[0..1] += <a,b>, out[2] += <b,b> (a may be null: only the norm)
-template <typename R> cudaError_t launch_dot_norm(int64_t n, const void* a, const void* b, double* out, cudaStream_t s);
+// The right-hand-side columns a batched launch works on: slot j -> column col[j].
+struct ColMap {
+  int n;
+  unsigned char col[MAXCOL];
+};
+// Every launcher below is batched: column c of a vector starts c * (column length) after the base pointer and
+// uses the scalar block sc[c]; reductions into a plain double* go to out + 4*c.
+// sc phase kernels (one thread per column): see tmw_blas.cu
+cudaError_t launch_sc_begin_iter(Scalars* sc, const ColMap& cm, cudaStream_t s);  // beta = (rho/rho_old)(alpha/omega); zero rhat_v, ts, tt
+cudaError_t launch_sc_alpha(Scalars* sc, const ColMap& cm, cudaStream_t s);       // alpha = rho / rhat_v
+cudaError_t launch_sc_omega(Scalars* sc, const ColMap& cm, cudaStream_t s);       // omega = ts/tt; rho_old = rho; zero rho, rr
+// n = number of 16-byte vectors in one column of each array
+template <typename R> cudaError_t launch_update_p(int64_t n, void* p, const void* r, const void* v, const Scalars* sc, const ColMap& cm, cudaStream_t s);      // p = r + beta (p - omega v)
+template <typename R> cudaError_t launch_update_s(int64_t n, void* sv, const void* r, const void* v, const Scalars* sc, const ColMap& cm, cudaStream_t s);     // s = r - alpha v
+template <typename R> cudaError_t launch_update_xr(int64_t n, void* x, void* r, const void* p, const void* sv, const void* t, const void* rhat, Scalars* sc, const ColMap& cm, cudaStream_t s);  // x += alpha p + omega s; r = s - omega t; rho += <rhat,r>; rr += <r,r>
+// out[4c+0..1] += <a,b>, out[4c+2] += <b,b> (a may be null: only the norm)
+template <typename R> cudaError_t launch_dot_norm(int64_t n, const void* a, const void* b, double* out, const ColMap& cm, cudaStream_t s);
 // fp64 helpers for the reliable update
-template <typename R> cudaError_t launch_acc_y(int64_t n64, void* y64, void* x, cudaStream_t s);  // y += x; x = 0   (n64 = number of double2 vectors)
+template <typename R> cudaError_t launch_acc_y(int64_t n64, void* y64, void* x, const ColMap& cm, cudaStream_t s);  // y += x; x = 0   (n64 = number of double2 vectors per column)
 // r64 = b64 - w64; r = (R) r64; rho += <rhat, r>; rr += <r64, r64>
-template <typename R> cudaError_t launch_resid_convert(int64_t n64, const void* b64, const void* w64, void* r64, void* r, const void* rhat, Scalars* sc, cudaStream_t s);
-// dst(R) = src(double), n64 double2 vectors
-template <typename R> cudaError_t launch_convert(int64_t n64, const void* src64, void* dst, cudaStream_t s);
-// d = a - b (fp64, n64 double2 vectors), out[2] += <d,d>
-cudaError_t launch_sub_norm(int64_t n64, const void* a, const void* b, void* d, double* out, cudaStream_t s);
+template <typename R> cudaError_t launch_resid_convert(int64_t n64, const void* b64, const void* w64, void* r64, void* r, const void* rhat, Scalars* sc, const ColMap& cm, cudaStream_t s);
+// dst(R) = src(double), n64 double2 vectors per column
+template <typename R> cudaError_t launch_convert(int64_t n64, const void* src64, void* dst, const ColMap& cm, cudaStream_t s);
+// d = a - b (fp64, n64 double2 vectors per column), out[4c+2] += <d,d>
+cudaError_t launch_sub_norm(int64_t n64, const void* a, const void* b, void* d, double* out, const ColMap& cm, cudaStream_t s);
 
 }  // namespace tmw

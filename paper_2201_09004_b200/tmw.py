@@ -24,7 +24,8 @@ D, DDAG = 0, 1
 FULL, EVEN, ODD = 0, 1, 2
 F32, F64 = 0, 1
 
-EXPORTS = ["tmw_create", "tmw_apply", "tmw_apply_schur", "tmw_solve", "tmw_spinor_bytes", "tmw_pack", "tmw_unpack",
+EXPORTS = ["tmw_create", "tmw_apply", "tmw_apply_schur", "tmw_solve", "tmw_apply_multi", "tmw_apply_schur_multi",
+           "tmw_solve_multi", "tmw_spinor_bytes", "tmw_pack", "tmw_unpack",
            "tmw_get_clover", "tmw_set_location", "tmw_launch_count", "tmw_destroy", "tmw_last_error"]
 
 
@@ -70,6 +71,12 @@ def load():
     lib.tmw_apply_schur.restype = I
     lib.tmw_solve.argtypes = [P, P, P, DBL, ctypes.POINTER(tmw_solve_info)]
     lib.tmw_solve.restype = I
+    lib.tmw_apply_multi.argtypes = [P, I, I, I, I, P, P]
+    lib.tmw_apply_multi.restype = I
+    lib.tmw_apply_schur_multi.argtypes = [P, I, I, I, P, P]
+    lib.tmw_apply_schur_multi.restype = I
+    lib.tmw_solve_multi.argtypes = [P, I, P, P, DBL, ctypes.POINTER(tmw_solve_info)]
+    lib.tmw_solve_multi.restype = I
     lib.tmw_spinor_bytes.argtypes = [P, I]
     lib.tmw_spinor_bytes.restype = LL
     lib.tmw_pack.argtypes = [P, I, I, P, P]
@@ -140,6 +147,19 @@ class Context:
                          allow=(ENOCONV,) if allow_noconv else ())
         return dict(status=rc, iters=info.iters, reliable_updates=info.reliable_updates, restarts=info.restarts,
                     iter_resid=info.iter_resid, true_resid=info.true_resid, device_ms=info.device_ms)
+
+    def apply_multi(self, op: int, parity: int, prec: int, nrhs: int, src, dst):
+        self._check(self._lib.tmw_apply_multi(self._h, op, parity, prec, nrhs, _ptr(src), _ptr(dst)))
+
+    def apply_schur_multi(self, op: int, prec: int, nrhs: int, src, dst):
+        self._check(self._lib.tmw_apply_schur_multi(self._h, op, prec, nrhs, _ptr(src), _ptr(dst)))
+
+    def solve_multi(self, nrhs: int, b, x, tol: float, allow_noconv: bool = False) -> list:
+        infos = (tmw_solve_info * nrhs)()
+        rc = self._check(self._lib.tmw_solve_multi(self._h, nrhs, _ptr(b), _ptr(x), float(tol), infos),
+                         allow=(ENOCONV,) if allow_noconv else ())
+        return [dict(status=rc, iters=i.iters, reliable_updates=i.reliable_updates, restarts=i.restarts,
+                     iter_resid=i.iter_resid, true_resid=i.true_resid, device_ms=i.device_ms) for i in infos]
 
     def spinor_bytes(self, prec: int) -> int:
         return int(self._lib.tmw_spinor_bytes(self._h, prec))

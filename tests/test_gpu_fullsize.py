@@ -211,6 +211,34 @@ def test_fullsize_config3_twelve_columns(tmw):
     torch.cuda.empty_cache()
 
 
+def test_fullsize_config3_twelve_columns_batched(tmw):
+    """configs[3] again, the 12 columns in ONE tmw_solve_multi call: every column checked through the
+    oracle's D like the one-after-another solves above, and against the single-column solve of the same library."""
+    cfg, U = config_fields(3)
+    L, T, m, c_sw = cfg["L"], cfg["T"], complex(*cfg["m"]), cfg["c_sw"]
+    origin_nb = [lex(L, *c) for c in [(0, 0, 0, 0), (1, 0, 0, 0), (L - 1, 0, 0, 0), (0, 1, 0, 0), (0, L - 1, 0, 0),
+                                      (0, 0, 1, 0), (0, 0, L - 1, 0), (0, 0, 0, 1), (0, 0, 0, T - 1)]]
+    det = np.concatenate([boundary_sites(L, T), np.array(origin_nb, dtype=np.int64)])
+    rnd = random_sites(L, T, 4000, seed=33)
+    dU = torch.from_numpy(U).cuda()
+    with tmw.Context(L, T, dU, m, c_sw) as ctx:
+        del dU
+        b = torch.zeros((12, T, L, L, L, 4, 3), dtype=torch.complex128, device="cuda")
+        for c in range(12):
+            b[c, 0, 0, 0, 0, c // 3, c % 3] = 1.0
+        x = torch.empty_like(b)
+        infos = ctx.solve_multi(12, b, x, 1e-10)
+        for c in range(12):
+            assert infos[c]["true_resid"] <= 1e-10 and infos[c]["iters"] > 0
+            mx, est = sampled_residual(U, synth.point_source(L, T, c // 3, c % 3), x[c].cpu().numpy(), m, c_sw, rnd, det)
+            assert mx <= 1e-10 and est <= EST_TOL, (c, mx, est)
+        x1 = torch.empty_like(x[0])
+        ctx.solve(b[5], x1, 1e-10)
+        assert float(torch.linalg.vector_norm(x1 - x[5]) / torch.linalg.vector_norm(x1)) <= 1e-8
+        del b, x, x1
+    torch.cuda.empty_cache()
+
+
 def test_fullsize_config4_solve(tmw):
     cfg, U = config_fields(4)
     L, T, m, c_sw = cfg["L"], cfg["T"], complex(*cfg["m"]), cfg["c_sw"]

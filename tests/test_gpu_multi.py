@@ -1,0 +1,186 @@
+"""Parity of the multi-right-hand-side calls (tmw_apply_multi / tmw_apply_schur_multi / tmw_solve_multi, SURVEY §8(f1):
+the "12 columns" of PAPER.md:78) with the fp64 CPU oracle, column by column, on identical seeded inputs.
+
+The oracle has no multi-column notion: each column is an independent application / solve of the same operator, so the
+expected values are the single-column oracle results. Tolerances as in test_gpu_parity.py.
+"""
+import os
+
+import numpy as np
+import pytest
+
+import helpers as H
+import oracle
+from paper_2201_09004_b200 import synth
+from test_gpu_parity import TOL32, TOL64, check_solution, dev, mask_parity, site_matrices
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def tmw():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2201_09004_b200 import tmw as m
+    m.load()
+    return m
+
+
+@pytest.fixture
+def nr_env():
+    """TMW_NR (columns per thread of the fp32 stencil) and TMW_TILE (thread -> site mapping) are read at tmw_create;
+    restore them afterwards"""
+    old = {k: os.environ.get(k) for k in ("TMW_NR", "TMW_TILE")}
+    yield
+    for k, v in old.items():
+        if v is None:
+            os.environ.pop(k, None)
+        else:
+            os.environ[k] = v
+
+
+def columns(L, T, n):
+    """n dense spinors with different seeds (Gaussian, every third one Z2)"""
+    return [synth.z2_source(L, T, seed=100 + c) if c % 3 == 2 else synth.gaussian_spinor(L, T, seed=10 + c) for c in range(n)]
+
+
+def pack_multi(ctx, tmw, cols, par, prec):
+    nb = ctx.spinor_bytes(prec)
+    buf = torch.empty(nb * len(cols), dtype=torch.uint8, device="cuda")
+    for c, psi in enumerate(cols):
+        ctx.pack(prec, tmw.ODD if par else tmw.EVEN, dev(psi), buf[c * nb:(c + 1) * nb])
+    torch.cuda.synchronize()
+    return buf
+
+
+def unpack_multi(ctx, tmw, buf, n, par, prec, L, T):
+    nb = ctx.spinor_bytes(prec)
+    out = []
+    for c in range(n):
+        o = torch.zeros((T, L, L, L, 4, 3), dtype=torch.complex128, device="cuda")
+        ctx.unpack(prec, tmw.ODD if par else tmw.EVEN, buf[c * nb:(c + 1) * nb], o)
+        out.append(o)
+    torch.cuda.synchronize()
+    return [o.cpu().numpy() for o in out]
+
+
+@pytest.mark.parametrize("nr", [1, 2, 3, 4])
+@pytest.mark.parametrize("L,T,nrhs,tile", [(8, 16, 5, "auto"), (8, 16, 5, None), (6, 4, 12, None), (4, 8, 7, "auto"), (4, 8, 3, "1,2,1,3")])
+def test_hopping_multi_vs_oracle(tmw, nr_env, L, T, nrhs, tile, nr):
+    os.environ["TMW_NR"] = str(nr)
+    if tile:
+        os.environ["TMW_TILE"] = tile  # 4-D tiles of 128 sites instead of 128 consecutive checkerboard indices
+    U = synth.gauge_field(L, T, 0.4, seed=1)
+    cols = columns(L, T, nrhs)
+    with tmw.Context(L, T, dev(U), 0.1) as ctx:
+        for prec, tol in ((tmw.F32, TOL32), (tmw.F64, TOL64)):
+            if prec == tmw.F64 and nr > 1:
+                continue  # the fp64 stencil always takes one column per thread
+            for op in (tmw.D, tmw.DDAG):
+                for par in (0, 1):
+                    inp = pack_multi(ctx, tmw, cols, 1 - par, prec)
+                    out = torch.full_like(inp, 0x7f)
+                    ctx.apply_multi(op, tmw.ODD if par else tmw.EVEN, prec, nrhs, inp, out)
+                    got = unpack_multi(ctx, tmw, out, nrhs, par, prec, L, T)
+                    for c in range(nrhs):
+                        ref = mask_parity(oracle.apply(U, mask_parity(cols[c], 1 - par), 0.1, dagger=(op == tmw.DDAG)), par)
+                        site, glob = H.per_site_rel_err(got[c], ref)
+                        assert site <= tol, (prec, op, par, c, site, glob)
+
+
+@pytest.mark.parametrize("nr", [2, 3, 4])
+@pytest.mark.parametrize("case", [
+    dict(L=8, T=4, eps=0.4, m=-0.0695 + 0.0j, c_sw=1.0509, nrhs=5),
+    dict(L=4, T=6, eps=0.3, m=-0.044 + 0.2j, c_sw=1.0349, nrhs=4),   # twisted clover: two-factor inverse
+    dict(L=6, T=4, eps=0.4, m=-0.0695 + 0.01j, c_sw=0.0, nrhs=12),
+])
+def test_schur_multi_vs_oracle(tmw, nr_env, case, nr):
+    os.environ["TMW_NR"] = str(nr)
+    if nr == 3:
+        os.environ["TMW_TILE"] = "auto"
+    L, T, m, c_sw, nrhs = case["L"], case["T"], case["m"], case["c_sw"], case["nrhs"]
+    V = L ** 3 * T
+    U = synth.gauge_field(L, T, case["eps"], seed=1)
+    cols = columns(L, T, nrhs)
+    F = oracle.field_strength(U) if c_sw != 0 else None
+    ev, od = H.parity_sites(L, T, 0), H.parity_sites(L, T, 1)
+    A = site_matrices(U, m, c_sw)
+    refs = []
+    for psi in cols:
+        Dx = oracle.apply(U, mask_parity(psi, 1), m, c_sw, F=F).reshape(V, 12)
+        t_e = np.zeros((V, 12), dtype=np.complex128)
+        t_e[ev] = np.linalg.solve(A[ev], Dx[ev][..., None])[..., 0]
+        Dt = oracle.apply(U, t_e.reshape(psi.shape), m, c_sw, F=F).reshape(V, 12)
+        ref = np.zeros((V, 12), dtype=np.complex128)
+        ref[od] = Dx[od] - Dt[od]
+        refs.append(ref.reshape(psi.shape))
+    with tmw.Context(L, T, dev(U), m, c_sw) as ctx:
+        for prec, tol in ((tmw.F32, TOL32), (tmw.F64, TOL64)):
+            inp = pack_multi(ctx, tmw, cols, 1, prec)
+            out = torch.full_like(inp, 0x7f)
+            ctx.apply_schur_multi(tmw.D, prec, nrhs, inp, out)
+            got = unpack_multi(ctx, tmw, out, nrhs, 1, prec, L, T)
+            for c in range(nrhs):
+                site, glob = H.per_site_rel_err(got[c], refs[c])
+                assert site <= tol, (prec, c, site, glob)
+
+
+@pytest.mark.parametrize("precision", ["mixed", "double"])
+def test_solve_multi_12_columns_vs_oracle(tmw, precision):
+    """configs[3] shape of work on a small lattice: the 12 point sources of a propagator (C13) in ONE call."""
+    L, T, m, c_sw = 4, 8, -0.0514 + 0.0j, 1.0424
+    U = synth.gauge_field(L, T, 0.35, seed=1)
+    F = oracle.field_strength(U)
+    b = np.stack([synth.point_source(L, T, c // 3, c % 3) for c in range(12)])
+    with tmw.Context(L, T, dev(U), m, c_sw, precision=tmw.MIXED if precision == "mixed" else tmw.DOUBLE) as ctx:
+        x = torch.empty(b.shape, dtype=torch.complex128, device="cuda")
+        infos = ctx.solve_multi(12, dev(b), x, 1e-10)
+        x = x.cpu().numpy()
+        for c in range(12):
+            assert infos[c]["true_resid"] <= 1e-10 and infos[c]["iters"] > 0
+            x_ref, _ = oracle.bicgstab(U, b[c], m, c_sw, tol=1e-12, F=F)
+            check_solution(U, b[c], x[c], m, c_sw, x_ref, F=F)
+
+
+def test_solve_multi_mixed_columns_host(tmw):
+    """columns of different kind (point, Z2, Gaussian, zero, a scaled copy) converge at different iterations: columns
+    drop out of the launches one by one; HOST pointers; twisted mass without clover (configs[1] parameters)."""
+    L, T, m = 8, 4, -0.0695 + 0.01j
+    U = synth.gauge_field(L, T, 0.4, seed=1)
+    g = synth.gaussian_spinor(L, T, 3)
+    b = np.stack([synth.point_source(L, T, 0, 0), synth.z2_source(L, T, 2), g, np.zeros_like(g), 1e-3 * g,
+                  synth.point_source(L, T, 3, 2), synth.gaussian_spinor(L, T, 4)])
+    n = b.shape[0]
+    with tmw.Context(L, T, U, m, 0.0, location=tmw.HOST) as ctx:
+        x = np.full(b.shape, 7.0 + 0j)
+        infos = ctx.solve_multi(n, b, x, 1e-10)
+        assert infos[3]["iters"] == 0 and np.count_nonzero(x[3]) == 0
+        for c in range(n):
+            if c == 3:
+                continue
+            assert infos[c]["true_resid"] <= 1e-10
+            x_ref, _ = oracle.bicgstab(U, b[c], m, 0.0, tol=1e-12)
+            check_solution(U, b[c], x[c], m, 0.0, x_ref)
+        # a single solve afterwards (smaller batch than the workspace) gives the same answer as column 0
+        x0 = np.empty_like(b[0])
+        ctx.solve(b[0], x0, 1e-10)
+        assert np.linalg.norm((x0 - x[0]).ravel()) <= 1e-9 * np.linalg.norm(x[0].ravel())
+
+
+def test_solve_multi_edge_cases(tmw):
+    L, T = 4, 4
+    U = synth.gauge_field(L, T, 0.3, seed=1)
+    b = np.stack([synth.gaussian_spinor(L, T, 3), synth.gaussian_spinor(L, T, 5)])
+    with tmw.Context(L, T, dev(U), 0.1, max_iter=2) as ctx:
+        x = torch.empty(b.shape, dtype=torch.complex128, device="cuda")
+        infos = ctx.solve_multi(2, dev(b), x, 1e-10, allow_noconv=True)
+        for c in range(2):
+            assert infos[c]["status"] == tmw.ENOCONV and infos[c]["iters"] == 2 and 1e-10 < infos[c]["true_resid"] < 1.0
+            r = b[c] - oracle.apply(U, x[c].cpu().numpy(), 0.1)
+            assert abs(np.linalg.norm(r.ravel()) / np.linalg.norm(b[c].ravel()) - infos[c]["true_resid"]) < 1e-9
+        for bad in (0, 17):
+            with pytest.raises(tmw.TmwError) as e:
+                ctx.solve_multi(bad, dev(b), x, 1e-10)
+            assert e.value.code == tmw.EINVAL
