@@ -45,6 +45,8 @@ def parse_args():
     ap.add_argument("--e2e-steps", type=int, default=2, help="timed host-buffer steps for the e2e figure")
     ap.add_argument("--tol", type=float, default=1e-10)
     ap.add_argument("--cpu-sites", type=int, default=0, help="oracle sample size in sites (0: sized for ~15 s)")
+    ap.add_argument("--multi-rhs", type=int, default=3,
+                    help="columns of the extra tmw_solve_multi / tmw_apply_multi leg (0 or 1: skip); 3 fit at 48^3 x 144")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--skip-solve", action="store_true",
@@ -126,7 +128,7 @@ def shared_gauge(cfg, rank: int, world: int, barrier):
     return np.memmap(path, dtype=np.complex128, mode="r", shape=shape), path
 
 
-def time_oracle_sample(U, psi, cfg, n_sites: int):
+def time_oracle_sample(U, psi, cfg, n_sites: int, passes: int = 1):
     """The oracle as it stands on a bounded sample of the workload: (D psi)(x) with the hopping + mass terms of Eq. (2)
     at n_sites sites spread evenly over the lattice (its per-site routine; c_sw = 0 so that one site = the 8 hops
     the GPU metric counts). Returns (seconds, sites, threads)."""
@@ -138,8 +140,9 @@ def time_oracle_sample(U, psi, cfg, n_sites: int):
     m = complex(*cfg["m"])
     oracle.apply_sites(U, psi, sites[:1024], m, 0.0)  # page in
     t0 = time.perf_counter()
-    oracle.apply_sites(U, psi, sites, m, 0.0)
-    return time.perf_counter() - t0, int(sites.size), oracle.num_threads()
+    for _ in range(passes):
+        oracle.apply_sites(U, psi, sites, m, 0.0)
+    return time.perf_counter() - t0, int(sites.size) * passes, oracle.num_threads()
 
 
 def run_reference(args, cfg, rank: int):
@@ -324,17 +327,55 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
                "solve_call": "tmw_solve with HOST pointers: b in (H2D), x out (D2H)", "steps": n_e2e}
         del hb, hx, hpsi
 
+    # ---- several right-hand sides in one call (the "12 columns" of PAPER.md:78): reported beside the
+    # single-column figures, outside the timed step. Columns = as many of this rank's propagator columns as fit. ----
+    multi = None
+    if args.multi_rhs > 1 and not args.skip_solve:
+        n = args.multi_rhs
+        mine = columns.columns_for_rank(rank, world)
+        bm = torch.zeros((n, T, L, L, L, 4, 3), dtype=torch.complex128, device="cuda")
+        for c in range(n):
+            sp, co = columns.spin_colour((mine[0] + c) % columns.N_COLUMNS)
+            bm[c, 0, 0, 0, 0, sp, co] = 1.0
+        xm = torch.empty_like(bm)
+        pm = torch.empty(nb * n, dtype=torch.uint8, device="cuda")
+        pm2 = torch.empty_like(pm)
+        for c in range(n):
+            pm[c * nb:(c + 1) * nb].copy_(pe)
+        m0, m1, m2 = ev(), ev(), ev()
+        for i in range(2):  # first pass untimed (grows the workspaces)
+            barrier()
+            m0.record()
+            minfos = ctx.solve_multi(n, bm, xm, args.tol)
+            m1.record()
+            for _ in range(napply // 2):
+                ctx.apply_multi(tmw.D, tmw.ODD, tmw.F32, n, pm, pm2)
+            m2.record()
+            torch.cuda.synchronize()
+        ms_solve = max_over_ranks(m0.elapsed_time(m1))
+        ms_hop = max_over_ranks(m1.elapsed_time(m2)) / (napply // 2)
+        multi = {"nrhs": n, "solve_ms_per_rhs": ms_solve / n, "solve_iters": [i["iters"] for i in minfos],
+                 "solve_reliable_updates": [i["reliable_updates"] for i in minfos],
+                 "solve_true_resid_max": max(i["true_resid"] for i in minfos),
+                 "dslash_ms_per_rhs": ms_hop / n, "dslash_gflops": FLOP_PER_SITE * float(Vh) * n * world / (ms_hop * 1e-3) / 1e9,
+                 "call": "tmw_solve_multi / tmw_apply_multi, columns resident in HBM"}
+        del bm, xm, pm, pm2
+        torch.cuda.empty_cache()
+
     # ---- the oracle beside it: rank 0, N = 1 only, a bounded sample of the same workload ----
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         n = args.cpu_sites
         if not n:
             dt, ns, _ = time_oracle_sample(U, psi_host, cfg, 100_000)
-            n = int(min(V, max(100_000, 12.0 * ns / dt)))
-        dt, ns, threads = time_oracle_sample(U, psi_host, cfg, n)
+            n = int(max(100_000, 30.0 * ns / dt))  # sized from a cold 100k-site probe: 10-15 s of oracle work once warm
+        passes = max(1, -(-n // V))
+        n = min(n, V)
+        dt, ns, threads = time_oracle_sample(U, psi_host, cfg, n, passes)
         cpu = {"value": FLOP_PER_SITE * ns / dt / 1e9, "unit": "GFLOP/s", "cores": threads, "kind": "oracle",
-               "sample": f"oracle.apply_sites (fp64, hopping + mass of Eq. (2), explicit 4x4 gamma matrices) at {ns} "
-                         f"evenly spaced sites of the same {L}^3x{T} field, {dt:.1f} s", "msites_per_s": ns / dt / 1e6}
+               "sample": f"oracle.apply_sites (fp64, hopping + mass of Eq. (2), explicit 4x4 gamma matrices) at {n} "
+                         f"evenly spaced sites of the same {L}^3x{T} field, {passes} pass(es), {dt:.1f} s",
+               "msites_per_s": ns / dt / 1e6}
 
     ctx.destroy()
     if rank == 0:
@@ -350,7 +391,7 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
                 "dslash_gsites_per_s": sites / (dsl_total_ms * 1e-3) / 1e9, "dslash_ms": dsl_total_ms / (napply * args.steps),
                 "solve_ms": solve_mean_ms, "solve_iters": info["iters"], "solve_reliable_updates": info["reliable_updates"],
                 "solve_true_resid": info["true_resid"], "setup_ms": setup_ms,
-                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
+                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "multi_rhs": multi, "gpu_launches": int(launches),
                 "clocks": sampler.summary()}
         print(json.dumps(line), flush=True)
     if dist is not None:

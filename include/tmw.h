@@ -68,6 +68,7 @@ typedef struct { double re, im; } tmw_complex;
 
 #define TMW_D 0
 #define TMW_DDAG 1
+#define TMW_G5D 2 /* gamma5 D (= H_w when m is real): gamma5 fused into the stencil's epilogue */
 
 #define TMW_FULL 0
 #define TMW_EVEN 1
@@ -82,7 +83,7 @@ typedef struct {
   int reconstruct;  /* fp32 gauge storage: 12 (default; third row rebuilt in-kernel, links must be SU(3)) | 18 */
   int mass_reading; /* TMW_TWIST_GAMMA5 (default) | TMW_MASS_SCALAR */
   int max_iter;     /* BiCGStab iterations; 0 -> 10000 */
-  double delta;     /* reliable-update threshold: fp64 true residual when |r| < delta * max|r|; 0 -> 1e-3 */
+  double delta;     /* reliable-update threshold: fp64 true residual when |r| < delta * max|r|; 0 -> 1e-5 */
   void* stream;     /* cudaStream_t all work is queued on; NULL = the legacy default stream */
 } tmw_options;
 
@@ -104,7 +105,9 @@ typedef struct {
 int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, double c_sw, const tmw_options* opt);
 
 /*
- * out = D in (op = TMW_D) or D^dag in (TMW_DDAG), Eq. (2)+(3).
+ * out = D in (op = TMW_D), D^dag in (TMW_DDAG) or gamma5 D in (TMW_G5D), Eq. (2)+(3). TMW_G5D is the paper's one
+ * explicit fusion ("we combine the gamma5 and D_w operations into one kernel to save the bandwidth"):
+ * gamma5 = diag(+1,+1,-1,-1) in spin (C5) multiplies the result inside the kernel, at no extra memory traffic.
  *   parity = TMW_FULL: in, out are canonical fp64 full-lattice spinors (HOST or DEVICE per location); fp64 arithmetic.
  *   parity = TMW_EVEN | TMW_ODD: the raw benchmark path. out (packed, parity p) = H_{p pbar} in (packed, the other
  *     parity) = only the hopping part of Eq. (2) (the 1/2 sum over mu), in precision `prec` (TMW_F32 | TMW_F64).
@@ -140,6 +143,17 @@ int tmw_solve(tmw_ctx* ctx, const double* b, double* x, double tol, tmw_solve_in
 int tmw_apply_multi(tmw_ctx* ctx, int op, int parity, int prec, int nrhs, const void* in, void* out);
 int tmw_apply_schur_multi(tmw_ctx* ctx, int op, int prec, int nrhs, const void* in_odd, void* out_odd);
 int tmw_solve_multi(tmw_ctx* ctx, int nrhs, const double* b, double* x, double tol, tmw_solve_info* info);
+
+/*
+ * out = sum_{k=0}^{ncoef-1} coef[k] T_k(X) in,  X = scale * (gamma5 D) + shift * 1,  T_k the Chebyshev polynomials of
+ * the first kind, evaluated with the Clenshaw recursion ("one should use the Clenshaw recursion to define the
+ * Chebyshev polynomial to suppress the round-off error"; the polynomial of gamma5 D_w is the inner loop
+ * of the paper's overlap sign function). gamma5 D is applied with the fused gamma5 epilogue
+ * (PAPER.md:315). coef: HOST array of real coefficients; in, out: canonical fp64 full-lattice spinors (HOST or
+ * DEVICE per location); fp64 arithmetic. The caller chooses scale and shift so that the spectrum of X lies where the
+ * series is wanted (usually [-1, 1]). Cost: ncoef - 1 applications of gamma5 D.
+ */
+int tmw_cheb_apply(tmw_ctx* ctx, int ncoef, const double* coef, double scale, double shift, const double* in, double* out);
 
 /* bytes of one packed parity spinor in precision prec (TMW_F32 | TMW_F64); 0 on bad arguments */
 long long tmw_spinor_bytes(const tmw_ctx* ctx, int prec);

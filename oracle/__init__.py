@@ -134,5 +134,27 @@ def bicgstab(gauge, b, m: complex, c_sw: float = 0.0, tol: float = 1e-12, max_it
     return x, dict(status=status, iters=iters.value, true_resid=resid.value)
 
 
+def gamma5_apply(gauge, psi, m: complex, c_sw: float = 0.0, F=None) -> np.ndarray:
+    """gamma5 D psi (the operator the paper's overlap work is built on; = H_w when m is real):
+    the oracle's D followed by the explicit 4x4 gamma5 = gx gy gz gt on the spin index."""
+    return np.einsum("st,...tc->...sc", gamma(4), apply(gauge, psi, m, c_sw, F=F))
+
+
+def cheb_series(gauge, psi, coef, scale: float, shift: float, m: complex, c_sw: float = 0.0, F=None) -> np.ndarray:
+    """sum_k coef[k] T_k(X) psi with X = scale * gamma5 D + shift, by the DEFINITION of the Chebyshev polynomials of the
+    first kind: T_0 = 1, T_1 = X, T_{k+1} = 2 X T_k - T_{k-1} (each T_k psi formed explicitly and summed). The CUDA path
+    evaluates the same series with the Clenshaw recursion; the two agree up to rounding."""
+    X = lambda v: scale * gamma5_apply(gauge, v, m, c_sw, F=F) + shift * v
+    psi = _c(psi)
+    t_prev, out = psi, coef[0] * psi
+    if len(coef) > 1:
+        t_cur = X(psi)
+        out = out + coef[1] * t_cur
+        for k in range(2, len(coef)):
+            t_prev, t_cur = t_cur, 2.0 * X(t_cur) - t_prev
+            out = out + coef[k] * t_cur
+    return out
+
+
 def num_threads() -> int:
     return int(_load().orc_num_threads())

@@ -37,7 +37,7 @@ struct tmw_ctx {
   void* w64[10];  // packed fp64 parity spinors
   void* w32[8];   // packed inner-precision parity spinors (fp32 for TMW_MIXED, fp64 for TMW_DOUBLE)
   void* canon[2]; // canonical fp64 full-lattice staging (HOST location only)
-  int nr32;          // most columns one thread of the fp32 stencil takes (1..4)
+  int nr32;          // forced columns per thread of the fp32 stencil (1..4), 0 = automatic
   Scalars* sc;       // MAXCOL scalar blocks
   Scalars* sc_host;  // pinned
   double* red;       // 4 * MAXCOL device doubles
@@ -130,6 +130,7 @@ static DslashArgs<R> make_args(const tmw_ctx* c, int par, int dagger, const void
   a.par = par;
   a.sig = dagger ? (R)-1 : (R)1;
   a.coef = (R)(0.5 * sgn);
+  a.g5 = 0;
   a.d = make_diag<R>(c, dagger);
   a.red_mode = 0;
   a.dotv = nullptr;
@@ -147,8 +148,9 @@ template <typename R> static int ng_of(const tmw_ctx* c) { return sizeof(R) == 4
 // red (if any) is the reduction target of column 0, column c's is red_stride doubles further per column.
 template <typename R>
 static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, void* out, const void* aux, double sgn, const ColMap& cm,
-                  int red_mode = 0, const void* dotv = nullptr, double* red = nullptr, int red_stride = 0) {
+                  int red_mode = 0, const void* dotv = nullptr, double* red = nullptr, int red_stride = 0, int g5 = 0) {
   DslashArgs<R> a = make_args<R>(ctx, par, dagger, in, out, aux, sgn, cm);
+  a.g5 = g5;
   a.red_mode = red_mode;
   a.dotv = dotv;
   a.red = red;
@@ -156,8 +158,12 @@ static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, vo
   // columns per thread: as even a split of the columns into groups of at most nr32 as possible
   int nr = 1;
   if (sizeof(R) == 4 && cm.n > 1) {
-    const int groups = (cm.n + ctx->nr32 - 1) / ctx->nr32;
-    nr = (cm.n + groups - 1) / groups;
+    if (ctx->nr32 > 0) {  // TMW_NR: as even a split into groups of at most nr32 columns as possible
+      const int groups = (cm.n + ctx->nr32 - 1) / ctx->nr32;
+      nr = (cm.n + groups - 1) / groups;
+    } else {  // 2 columns per thread (the fastest) unless 3 wastes fewer slots of a ragged last group
+      nr = ((cm.n + 2) / 3 * 3 < (cm.n + 1) / 2 * 2) ? 3 : 2;
+    }
   }
   LAUNCH(launch_dslash(a, ng_of<R>(ctx), epi, ctx->clover, nr, ctx->stream));
   return TMW_OK;
@@ -239,7 +245,7 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
   if (opt) o = *opt;
   if (o.reconstruct == 0) o.reconstruct = 12;
   if (o.max_iter == 0) o.max_iter = 10000;
-  if (o.delta == 0.0) o.delta = 1e-3;
+  if (o.delta == 0.0) o.delta = 1e-5;  // the fewest fp64 passes without costing iterations
   if ((o.location != TMW_DEVICE && o.location != TMW_HOST) || (o.precision != TMW_MIXED && o.precision != TMW_DOUBLE) ||
       (o.reconstruct != 12 && o.reconstruct != 18) || (o.mass_reading != TMW_TWIST_GAMMA5 && o.mass_reading != TMW_MASS_SCALAR) ||
       o.max_iter < 0 || !(o.delta > 0.0) || !(o.delta < 1.0))
@@ -251,7 +257,7 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
   ctx->g.sy = L / 2; ctx->g.sz = (L / 2) * L; ctx->g.st = (L / 2) * L * L;
   choose_tile(ctx->g);
   ctx->ws_cols = 1;
-  ctx->nr32 = 2;  // 2 columns per thread at 168 registers is the fastest split on B200
+  ctx->nr32 = 0;  // 0: automatic (2 or 3 columns per thread); TMW_NR=1..4 forces the group size (tuning, tests)
   if (const char* e = getenv("TMW_NR")) { const int v = atoi(e); if (v >= 1 && v <= 4) ctx->nr32 = v; }
   ctx->V = V;
   ctx->m_re = m.re; ctx->m_im = m.im; ctx->c_sw = c_sw;
@@ -396,24 +402,24 @@ static inline void* colp(void* base, int c, size_t bytes) { return (char*)base +
 static inline const void* colp(const void* base, int c, size_t bytes) { return (const char*)base + (size_t)c * bytes; }
 
 // out_p = A in_p + H in_pbar for both parities, fp64 packed
-static int full_apply64(tmw_ctx* ctx, int dagger, const void* in_e, const void* in_o, void* out_e, void* out_o, const ColMap& cm) {
-  int rc = dslash<double>(ctx, EPI_A_XPAY, 0, dagger, in_o, out_e, in_e, 1.0, cm);
+static int full_apply64(tmw_ctx* ctx, int dagger, const void* in_e, const void* in_o, void* out_e, void* out_o, const ColMap& cm, int g5 = 0) {
+  int rc = dslash<double>(ctx, EPI_A_XPAY, 0, dagger, in_o, out_e, in_e, 1.0, cm, 0, nullptr, nullptr, 0, g5);
   if (rc) return rc;
-  return dslash<double>(ctx, EPI_A_XPAY, 1, dagger, in_e, out_o, in_o, 1.0, cm);
+  return dslash<double>(ctx, EPI_A_XPAY, 1, dagger, in_e, out_o, in_o, 1.0, cm, 0, nullptr, nullptr, 0, g5);
 }
 
 extern "C" int tmw_apply_multi(tmw_ctx* ctx, int op, int parity, int prec, int nrhs, const void* in, void* out) {
   if (!ctx) return TMW_EINVAL;
   if (!in || !out || in == out) return fail(ctx, TMW_EINVAL, "tmw_apply: null or aliased pointers");
-  if ((op != TMW_D && op != TMW_DDAG) || (parity != TMW_FULL && parity != TMW_EVEN && parity != TMW_ODD)) return fail(ctx, TMW_EINVAL, "tmw_apply: bad op or parity");
+  if ((op != TMW_D && op != TMW_DDAG && op != TMW_G5D) || (parity != TMW_FULL && parity != TMW_EVEN && parity != TMW_ODD)) return fail(ctx, TMW_EINVAL, "tmw_apply: bad op or parity");
   if (nrhs < 1 || nrhs > MAXCOL) return fail(ctx, TMW_EINVAL, "tmw_apply: nrhs must be in 1..16");
-  const int dagger = (op == TMW_DDAG);
+  const int dagger = (op == TMW_DDAG), g5 = (op == TMW_G5D);
   const ColMap cm = cols_first(nrhs);
   if (parity != TMW_FULL) {
     if (prec != TMW_F32 && prec != TMW_F64) return fail(ctx, TMW_EINVAL, "tmw_apply: bad precision");
     const int par = (parity == TMW_ODD);
-    if (prec == TMW_F32) return dslash<float>(ctx, EPI_HOP, par, dagger, in, out, nullptr, 1.0, cm);
-    return dslash<double>(ctx, EPI_HOP, par, dagger, in, out, nullptr, 1.0, cm);
+    if (prec == TMW_F32) return dslash<float>(ctx, EPI_HOP, par, dagger, in, out, nullptr, 1.0, cm, 0, nullptr, nullptr, 0, g5);
+    return dslash<double>(ctx, EPI_HOP, par, dagger, in, out, nullptr, 1.0, cm, 0, nullptr, nullptr, 0, g5);
   }
   int rc = need_cols(ctx, nrhs);
   if (rc) return rc;
@@ -432,7 +438,7 @@ extern "C" int tmw_apply_multi(tmw_ctx* ctx, int op, int parity, int prec, int n
     LAUNCH(launch_pack_spinor(ctx->g, 0, 1, (const double*)colp(cin, c, cbytes), colp(ctx->w64[0], c, b64), ctx->stream));
     LAUNCH(launch_pack_spinor(ctx->g, 1, 1, (const double*)colp(cin, c, cbytes), colp(ctx->w64[1], c, b64), ctx->stream));
   }
-  rc = full_apply64(ctx, dagger, ctx->w64[0], ctx->w64[1], ctx->w64[2], ctx->w64[3], cm);
+  rc = full_apply64(ctx, dagger, ctx->w64[0], ctx->w64[1], ctx->w64[2], ctx->w64[3], cm, g5);
   if (rc) return rc;
   for (int c = 0; c < nrhs; c++) {
     LAUNCH(launch_unpack_spinor(ctx->g, 0, 1, colp(ctx->w64[2], c, b64), (double*)colp(cout, c, cbytes), ctx->stream));
@@ -446,6 +452,56 @@ extern "C" int tmw_apply_multi(tmw_ctx* ctx, int op, int parity, int prec, int n
 }
 extern "C" int tmw_apply(tmw_ctx* ctx, int op, int parity, int prec, const void* in, void* out) {
   return tmw_apply_multi(ctx, op, parity, prec, 1, in, out);
+}
+
+// Chebyshev series of X = scale * gamma5 D + shift by the Clenshaw recursion, fp64, full lattice:
+//   b_{n} = b_{n+1} = 0;  b_k = c_k psi + 2 X b_{k+1} - b_{k+2} (k = n-1 .. 1);  out = c_0 psi + X b_1 - b_2.
+// Each step = gamma5 D fused in the two stencil launches + one fused vector kernel per parity.
+//   w64: 0,1 psi (e,o); 2,3 and 4,5 the two recursion vectors; 6,7 H b_1
+extern "C" int tmw_cheb_apply(tmw_ctx* ctx, int ncoef, const double* coef, double scale, double shift, const double* in, double* out) {
+  if (!ctx) return TMW_EINVAL;
+  if (!coef || !in || !out || in == out) return fail(ctx, TMW_EINVAL, "tmw_cheb_apply: null or aliased pointers");
+  if (ncoef < 1 || !isfinite(scale) || !isfinite(shift)) return fail(ctx, TMW_EINVAL, "tmw_cheb_apply: ncoef must be >= 1, scale and shift finite");
+  for (int k = 0; k < ncoef; k++) if (!isfinite(coef[k])) return fail(ctx, TMW_EINVAL, "tmw_cheb_apply: non-finite coefficient");
+  int rc;
+  if ((rc = need_w64(ctx, 8))) return rc;
+  cudaStream_t s = ctx->stream;
+  const double* cin = in;
+  double* cout = out;
+  const size_t cbytes = (size_t)ctx->V * 24 * 8;
+  if (ctx->opt.location == TMW_HOST) {
+    if ((rc = need_canon(ctx))) return rc;
+    CK(cudaMemcpyAsync(ctx->canon[0], in, cbytes, cudaMemcpyHostToDevice, s));
+    cin = (const double*)ctx->canon[0];
+    cout = (double*)ctx->canon[1];
+  }
+  void** W = ctx->w64;
+  const int64_t n64 = (int64_t)ctx->g.Vh * 12;
+  const ColMap one = cols_first(1);
+  LAUNCH(launch_pack_spinor(ctx->g, 0, 1, cin, W[0], s));
+  LAUNCH(launch_pack_spinor(ctx->g, 1, 1, cin, W[1], s));
+  int b1 = 2, b2 = 4;  // indices of the (even) buffers of b_{k+1}, b_{k+2}
+  if (ncoef == 1) {
+    for (int p = 0; p < 2; p++) LAUNCH(launch_scale(n64, W[b1 + p], W[p], coef[0], s));
+  } else {
+    for (int p = 0; p < 2; p++) {
+      LAUNCH(launch_scale(n64, W[b1 + p], W[p], coef[ncoef - 1], s));  // b_{n-1} = c_{n-1} psi
+      CK(cudaMemsetAsync(W[b2 + p], 0, (size_t)n64 * 16, s));
+    }
+    for (int k = ncoef - 2; k >= 0; k--) {
+      if ((rc = full_apply64(ctx, 0, W[b1], W[b1 + 1], W[6], W[7], one, 1))) return rc;
+      const double f = (k == 0) ? 1.0 : 2.0;
+      for (int p = 0; p < 2; p++) LAUNCH(launch_clenshaw(n64, W[b2 + p], W[p], W[6 + p], W[b1 + p], W[b2 + p], coef[k], f, scale, shift, s));
+      const int t = b1; b1 = b2; b2 = t;  // the new vector was written over b_{k+2}
+    }
+  }
+  LAUNCH(launch_unpack_spinor(ctx->g, 0, 1, W[b1], cout, s));
+  LAUNCH(launch_unpack_spinor(ctx->g, 1, 1, W[b1 + 1], cout, s));
+  if (ctx->opt.location == TMW_HOST) {
+    CK(cudaMemcpyAsync(out, cout, cbytes, cudaMemcpyDeviceToHost, s));
+    CK(cudaStreamSynchronize(s));
+  }
+  return TMW_OK;
 }
 
 extern "C" int tmw_apply_schur_multi(tmw_ctx* ctx, int op, int prec, int nrhs, const void* in_odd, void* out_odd) {

@@ -245,6 +245,40 @@ __global__ void __launch_bounds__(BB) sub_norm_kernel(int64_t n, const double* a
   reduce_atomic<1>(acc, dst);
 }
 
+// One step of the Clenshaw recursion for a Chebyshev series in X = scale*H + shift:
+// out = c*psi + f*(scale*hb + shift*b1) - b2, hb = H b1; out may alias b2. Real coefficients, fp64.
+__global__ void __launch_bounds__(BB) clenshaw_kernel(int64_t n, double* out, const double* psi, const double* hb, const double* b1, const double* b2,
+                                                      double c, double f, double scale, double shift) {
+  for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
+    double pp[4], hh[4], u1[4], u2[4], oo[4];
+    ldp(psi, i, pp); ldp(hb, i, hh); ldp(b1, i, u1); ldp(b2, i, u2);
+#pragma unroll
+    for (int k = 0; k < 4; k++) oo[k] = c * pp[k] + f * (scale * hh[k] + shift * u1[k]) - u2[k];
+    stp(out, i, oo);
+  }
+}
+cudaError_t launch_clenshaw(int64_t n64, void* out, const void* psi, const void* hb, const void* b1, const void* b2, double c, double f, double scale,
+                            double shift, cudaStream_t s) {
+  const int64_t np = n64 / 2;
+  clenshaw_kernel<<<blas_grid(np), BB, 0, s>>>(np, (double*)out, (const double*)psi, (const double*)hb, (const double*)b1, (const double*)b2, c, f, scale, shift);
+  return cudaGetLastError();
+}
+// dst = c * src (fp64)
+__global__ void __launch_bounds__(BB) scale_kernel(int64_t n, double* dst, const double* src, double c) {
+  for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
+    double v[4];
+    ldp(src, i, v);
+#pragma unroll
+    for (int k = 0; k < 4; k++) v[k] *= c;
+    stp(dst, i, v);
+  }
+}
+cudaError_t launch_scale(int64_t n64, void* dst, const void* src, double c, cudaStream_t s) {
+  const int64_t np = n64 / 2;
+  scale_kernel<<<blas_grid(np), BB, 0, s>>>(np, (double*)dst, (const double*)src, c);
+  return cudaGetLastError();
+}
+
 // n16 = number of 16-byte vectors of R in ONE column; pairs = n16 (float) or n16/2 (double)
 template <typename R> static inline int64_t pairs_of(int64_t n16) { return sizeof(R) == 4 ? n16 : n16 / 2; }
 static inline dim3 grid_of(int64_t np, const ColMap& cm) { return dim3((unsigned)blas_grid(np), (unsigned)cm.n, 1); }

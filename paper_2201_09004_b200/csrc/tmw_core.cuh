@@ -458,6 +458,7 @@ template <typename R> struct DslashArgs {
   int par;           // parity of the output sites
   R sig;             // +1 for D, -1 for D^dagger (sign of gamma_mu in the projectors)
   R coef;            // 1/2 * sgn
+  int g5;            // multiply the result by gamma5 = diag(1,1,-1,-1) (the fused gamma5 D_w of PAPER.md:315)
   Diag<R> d;
   // fused reductions (kernel wrapper): red_mode 0 none; 1: red[0..1] += <dotv, out>; 2: red[0..1] += <out, aux>, red[2] += <out,out>
   int red_mode;

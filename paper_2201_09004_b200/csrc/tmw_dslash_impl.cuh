@@ -52,6 +52,12 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<R>
   R o[NR][24], r2[NR][3];
   if (active) {
     dslash_site<R, NG, EPI, CLOVER, NR>(a, s, coff, o, r2);
+    if (a.g5) {  // uniform across the grid
+#pragma unroll
+      for (int j = 0; j < NR; j++)
+#pragma unroll
+        for (int i = 12; i < 24; i++) o[j][i] = -o[j][i];
+    }
 #pragma unroll
     for (int j = 0; j < NR; j++)
       if (valid[j]) store_reals_s<24>((V*)a.out + coff[j], a.g.Vh, s.cb, o[j]);

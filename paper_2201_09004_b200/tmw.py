@@ -20,12 +20,12 @@ OK, EINVAL, ENOMEM, ECUDA, ESINGULAR, ENOCONV, EBREAKDOWN = 0, -1, -2, -3, -4, -
 DEVICE, HOST = 0, 1
 MIXED, DOUBLE = 0, 1
 TWIST_GAMMA5, MASS_SCALAR = 0, 1
-D, DDAG = 0, 1
+D, DDAG, G5D = 0, 1, 2
 FULL, EVEN, ODD = 0, 1, 2
 F32, F64 = 0, 1
 
 EXPORTS = ["tmw_create", "tmw_apply", "tmw_apply_schur", "tmw_solve", "tmw_apply_multi", "tmw_apply_schur_multi",
-           "tmw_solve_multi", "tmw_spinor_bytes", "tmw_pack", "tmw_unpack",
+           "tmw_solve_multi", "tmw_cheb_apply", "tmw_spinor_bytes", "tmw_pack", "tmw_unpack",
            "tmw_get_clover", "tmw_set_location", "tmw_launch_count", "tmw_destroy", "tmw_last_error"]
 
 
@@ -77,6 +77,8 @@ def load():
     lib.tmw_apply_schur_multi.restype = I
     lib.tmw_solve_multi.argtypes = [P, I, P, P, DBL, ctypes.POINTER(tmw_solve_info)]
     lib.tmw_solve_multi.restype = I
+    lib.tmw_cheb_apply.argtypes = [P, I, ctypes.POINTER(DBL), DBL, DBL, P, P]
+    lib.tmw_cheb_apply.restype = I
     lib.tmw_spinor_bytes.argtypes = [P, I]
     lib.tmw_spinor_bytes.restype = LL
     lib.tmw_pack.argtypes = [P, I, I, P, P]
@@ -160,6 +162,10 @@ class Context:
                          allow=(ENOCONV,) if allow_noconv else ())
         return [dict(status=rc, iters=i.iters, reliable_updates=i.reliable_updates, restarts=i.restarts,
                      iter_resid=i.iter_resid, true_resid=i.true_resid, device_ms=i.device_ms) for i in infos]
+
+    def cheb_apply(self, coef, scale: float, shift: float, src, dst):
+        c = (ctypes.c_double * len(coef))(*[float(v) for v in coef])
+        self._check(self._lib.tmw_cheb_apply(self._h, len(coef), c, float(scale), float(shift), _ptr(src), _ptr(dst)))
 
     def spinor_bytes(self, prec: int) -> int:
         return int(self._lib.tmw_spinor_bytes(self._h, prec))

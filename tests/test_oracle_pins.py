@@ -406,3 +406,60 @@ def test_zero_source_gives_zero_solution():
     U = synth.gauge_field(2, 2, 0.3, seed=1)
     x, info = oracle.bicgstab(U, np.zeros((2, 2, 2, 2, 4, 3), dtype=np.complex128), 0.1)
     assert info["status"] == 0 and np.all(x == 0)
+
+
+# ----------------------------------------------------------------------------------------------------------
+# (e) gamma5 D and the Chebyshev series of it
+# ----------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("c_sw", [0.0, 1.1])
+def test_gamma5_D_is_hermitian_for_real_mass(c_sw):
+    """gamma5-hermiticity D^dag = g5 D g5 (pin (b)) makes H_w = g5 D Hermitian when m is real: <y, H x> = <H y, x>,
+    and H^2 = D^dag D. A wrong gamma5 (sign, basis, acting on colour instead of spin) breaks one of the two."""
+    L, T, m = 4, 4, -0.3
+    U = synth.gauge_field(L, T, 0.4, seed=1)
+    x, y = synth.gaussian_spinor(L, T, 3), synth.gaussian_spinor(L, T, 4)
+    Hx, Hy = oracle.gamma5_apply(U, x, m, c_sw), oracle.gamma5_apply(U, y, m, c_sw)
+    assert abs(vdot(y, Hx) - vdot(Hy, x)) <= 1e-12 * abs(vdot(y, Hx))
+    HHx = oracle.gamma5_apply(U, Hx, m, c_sw)
+    DdDx = oracle.apply(U, oracle.apply(U, x, m, c_sw), m, c_sw, dagger=True)
+    assert rel(HHx, DdDx) <= 1e-13
+    # gamma5 itself: diag(+1,+1,-1,-1) on the spin index (golden table, C5)
+    assert np.array_equal(oracle.gamma5_apply(U, x, m, c_sw)[..., 2:, :], -oracle.apply(U, x, m, c_sw)[..., 2:, :])
+    assert np.array_equal(oracle.gamma5_apply(U, x, m, c_sw)[..., :2, :], oracle.apply(U, x, m, c_sw)[..., :2, :])
+
+
+def test_cheb_series_vs_eigendecomposition_2x2x2x2():
+    """On 2^4 the Hermitian X = scale * g5 D + shift is a 192 x 192 matrix: sum_k c_k T_k(X) psi must equal
+    V chebval(lambda, c) V^dag psi (numpy's Chebyshev evaluation on the eigenvalues). Pins the recurrence
+    (T_{k+1} = 2 X T_k - T_{k-1}), the role of scale and shift, and the coefficient order."""
+    L = T = 2
+    m, c_sw = -0.2, 1.0
+    U = synth.gauge_field(L, T, 0.4, seed=1)
+    psi = synth.gaussian_spinor(L, T, 3)
+    g5 = np.kron(np.eye(L ** 3 * T), np.kron(oracle.gamma(4), np.eye(3)))
+    H = g5 @ dense_matrix(U, m, c_sw)
+    assert np.linalg.norm(H - H.conj().T) <= 1e-12 * np.linalg.norm(H)
+    lam = np.linalg.eigvalsh(H)
+    scale, shift = 1.7 / (lam.max() - lam.min()), 0.05
+    X = scale * H + shift * np.eye(H.shape[0])
+    w, V = np.linalg.eigh(X)
+    assert w.min() > -1 and w.max() < 1
+    rng = np.random.default_rng(5)
+    for n in (1, 2, 3, 12):
+        coef = rng.standard_normal(n)
+        ref = V @ (np.polynomial.chebyshev.chebval(w, coef) * (V.conj().T @ psi.ravel()))
+        got = oracle.cheb_series(U, psi, coef, scale, shift, m, c_sw).ravel()
+        assert rel(got, ref) <= 1e-12, n
+
+
+def test_cheb_series_single_polynomials_free_field():
+    """T_k(cos theta) = cos(k theta): on a free-field plane-wave eigenvector of H^2 = D^dag D ... use instead the
+    exact operator identity T_2(X) = 2 X^2 - 1 and T_3(X) = 4 X^3 - 3 X on a random field."""
+    L, T, m = 4, 4, 0.1
+    U = synth.gauge_field(L, T, 0.3, seed=1)
+    psi = synth.gaussian_spinor(L, T, 3)
+    scale, shift = 0.2, -0.1
+    X = lambda v: scale * oracle.gamma5_apply(U, v, m) + shift * v
+    X1 = X(psi); X2 = X(X1); X3 = X(X2)
+    assert rel(oracle.cheb_series(U, psi, [0, 0, 1.0], scale, shift, m), 2 * X2 - psi) <= 1e-13
+    assert rel(oracle.cheb_series(U, psi, [0, 0, 0, 1.0], scale, shift, m), 4 * X3 - 3 * X1) <= 1e-13
