@@ -63,6 +63,9 @@ typedef struct { double re, im; } tmw_complex;
 #define TMW_MIXED 0  /* fp32 inner BiCGStab, fp64 reliable updates (default) */
 #define TMW_DOUBLE 1 /* everything in fp64 */
 
+#define TMW_BICGSTAB 0
+#define TMW_GCR 1
+
 #define TMW_TWIST_GAMMA5 0 /* mass term -(4+Re m) - i Im m g5  (default, reading C4) */
 #define TMW_MASS_SCALAR 1  /* mass term -(4+m) with a complex scalar m (the literal alternative) */
 
@@ -85,10 +88,13 @@ typedef struct {
   int max_iter;     /* BiCGStab iterations; 0 -> 10000 */
   double delta;     /* reliable-update threshold: fp64 true residual when |r| < delta * max|r|; 0 -> 1e-5 */
   void* stream;     /* cudaStream_t all work is queued on; NULL = the legacy default stream */
+  int solver;       /* TMW_BICGSTAB (default; the paper's CPU solver) | TMW_GCR (its "standard GPU inverter with
+                       GCR algorithm"): restarted GCR(nkrylov) on the same Schur system and kernels */
+  int nkrylov;      /* GCR restart length, 1..16; 0 -> 8 */
 } tmw_options;
 
 typedef struct {
-  int iters;            /* BiCGStab iterations (each = 2 Schur-operator applications) */
+  int iters;            /* BiCGStab iterations (each = 2 Schur-operator applications) or GCR steps (1 application each) */
   int reliable_updates; /* fp64 true-residual recomputations */
   int restarts;         /* breakdown restarts (rhat := r) */
   double iter_resid;    /* last iterated |r| / |b| */

@@ -37,6 +37,10 @@ struct tmw_ctx {
   void* w64[10];  // packed fp64 parity spinors
   void* w32[8];   // packed inner-precision parity spinors (fp32 for TMW_MIXED, fp64 for TMW_DOUBLE)
   void* canon[2]; // canonical fp64 full-lattice staging (HOST location only)
+  void* gcr_q;       // GCR Krylov vectors q_j, p_j: nkrylov inner-precision parity spinors each (lazily allocated)
+  void* gcr_p;
+  GcrScalars* gs;       // device
+  GcrScalars* gs_host;  // pinned
   int nr32;          // forced columns per thread of the fp32 stencil (1..4), 0 = automatic
   Scalars* sc;       // MAXCOL scalar blocks
   Scalars* sc_host;  // pinned
@@ -228,6 +232,7 @@ void tmw_destroy(tmw_ctx* ctx) {
   for (void* p : ctx->owned) cudaFree(p);
   if (ctx->sc_host) cudaFreeHost(ctx->sc_host);
   if (ctx->red_host) cudaFreeHost(ctx->red_host);
+  if (ctx->gs_host) cudaFreeHost(ctx->gs_host);
   if (ctx->ev0) cudaEventDestroy(ctx->ev0);
   if (ctx->ev1) cudaEventDestroy(ctx->ev1);
   delete ctx;
@@ -245,10 +250,12 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
   if (opt) o = *opt;
   if (o.reconstruct == 0) o.reconstruct = 12;
   if (o.max_iter == 0) o.max_iter = 10000;
+  if (o.nkrylov == 0) o.nkrylov = 8;  // GCR(8) beats GCR(16) on every config (orthogonalisation traffic)
   if (o.delta == 0.0) o.delta = 1e-5;  // the fewest fp64 passes without costing iterations
   if ((o.location != TMW_DEVICE && o.location != TMW_HOST) || (o.precision != TMW_MIXED && o.precision != TMW_DOUBLE) ||
       (o.reconstruct != 12 && o.reconstruct != 18) || (o.mass_reading != TMW_TWIST_GAMMA5 && o.mass_reading != TMW_MASS_SCALAR) ||
-      o.max_iter < 0 || !(o.delta > 0.0) || !(o.delta < 1.0))
+      o.max_iter < 0 || !(o.delta > 0.0) || !(o.delta < 1.0) || (o.solver != TMW_BICGSTAB && o.solver != TMW_GCR) || o.nkrylov < 1 ||
+      o.nkrylov > GCR_KMAX)
     return fail(nullptr, TMW_EINVAL, "tmw_create: bad option value");
   if (!isfinite(m.re) || !isfinite(m.im) || !isfinite(c_sw)) return fail(nullptr, TMW_EINVAL, "tmw_create: non-finite parameter");
   tmw_ctx* ctx = new (std::nothrow) tmw_ctx();
@@ -292,6 +299,8 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
   CKC(cudaEventCreate(&ctx->ev1));
   CKA(&ctx->sc, MAXCOL * sizeof(Scalars));
   CKA(&ctx->red, 4 * MAXCOL * sizeof(double));
+  CKC(cudaMallocHost((void**)&ctx->gs_host, sizeof(GcrScalars)));
+  CKA(&ctx->gs, sizeof(GcrScalars));
   const size_t Vh = (size_t)ctx->g.Vh;
   const int np32 = (ctx->ng32 == 12) ? 3 : 5;
   for (int p = 0; p < 2; p++) {
@@ -706,6 +715,72 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
   return TMW_OK;
 }
 
+
+// Restarted GCR(k) (the paper's GPU solver) on the Schur system of column c, inner
+// precision R, restarted from the fp64 true residual (the same reliable update as in solve_schur): per step one Mhat
+// application (K1, K2) and the five launches of launch_gcr_step.
+//   w64 as in solve_schur; w32: 0 r, 1 zero (the rhat slot of resid_convert), 6 x, 7 tmp_e
+template <typename R>
+int solve_gcr(tmw_ctx* ctx, int c, double tol, ColState& q) {
+  cudaStream_t s = ctx->stream;
+  const int64_t n64 = (int64_t)ctx->g.Vh * 12;
+  const int64_t nR = (int64_t)ctx->g.Vh * 24 * (int64_t)sizeof(R) / 16;
+  const size_t bytesR = (size_t)nR * 16;
+  const int k = ctx->opt.nkrylov;
+  void** W = ctx->w64;
+  void** X = ctx->w32;
+  int rc;
+  if (!ctx->gcr_q) { if ((rc = dev_alloc(ctx, &ctx->gcr_q, bytesR * GCR_KMAX))) return rc; }
+  if (!ctx->gcr_p) { if ((rc = dev_alloc(ctx, &ctx->gcr_p, bytesR * GCR_KMAX))) return rc; }
+  ColMap one;
+  one.n = 0;
+  cols_add(one, c);
+  void* r = colp(X[0], c, bytesR);
+  void* x = colp(X[6], c, bytesR);
+  void* tmp = colp(X[7], c, bytesR);
+  Scalars* h = ctx->sc_host;
+  GcrScalars* gh = ctx->gs_host;
+  const bool verbose = getenv("TMW_VERBOSE") != nullptr;
+  const ColMap zero = cols_first(1);
+  CK(cudaMemsetAsync(colp(W[3], c, (size_t)n64 * 16), 0, (size_t)n64 * 16, s));
+  CK(cudaMemsetAsync(colp(W[6], c, (size_t)n64 * 16), 0, (size_t)n64 * 16, s));
+  CK(cudaMemsetAsync(colp(X[1], c, bytesR), 0, bytesR, s));
+  const int max_iter = ctx->opt.max_iter;
+  for (;;) {
+    // true residual r64 = bhat - Mhat y (W[6] holds Mhat y), r = (R) r64, |r64|^2
+    memset(h, 0, MAXCOL * sizeof(Scalars));
+    if ((rc = push_scalars(ctx))) return rc;
+    LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], X[0], X[1], ctx->sc, one, s));
+    if ((rc = fetch_scalars(ctx))) return rc;
+    q.rnorm = q.maxr = sqrt(h[c].rr);
+    q.iter_resid = q.rnorm / q.bnorm;
+    if (verbose) fprintf(stderr, "[tmw] gcr col %d cycle %d it %d true |r|/|b| %.3e\n", c, q.updates, q.iters, q.iter_resid);
+    if (!isfinite(q.rnorm)) return fail(ctx, TMW_EBREAKDOWN, "tmw_solve: non-finite true residual");
+    if (q.rnorm <= tol * q.bnorm) { q.done = true; return TMW_OK; }
+    if (q.iters >= max_iter) return fail(ctx, TMW_ENOCONV, "tmw_solve: max_iter reached");
+    CK(cudaMemsetAsync(x, 0, bytesR, s));
+    CK(cudaMemsetAsync(ctx->gs, 0, sizeof(GcrScalars), s));
+    for (int i = 0; i < k && q.iters < max_iter; i++) {
+      // q_i = Mhat r (orthogonalised in launch_gcr_step), p_i = r - ...
+      if ((rc = schur<R>(ctx, 0, r, colp(ctx->gcr_q, i, bytesR), tmp, zero))) return rc;
+      LAUNCH(launch_gcr_step<R>(nR, i, ctx->gcr_q, ctx->gcr_p, x, r, ctx->gs, s));
+      ctx->launches += (i > 0) ? 4 : 3;  // launch_gcr_step is 5 launches (4 for the first vector)
+      CK(cudaMemcpyAsync(gh, ctx->gs, sizeof(GcrScalars), cudaMemcpyDeviceToHost, s));
+      CK(cudaStreamSynchronize(s));
+      q.iters++;
+      if (!isfinite(gh->rr) || !(gh->nw > 0.0)) return fail(ctx, TMW_EBREAKDOWN, "tmw_solve: GCR breakdown (Mhat p vanished or non-finite)");
+      const double rn = sqrt(gh->rr);
+      q.iter_resid = rn / q.bnorm;
+      if (verbose) fprintf(stderr, "[tmw] gcr col %d it %d |r|/|b| %.3e\n", c, q.iters, q.iter_resid);
+      if (rn <= tol * q.bnorm || rn < ctx->opt.delta * q.maxr) break;
+    }
+    // restart: y += x, Mhat y in fp64
+    LAUNCH(launch_acc_y<R>(n64, W[3], X[6], one, s));
+    if ((rc = schur<double>(ctx, 0, W[3], W[6], W[5], one))) return rc;
+    q.updates++;
+  }
+}
+
 }  // namespace
 
 extern "C" int tmw_solve_multi(tmw_ctx* ctx, int nrhs, const double* b, double* x, double tol, tmw_solve_info* info) {
@@ -761,7 +836,15 @@ extern "C" int tmw_solve_multi(tmw_ctx* ctx, int nrhs, const double* b, double* 
     Diag<double> d = make_diag<double>(ctx, 0);
     for (int i = 0; i < nz.n; i++) LAUNCH(launch_diag(d, ctx->g, 0, ctx->clover, 1, colp(W[0], nz.col[i], b64), colp(W[5], nz.col[i], b64), s));
     if ((rc = dslash<double>(ctx, EPI_XPAY, 1, 0, W[5], W[2], W[1], -1.0, nz))) return rc;
-    status = dbl ? solve_schur<double>(ctx, nrhs, tol, cs) : solve_schur<float>(ctx, nrhs, tol, cs);
+    if (ctx->opt.solver == TMW_GCR) {
+      for (int i = 0; i < nz.n; i++) {  // GCR keeps 2 k Krylov vectors per system: the columns go one after another
+        rc = dbl ? solve_gcr<double>(ctx, nz.col[i], tol, cs[nz.col[i]]) : solve_gcr<float>(ctx, nz.col[i], tol, cs[nz.col[i]]);
+        if (rc != TMW_OK && rc != TMW_ENOCONV) return rc;
+        if (rc == TMW_ENOCONV) status = rc;
+      }
+    } else {
+      status = dbl ? solve_schur<double>(ctx, nrhs, tol, cs) : solve_schur<float>(ctx, nrhs, tol, cs);
+    }
     if (status != TMW_OK && status != TMW_ENOCONV) return status;
     // A7: x_o = y, x_e = A_ee^{-1} (b_e - H_eo x_o)
     if ((rc = dslash<double>(ctx, EPI_AINV_XPAY, 0, 0, W[3], W[7], W[0], -1.0, nz))) return rc;

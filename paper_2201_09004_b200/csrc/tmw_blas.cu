@@ -279,6 +279,125 @@ cudaError_t launch_scale(int64_t n64, void* dst, const void* src, double c, cuda
   return cudaGetLastError();
 }
 
+// ---- GCR(k) kernels (the paper's "standard GPU inverter with GCR algorithm") ----
+// Krylov vectors q_j (= Mhat p_j, orthogonal, NOT normalised: nq[j] = <q_j,q_j>) and p_j, j < KMAX, are stored back to
+// back: vector j starts j*n work items after the base pointer. All scalars stay in a GcrScalars block on the device.
+
+// dots[2j..2j+1] += <q_j, w> for j < i: one pass over w and the i vectors q_j
+template <typename R> __global__ void __launch_bounds__(BB) gcr_dots_kernel(int64_t n, int i, const R* Q, const R* w, GcrScalars* gs) {
+  double acc[2 * GCR_KMAX];
+#pragma unroll
+  for (int j = 0; j < 2 * GCR_KMAX; j++) acc[j] = 0.0;
+  for (int64_t e = (int64_t)blockIdx.x * BB + threadIdx.x; e < n; e += (int64_t)gridDim.x * BB) {
+    R ww[4];
+    ldp(w, e, ww);
+#pragma unroll
+    for (int j = 0; j < GCR_KMAX; j++) {
+      if (j < i) {
+        R qq[4];
+        ldp(Q + 4 * n * j, e, qq);
+        acc[2 * j] += (double)(qq[0] * ww[0] + qq[1] * ww[1] + qq[2] * ww[2] + qq[3] * ww[3]);
+        acc[2 * j + 1] += (double)(qq[0] * ww[1] - qq[1] * ww[0] + qq[2] * ww[3] - qq[3] * ww[2]);
+      }
+    }
+  }
+  __shared__ double sm[BB / 32];
+  const int lane = threadIdx.x & 31, wp = threadIdx.x >> 5;
+  for (int j = 0; j < 2 * i; j++) {
+    double v = acc[j];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_down_sync(0xffffffffu, v, off);
+    if (lane == 0) sm[wp] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      double t = 0;
+#pragma unroll
+      for (int k = 0; k < BB / 32; k++) t += sm[k];
+      atomicAdd(&gs->dots[j], t);
+    }
+    __syncthreads();
+  }
+}
+// coef_j = dots_j / nq_j (j < i); zero the accumulators of the next two kernels
+__global__ void gcr_coef_kernel(int i, GcrScalars* gs) {
+  const int j = threadIdx.x;
+  if (j < i) {
+    gs->coef[2 * j] = gs->dots[2 * j] / gs->nq[j];
+    gs->coef[2 * j + 1] = gs->dots[2 * j + 1] / gs->nq[j];
+    gs->dots[2 * j] = gs->dots[2 * j + 1] = 0.0;
+  }
+  if (j == 0) { gs->nw = 0.0; gs->g[0] = gs->g[1] = 0.0; gs->rr = 0.0; }
+}
+// w -= sum_j coef_j q_j (stored as q_i);  p_i = r - sum_j coef_j p_j;  nw += <w,w>;  g += <w,r>
+template <typename R> __global__ void __launch_bounds__(BB) gcr_orth_kernel(int64_t n, int i, R* Q, R* P, const R* r, GcrScalars* gs) {
+  R cr[GCR_KMAX], ci[GCR_KMAX];
+#pragma unroll
+  for (int j = 0; j < GCR_KMAX; j++) {
+    cr[j] = j < i ? (R)gs->coef[2 * j] : (R)0;
+    ci[j] = j < i ? (R)gs->coef[2 * j + 1] : (R)0;
+  }
+  double acc[3] = {0, 0, 0};
+  R* w = Q + 4 * n * i;
+  R* p = P + 4 * n * i;
+  for (int64_t e = (int64_t)blockIdx.x * BB + threadIdx.x; e < n; e += (int64_t)gridDim.x * BB) {
+    R ww[4], pp[4], rr[4];
+    ldp(w, e, ww); ldp(r, e, rr);
+#pragma unroll
+    for (int c = 0; c < 4; c++) pp[c] = rr[c];
+#pragma unroll
+    for (int j = 0; j < GCR_KMAX; j++) {
+      if (j < i) {
+        R qq[4], pj[4];
+        ldp(Q + 4 * n * j, e, qq); ldp(P + 4 * n * j, e, pj);
+#pragma unroll
+        for (int c = 0; c < 2; c++) {
+          ww[2 * c] -= cr[j] * qq[2 * c] - ci[j] * qq[2 * c + 1];
+          ww[2 * c + 1] -= cr[j] * qq[2 * c + 1] + ci[j] * qq[2 * c];
+          pp[2 * c] -= cr[j] * pj[2 * c] - ci[j] * pj[2 * c + 1];
+          pp[2 * c + 1] -= cr[j] * pj[2 * c + 1] + ci[j] * pj[2 * c];
+        }
+      }
+    }
+    stp(w, e, ww); stp(p, e, pp);
+#pragma unroll
+    for (int c = 0; c < 2; c++) {
+      acc[0] += (double)(ww[2 * c] * ww[2 * c] + ww[2 * c + 1] * ww[2 * c + 1]);
+      acc[1] += (double)(ww[2 * c] * rr[2 * c] + ww[2 * c + 1] * rr[2 * c + 1]);
+      acc[2] += (double)(ww[2 * c] * rr[2 * c + 1] - ww[2 * c + 1] * rr[2 * c]);
+    }
+  }
+  double* dst[3] = {&gs->nw, &gs->g[0], &gs->g[1]};
+  reduce_atomic<3>(acc, dst);
+}
+// a = g / nw; nq[i] = nw
+__global__ void gcr_alpha_kernel(int i, GcrScalars* gs) {
+  gs->nq[i] = gs->nw;
+  gs->a[0] = gs->g[0] / gs->nw;
+  gs->a[1] = gs->g[1] / gs->nw;
+}
+// x += a p_i;  r -= a q_i;  rr += <r,r>
+template <typename R> __global__ void __launch_bounds__(BB) gcr_update_kernel(int64_t n, int i, R* x, R* r, const R* Q, const R* P, GcrScalars* gs) {
+  const R ar = (R)gs->a[0], ai = (R)gs->a[1];
+  const R* w = Q + 4 * n * i;
+  const R* p = P + 4 * n * i;
+  double acc[1] = {0};
+  for (int64_t e = (int64_t)blockIdx.x * BB + threadIdx.x; e < n; e += (int64_t)gridDim.x * BB) {
+    R xx[4], rr[4], ww[4], pp[4];
+    ldp(x, e, xx); ldp(r, e, rr); ldp(w, e, ww); ldp(p, e, pp);
+#pragma unroll
+    for (int c = 0; c < 2; c++) {
+      xx[2 * c] += ar * pp[2 * c] - ai * pp[2 * c + 1];
+      xx[2 * c + 1] += ar * pp[2 * c + 1] + ai * pp[2 * c];
+      rr[2 * c] -= ar * ww[2 * c] - ai * ww[2 * c + 1];
+      rr[2 * c + 1] -= ar * ww[2 * c + 1] + ai * ww[2 * c];
+      acc[0] += (double)(rr[2 * c] * rr[2 * c] + rr[2 * c + 1] * rr[2 * c + 1]);
+    }
+    stp(x, e, xx); stp(r, e, rr);
+  }
+  double* dst[1] = {&gs->rr};
+  reduce_atomic<1>(acc, dst);
+}
+
 // n16 = number of 16-byte vectors of R in ONE column; pairs = n16 (float) or n16/2 (double)
 template <typename R> static inline int64_t pairs_of(int64_t n16) { return sizeof(R) == 4 ? n16 : n16 / 2; }
 static inline dim3 grid_of(int64_t np, const ColMap& cm) { return dim3((unsigned)blas_grid(np), (unsigned)cm.n, 1); }
@@ -323,6 +442,20 @@ cudaError_t launch_sub_norm(int64_t n64, const void* a, const void* b, void* d, 
   sub_norm_kernel<<<grid_of(np, cm), BB, 0, s>>>(np, (const double*)a, (const double*)b, (double*)d, out, cm);
   return cudaGetLastError();
 }
+
+template <typename R> cudaError_t launch_gcr_step(int64_t n16, int i, void* Q, void* P, void* x, void* r, GcrScalars* gs, cudaStream_t s) {
+  const int64_t np = pairs_of<R>(n16);
+  if (i > 0) {
+    gcr_dots_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, i, (const R*)Q, (const R*)Q + 4 * np * i, gs);
+  }
+  gcr_coef_kernel<<<1, GCR_KMAX, 0, s>>>(i, gs);
+  gcr_orth_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, i, (R*)Q, (R*)P, (const R*)r, gs);
+  gcr_alpha_kernel<<<1, 1, 0, s>>>(i, gs);
+  gcr_update_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, i, (R*)x, (R*)r, (const R*)Q, (const R*)P, gs);
+  return cudaGetLastError();
+}
+template cudaError_t launch_gcr_step<float>(int64_t, int, void*, void*, void*, void*, GcrScalars*, cudaStream_t);
+template cudaError_t launch_gcr_step<double>(int64_t, int, void*, void*, void*, void*, GcrScalars*, cudaStream_t);
 
 #define TMW_INST(R)                                                                                                          \
   template cudaError_t launch_update_p<R>(int64_t, void*, const void*, const void*, const Scalars*, const ColMap&, cudaStream_t);           \

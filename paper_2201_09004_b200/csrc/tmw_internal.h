@@ -45,6 +45,23 @@ struct Scalars {
   double nrm;         // generic norm^2 accumulator
   double pad;
 };
+// GCR(k) scalars (device): see the gcr_* kernels of tmw_blas.cu
+enum { GCR_KMAX = 16 };
+struct GcrScalars {
+  double dots[2 * GCR_KMAX];  // <q_j, w>
+  double coef[2 * GCR_KMAX];  // dots_j / nq_j
+  double nq[GCR_KMAX];        // <q_j, q_j>
+  double nw;                  // <w, w> after orthogonalisation
+  double g[2];                // <w, r>
+  double a[2];                // g / nw
+  double rr;                  // <r, r> after the update
+  double pad[2];
+};
+// One GCR step after q_i = Mhat p_i(= Mhat r) has been stored as vector i of Q: orthogonalise it against q_0..q_{i-1}
+// (classical Gram-Schmidt, one pass for the dot products and one for the updates), build p_i alongside, then
+// x += a p_i, r -= a q_i with a = <q_i, r>/<q_i, q_i>; gs->rr = |r|^2. n16 = 16-byte vectors per spinor; 5 launches.
+template <typename R> cudaError_t launch_gcr_step(int64_t n16, int i, void* Q, void* P, void* x, void* r, GcrScalars* gs, cudaStream_t s);
+
 // The right-hand-side columns a batched launch works on: slot j -> column col[j].
 struct ColMap {
   int n;

@@ -19,6 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libtmw.so")
 OK, EINVAL, ENOMEM, ECUDA, ESINGULAR, ENOCONV, EBREAKDOWN = 0, -1, -2, -3, -4, -5, -6
 DEVICE, HOST = 0, 1
 MIXED, DOUBLE = 0, 1
+BICGSTAB, GCR = 0, 1
 TWIST_GAMMA5, MASS_SCALAR = 0, 1
 D, DDAG, G5D = 0, 1, 2
 FULL, EVEN, ODD = 0, 1, 2
@@ -36,7 +37,7 @@ class tmw_complex(ctypes.Structure):
 class tmw_options(ctypes.Structure):
     _fields_ = [("location", ctypes.c_int), ("precision", ctypes.c_int), ("reconstruct", ctypes.c_int),
                 ("mass_reading", ctypes.c_int), ("max_iter", ctypes.c_int), ("delta", ctypes.c_double),
-                ("stream", ctypes.c_void_p)]
+                ("stream", ctypes.c_void_p), ("solver", ctypes.c_int), ("nkrylov", ctypes.c_int)]
 
 
 class tmw_solve_info(ctypes.Structure):
@@ -118,13 +119,13 @@ class Context:
 
     def __init__(self, L: int, T: int, gauge, m: complex, c_sw: float = 0.0, *, location: int = DEVICE,
                  precision: int = MIXED, reconstruct: int = 12, mass_reading: int = TWIST_GAMMA5, max_iter: int = 0,
-                 delta: float = 0.0, stream: int | None = None):
+                 delta: float = 0.0, stream: int | None = None, solver: int = BICGSTAB, nkrylov: int = 0):
         lib = load()
         self._lib = lib
         self.L, self.T = L, T
         self.V = L * L * L * T
         self.location = location
-        opt = tmw_options(location, precision, reconstruct, mass_reading, max_iter, delta, stream)
+        opt = tmw_options(location, precision, reconstruct, mass_reading, max_iter, delta, stream, solver, nkrylov)
         h = ctypes.c_void_p()
         rc = lib.tmw_create(ctypes.byref(h), L, T, _ptr(gauge), tmw_complex(float(np.real(m)), float(np.imag(m))),
                             float(c_sw), ctypes.byref(opt))
