@@ -32,10 +32,14 @@ template <bool DA, bool DB> __device__ __forceinline__ void mm(const zd* A, cons
 }
 
 struct Lat {
-  int L, T;
-  int64_t V;
+  int L, T, Lh;
+  int64_t Vh;
+  const double2* U[2];  // packed fp64 gauge per parity: [mu][9 planes][Vh] (tmw_pack.cu)
 };
-__device__ __forceinline__ int64_t lex(const Lat& g, const int* c) { return c[0] + (int64_t)g.L * (c[1] + (int64_t)g.L * (c[2] + (int64_t)g.L * c[3])); }
+// site code: (lexicographic index << 1) | parity; lex >> 1 is the checkerboard index (L is even)
+__device__ __forceinline__ int64_t lex(const Lat& g, const int* c) {
+  return ((c[0] + (int64_t)g.L * (c[1] + (int64_t)g.L * (c[2] + (int64_t)g.L * c[3]))) << 1) | ((c[0] + c[1] + c[2] + c[3]) & 1);
+}
 // site c shifted by dm in direction mu and dn in direction nu, periodic
 __device__ __forceinline__ int64_t shifted(const Lat& g, const int* c, int mu, int dm, int nu, int dn) {
   int n[4] = {c[0], c[1], c[2], c[3]};
@@ -44,12 +48,16 @@ __device__ __forceinline__ int64_t shifted(const Lat& g, const int* c, int mu, i
   n[nu] = (n[nu] + dn + en) % en;
   return lex(g, n);
 }
-__device__ __forceinline__ void ld_link(const Lat& g, const double* __restrict__ canon, int mu, int64_t site, zd* U) {
-  const double2* p = (const double2*)(canon + 18 * ((int64_t)mu * g.V + site));
+// link U_mu at the lexicographic site index: read from the packed (checkerboarded, plane-major) fp64 copy, so that the
+// 32 lanes of a warp (consecutive checkerboard sites of one parity) read 512 contiguous bytes per plane. Reading the
+// canonical array-of-structures field instead costs 36 L1 wavefronts per warp load instead of 4 and made this kernel
+// L1-bound (38.6 ms at 48^3 x 144).
+__device__ __forceinline__ void ld_link(const Lat& g, const double* __restrict__, int mu, int64_t site, zd* U) {
+  const double2* p = g.U[site & 1] + (int64_t)mu * 9 * g.Vh + (site >> 2);
 #pragma unroll
   for (int i = 0; i < 9; i++) {
-    const double2 q = __ldg(p + i);
-    U[i] = mk<double>(q.x, q.y);
+    const double2 v = __ldg(p + i * g.Vh);
+    U[i] = mk<double>(v.x, v.y);
   }
 }
 
@@ -68,7 +76,7 @@ __device__ __forceinline__ void leaf(const Lat& g, const double* canon, int m0, 
   for (int i = 0; i < 9; i++) Q[i] = Q[i] + P[i];
 }
 
-__device__ void field_strength(const Lat& g, const double* canon, const int* c, int mu, int nu, zd* F) {
+__device__ __noinline__ void field_strength(const Lat& g, const double* canon, const int* c, int mu, int nu, zd* F) {
   zd Q[9];
 #pragma unroll
   for (int i = 0; i < 9; i++) Q[i] = mk<double>(0.0, 0.0);
@@ -118,58 +126,88 @@ __device__ __forceinline__ void pack_block(const zd* E1, const zd* E2, const zd*
     }
 }
 
-__global__ void __launch_bounds__(128) clover_build_kernel(const Geom g, const double* __restrict__ canon, double k, double diag, double2* c64e, double2* c64o, float4* c32e, float4* c32o) {
-  const int64_t site = (int64_t)blockIdx.x * 128 + threadIdx.x;
+// One warp per plane: CTA = 32 consecutive lexicographic sites x 6 planes (192 threads). Thread (site, plane) computes
+// the Hermitian F_plane(site) (4 leaves = 12 SU(3) products in fp64) and leaves its 9 independent reals in shared
+// memory; warps 0 and 1 then assemble the packed block of chirality 0 / 1 of the 32 sites and store the fp64 and fp32
+// copies (one 16-byte vector per lane and plane: coalesced). The earlier one-thread-per-site version kept six field
+// strengths and both blocks in one thread (255 registers + 1.9 KB of spills) and ran 4x slower.
+enum { CB_SITES = 32 };
+__global__ void __launch_bounds__(6 * CB_SITES, 2) clover_build_kernel(const Geom g, const double2* __restrict__ u64e, const double2* __restrict__ u64o, double k, double diag, double2* c64e, double2* c64o, float4* c32e, float4* c32o) {
+  __shared__ double Fs[6][9][CB_SITES];  // [plane][re(0,0) re(1,1) re(2,2) re/im(1,0) re/im(2,0) re/im(2,1)][site]
+  const int lane = threadIdx.x & 31, plane = threadIdx.x >> 5;
+  const int par = blockIdx.y;
+  const int cb = blockIdx.x * CB_SITES + lane;  // 32 consecutive checkerboard sites of parity par
+  const double* canon = nullptr;
   Lat lt;
   lt.L = g.L;
   lt.T = g.T;
-  lt.V = 2 * (int64_t)g.Vh;
-  if (site >= lt.V) return;
-  int c[4];
-  int64_t q = site;
-  c[0] = (int)(q % g.L); q /= g.L;
-  c[1] = (int)(q % g.L); q /= g.L;
-  c[2] = (int)(q % g.L); q /= g.L;
-  c[3] = (int)q;
-  const int par = (c[0] + c[1] + c[2] + c[3]) & 1;
-  const int cb = (int)(site >> 1);
-  // planes: xy=0 xz=1 xt=2 yz=3 yt=4 zt=5
-  zd Fa[9], Fb[9], E1u[9], E2u[9], E3u[9], E1l[9], E2l[9], E3l[9];
-  field_strength(lt, canon, c, 0, 1, Fa);  // xy
-  field_strength(lt, canon, c, 2, 3, Fb);  // zt
+  lt.Lh = g.Lh;
+  lt.Vh = g.Vh;
+  lt.U[0] = u64e;
+  lt.U[1] = u64o;
+  const bool active = cb < g.Vh;
+  int c[4] = {0, 0, 0, 0};
+  if (active) {
+    int q = cb / g.Lh;
+    c[1] = q % g.L; q /= g.L;
+    c[2] = q % g.L;
+    c[3] = q / g.L;
+    c[0] = 2 * (cb % g.Lh) + ((c[1] + c[2] + c[3] + par) & 1);
+    zd F[9];
+    // planes: xy=0 xz=1 xt=2 yz=3 yt=4 zt=5. mu, nu are RUNTIME values (one copy of the 12 unrolled 3x3 products for
+    // all six warps): with one specialised copy per plane the kernel was instruction-fetch bound (ncu: stall
+    // no_instruction 8.9 per issue, fp64 pipe 24 %).
+    const int mu = (plane < 3) ? 0 : (plane < 5 ? 1 : 2);
+    const int nu = (plane < 3) ? plane + 1 : (plane < 5 ? plane - 1 : 3);
+    field_strength(lt, canon, c, mu, nu, F);
+    Fs[plane][0][lane] = F[0].re;
+    Fs[plane][1][lane] = F[4].re;
+    Fs[plane][2][lane] = F[8].re;
+    Fs[plane][3][lane] = F[3].re; Fs[plane][4][lane] = F[3].im;
+    Fs[plane][5][lane] = F[6].re; Fs[plane][6][lane] = F[6].im;
+    Fs[plane][7][lane] = F[7].re; Fs[plane][8][lane] = F[7].im;
+  }
+  __syncthreads();
+  if (plane >= 2 || !active) return;
+  // chirality b = plane: upper (b = 0): E1 = F_yz - F_xt, E2 = F_xz + F_yt, E3 = F_xy - F_zt; lower: opposite signs
+  const double sg = plane ? 1.0 : -1.0;
+  zd E1[9], E2[9], E3[9];
+  {
+    // rebuild full Hermitian matrices from the 9 reals
+    auto herm = [&](int pa, int pb, double sa, double sb, zd* E) {
+      double v[9];
 #pragma unroll
-  for (int i = 0; i < 9; i++) { E3u[i] = Fa[i] - Fb[i]; E3l[i] = Fa[i] + Fb[i]; }
-  field_strength(lt, canon, c, 0, 2, Fa);  // xz
-  field_strength(lt, canon, c, 1, 3, Fb);  // yt
+      for (int i = 0; i < 9; i++) v[i] = sa * Fs[pa][i][lane] + sb * Fs[pb][i][lane];
+      E[0] = mk<double>(v[0], 0.0); E[4] = mk<double>(v[1], 0.0); E[8] = mk<double>(v[2], 0.0);
+      E[3] = mk<double>(v[3], v[4]); E[1] = mk<double>(v[3], -v[4]);
+      E[6] = mk<double>(v[5], v[6]); E[2] = mk<double>(v[5], -v[6]);
+      E[7] = mk<double>(v[7], v[8]); E[5] = mk<double>(v[7], -v[8]);
+    };
+    herm(3, 2, 1.0, sg, E1);    // F_yz -/+ F_xt
+    herm(1, 4, 1.0, -sg, E2);   // F_xz +/- F_yt
+    herm(0, 5, 1.0, sg, E3);    // F_xy -/+ F_zt
+  }
+  double B[36];
+  pack_block(E1, E2, E3, k, diag, B);
+  double2* d64 = (par ? c64o : c64e) + (int64_t)plane * 18 * g.Vh;
+  float4* d32 = (par ? c32o : c32e) + (int64_t)plane * 9 * g.Vh;
+  float Bf[36];
 #pragma unroll
-  for (int i = 0; i < 9; i++) { E2u[i] = Fa[i] + Fb[i]; E2l[i] = Fa[i] - Fb[i]; }
-  field_strength(lt, canon, c, 1, 2, Fa);  // yz
-  field_strength(lt, canon, c, 0, 3, Fb);  // xt
-#pragma unroll
-  for (int i = 0; i < 9; i++) { E1u[i] = Fa[i] - Fb[i]; E1l[i] = Fa[i] + Fb[i]; }
-  double B[72];
-  pack_block(E1u, E2u, E3u, k, diag, B);
-  pack_block(E1l, E2l, E3l, k, diag, B + 36);
-  double2* d64 = par ? c64o : c64e;
-  float4* d32 = par ? c32o : c32e;
-  float Bf[72];
-#pragma unroll
-  for (int i = 0; i < 72; i++) Bf[i] = (float)B[i];
+  for (int i = 0; i < 36; i++) Bf[i] = (float)B[i];
   store_reals<36>(d64, g.Vh, cb, B);
-  store_reals<36>(d64 + (int64_t)18 * g.Vh, g.Vh, cb, B + 36);
   store_reals<36>(d32, g.Vh, cb, Bf);
-  store_reals<36>(d32 + (int64_t)9 * g.Vh, g.Vh, cb, Bf + 36);
 }
 
-cudaError_t launch_clover_build(const Geom& g, const double* canon_gauge, double c_sw, double diag, void* c64_even, void* c64_odd, void* c32_even, void* c32_odd, cudaStream_t s) {
-  const int64_t V = 2 * (int64_t)g.Vh;
-  clover_build_kernel<<<(unsigned)((V + 127) / 128), 128, 0, s>>>(g, canon_gauge, 0.5 * c_sw, diag, (double2*)c64_even, (double2*)c64_odd, (float4*)c32_even, (float4*)c32_odd);
+cudaError_t launch_clover_build(const Geom& g, const void* g64_even, const void* g64_odd, double c_sw, double diag, void* c64_even, void* c64_odd, void* c32_even, void* c32_odd, cudaStream_t s) {
+  const dim3 grid((unsigned)((g.Vh + CB_SITES - 1) / CB_SITES), 2, 1);
+  clover_build_kernel<<<grid, 6 * CB_SITES, 0, s>>>(g, (const double2*)g64_even, (const double2*)g64_odd, 0.5 * c_sw, diag, (double2*)c64_even, (double2*)c64_odd, (float4*)c32_even, (float4*)c32_odd);
   return cudaGetLastError();
 }
 
-// ---- inverse of a packed Hermitian block: Gauss-Jordan with partial pivoting on the full complex 6x6 ----
+// ---- fallback inverse of a packed Hermitian block: Gauss-Jordan with partial pivoting on the full complex 6x6 (used only
+// when the unpivoted factorisation below met a tiny pivot; dynamic row indexing puts M and X in local memory) ----
 // M = C (tw2 == 0) or C^2 + tw2 (twisted clover: (C + i tw)^{-1} = (C - i tw)(C^2 + tw^2)^{-1}); result Hermitian.
-__global__ void __launch_bounds__(64) clover_invert_kernel(const Geom g, const double2* __restrict__ c64, double tw2, double2* inv64, float4* inv32, int* singular) {
+__global__ void __launch_bounds__(64) clover_invert_pivot_kernel(const Geom g, const double2* __restrict__ c64, double tw2, double2* inv64, float4* inv32, int* singular) {
   const int idx = blockIdx.x * 64 + threadIdx.x;  // (block b, cb)
   if (idx >= 2 * g.Vh) return;
   const int b = idx / g.Vh, cb = idx % g.Vh;
@@ -241,9 +279,143 @@ __global__ void __launch_bounds__(64) clover_invert_kernel(const Geom g, const d
   store_reals<36>(inv32 + (int64_t)b * 9 * g.Vh, g.Vh, cb, Pf);
 }
 
-cudaError_t launch_clover_invert(const Geom& g, const void* c64, double tw2, void* inv64, void* inv32, int* singular, cudaStream_t s) {
+// ---- inverse of a packed Hermitian block by an unpivoted L D L^dag factorisation, fully unrolled so that every index is
+// static and the factors live in registers: A = L D L^dag, A^{-1} = L^{-dag} D^{-1} L^{-1}. M = C, or C^2 + tw2 for
+// twisted clover ((C + i tw)^{-1} = (C - i tw)(C^2 + tw^2)^{-1}). Without pivoting the factorisation is backward stable
+// for DEFINITE blocks only — which is what physical parameters give (|clover term| <= 3 c_sw < 4 + m) — so a pivot of
+// the wrong sign or below 1e-6 of the block's scale sets *retry: the host then reruns the field with the pivoted kernel
+// above, which alone decides whether a block is singular. ----
+__global__ void __launch_bounds__(64) clover_invert_kernel(const Geom g, const double2* __restrict__ c64, double tw2, double2* inv64, float4* inv32, int* retry) {
+  const int idx = blockIdx.x * 64 + threadIdx.x;  // (block b, cb)
+  if (idx >= 2 * g.Vh) return;
+  const int b = idx / g.Vh, cb = idx % g.Vh;
+  double P[36];
+  load_reals<36>(c64 + (int64_t)b * 18 * g.Vh, g.Vh, cb, P);
+  // lower triangle of A: a[i][j], j <= i (diagonal real)
+  zd a[6][6];
+#pragma unroll
+  for (int i = 0; i < 6; i++) {
+    a[i][i] = mk<double>(P[i], 0.0);
+#pragma unroll
+    for (int j = 0; j < 6; j++)
+      if (j < i) a[i][j] = mk<double>(P[6 + 2 * (i * (i - 1) / 2 + j)], P[6 + 2 * (i * (i - 1) / 2 + j) + 1]);
+  }
+  if (tw2 != 0.0) {  // A <- A^2 + tw2 (Hermitian): (A^2)_ij = sum_k A_ik conj(A_jk)
+    zd q[6][6];
+#pragma unroll
+    for (int i = 0; i < 6; i++)
+#pragma unroll
+      for (int j = 0; j < 6; j++)
+        if (j <= i) {
+          zd sum = mk<double>(i == j ? tw2 : 0.0, 0.0);
+#pragma unroll
+          for (int k = 0; k < 6; k++) {
+            const zd aik = (k <= i) ? a[i][k] : conj(a[k][i]);
+            const zd ajk = (k <= j) ? a[j][k] : conj(a[k][j]);
+            cmad(sum, aik, conj(ajk));
+          }
+          q[i][j] = sum;
+        }
+#pragma unroll
+    for (int i = 0; i < 6; i++)
+#pragma unroll
+      for (int j = 0; j < 6; j++)
+        if (j <= i) a[i][j] = q[i][j];
+#pragma unroll
+    for (int i = 0; i < 6; i++) a[i][i].im = 0.0;
+  }
+  double scale = 0.0;
+#pragma unroll
+  for (int i = 0; i < 6; i++)
+#pragma unroll
+    for (int j = 0; j < 6; j++)
+      if (j <= i) scale = fmax(scale, fabs(a[i][j].re) + fabs(a[i][j].im));
+  // in place: a[i][j] (j < i) <- L_ij, d[j] <- D_j
+  double d[6], dinv[6];
+  bool bad = !(scale > 0.0);
+#pragma unroll
+  for (int j = 0; j < 6; j++) {
+    double dj = a[j][j].re;
+#pragma unroll
+    for (int k = 0; k < 6; k++)
+      if (k < j) dj -= (a[j][k].re * a[j][k].re + a[j][k].im * a[j][k].im) * d[k];
+    d[j] = dj;
+    // stable only for definite blocks (all pivots of one sign, none tiny): anything else goes to the pivoted kernel
+    if (!(fabs(dj) > 1e-6 * scale) || dj * d[0] < 0.0) bad = true;
+    dinv[j] = 1.0 / dj;
+#pragma unroll
+    for (int i = 0; i < 6; i++)
+      if (i > j) {
+        zd v = a[i][j];
+#pragma unroll
+        for (int k = 0; k < 6; k++)
+          if (k < j) {
+            const zd t = a[i][k] * conj(a[j][k]);
+            v.re -= t.re * d[k];
+            v.im -= t.im * d[k];
+          }
+        a[i][j] = mk<double>(v.re * dinv[j], v.im * dinv[j]);
+      }
+  }
+  // W = L^{-1} (unit lower), in place column by column: W_ij = -L_ij - sum_{j<k<i} L_ik W_kj
+  zd w[6][6];
+#pragma unroll
+  for (int j = 0; j < 6; j++)
+#pragma unroll
+    for (int i = 0; i < 6; i++)
+      if (i > j) {
+        zd v = mk<double>(-a[i][j].re, -a[i][j].im);
+#pragma unroll
+        for (int k = 0; k < 6; k++)
+          if (k > j && k < i) {
+            const zd t = a[i][k] * w[k][j];
+            v.re -= t.re;
+            v.im -= t.im;
+          }
+        w[i][j] = v;
+      }
+  // A^{-1}_ij = sum_{k >= i} conj(W_ki) W_kj / D_k  (i >= j; W_kk = 1)
+  if (bad) {
+    atomicExch(retry, 1);
+    return;
+  }
+#pragma unroll
+  for (int i = 0; i < 6; i++) {
+#pragma unroll
+    for (int j = 0; j < 6; j++)
+      if (j <= i) {
+        zd sum = mk<double>(0.0, 0.0);
+#pragma unroll
+        for (int k = 0; k < 6; k++)
+          if (k >= i) {
+            const zd wki = (k == i) ? mk<double>(1.0, 0.0) : w[k][i];
+            const zd wkj = (k == j) ? mk<double>(1.0, 0.0) : w[k][j];
+            const zd t = conj(wki) * wkj;
+            sum.re += t.re * dinv[k];
+            sum.im += t.im * dinv[k];
+          }
+        if (i == j) P[i] = sum.re;
+        else {
+          P[6 + 2 * (i * (i - 1) / 2 + j)] = sum.re;
+          P[6 + 2 * (i * (i - 1) / 2 + j) + 1] = sum.im;
+        }
+      }
+  }
+  float Pf[36];
+#pragma unroll
+  for (int i = 0; i < 36; i++) Pf[i] = (float)P[i];
+  store_reals<36>(inv64 + (int64_t)b * 18 * g.Vh, g.Vh, cb, P);
+  store_reals<36>(inv32 + (int64_t)b * 9 * g.Vh, g.Vh, cb, Pf);
+}
+
+cudaError_t launch_clover_invert(const Geom& g, const void* c64, double tw2, void* inv64, void* inv32, int* flag, cudaStream_t s) {
   const int n = 2 * g.Vh;
-  clover_invert_kernel<<<(n + 63) / 64, 64, 0, s>>>(g, (const double2*)c64, tw2, (double2*)inv64, (float4*)inv32, singular);
+  clover_invert_kernel<<<(n + 63) / 64, 64, 0, s>>>(g, (const double2*)c64, tw2, (double2*)inv64, (float4*)inv32, flag);
+  return cudaGetLastError();
+}
+cudaError_t launch_clover_invert_pivot(const Geom& g, const void* c64, double tw2, void* inv64, void* inv32, int* singular, cudaStream_t s) {
+  const int n = 2 * g.Vh;
+  clover_invert_pivot_kernel<<<(n + 63) / 64, 64, 0, s>>>(g, (const double2*)c64, tw2, (double2*)inv64, (float4*)inv32, singular);
   return cudaGetLastError();
 }
 

@@ -22,11 +22,14 @@ cudaError_t launch_pack_spinor(const Geom& g, int par, int prec, const double* c
 cudaError_t launch_unpack_spinor(const Geom& g, int par, int prec, const void* packed, double* canon, cudaStream_t s);
 
 // ---- clover (tmw_clover.cu) ----
-// From the canonical fp64 gauge: packed Hermitian blocks C = (c_sw/2) sum sigma F + diag, both parities,
-// fp64 [36 planes][Vh] double2 and fp32 [18 planes][Vh] float4.
-cudaError_t launch_clover_build(const Geom& g, const double* canon_gauge, double c_sw, double diag, void* c64_even, void* c64_odd, void* c32_even, void* c32_odd, cudaStream_t s);
-// inverse blocks of one parity: (C^2 + tw2)^{-1} if tw2 != 0 else C^{-1}; *singular (device int) is set on failure
-cudaError_t launch_clover_invert(const Geom& g, const void* c64, double tw2, void* inv64, void* inv32, int* singular, cudaStream_t s);
+// From the packed fp64 gauge (launch_pack_gauge's g64): packed Hermitian blocks C = (c_sw/2) sum sigma F + diag, both
+// parities, fp64 [36 planes][Vh] double2 and fp32 [18 planes][Vh] float4.
+cudaError_t launch_clover_build(const Geom& g, const void* g64_even, const void* g64_odd, double c_sw, double diag, void* c64_even, void* c64_odd, void* c32_even, void* c32_odd, cudaStream_t s);
+// inverse blocks of one parity: (C^2 + tw2)^{-1} if tw2 != 0 else C^{-1}. launch_clover_invert: unpivoted LDL^dag in
+// registers; *flag (device int) is set if any block met a tiny pivot (its output is then not written) and the caller
+// reruns the field with launch_clover_invert_pivot (Gauss-Jordan with pivoting), whose *singular is set on failure.
+cudaError_t launch_clover_invert(const Geom& g, const void* c64, double tw2, void* inv64, void* inv32, int* flag, cudaStream_t s);
+cudaError_t launch_clover_invert_pivot(const Geom& g, const void* c64, double tw2, void* inv64, void* inv32, int* singular, cudaStream_t s);
 // packed [planes][Vh] double2 blocks -> [cb][2][36] doubles
 cudaError_t launch_clover_export(const Geom& g, const void* c64, double* dst, cudaStream_t s);
 

@@ -181,8 +181,13 @@ def test_full_apply_vs_oracle(tmw, case):
 # ------------------------------------------------------------------------------------------------------
 # clover blocks (A1) and their inverse (A2) against the oracle's F and sigma
 # ------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("L,T,m,c_sw", [(4, 6, -0.0695 + 0.0j, 1.0509), (6, 4, -0.044 + 0.2j, 1.0349)])
-def test_clover_blocks_and_inverse(tmw, L, T, m, c_sw):
+@pytest.mark.parametrize("pivot", [False, True])
+@pytest.mark.parametrize("L,T,m,c_sw", [(4, 6, -0.0695 + 0.0j, 1.0509), (6, 4, -0.044 + 0.2j, 1.0349), (8, 4, -3.9 + 0.0j, 2.5)])
+def test_clover_blocks_and_inverse(tmw, L, T, m, c_sw, pivot, monkeypatch):
+    """the third case makes the blocks indefinite (diagonal -(4+m) = -0.1, clover term of order 1): the unpivoted
+    L D L^dag still has to invert them; pivot = True forces the Gauss-Jordan fallback kernel (TMW_CLOVER_PIVOT)."""
+    if pivot:
+        monkeypatch.setenv("TMW_CLOVER_PIVOT", "1")
     U = synth.gauge_field(L, T, 0.4, seed=1)
     blocks = H.site_diagonal_blocks(U, c_sw, m.real)  # (V,2,6,6)
     Vh = L ** 3 * T // 2
@@ -199,7 +204,11 @@ def test_clover_blocks_and_inverse(tmw, L, T, m, c_sw):
         be = blocks[H.parity_sites(L, T, 0)]
         ref_inv = np.linalg.inv(be @ be + m.imag ** 2 * np.eye(6)) if m.imag != 0 else np.linalg.inv(be)
         ref = H.pack_hermitian(ref_inv)
-        assert np.max(np.abs(dst.cpu().numpy() - ref) / np.max(np.abs(ref))) <= 1e-12
+        got = dst.cpu().numpy()
+        # relative to each block's own largest entry (indefinite blocks can have large inverses)
+        scale = np.max(np.abs(ref), axis=-1, keepdims=True)
+        cond = np.linalg.cond(be @ be + m.imag ** 2 * np.eye(6) if m.imag != 0 else be)
+        assert np.max(np.abs(got - ref) / scale / cond[..., None]) <= 1e-13
 
 
 # ------------------------------------------------------------------------------------------------------
