@@ -47,6 +47,8 @@ def parse_args():
     ap.add_argument("--cpu-sites", type=int, default=0, help="oracle sample size in sites (0: sized for ~15 s)")
     ap.add_argument("--multi-rhs", type=int, default=3,
                     help="columns of the extra tmw_solve_multi / tmw_apply_multi leg (0 or 1: skip); 3 fit at 48^3 x 144")
+    ap.add_argument("--cpu-solve", action="store_true",
+                    help="also time the oracle's full-lattice fp64 BiCGStab on this config's source (minutes at 32^3 x 96)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--skip-solve", action="store_true",
@@ -225,8 +227,11 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
     # ---- inputs resident in HBM: a point source for the solve, a Gaussian spinor for the Dslash-only run ----
     from paper_2201_09004_b200 import columns
     spin, colour = columns.spin_colour(columns.columns_for_rank(rank, world)[0])
-    b = torch.zeros((T, L, L, L, 4, 3), dtype=torch.complex128, device="cuda")
-    b[0, 0, 0, 0, spin, colour] = 1.0
+    if cfg["source"] == "z2":  # configs[1]: Z2 noise (C15); the others: a point source at the origin (C13)
+        b = torch.from_numpy(synth.z2_source(L, T, 2)).cuda()
+    else:
+        b = torch.zeros((T, L, L, L, 4, 3), dtype=torch.complex128, device="cuda")
+        b[0, 0, 0, 0, spin, colour] = 1.0
     x = torch.empty_like(b)
     psi_host = synth.gaussian_spinor(L, T, seed=3)
     nb = ctx.spinor_bytes(tmw.F32)
@@ -299,8 +304,7 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
     e2e = None
     if not args.no_e2e:
         cbytes = V * 24 * 8
-        hb = torch.zeros((T, L, L, L, 4, 3), dtype=torch.complex128).pin_memory()
-        hb[0, 0, 0, 0, spin, colour] = 1.0
+        hb = b.cpu().pin_memory()
         hx = torch.empty((T, L, L, L, 4, 3), dtype=torch.complex128).pin_memory()
         hpsi = torch.from_numpy(psi_host).pin_memory()
         ctx.set_location(tmw.HOST)
@@ -376,6 +380,13 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
                "sample": f"oracle.apply_sites (fp64, hopping + mass of Eq. (2), explicit 4x4 gamma matrices) at {n} "
                          f"evenly spaced sites of the same {L}^3x{T} field, {passes} pass(es), {dt:.1f} s",
                "msites_per_s": ns / dt / 1e6}
+        if args.cpu_solve:
+            import oracle
+            bsrc = synth.z2_source(L, T, 2) if cfg["source"] == "z2" else synth.point_source(L, T, spin, colour)
+            t0 = time.perf_counter()
+            _, oinfo = oracle.bicgstab(np.asarray(U), bsrc, m, c_sw, tol=args.tol)
+            cpu.update(solve_s=time.perf_counter() - t0, solve_iters=oinfo["iters"], solve_true_resid=oinfo["true_resid"],
+                       solve="oracle.bicgstab (full-lattice fp64 BiCGStab, no preconditioning), incl. its clover-leaf setup")
 
     ctx.destroy()
     if rank == 0:
@@ -383,7 +394,8 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
                 "warmup": max(3, args.warmup), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": cfg["name"], "L": L, "T": T, "m": list(cfg["m"]), "c_sw": c_sw, "eps": cfg["eps"],
-                           "gauge": "fp32 12-real (fp64 18-real for the outer residual)", "source": "point, origin",
+                           "gauge": "fp32 12-real (fp64 18-real for the outer residual)",
+                           "source": "Z2 noise, seed 2" if cfg["source"] == "z2" else "point, origin",
                            "step": ("SOLVE SKIPPED (profiling run, not a bench value): " if args.skip_solve else
                                     f"1 tmw_solve(tol={args.tol:g}) + ") + f"{napply} fp32 Dslash applications",
                            "parallelism": "replicas" if world > 1 else "single",
