@@ -141,7 +141,7 @@ static DslashArgs<R> make_args(const tmw_ctx* c, int par, int dagger, const void
   a.red = nullptr;
   a.ncol = cm.n;
   a.ngroups = 1;
-  a.cstride = (int64_t)c->g.Vh * 24 * (int64_t)sizeof(R) / 16;
+  a.cstride = (int)((int64_t)c->g.Vh * 24 * (int64_t)sizeof(R) / 16);
   a.red_stride = 0;
   for (int i = 0; i < MAXCOL; i++) a.col[i] = cm.col[i];
   return a;
@@ -154,6 +154,9 @@ template <typename R>
 static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, void* out, const void* aux, double sgn, const ColMap& cm,
                   int red_mode = 0, const void* dotv = nullptr, double* red = nullptr, int red_stride = 0, int g5 = 0) {
   DslashArgs<R> a = make_args<R>(ctx, par, dagger, in, out, aux, sgn, cm);
+  for (int i = 0; i < cm.n; i++)  // the kernels add column * cstride to a 32-bit site index
+    if (((int64_t)cm.col[i] + 1) * ((int64_t)ctx->g.Vh * 24 * (int64_t)sizeof(R) / 16) >= ((int64_t)1 << 31))
+      return fail(ctx, TMW_EINVAL, "lattice too large for this many right-hand-side columns in one call");
   a.g5 = g5;
   a.red_mode = red_mode;
   a.dotv = dotv;
@@ -169,7 +172,7 @@ static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, vo
       nr = ((cm.n + 2) / 3 * 3 < (cm.n + 1) / 2 * 2) ? 3 : 2;
     }
   }
-  LAUNCH(launch_dslash(a, ng_of<R>(ctx), epi, ctx->clover, nr, ctx->stream));
+  LAUNCH(launch_dslash(a, ng_of<R>(ctx), epi, !ctx->clover ? CL_NONE : (ctx->m_im != 0.0 ? CL_TWISTED : CL_CLOVER), nr, ctx->stream));
   return TMW_OK;
 }
 // Schur operator on the odd sites: out = A_oo in - H_oe A_ee^{-1} H_eo in  (tmp: even-parity scratch)
@@ -389,30 +392,44 @@ int tmw_get_clover(tmw_ctx* ctx, int parity, int inverse, double* dst) {
 }  // extern "C"
 
 // ---- workspaces ----
+static void release_ws(tmw_ctx* ctx) {
+  for (int i = 0; i < 10; i++) if (ctx->w64[i]) { dev_free(ctx, ctx->w64[i]); ctx->w64[i] = nullptr; }
+  for (int i = 0; i < 8; i++) if (ctx->w32[i]) { dev_free(ctx, ctx->w32[i]); ctx->w32[i] = nullptr; }
+  for (int i = 0; i < 2; i++) if (ctx->canon[i]) { dev_free(ctx, ctx->canon[i]); ctx->canon[i] = nullptr; }
+}
 // make the workspaces hold `cols` columns (existing smaller ones are released and re-made on demand)
 static int need_cols(tmw_ctx* ctx, int cols) {
   if (cols <= ctx->ws_cols) return TMW_OK;
   cudaError_t e = cudaStreamSynchronize(ctx->stream);
   if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaStreamSynchronize");
-  for (int i = 0; i < 10; i++) if (ctx->w64[i]) { dev_free(ctx, ctx->w64[i]); ctx->w64[i] = nullptr; }
-  for (int i = 0; i < 8; i++) if (ctx->w32[i]) { dev_free(ctx, ctx->w32[i]); ctx->w32[i] = nullptr; }
-  for (int i = 0; i < 2; i++) if (ctx->canon[i]) { dev_free(ctx, ctx->canon[i]); ctx->canon[i] = nullptr; }
+  release_ws(ctx);
   ctx->ws_cols = cols;
   return TMW_OK;
 }
+// A failed workspace allocation (TMW_ENOMEM: too many columns for this lattice) releases every workspace and goes back
+// to one column, so that the context stays usable for smaller calls.
+static int ws_alloc(tmw_ctx* ctx, void** p, size_t bytes) {
+  const int rc = dev_alloc(ctx, p, bytes);
+  if (rc) {
+    cudaStreamSynchronize(ctx->stream);
+    release_ws(ctx);
+    ctx->ws_cols = 1;
+  }
+  return rc;
+}
 static int need_w64(tmw_ctx* ctx, int n) {
   for (int i = 0; i < n; i++)
-    if (!ctx->w64[i]) { int rc = dev_alloc(ctx, &ctx->w64[i], spinor_bytes(ctx, TMW_F64) * ctx->ws_cols); if (rc) return rc; }
+    if (!ctx->w64[i]) { int rc = ws_alloc(ctx, &ctx->w64[i], spinor_bytes(ctx, TMW_F64) * ctx->ws_cols); if (rc) return rc; }
   return TMW_OK;
 }
 static int need_w32(tmw_ctx* ctx, int n, int prec) {
   for (int i = 0; i < n; i++)
-    if (!ctx->w32[i]) { int rc = dev_alloc(ctx, &ctx->w32[i], spinor_bytes(ctx, prec) * ctx->ws_cols); if (rc) return rc; }
+    if (!ctx->w32[i]) { int rc = ws_alloc(ctx, &ctx->w32[i], spinor_bytes(ctx, prec) * ctx->ws_cols); if (rc) return rc; }
   return TMW_OK;
 }
 static int need_canon(tmw_ctx* ctx) {
   for (int i = 0; i < 2; i++)
-    if (!ctx->canon[i]) { int rc = dev_alloc(ctx, &ctx->canon[i], (size_t)ctx->V * 24 * 8 * ctx->ws_cols); if (rc) return rc; }
+    if (!ctx->canon[i]) { int rc = ws_alloc(ctx, &ctx->canon[i], (size_t)ctx->V * 24 * 8 * ctx->ws_cols); if (rc) return rc; }
   return TMW_OK;
 }
 static inline void* colp(void* base, int c, size_t bytes) { return (char*)base + (size_t)c * bytes; }
@@ -529,10 +546,10 @@ extern "C" int tmw_apply_schur_multi(tmw_ctx* ctx, int op, int prec, int nrhs, c
   const int dagger = (op == TMW_DDAG);
   int rc;
   if ((rc = need_cols(ctx, nrhs))) return rc;
-  if ((rc = need_w64(ctx, 1))) return rc;  // even-parity scratch (an fp32 call uses the head of each fp64 column... see below)
+  if ((rc = need_w64(ctx, 1))) return rc;  // even-parity scratch for nrhs columns
   const ColMap cm = cols_first(nrhs);
   if (prec == TMW_F64) return schur<double>(ctx, dagger, in_odd, out_odd, ctx->w64[0], cm);
-  // fp32: columns of the scratch are fp32 spinors packed back to back at the start of the fp64 workspace
+  // fp32: the scratch columns are fp32 spinors back to back at the start of the (twice as large) fp64 workspace
   return schur<float>(ctx, dagger, in_odd, out_odd, ctx->w64[0], cm);
 }
 extern "C" int tmw_apply_schur(tmw_ctx* ctx, int op, int prec, const void* in_odd, void* out_odd) {

@@ -442,6 +442,11 @@ template <typename R, bool CLOVER> TMW_HD void apply_Ainv(const Diag<R>& d, int 
 // ---------------------------------------------------------------------------------------------------------
 enum { MAXCOL = 16 };  // most right-hand sides per call
 
+// kind of site-diagonal part a stencil kernel is compiled for: no clover (a complex scalar per chirality), clover, or
+// clover with a twist, whose inverse is two factors. A compile-time choice: as a runtime branch the
+// two-factor path cost the common K1 kernel 32 bytes of register spills.
+enum { CL_NONE = 0, CL_CLOVER = 1, CL_TWISTED = 2 };
+
 enum { EPI_HOP = 0,        // out = h
        EPI_AINV_HOP = 1,   // out = A^{-1} h                      (K1 of the Schur operator)
        EPI_A_XPAY = 2,     // out = A aux + sgn*h                 (K2: sgn = -1; full apply: sgn = +1)
@@ -470,7 +475,7 @@ template <typename R> struct DslashArgs {
   // are loaded once for the NR columns); CTAs of the ngroups = ceil(ncol/NR) slot groups of one site block are
   // adjacent in blockIdx.x, so the groups after the first find the links in L2.
   int ncol, ngroups;
-  int64_t cstride;
+  int cstride;  // 16-byte vectors per column; (columns in the buffers) * cstride < 2^31 (checked by the host)
   int red_stride;
   unsigned char col[MAXCOL];
 };
@@ -500,7 +505,7 @@ TMW_HD Nbr neighbours(const Geom& g, int par, const Site& s) {
 }
 
 template <typename R, int NG, int MU, int NR>
-__device__ __forceinline__ void hop_pair(const DslashArgs<R>& a, const Nbr& n, int cb, const int64_t (&coff)[NR], R (&acc)[NR][24]) {
+__device__ __forceinline__ void hop_pair(const DslashArgs<R>& a, const Nbr& n, int cb, const int (&cofs)[NR], R (&acc)[NR][24]) {
   const int NPG = Planes<R, NG>::N;
   const int64_t Vh = a.g.Vh;
   typedef typename Vec16<R>::T V;
@@ -511,7 +516,7 @@ __device__ __forceinline__ void hop_pair(const DslashArgs<R>& a, const Nbr& n, i
 #pragma unroll
     for (int j = 0; j < NR; j++) {
       R psi[24];
-      load_reals<24>((const V*)a.in + coff[j], Vh, n.fwd[MU], psi);
+      load_reals<24>(a.in, Vh, n.fwd[MU] + cofs[j], psi);
       hop<R, MU, true>(psi, U, a.sig, bc, acc[j]);
     }
   }
@@ -522,7 +527,7 @@ __device__ __forceinline__ void hop_pair(const DslashArgs<R>& a, const Nbr& n, i
 #pragma unroll
     for (int j = 0; j < NR; j++) {
       R psi[24];
-      load_reals<24>((const V*)a.in + coff[j], Vh, n.bwd[MU], psi);
+      load_reals<24>(a.in, Vh, n.bwd[MU] + cofs[j], psi);
       hop<R, MU, false>(psi, U, -a.sig, bc, acc[j]);
     }
   }
@@ -530,10 +535,10 @@ __device__ __forceinline__ void hop_pair(const DslashArgs<R>& a, const Nbr& n, i
 
 // One chirality b (12 reals: spins 2b, 2b+1) of the site-diagonal part, with the block held in registers so that it
 // serves several right-hand sides: w = A_b v and w = A_b^{-1} v as in apply_A / apply_Ainv above.
-template <typename R, bool CLOVER> TMW_HD void load_block(const void* base, int b, int64_t Vh, int64_t cb, R* B) {
+template <typename R, int CLOVER> TMW_HD void load_block(const void* base, int b, int64_t Vh, int64_t cb, R* B) {
   if (CLOVER) load_reals_s<36>((const typename Vec16<R>::T*)base + (int64_t)b * Planes<R, 36>::N * Vh, Vh, cb, B);
 }
-template <typename R, bool CLOVER> TMW_HD void half_A(const Diag<R>& d, int b, const R* B, const R* v, R* w) {
+template <typename R, int CLOVER> TMW_HD void half_A(const Diag<R>& d, int b, const R* B, const R* v, R* w) {
   if (CLOVER) {
     herm6_mul(B, v, w);
   } else {
@@ -549,7 +554,7 @@ template <typename R, bool CLOVER> TMW_HD void half_A(const Diag<R>& d, int b, c
 }
 // no clover: the complex scalar inverse; clover: w = Binv v (Binv = C^{-1}, or (C^2 + tw^2)^{-1} when twisted: the
 // caller then multiplies by (C - i tw) with half_twfix)
-template <typename R, bool CLOVER> TMW_HD void half_Ainv(const Diag<R>& d, int b, const R* Binv, const R* v, R* w) {
+template <typename R, int CLOVER> TMW_HD void half_Ainv(const Diag<R>& d, int b, const R* Binv, const R* v, R* w) {
   if (CLOVER) {
     herm6_mul(Binv, v, w);
   } else {
@@ -571,21 +576,26 @@ template <typename R> TMW_HD void half_twfix(const Diag<R>& d, int b, const R* C
   }
 }
 
+// true if dslash_site has already stored the result (the untwisted clover K1)
+template <int EPI, int CLOVER> __device__ __forceinline__ constexpr bool stored_in_site() { return EPI == EPI_AINV_HOP && CLOVER == CL_CLOVER; }
+
 // The stencil at one site for NR right-hand sides: on return acc[j] holds the output spinor of column slot j.
 // red[j] = {Re, Im <out, aux>, <out, out>} when WANT_RED2 (EPI >= 2), accumulated chirality by chirality.
-template <typename R, int NG, int EPI, bool CLOVER, int NR>
-__device__ __forceinline__ void dslash_site(const DslashArgs<R>& a, const Site& s, const int64_t (&coff)[NR], R (&acc)[NR][24], R (&red2)[NR][3]) {
+template <typename R, int NG, int EPI, int CLOVER, int NR>
+__device__ __forceinline__ void dslash_site(const DslashArgs<R>& a, const Site& s, const int (&cofs)[NR], const bool (&valid)[NR], R (&acc)[NR][24], R (&red2)[NR][3]) {
   typedef typename Vec16<R>::T V;
+  // cofs[j] = column * cstride: the column offset is added to the 32-bit SITE INDEX (the host checks that it fits), so
+  // that every load address stays one IMAD.WIDE on a kernel-parameter base pointer, as with a single column
   const Nbr n = neighbours(a.g, a.par, s);
   const int cb = s.cb;
 #pragma unroll
   for (int j = 0; j < NR; j++)
 #pragma unroll
     for (int i = 0; i < 24; i++) acc[j][i] = (R)0;
-  hop_pair<R, NG, 0, NR>(a, n, cb, coff, acc);
-  hop_pair<R, NG, 1, NR>(a, n, cb, coff, acc);
-  hop_pair<R, NG, 2, NR>(a, n, cb, coff, acc);
-  hop_pair<R, NG, 3, NR>(a, n, cb, coff, acc);
+  hop_pair<R, NG, 0, NR>(a, n, cb, cofs, acc);
+  hop_pair<R, NG, 1, NR>(a, n, cb, cofs, acc);
+  hop_pair<R, NG, 2, NR>(a, n, cb, cofs, acc);
+  hop_pair<R, NG, 3, NR>(a, n, cb, cofs, acc);
   const int64_t Vh = a.g.Vh;
 #pragma unroll
   for (int j = 0; j < NR; j++) {
@@ -604,11 +614,17 @@ __device__ __forceinline__ void dslash_site(const DslashArgs<R>& a, const Site& 
     for (int j = 0; j < NR; j++) {
       R* o = acc[j] + 12 * b;
       R ax[12], w[12];
-      if (EPI >= 2) load_reals<12>((const V*)a.aux + coff[j] + (int64_t)b * HP * Vh, Vh, cb, ax);
+      if (EPI >= 2) load_reals<12>((const V*)a.aux + (int64_t)b * HP * Vh, Vh, cb + cofs[j], ax);
       if (EPI == EPI_AINV_HOP) {
         half_Ainv<R, CLOVER>(a.d, b, B, o, w);
+        if (stored_in_site<EPI, CLOVER>()) {
+          // K1 has no fused reduction and no gamma5: store this chirality now, so that its accumulators are dead
+          // before the block of the other chirality is loaded (the kernel wrapper skips its store, see stored_in_site)
+          if (valid[j]) store_reals_s<12>((V*)a.out + (int64_t)b * HP * Vh, Vh, cb + cofs[j], w);
+        } else {
 #pragma unroll
-        for (int i = 0; i < 12; i++) o[i] = w[i];
+          for (int i = 0; i < 12; i++) o[i] = w[i];
+        }
       } else if (EPI == EPI_A_XPAY) {
         half_A<R, CLOVER>(a.d, b, B, ax, w);
 #pragma unroll
@@ -632,8 +648,8 @@ __device__ __forceinline__ void dslash_site(const DslashArgs<R>& a, const Site& 
         }
       }
     }
-    if (CLOVER && (EPI == EPI_AINV_HOP || EPI == EPI_AINV_XPAY)) {
-      if (a.d.twisted_clover) {  // (C + i tw)^{-1} = (C - i tw)(C^2 + tw^2)^{-1}: second factor, same registers
+    if (CLOVER == CL_TWISTED && (EPI == EPI_AINV_HOP || EPI == EPI_AINV_XPAY)) {
+      {  // (C + i tw)^{-1} = (C - i tw)(C^2 + tw^2)^{-1}: second factor, same registers
         load_block<R, CLOVER>(a.d.c[a.par], b, Vh, cb, B);
 #pragma unroll
         for (int j = 0; j < NR; j++) {

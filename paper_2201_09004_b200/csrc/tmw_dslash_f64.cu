@@ -3,7 +3,7 @@
 #include "tmw_dslash_impl.cuh"
 
 namespace tmw {
-cudaError_t launch_dslash(const DslashArgs<double>& a, int ng, int epi, bool clover, int nr, cudaStream_t s) {
+cudaError_t launch_dslash(const DslashArgs<double>& a, int ng, int epi, int clover, int nr, cudaStream_t s) {
   (void)nr;
   if (ng == 18) return launch_epi<double, 18, 1>(a, epi, clover, s);
   return cudaErrorInvalidValue;

@@ -28,7 +28,7 @@ template <int NV, int BLOCK> __device__ __forceinline__ void block_reduce_atomic
   }
 }
 
-template <typename R, int NG, int EPI, bool CLOVER, int NR, int BLOCK, int MINB>
+template <typename R, int NG, int EPI, int CLOVER, int NR, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<R> a) {
   typedef typename Vec16<R>::T V;
   // blockIdx.x = group + ngroups * site block: the CTAs that share the links of a site block are launched together
@@ -39,28 +39,29 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<R>
   }
   Site s;
   const bool active = thread_site<BLOCK>(a.g, sblock, s);
-  int64_t coff[NR];
-  int colj[NR];
+  int colj[NR], cofs[NR];
   bool valid[NR];
 #pragma unroll
   for (int j = 0; j < NR; j++) {
     const int slot = grp * NR + j;
     valid[j] = slot < a.ncol;  // a ragged last group recomputes the last column and drops the result
     colj[j] = a.col[valid[j] ? slot : a.ncol - 1];
-    coff[j] = (int64_t)colj[j] * a.cstride;
+    cofs[j] = colj[j] * a.cstride;
   }
   R o[NR][24], r2[NR][3];
   if (active) {
-    dslash_site<R, NG, EPI, CLOVER, NR>(a, s, coff, o, r2);
-    if (a.g5) {  // uniform across the grid
+    dslash_site<R, NG, EPI, CLOVER, NR>(a, s, cofs, valid, o, r2);
+    if (!stored_in_site<EPI, CLOVER>()) {
+      if (a.g5) {  // uniform across the grid
+#pragma unroll
+        for (int j = 0; j < NR; j++)
+#pragma unroll
+          for (int i = 12; i < 24; i++) o[j][i] = -o[j][i];
+      }
 #pragma unroll
       for (int j = 0; j < NR; j++)
-#pragma unroll
-        for (int i = 12; i < 24; i++) o[j][i] = -o[j][i];
+        if (valid[j]) store_reals_s<24>(a.out, a.g.Vh, s.cb + cofs[j], o[j]);
     }
-#pragma unroll
-    for (int j = 0; j < NR; j++)
-      if (valid[j]) store_reals_s<24>((V*)a.out + coff[j], a.g.Vh, s.cb, o[j]);
   }
   if (a.red_mode != 0) {  // uniform across the grid
 #pragma unroll
@@ -69,7 +70,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<R>
       if (active && valid[j]) {
         if (a.red_mode == 1) {
           R d[24];
-          load_reals<24>((const V*)a.dotv + coff[j], a.g.Vh, s.cb, d);
+          load_reals<24>(a.dotv, a.g.Vh, s.cb + cofs[j], d);
           R re = 0, im = 0;
 #pragma unroll
           for (int i = 0; i < 12; i++) {  // conj(d) * o
@@ -109,7 +110,7 @@ template <> struct Tune<float, 3> { enum { BLOCK = 128, MINB = 3 }; };
 template <> struct Tune<float, 4> { enum { BLOCK = 128, MINB = 2 }; };
 template <> struct Tune<double, 1> { enum { BLOCK = 128, MINB = 2 }; };
 
-template <typename R, int NG, int EPI, bool CLOVER, int NR> static cudaError_t launch_one(DslashArgs<R> a, cudaStream_t s) {
+template <typename R, int NG, int EPI, int CLOVER, int NR> static cudaError_t launch_one(DslashArgs<R> a, cudaStream_t s) {
   const int B = Tune<R, NR>::BLOCK;
   a.ngroups = (a.ncol + NR - 1) / NR;
   dim3 grid;
@@ -119,13 +120,18 @@ template <typename R, int NG, int EPI, bool CLOVER, int NR> static cudaError_t l
   return cudaGetLastError();
 }
 
-template <typename R, int NG, int NR> static cudaError_t launch_epi(const DslashArgs<R>& a, int epi, bool clover, cudaStream_t s) {
+// clover: CL_NONE | CL_CLOVER | CL_TWISTED; only the kernels that apply A^{-1} have a separate twisted instantiation
+template <typename R, int NG, int NR> static cudaError_t launch_epi(const DslashArgs<R>& a, int epi, int clover, cudaStream_t s) {
   switch (epi) {
-    case EPI_HOP: return launch_one<R, NG, EPI_HOP, false, NR>(a, s);
-    case EPI_AINV_HOP: return clover ? launch_one<R, NG, EPI_AINV_HOP, true, NR>(a, s) : launch_one<R, NG, EPI_AINV_HOP, false, NR>(a, s);
-    case EPI_A_XPAY: return clover ? launch_one<R, NG, EPI_A_XPAY, true, NR>(a, s) : launch_one<R, NG, EPI_A_XPAY, false, NR>(a, s);
-    case EPI_XPAY: return launch_one<R, NG, EPI_XPAY, false, NR>(a, s);
-    case EPI_AINV_XPAY: return clover ? launch_one<R, NG, EPI_AINV_XPAY, true, NR>(a, s) : launch_one<R, NG, EPI_AINV_XPAY, false, NR>(a, s);
+    case EPI_HOP: return launch_one<R, NG, EPI_HOP, CL_NONE, NR>(a, s);
+    case EPI_AINV_HOP:
+      if (clover == CL_TWISTED) return launch_one<R, NG, EPI_AINV_HOP, CL_TWISTED, NR>(a, s);
+      return clover ? launch_one<R, NG, EPI_AINV_HOP, CL_CLOVER, NR>(a, s) : launch_one<R, NG, EPI_AINV_HOP, CL_NONE, NR>(a, s);
+    case EPI_A_XPAY: return clover ? launch_one<R, NG, EPI_A_XPAY, CL_CLOVER, NR>(a, s) : launch_one<R, NG, EPI_A_XPAY, CL_NONE, NR>(a, s);
+    case EPI_XPAY: return launch_one<R, NG, EPI_XPAY, CL_NONE, NR>(a, s);
+    case EPI_AINV_XPAY:
+      if (clover == CL_TWISTED) return launch_one<R, NG, EPI_AINV_XPAY, CL_TWISTED, NR>(a, s);
+      return clover ? launch_one<R, NG, EPI_AINV_XPAY, CL_CLOVER, NR>(a, s) : launch_one<R, NG, EPI_AINV_XPAY, CL_NONE, NR>(a, s);
   }
   return cudaErrorInvalidValue;
 }

@@ -5,10 +5,10 @@
 namespace tmw {
 
 // ---- stencil (tmw_dslash_f32.cu / tmw_dslash_f64.cu) ----
-// ng = stored reals per link (12 | 18), epi = EPI_*, clover = the diagonal part has clover blocks,
+// ng = stored reals per link (12 | 18), epi = EPI_*, clover = CL_NONE | CL_CLOVER | CL_TWISTED (kind of diagonal part),
 // nr = right-hand-side columns per thread (fp32: 1..4; fp64: always 1)
-cudaError_t launch_dslash(const DslashArgs<float>& a, int ng, int epi, bool clover, int nr, cudaStream_t s);
-cudaError_t launch_dslash(const DslashArgs<double>& a, int ng, int epi, bool clover, int nr, cudaStream_t s);
+cudaError_t launch_dslash(const DslashArgs<float>& a, int ng, int epi, int clover, int nr, cudaStream_t s);
+cudaError_t launch_dslash(const DslashArgs<double>& a, int ng, int epi, int clover, int nr, cudaStream_t s);
 // out = A in (inverse = 0) or A^{-1} in (inverse = 1) on parity par, site-local
 cudaError_t launch_diag(const Diag<float>& d, const Geom& g, int par, bool clover, int inverse, const void* in, void* out, cudaStream_t s);
 cudaError_t launch_diag(const Diag<double>& d, const Geom& g, int par, bool clover, int inverse, const void* in, void* out, cudaStream_t s);

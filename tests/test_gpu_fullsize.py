@@ -251,9 +251,15 @@ def test_fullsize_config4_solve(tmw):
     with tmw.Context(L, T, dU, m, c_sw) as ctx:
         del dU
         x = torch.empty((T, L, L, L, 4, 3), dtype=torch.complex128, device="cuda")
-        info = ctx.solve(torch.from_numpy(b).cuda(), x, 1e-10)
+        db = torch.from_numpy(b).cuda()
+        # 16 columns need 16 x 18.3 GB of workspace here: more than the GPU has. The call must fail with TMW_ENOMEM before
+        # it touches b or x (so one-column buffers are enough), release what it allocated, and leave the context usable.
+        with pytest.raises(tmw.TmwError) as e:
+            ctx.solve_multi(16, db, x, 1e-10)
+        assert e.value.code == tmw.ENOMEM
+        info = ctx.solve(db, x, 1e-10)
         xg = x.cpu().numpy()
-        del x
+        del x, db
     torch.cuda.empty_cache()
     assert info["true_resid"] <= 1e-10
     mx, est = sampled_residual(U, b, xg, m, c_sw, rnd, det)
