@@ -12,8 +12,17 @@
 #include <string>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>  // header-only: ranges around the phases of create / apply / solve for nsys and ncu --nvtx
+
 #include "../../include/tmw.h"
 #include "tmw_internal.h"
+
+namespace {
+struct NvtxRange {
+  explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+  ~NvtxRange() { nvtxRangePop(); }
+};
+}  // namespace
 
 using namespace tmw;
 
@@ -242,6 +251,7 @@ void tmw_destroy(tmw_ctx* ctx) {
 }
 
 int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, double c_sw, const tmw_options* opt) {
+  NvtxRange nvtx("tmw_create");
   if (!out) return fail(nullptr, TMW_EINVAL, "tmw_create: out is null");
   *out = nullptr;
   if (!gauge) return fail(nullptr, TMW_EINVAL, "tmw_create: gauge is null");
@@ -443,6 +453,7 @@ static int full_apply64(tmw_ctx* ctx, int dagger, const void* in_e, const void* 
 }
 
 extern "C" int tmw_apply_multi(tmw_ctx* ctx, int op, int parity, int prec, int nrhs, const void* in, void* out) {
+  NvtxRange nvtx("tmw_apply");
   if (!ctx) return TMW_EINVAL;
   if (!in || !out || in == out) return fail(ctx, TMW_EINVAL, "tmw_apply: null or aliased pointers");
   if ((op != TMW_D && op != TMW_DDAG && op != TMW_G5D) || (parity != TMW_FULL && parity != TMW_EVEN && parity != TMW_ODD)) return fail(ctx, TMW_EINVAL, "tmw_apply: bad op or parity");
@@ -809,6 +820,7 @@ int solve_gcr(tmw_ctx* ctx, int c, double tol, ColState& q) {
 }  // namespace
 
 extern "C" int tmw_solve_multi(tmw_ctx* ctx, int nrhs, const double* b, double* x, double tol, tmw_solve_info* info) {
+  NvtxRange nvtx("tmw_solve");
   if (!ctx) return TMW_EINVAL;
   if (!b || !x || b == x) return fail(ctx, TMW_EINVAL, "tmw_solve: null or aliased pointers");
   if (!(tol > 0.0) || !isfinite(tol)) return fail(ctx, TMW_EINVAL, "tmw_solve: tol must be > 0");
@@ -861,6 +873,8 @@ extern "C" int tmw_solve_multi(tmw_ctx* ctx, int nrhs, const double* b, double* 
     Diag<double> d = make_diag<double>(ctx, 0);
     for (int i = 0; i < nz.n; i++) LAUNCH(launch_diag(d, ctx->g, 0, ctx->clover, 1, colp(W[0], nz.col[i], b64), colp(W[5], nz.col[i], b64), s));
     if ((rc = dslash<double>(ctx, EPI_XPAY, 1, 0, W[5], W[2], W[1], -1.0, nz))) return rc;
+    {
+    NvtxRange nvtx_it("tmw_solve: Krylov iterations");
     if (ctx->opt.solver == TMW_GCR) {
       for (int i = 0; i < nz.n; i++) {  // GCR keeps 2 k Krylov vectors per system: the columns go one after another
         rc = dbl ? solve_gcr<double>(ctx, nz.col[i], tol, cs[nz.col[i]]) : solve_gcr<float>(ctx, nz.col[i], tol, cs[nz.col[i]]);
@@ -869,6 +883,7 @@ extern "C" int tmw_solve_multi(tmw_ctx* ctx, int nrhs, const double* b, double* 
       }
     } else {
       status = dbl ? solve_schur<double>(ctx, nrhs, tol, cs) : solve_schur<float>(ctx, nrhs, tol, cs);
+    }
     }
     if (status != TMW_OK && status != TMW_ENOCONV) return status;
     // A7: x_o = y, x_e = A_ee^{-1} (b_e - H_eo x_o)
