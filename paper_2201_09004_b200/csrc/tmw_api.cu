@@ -480,14 +480,12 @@ extern "C" int tmw_apply_multi(tmw_ctx* ctx, int op, int parity, int prec, int n
     cout = (double*)ctx->canon[1];
   }
   for (int c = 0; c < nrhs; c++) {
-    LAUNCH(launch_pack_spinor(ctx->g, 0, 1, (const double*)colp(cin, c, cbytes), colp(ctx->w64[0], c, b64), ctx->stream));
-    LAUNCH(launch_pack_spinor(ctx->g, 1, 1, (const double*)colp(cin, c, cbytes), colp(ctx->w64[1], c, b64), ctx->stream));
+    LAUNCH(launch_pack_spinor_both(ctx->g, 1, (const double*)colp(cin, c, cbytes), colp(ctx->w64[0], c, b64), colp(ctx->w64[1], c, b64), ctx->stream));
   }
   rc = full_apply64(ctx, dagger, ctx->w64[0], ctx->w64[1], ctx->w64[2], ctx->w64[3], cm, g5);
   if (rc) return rc;
   for (int c = 0; c < nrhs; c++) {
-    LAUNCH(launch_unpack_spinor(ctx->g, 0, 1, colp(ctx->w64[2], c, b64), (double*)colp(cout, c, cbytes), ctx->stream));
-    LAUNCH(launch_unpack_spinor(ctx->g, 1, 1, colp(ctx->w64[3], c, b64), (double*)colp(cout, c, cbytes), ctx->stream));
+    LAUNCH(launch_unpack_spinor_both(ctx->g, 1, colp(ctx->w64[2], c, b64), colp(ctx->w64[3], c, b64), (double*)colp(cout, c, cbytes), ctx->stream));
   }
   if (ctx->opt.location == TMW_HOST) {
     CK(cudaMemcpyAsync(out, cout, cbytes * nrhs, cudaMemcpyDeviceToHost, ctx->stream));
@@ -523,8 +521,7 @@ extern "C" int tmw_cheb_apply(tmw_ctx* ctx, int ncoef, const double* coef, doubl
   void** W = ctx->w64;
   const int64_t n64 = (int64_t)ctx->g.Vh * 12;
   const ColMap one = cols_first(1);
-  LAUNCH(launch_pack_spinor(ctx->g, 0, 1, cin, W[0], s));
-  LAUNCH(launch_pack_spinor(ctx->g, 1, 1, cin, W[1], s));
+  LAUNCH(launch_pack_spinor_both(ctx->g, 1, cin, W[0], W[1], s));
   int b1 = 2, b2 = 4;  // indices of the (even) buffers of b_{k+1}, b_{k+2}
   if (ncoef == 1) {
     for (int p = 0; p < 2; p++) LAUNCH(launch_scale(n64, W[b1 + p], W[p], coef[0], s));
@@ -540,8 +537,7 @@ extern "C" int tmw_cheb_apply(tmw_ctx* ctx, int ncoef, const double* coef, doubl
       const int t = b1; b1 = b2; b2 = t;  // the new vector was written over b_{k+2}
     }
   }
-  LAUNCH(launch_unpack_spinor(ctx->g, 0, 1, W[b1], cout, s));
-  LAUNCH(launch_unpack_spinor(ctx->g, 1, 1, W[b1 + 1], cout, s));
+  LAUNCH(launch_unpack_spinor_both(ctx->g, 1, W[b1], W[b1 + 1], cout, s));
   if (ctx->opt.location == TMW_HOST) {
     CK(cudaMemcpyAsync(out, cout, cbytes, cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));
@@ -849,8 +845,7 @@ extern "C" int tmw_solve_multi(tmw_ctx* ctx, int nrhs, const double* b, double* 
   const ColMap all = cols_first(nrhs);
   // A0/A7: split b, |b|, bhat_o = b_o - H_oe A_ee^{-1} b_e
   for (int c = 0; c < nrhs; c++) {
-    LAUNCH(launch_pack_spinor(ctx->g, 0, 1, (const double*)colp(cb, c, cbytes), colp(W[0], c, b64), s));
-    LAUNCH(launch_pack_spinor(ctx->g, 1, 1, (const double*)colp(cb, c, cbytes), colp(W[1], c, b64), s));
+    LAUNCH(launch_pack_spinor_both(ctx->g, 1, (const double*)colp(cb, c, cbytes), colp(W[0], c, b64), colp(W[1], c, b64), s));
   }
   CK(cudaMemsetAsync(ctx->red, 0, 4 * MAXCOL * sizeof(double), s));
   LAUNCH(launch_dot_norm<double>(n64, nullptr, W[0], ctx->red, all, s));
@@ -890,14 +885,13 @@ extern "C" int tmw_solve_multi(tmw_ctx* ctx, int nrhs, const double* b, double* 
     if ((rc = dslash<double>(ctx, EPI_AINV_XPAY, 0, 0, W[3], W[7], W[0], -1.0, nz))) return rc;
     for (int i = 0; i < nz.n; i++) {
       const int c = nz.col[i];
-      LAUNCH(launch_unpack_spinor(ctx->g, 0, 1, colp(W[7], c, b64), (double*)colp(cx_, c, cbytes), s));
-      LAUNCH(launch_unpack_spinor(ctx->g, 1, 1, colp(W[3], c, b64), (double*)colp(cx_, c, cbytes), s));
+      LAUNCH(launch_unpack_spinor_both(ctx->g, 1, colp(W[7], c, b64), colp(W[3], c, b64), (double*)colp(cx_, c, cbytes), s));
     }
-    // true residual of the full system in fp64: |b - D x|
-    if ((rc = full_apply64(ctx, 0, W[7], W[3], W[5], W[6], nz))) return rc;
+    // true residual of the full system in fp64: |b - D x|, the difference and its norm fused into the two launches of
+    // the full operator (out_p = A x_p + H x_pbar is not stored)
     CK(cudaMemsetAsync(ctx->red, 0, 4 * MAXCOL * sizeof(double), s));
-    LAUNCH(launch_sub_norm(n64, W[0], W[5], W[5], ctx->red, nz, s));
-    LAUNCH(launch_sub_norm(n64, W[1], W[6], W[6], ctx->red, nz, s));
+    if ((rc = dslash<double>(ctx, EPI_A_XPAY, 0, 0, W[3], nullptr, W[7], 1.0, nz, 3, W[0], ctx->red, 4))) return rc;
+    if ((rc = dslash<double>(ctx, EPI_A_XPAY, 1, 0, W[7], nullptr, W[3], 1.0, nz, 3, W[1], ctx->red, 4))) return rc;
     if ((rc = fetch_red(ctx))) return rc;
     for (int i = 0; i < nz.n; i++) cs[nz.col[i]].true_resid = sqrt(ctx->red_host[4 * nz.col[i] + 2]) / cs[nz.col[i]].bnorm;
   }

@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<R>
       }
 #pragma unroll
       for (int j = 0; j < NR; j++)
-        if (valid[j]) store_reals_s<24>(a.out, a.g.Vh, s.cb + cofs[j], o[j]);
+        if (valid[j] && a.out) store_reals_s<24>(a.out, a.g.Vh, s.cb + cofs[j], o[j]);
     }
   }
   if (a.red_mode != 0) {  // uniform across the grid
@@ -79,6 +79,13 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<R>
           }
           v[0] = re;
           v[1] = im;
+        } else if (a.red_mode == 3) {  // |dotv - o|^2: the residual norm of the final check, o itself is not kept
+          R d[24];
+          load_reals<24>(a.dotv, a.g.Vh, s.cb + cofs[j], d);
+          R nn = 0;
+#pragma unroll
+          for (int i = 0; i < 24; i++) nn += (d[i] - o[j][i]) * (d[i] - o[j][i]);
+          v[2] = nn;
         } else {
           v[0] = r2[j][0];
           v[1] = r2[j][1];
