@@ -55,6 +55,12 @@ def test_argument_validation_before_any_cuda_call(lib):
     # null context
     assert lib.tmw_apply(None, 0, 0, 0, None, None) == tmw.EINVAL
     assert lib.tmw_solve(None, None, None, 1e-10, None) == tmw.EINVAL
+    assert lib.tmw_apply_multi(None, 0, 0, 0, 2, None, None) == tmw.EINVAL
+    assert lib.tmw_apply_schur_multi(None, 0, 0, 2, None, None) == tmw.EINVAL
+    assert lib.tmw_solve_multi(None, 2, None, None, 1e-10, None) == tmw.EINVAL
+    assert lib.tmw_cheb_apply(None, 1, (ctypes.c_double * 1)(1.0), 1.0, 0.0, None, None) == tmw.EINVAL
+    bad = tmw.tmw_options(0, 0, 12, 0, 0, 0.0, None, 7, 0)  # unknown solver
+    assert lib.tmw_create(ctypes.byref(h), 4, 4, g.ctypes.data, m, 0.0, ctypes.byref(bad)) == tmw.EINVAL
     assert lib.tmw_spinor_bytes(None, 0) == 0
     assert lib.tmw_launch_count(None) == 0
     lib.tmw_destroy(None)
