@@ -143,8 +143,9 @@ int tmw_solve(tmw_ctx* ctx, const double* b, double* x, double tol, tmw_solve_in
  * tmw_solve_multi: BiCGStab on all columns in lockstep, each with its own recurrence scalars, reliable updates and
  *   stopping test (|b_c - D x_c| / |b_c| <= tol for every column c); columns that have converged drop out of the
  *   launches. info (nullable) points to nrhs records; device_ms is the time of the whole call in each of them.
- *   Returns TMW_ENOCONV if any column reached max_iter. Workspace grows with nrhs (16 parity spinors per column):
- *   TMW_ENOMEM if it does not fit.
+ *   Returns TMW_ENOCONV if any column reached max_iter. Workspace grows with nrhs (16 parity spinors per column); if
+ *   the columns do not all fit in the free device memory they are solved in chunks of as many as fit (device_ms is
+ *   then the time of the column's chunk). TMW_ENOMEM if not even one column fits.
  */
 int tmw_apply_multi(tmw_ctx* ctx, int op, int parity, int prec, int nrhs, const void* in, void* out);
 int tmw_apply_schur_multi(tmw_ctx* ctx, int op, int prec, int nrhs, const void* in_odd, void* out_odd);

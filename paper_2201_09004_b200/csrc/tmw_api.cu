@@ -815,13 +815,8 @@ int solve_gcr(tmw_ctx* ctx, int c, double tol, ColState& q) {
 
 }  // namespace
 
-extern "C" int tmw_solve_multi(tmw_ctx* ctx, int nrhs, const double* b, double* x, double tol, tmw_solve_info* info) {
-  NvtxRange nvtx("tmw_solve");
-  if (!ctx) return TMW_EINVAL;
-  if (!b || !x || b == x) return fail(ctx, TMW_EINVAL, "tmw_solve: null or aliased pointers");
-  if (!(tol > 0.0) || !isfinite(tol)) return fail(ctx, TMW_EINVAL, "tmw_solve: tol must be > 0");
-  if (nrhs < 1 || nrhs > MAXCOL) return fail(ctx, TMW_EINVAL, "tmw_solve: nrhs must be in 1..16");
-  if (info) memset(info, 0, sizeof(*info) * nrhs);
+// nrhs columns that are known to fit in the workspaces (tmw_solve_multi below splits a call into such chunks)
+static int solve_chunk(tmw_ctx* ctx, int nrhs, const double* b, double* x, double tol, tmw_solve_info* info) {
   const bool dbl = ctx->opt.precision == TMW_DOUBLE;
   int rc;
   if ((rc = need_cols(ctx, nrhs))) return rc;
@@ -909,6 +904,47 @@ extern "C" int tmw_solve_multi(tmw_ctx* ctx, int nrhs, const double* b, double* 
       info[c].true_resid = cs[c].true_resid;
       info[c].device_ms = ms;
     }
+  }
+  return status;
+}
+
+extern "C" int tmw_solve_multi(tmw_ctx* ctx, int nrhs, const double* b, double* x, double tol, tmw_solve_info* info) {
+  NvtxRange nvtx("tmw_solve");
+  if (!ctx) return TMW_EINVAL;
+  if (!b || !x || b == x) return fail(ctx, TMW_EINVAL, "tmw_solve: null or aliased pointers");
+  if (!(tol > 0.0) || !isfinite(tol)) return fail(ctx, TMW_EINVAL, "tmw_solve: tol must be > 0");
+  if (nrhs < 1 || nrhs > MAXCOL) return fail(ctx, TMW_EINVAL, "tmw_solve: nrhs must be in 1..16");
+  if (info) memset(info, 0, sizeof(*info) * nrhs);
+  // How many columns fit at once: 8 fp64 + 8 inner-precision parity spinors per column (+ 2 canonical staging spinors
+  // for HOST pointers) out of the free device memory plus what the workspaces already hold. More columns than that are
+  // solved chunk after chunk (as even as possible); TMW_NO_CHUNK=1 disables the split (the call then fails with
+  // TMW_ENOMEM if the columns do not fit).
+  int chunk = nrhs;
+  if (nrhs > 1 && !getenv("TMW_NO_CHUNK")) {
+    const size_t b64 = spinor_bytes(ctx, TMW_F64), bin = spinor_bytes(ctx, ctx->opt.precision == TMW_DOUBLE ? TMW_F64 : TMW_F32);
+    const size_t cbytes = (size_t)ctx->V * 24 * 8;
+    const size_t per_col = 8 * b64 + 8 * bin + (ctx->opt.location == TMW_HOST ? 2 * cbytes : 0);
+    size_t held = 0;
+    for (int i = 0; i < 10; i++) if (ctx->w64[i]) held += b64 * ctx->ws_cols;
+    for (int i = 0; i < 8; i++) if (ctx->w32[i]) held += bin * ctx->ws_cols;
+    for (int i = 0; i < 2; i++) if (ctx->canon[i]) held += cbytes * ctx->ws_cols;
+    size_t free_b = 0, total_b = 0;
+    CK(cudaMemGetInfo(&free_b, &total_b));
+    const size_t fit = (size_t)(0.92 * (double)(free_b + held)) / per_col;
+    if (fit < (size_t)nrhs && ctx->ws_cols < nrhs) {
+      chunk = fit < 1 ? 1 : (int)fit;
+      if (chunk < ctx->ws_cols) chunk = ctx->ws_cols;  // what is already allocated fits by construction
+      const int nchunks = (nrhs + chunk - 1) / chunk;
+      chunk = (nrhs + nchunks - 1) / nchunks;
+    }
+  }
+  int status = TMW_OK;
+  const size_t cdoubles = (size_t)ctx->V * 24;
+  for (int c0 = 0; c0 < nrhs; c0 += chunk) {
+    const int n = nrhs - c0 < chunk ? nrhs - c0 : chunk;
+    const int rc = solve_chunk(ctx, n, b + c0 * cdoubles, x + c0 * cdoubles, tol, info ? info + c0 : nullptr);
+    if (rc != TMW_OK && rc != TMW_ENOCONV) return rc;
+    if (rc == TMW_ENOCONV) status = rc;
   }
   return status;
 }

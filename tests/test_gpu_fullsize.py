@@ -239,7 +239,7 @@ def test_fullsize_config3_twelve_columns_batched(tmw):
     torch.cuda.empty_cache()
 
 
-def test_fullsize_config4_solve(tmw):
+def test_fullsize_config4_solve(tmw, monkeypatch):
     cfg, U = config_fields(4)
     L, T, m, c_sw = cfg["L"], cfg["T"], complex(*cfg["m"]), cfg["c_sw"]
     b = synth.point_source(L, T, 0, 0)
@@ -254,13 +254,28 @@ def test_fullsize_config4_solve(tmw):
         db = torch.from_numpy(b).cuda()
         # 16 columns need 16 x 18.3 GB of workspace here: more than the GPU has. The call must fail with TMW_ENOMEM before
         # it touches b or x (so one-column buffers are enough), release what it allocated, and leave the context usable.
+        monkeypatch.setenv("TMW_NO_CHUNK", "1")
         with pytest.raises(tmw.TmwError) as e:
             ctx.solve_multi(16, db, x, 1e-10)
         assert e.value.code == tmw.ENOMEM
+        monkeypatch.delenv("TMW_NO_CHUNK")
         info = ctx.solve(db, x, 1e-10)
         xg = x.cpu().numpy()
-        del x, db
+        del x
+        # without TMW_NO_CHUNK more columns than fit are solved chunk after chunk: 8 columns = 147 GB of workspace
+        n = 8
+        bm = torch.zeros((n, T, L, L, L, 4, 3), dtype=torch.complex128, device="cuda")
+        for c in range(n):
+            bm[c, 0, 0, 0, 0, c // 3, c % 3] = 1.0
+        xm = torch.empty_like(bm)
+        infos = ctx.solve_multi(n, bm, xm, 1e-10)
+        assert all(i["true_resid"] <= 1e-10 and i["iters"] > 0 for i in infos)
+        assert float(torch.linalg.vector_norm(xm[0] - torch.from_numpy(xg).cuda()) / torch.linalg.vector_norm(xm[0])) <= 1e-8
+        x7 = xm[7].cpu().numpy()
+        del bm, xm, db
     torch.cuda.empty_cache()
+    mx7, est7 = sampled_residual(U, synth.point_source(L, T, 2, 1), x7, m, c_sw, rnd, det)
+    assert mx7 <= 1e-10 and est7 <= EST_TOL, (mx7, est7)
     assert info["true_resid"] <= 1e-10
     mx, est = sampled_residual(U, b, xg, m, c_sw, rnd, det)
     assert mx <= 1e-10 and est <= EST_TOL, (mx, est)
