@@ -629,7 +629,7 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
   LAUNCH(launch_convert<R>(n64, W[2], rhat, act, s));
   memset(h, 0, MAXCOL * sizeof(Scalars));
   if ((rc = push_scalars(ctx))) return rc;
-  LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], r, rhat, ctx->sc, act, s));  // r64 = bhat - 0; rho = <rhat,r>; rr = |r64|^2
+  LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], r, rhat, nullptr, ctx->sc, act, s));  // r64 = bhat - 0; rho = <rhat,r>; rr = |r64|^2
   if ((rc = fetch_scalars(ctx))) return rc;
   for (int i = 0; i < act.n; i++) {
     const int c = act.col[i];
@@ -639,19 +639,19 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
     if (cs[c].rnorm <= tol * cs[c].bnorm) cs[c].done = true;
   }
   if ((rc = push_scalars(ctx))) return rc;
+  LAUNCH(launch_update_p<R>(nR, p, r, v, ctx->sc, act, s));  // p = r (p = v = 0); later p comes out of update_xrp
   const int max_iter = ctx->opt.max_iter;
   for (int k = 1; k <= max_iter; k++) {
     act.n = 0;
     for (int c = 0; c < ncols; c++) if (!cs[c].done) cols_add(act, c);
     if (act.n == 0) return TMW_OK;
     LAUNCH(launch_sc_begin_iter(ctx->sc, act, s));
-    LAUNCH(launch_update_p<R>(nR, p, r, v, ctx->sc, act, s));
     if ((rc = schur<R>(ctx, 0, p, v, tmp, act, 1, rhat, red_rhat_v, SCD))) return rc;
     LAUNCH(launch_sc_alpha(ctx->sc, act, s));
     LAUNCH(launch_update_s<R>(nR, sv, r, v, ctx->sc, act, s));
-    if ((rc = schur<R>(ctx, 0, sv, t, tmp, act, 2, nullptr, red_ts, SCD))) return rc;
-    LAUNCH(launch_sc_omega(ctx->sc, act, s));
-    LAUNCH(launch_update_xr<R>(nR, x, r, p, sv, t, rhat, ctx->sc, act, s));
+    if ((rc = schur<R>(ctx, 0, sv, t, tmp, act, 4, rhat, red_ts, SCD))) return rc;  // <t,s>, <t,t>, <rhat,t>, <rhat,s>
+    LAUNCH(launch_sc_omega(ctx->sc, act, s));                                        // omega, rho' = <rhat, s - omega t>, beta
+    LAUNCH(launch_update_xrp<R>(nR, x, r, p, sv, t, v, ctx->sc, act, s));             // x, r, and p of the next iteration
     if ((rc = fetch_scalars(ctx))) return rc;
     ColMap upd, brk;  // columns that take a reliable update now / whose iterate is corrupted
     upd.n = brk.n = 0;
@@ -690,7 +690,8 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
         if (broken[c]) reset_recurrence(&h[c]);
       }
       if ((rc = push_scalars(ctx))) return rc;
-      LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], r, rhat, ctx->sc, upd, s));
+      // r := true residual; the search direction update_xrp already built from the iterated r moves with it
+      LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], r, rhat, p, ctx->sc, upd, s));
       if ((rc = fetch_scalars(ctx))) return rc;
       for (int i = 0; i < upd.n; i++) {
         const int c = upd.col[i];
@@ -730,7 +731,8 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
       if ((rc = push_scalars(ctx))) return rc;
       LAUNCH(launch_sub_norm(n64, W[2], W[6], W[4], ctx->red, rst, s));  // r64 = bhat - Mhat y (norm discarded)
       LAUNCH(launch_convert<R>(n64, W[4], rhat, rst, s));
-      LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], r, rhat, ctx->sc, rst, s));
+      LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], r, rhat, nullptr, ctx->sc, rst, s));
+      LAUNCH(launch_update_p<R>(nR, p, r, v, ctx->sc, rst, s));  // p = r (p = v = 0, beta = 0)
       if ((rc = fetch_scalars(ctx))) return rc;
       for (int i = 0; i < rst.n; i++) {
         const int c = rst.col[i];
@@ -782,7 +784,7 @@ int solve_gcr(tmw_ctx* ctx, int c, double tol, ColState& q) {
     // true residual r64 = bhat - Mhat y (W[6] holds Mhat y), r = (R) r64, |r64|^2
     memset(h, 0, MAXCOL * sizeof(Scalars));
     if ((rc = push_scalars(ctx))) return rc;
-    LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], X[0], X[1], ctx->sc, one, s));
+    LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], X[0], X[1], nullptr, ctx->sc, one, s));
     if ((rc = fetch_scalars(ctx))) return rc;
     q.rnorm = q.maxr = sqrt(h[c].rr);
     q.iter_resid = q.rnorm / q.bnorm;

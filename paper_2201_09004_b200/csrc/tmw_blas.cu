@@ -72,16 +72,13 @@ __device__ __forceinline__ void cdiv(const double* a, const double* b, double* q
   const double re = (a[0] * b[0] + a[1] * b[1]) / d, im = (a[1] * b[0] - a[0] * b[1]) / d;
   q[0] = re; q[1] = im;
 }
-__global__ void sc_begin_iter_kernel(Scalars* sc0, ColMap cm) {  // beta = (rho/rho_old)(alpha/omega)
+__global__ void sc_begin_iter_kernel(Scalars* sc0, ColMap cm) {  // zero the accumulators of the two K2 launches
   Scalars* sc = sc0 + cm.col[threadIdx.x];
-  double a[2], b[2];
-  cdiv(sc->rho, sc->rho_old, a);
-  cdiv(sc->alpha, sc->omega, b);
-  sc->beta[0] = a[0] * b[0] - a[1] * b[1];
-  sc->beta[1] = a[0] * b[1] + a[1] * b[0];
   sc->rhat_v[0] = sc->rhat_v[1] = 0.0;
   sc->ts[0] = sc->ts[1] = 0.0;
   sc->tt = 0.0;
+  sc->rhat_t[0] = sc->rhat_t[1] = 0.0;
+  sc->rhat_s[0] = sc->rhat_s[1] = 0.0;
 }
 __global__ void sc_alpha_kernel(Scalars* sc0, ColMap cm) {
   Scalars* sc = sc0 + cm.col[threadIdx.x];
@@ -89,11 +86,19 @@ __global__ void sc_alpha_kernel(Scalars* sc0, ColMap cm) {
 }
 __global__ void sc_omega_kernel(Scalars* sc0, ColMap cm) {
   Scalars* sc = sc0 + cm.col[threadIdx.x];
-  sc->omega[0] = sc->ts[0] / sc->tt;
-  sc->omega[1] = sc->ts[1] / sc->tt;
+  const double wr = sc->ts[0] / sc->tt, wi = sc->ts[1] / sc->tt;
+  sc->omega[0] = wr;
+  sc->omega[1] = wi;
   sc->rho_old[0] = sc->rho[0];
   sc->rho_old[1] = sc->rho[1];
-  sc->rho[0] = sc->rho[1] = 0.0;
+  // <rhat, r_new> with r_new = s - omega t, from the two dot products the second K2 reduced
+  sc->rho[0] = sc->rhat_s[0] - (wr * sc->rhat_t[0] - wi * sc->rhat_t[1]);
+  sc->rho[1] = sc->rhat_s[1] - (wr * sc->rhat_t[1] + wi * sc->rhat_t[0]);
+  double a[2], b[2];
+  cdiv(sc->rho, sc->rho_old, a);
+  cdiv(sc->alpha, sc->omega, b);
+  sc->beta[0] = a[0] * b[0] - a[1] * b[1];
+  sc->beta[1] = a[0] * b[1] + a[1] * b[0];
   sc->rr = 0.0;
 }
 cudaError_t launch_sc_begin_iter(Scalars* sc, const ColMap& cm, cudaStream_t s) { sc_begin_iter_kernel<<<1, cm.n, 0, s>>>(sc, cm); return cudaGetLastError(); }
@@ -135,32 +140,35 @@ template <typename R> __global__ void __launch_bounds__(BB) update_s_kernel(int6
     stp(s, i, ss);
   }
 }
-template <typename R> __global__ void __launch_bounds__(BB) update_xr_kernel(int64_t n, R* x, R* r, const R* p, const R* s, const R* t, const R* rhat, Scalars* sc, ColMap cm) {
+template <typename R> __global__ void __launch_bounds__(BB) update_xrp_kernel(int64_t n, R* x, R* r, R* p, const R* s, const R* t, const R* v, Scalars* sc, ColMap cm) {
   const int c = cm.col[blockIdx.y];
   sc += c;
-  { const int64_t o = 4 * n * c; x += o; r += o; p += o; s += o; t += o; rhat += o; }
-  const R ar = (R)sc->alpha[0], ai = (R)sc->alpha[1], wr = (R)sc->omega[0], wi = (R)sc->omega[1];
-  double acc[3] = {0, 0, 0};
+  { const int64_t o = 4 * n * c; x += o; r += o; p += o; s += o; t += o; v += o; }
+  const R ar = (R)sc->alpha[0], ai = (R)sc->alpha[1], wr = (R)sc->omega[0], wi = (R)sc->omega[1], br = (R)sc->beta[0], bi = (R)sc->beta[1];
+  double acc[1] = {0};
   for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
-    R xx[4], pp[4], ss[4], tt[4], hh[4], rr[4];
-    ldp(x, i, xx); ldp(p, i, pp); ldp(s, i, ss); ldp(t, i, tt); ldp(rhat, i, hh);
-    R re = 0, im = 0, nn = 0;
+    R xx[4], pp[4], ss[4], tt[4], vv[4], rr[4];
+    ldp(x, i, xx); ldp(p, i, pp); ldp(s, i, ss); ldp(t, i, tt); ldp(v, i, vv);
+    R nn = 0;
 #pragma unroll
-    for (int c = 0; c < 2; c++) {
-      xx[2 * c] += (ar * pp[2 * c] - ai * pp[2 * c + 1]) + (wr * ss[2 * c] - wi * ss[2 * c + 1]);
-      xx[2 * c + 1] += (ar * pp[2 * c + 1] + ai * pp[2 * c]) + (wr * ss[2 * c + 1] + wi * ss[2 * c]);
-      rr[2 * c] = ss[2 * c] - (wr * tt[2 * c] - wi * tt[2 * c + 1]);
-      rr[2 * c + 1] = ss[2 * c + 1] - (wr * tt[2 * c + 1] + wi * tt[2 * c]);
-      re += hh[2 * c] * rr[2 * c] + hh[2 * c + 1] * rr[2 * c + 1];
-      im += hh[2 * c] * rr[2 * c + 1] - hh[2 * c + 1] * rr[2 * c];
-      nn += rr[2 * c] * rr[2 * c] + rr[2 * c + 1] * rr[2 * c + 1];
+    for (int k = 0; k < 2; k++) {
+      xx[2 * k] += (ar * pp[2 * k] - ai * pp[2 * k + 1]) + (wr * ss[2 * k] - wi * ss[2 * k + 1]);
+      xx[2 * k + 1] += (ar * pp[2 * k + 1] + ai * pp[2 * k]) + (wr * ss[2 * k + 1] + wi * ss[2 * k]);
+      rr[2 * k] = ss[2 * k] - (wr * tt[2 * k] - wi * tt[2 * k + 1]);
+      rr[2 * k + 1] = ss[2 * k + 1] - (wr * tt[2 * k + 1] + wi * tt[2 * k]);
+      nn += rr[2 * k] * rr[2 * k] + rr[2 * k + 1] * rr[2 * k + 1];
+      const R ur = pp[2 * k] - (wr * vv[2 * k] - wi * vv[2 * k + 1]);
+      const R ui = pp[2 * k + 1] - (wr * vv[2 * k + 1] + wi * vv[2 * k]);
+      pp[2 * k] = rr[2 * k] + (br * ur - bi * ui);
+      pp[2 * k + 1] = rr[2 * k + 1] + (br * ui + bi * ur);
     }
     stp(x, i, xx);
     stp(r, i, rr);
-    acc[0] += re; acc[1] += im; acc[2] += nn;
+    stp(p, i, pp);
+    acc[0] += nn;
   }
-  double* dst[3] = {&sc->rho[0], &sc->rho[1], &sc->rr};
-  reduce_atomic<3>(acc, dst);
+  double* dst[1] = {&sc->rr};
+  reduce_atomic<1>(acc, dst);
 }
 template <typename R> __global__ void __launch_bounds__(BB) dot_norm_kernel(int64_t n, const R* a, const R* b, double* out, ColMap cm) {
   const int c = cm.col[blockIdx.y];
@@ -195,10 +203,10 @@ template <typename R> __global__ void __launch_bounds__(BB) acc_y_kernel(int64_t
     stm(x, i, Vh, xx);
   }
 }
-template <typename R> __global__ void __launch_bounds__(BB) resid_convert_kernel(int64_t n, int64_t Vh, const double* b, const double* w, double* r64, R* r, const R* rhat, Scalars* sc, ColMap cm) {
+template <typename R> __global__ void __launch_bounds__(BB) resid_convert_kernel(int64_t n, int64_t Vh, const double* b, const double* w, double* r64, R* r, const R* rhat, R* p, Scalars* sc, ColMap cm) {
   const int c = cm.col[blockIdx.y];
   sc += c;
-  { const int64_t o = 4 * n * c; b += o; w += o; r64 += o; r += o; rhat += o; }
+  { const int64_t o = 4 * n * c; b += o; w += o; r64 += o; r += o; rhat += o; if (p) p += o; }
   double acc[3] = {0, 0, 0};
   for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
     double bb[4], ww[4], dd[4];
@@ -206,6 +214,13 @@ template <typename R> __global__ void __launch_bounds__(BB) resid_convert_kernel
     ldm(b, i, Vh, bb); ldm(w, i, Vh, ww); ldm(rhat, i, Vh, hh);
 #pragma unroll
     for (int c = 0; c < 4; c++) { dd[c] = bb[c] - ww[c]; rr[c] = (R)dd[c]; }
+    if (p) {  // p += r_new - r_old
+      R ro[4], pp[4];
+      ldm(r, i, Vh, ro); ldm(p, i, Vh, pp);
+#pragma unroll
+      for (int c = 0; c < 4; c++) pp[c] += rr[c] - ro[c];
+      stm(p, i, Vh, pp);
+    }
     stm(r64, i, Vh, dd);
     stm(r, i, Vh, rr);
 #pragma unroll
@@ -412,9 +427,9 @@ template <typename R> cudaError_t launch_update_s(int64_t n, void* sv, const voi
   update_s_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, (R*)sv, (const R*)r, (const R*)v, sc, cm);
   return cudaGetLastError();
 }
-template <typename R> cudaError_t launch_update_xr(int64_t n, void* x, void* r, const void* p, const void* sv, const void* t, const void* rhat, Scalars* sc, const ColMap& cm, cudaStream_t s) {
+template <typename R> cudaError_t launch_update_xrp(int64_t n, void* x, void* r, void* p, const void* sv, const void* t, const void* v, Scalars* sc, const ColMap& cm, cudaStream_t s) {
   const int64_t np = pairs_of<R>(n);
-  update_xr_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, (R*)x, (R*)r, (const R*)p, (const R*)sv, (const R*)t, (const R*)rhat, sc, cm);
+  update_xrp_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, (R*)x, (R*)r, (R*)p, (const R*)sv, (const R*)t, (const R*)v, sc, cm);
   return cudaGetLastError();
 }
 template <typename R> cudaError_t launch_dot_norm(int64_t n, const void* a, const void* b, double* out, const ColMap& cm, cudaStream_t s) {
@@ -427,9 +442,9 @@ template <typename R> cudaError_t launch_acc_y(int64_t n64, void* y64, void* x, 
   acc_y_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, np / 6, (double*)y64, (R*)x, cm);
   return cudaGetLastError();
 }
-template <typename R> cudaError_t launch_resid_convert(int64_t n64, const void* b64, const void* w64, void* r64, void* r, const void* rhat, Scalars* sc, const ColMap& cm, cudaStream_t s) {
+template <typename R> cudaError_t launch_resid_convert(int64_t n64, const void* b64, const void* w64, void* r64, void* r, const void* rhat, void* p, Scalars* sc, const ColMap& cm, cudaStream_t s) {
   const int64_t np = n64 / 2;
-  resid_convert_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, np / 6, (const double*)b64, (const double*)w64, (double*)r64, (R*)r, (const R*)rhat, sc, cm);
+  resid_convert_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, np / 6, (const double*)b64, (const double*)w64, (double*)r64, (R*)r, (const R*)rhat, (R*)p, sc, cm);
   return cudaGetLastError();
 }
 template <typename R> cudaError_t launch_convert(int64_t n64, const void* src64, void* dst, const ColMap& cm, cudaStream_t s) {
@@ -460,10 +475,10 @@ template cudaError_t launch_gcr_step<double>(int64_t, int, void*, void*, void*, 
 #define TMW_INST(R)                                                                                                          \
   template cudaError_t launch_update_p<R>(int64_t, void*, const void*, const void*, const Scalars*, const ColMap&, cudaStream_t);           \
   template cudaError_t launch_update_s<R>(int64_t, void*, const void*, const void*, const Scalars*, const ColMap&, cudaStream_t);           \
-  template cudaError_t launch_update_xr<R>(int64_t, void*, void*, const void*, const void*, const void*, const void*, Scalars*, const ColMap&, cudaStream_t); \
+  template cudaError_t launch_update_xrp<R>(int64_t, void*, void*, void*, const void*, const void*, const void*, Scalars*, const ColMap&, cudaStream_t); \
   template cudaError_t launch_dot_norm<R>(int64_t, const void*, const void*, double*, const ColMap&, cudaStream_t);                         \
   template cudaError_t launch_acc_y<R>(int64_t, void*, void*, const ColMap&, cudaStream_t);                                                 \
-  template cudaError_t launch_resid_convert<R>(int64_t, const void*, const void*, void*, void*, const void*, Scalars*, const ColMap&, cudaStream_t); \
+  template cudaError_t launch_resid_convert<R>(int64_t, const void*, const void*, void*, void*, const void*, void*, Scalars*, const ColMap&, cudaStream_t); \
   template cudaError_t launch_convert<R>(int64_t, const void*, void*, const ColMap&, cudaStream_t);
 TMW_INST(float)
 TMW_INST(double)

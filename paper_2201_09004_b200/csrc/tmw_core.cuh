@@ -466,7 +466,8 @@ template <typename R> struct DslashArgs {
   int g5;            // multiply the result by gamma5 = diag(1,1,-1,-1) (the fused gamma5 D_w of PAPER.md:315)
   Diag<R> d;
   // fused reductions (kernel wrapper): red_mode 0 none; 1: red[0..1] += <dotv, out>; 2: red[0..1] += <out, aux>, red[2] += <out,out>;
-  // 3: red[2] += |dotv - out|^2 (out may then be null: nothing is stored)
+  // 3: red[2] += |dotv - out|^2 (out may then be null: nothing is stored); 4: as 2 plus red[3..4] += <dotv, out>,
+  // red[5..6] += <dotv, aux>
   int red_mode;
   const void* dotv;
   double* red;

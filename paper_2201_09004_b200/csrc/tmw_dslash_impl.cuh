@@ -66,7 +66,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<R>
   if (a.red_mode != 0) {  // uniform across the grid
 #pragma unroll
     for (int j = 0; j < NR; j++) {
-      double v[3] = {0, 0, 0};
+      double v[7] = {0, 0, 0, 0, 0, 0, 0};
       if (active && valid[j]) {
         if (a.red_mode == 1) {
           R d[24];
@@ -90,10 +90,38 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<R>
           v[0] = r2[j][0];
           v[1] = r2[j][1];
           v[2] = r2[j][2];
+          if (a.red_mode == 4) {  // also <dotv, o> and <dotv, aux> (aux is re-read: it was consumed chirality by chirality)
+            R d[24], x[24];
+            load_reals<24>(a.dotv, a.g.Vh, s.cb + cofs[j], d);
+            R re = 0, im = 0;
+#pragma unroll
+            for (int i = 0; i < 12; i++) {
+              re += d[2 * i] * o[j][2 * i] + d[2 * i + 1] * o[j][2 * i + 1];
+              im += d[2 * i] * o[j][2 * i + 1] - d[2 * i + 1] * o[j][2 * i];
+            }
+            v[3] = re;
+            v[4] = im;
+            load_reals<24>(a.aux, a.g.Vh, s.cb + cofs[j], x);
+            re = 0;
+            im = 0;
+#pragma unroll
+            for (int i = 0; i < 12; i++) {
+              re += d[2 * i] * x[2 * i] + d[2 * i + 1] * x[2 * i + 1];
+              im += d[2 * i] * x[2 * i + 1] - d[2 * i + 1] * x[2 * i];
+            }
+            v[5] = re;
+            v[6] = im;
+          }
         }
       }
       if (j > 0) __syncthreads();  // the shared scratch of block_reduce_atomic is reused
-      block_reduce_atomic<3, BLOCK>(v, a.red + (int64_t)colj[j] * a.red_stride);
+      double* dst = a.red + (int64_t)colj[j] * a.red_stride;
+      if (a.red_mode == 4) {
+        block_reduce_atomic<7, BLOCK>(v, dst);
+      } else {
+        double v3[3] = {v[0], v[1], v[2]};
+        block_reduce_atomic<3, BLOCK>(v3, dst);
+      }
     }
   }
 }

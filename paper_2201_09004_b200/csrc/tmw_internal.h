@@ -39,17 +39,19 @@ cudaError_t launch_clover_export(const Geom& g, const void* c64, double* dst, cu
 // ---- BLAS-1 with fused reductions (tmw_blas.cu) ----
 // Device scalar block of the BiCGStab recurrences (all complex as re,im doubles).
 struct Scalars {
-  double rho[2];      // <rhat, r>           (accumulated by blas_update_xr / blas_convert)
+  double rho[2];      // <rhat, r>           (sc_omega: <rhat,s> - omega <rhat,t>; resid_convert after a reliable update)
   double rho_old[2];
   double alpha[2];
   double omega[2];
   double beta[2];
   double rhat_v[2];   // <rhat, v>           (accumulated by the first K2)
-  double ts[2];       // <t, s>              (accumulated by the second K2)
+  double ts[2];       // <t, s>              (accumulated by the second K2, red_mode 4: the next 7 doubles in this order)
   double tt;          // <t, t>
-  double rr;          // <r, r>              (accumulated by blas_update_xr / blas_convert)
+  double rhat_t[2];   // <rhat, t>
+  double rhat_s[2];   // <rhat, s>
+  double rr;          // <r, r>              (accumulated by update_xrp / resid_convert)
   double nrm;         // generic norm^2 accumulator
-  double pad;
+  double pad[3];
 };
 // GCR(k) scalars (device): see the gcr_* kernels of tmw_blas.cu
 enum { GCR_KMAX = 16 };
@@ -76,19 +78,25 @@ struct ColMap {
 // Every launcher below is batched: column c of a vector starts c * (column length) after the base pointer and
 // uses the scalar block sc[c]; reductions into a plain double* go to out + 4*c.
 // sc phase kernels (one thread per column): see tmw_blas.cu
-cudaError_t launch_sc_begin_iter(Scalars* sc, const ColMap& cm, cudaStream_t s);  // beta = (rho/rho_old)(alpha/omega); zero rhat_v, ts, tt
+cudaError_t launch_sc_begin_iter(Scalars* sc, const ColMap& cm, cudaStream_t s);  // zero the accumulators of the two K2 launches
 cudaError_t launch_sc_alpha(Scalars* sc, const ColMap& cm, cudaStream_t s);       // alpha = rho / rhat_v
-cudaError_t launch_sc_omega(Scalars* sc, const ColMap& cm, cudaStream_t s);       // omega = ts/tt; rho_old = rho; zero rho, rr
+// omega = ts/tt; rho_old = rho; rho = <rhat,s> - omega <rhat,t> (= <rhat, s - omega t>, the new <rhat,r>);
+// beta = (rho/rho_old)(alpha/omega); zero rr
+cudaError_t launch_sc_omega(Scalars* sc, const ColMap& cm, cudaStream_t s);
 // n = number of 16-byte vectors in one column of each array
 template <typename R> cudaError_t launch_update_p(int64_t n, void* p, const void* r, const void* v, const Scalars* sc, const ColMap& cm, cudaStream_t s);      // p = r + beta (p - omega v)
 template <typename R> cudaError_t launch_update_s(int64_t n, void* sv, const void* r, const void* v, const Scalars* sc, const ColMap& cm, cudaStream_t s);     // s = r - alpha v
-template <typename R> cudaError_t launch_update_xr(int64_t n, void* x, void* r, const void* p, const void* sv, const void* t, const void* rhat, Scalars* sc, const ColMap& cm, cudaStream_t s);  // x += alpha p + omega s; r = s - omega t; rho += <rhat,r>; rr += <r,r>
+// x += alpha p + omega s; r = s - omega t; p = r + beta (p - omega v); rr += <r,r>  (the end of one BiCGStab iteration and
+// the search direction of the next in one pass: 5 reads + 3 writes instead of 8 + 3 in two kernels)
+template <typename R> cudaError_t launch_update_xrp(int64_t n, void* x, void* r, void* p, const void* sv, const void* t, const void* v, Scalars* sc, const ColMap& cm, cudaStream_t s);
 // out[4c+0..1] += <a,b>, out[4c+2] += <b,b> (a may be null: only the norm)
 template <typename R> cudaError_t launch_dot_norm(int64_t n, const void* a, const void* b, double* out, const ColMap& cm, cudaStream_t s);
 // fp64 helpers for the reliable update
 template <typename R> cudaError_t launch_acc_y(int64_t n64, void* y64, void* x, const ColMap& cm, cudaStream_t s);  // y += x; x = 0   (n64 = number of double2 vectors per column)
-// r64 = b64 - w64; r = (R) r64; rho += <rhat, r>; rr += <r64, r64>
-template <typename R> cudaError_t launch_resid_convert(int64_t n64, const void* b64, const void* w64, void* r64, void* r, const void* rhat, Scalars* sc, const ColMap& cm, cudaStream_t s);
+// r64 = b64 - w64; r = (R) r64; rho += <rhat, r>; rr += <r64, r64>. If p is not null (reliable update in the middle of
+// the recurrence): p += r_new - r_old, i.e. the search direction already built from the iterated residual is moved to
+// the true one.
+template <typename R> cudaError_t launch_resid_convert(int64_t n64, const void* b64, const void* w64, void* r64, void* r, const void* rhat, void* p, Scalars* sc, const ColMap& cm, cudaStream_t s);
 // dst(R) = src(double), n64 double2 vectors per column
 template <typename R> cudaError_t launch_convert(int64_t n64, const void* src64, void* dst, const ColMap& cm, cudaStream_t s);
 // d = a - b (fp64, n64 double2 vectors per column), out[4c+2] += <d,d>
