@@ -622,14 +622,11 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
   if (act.n == 0) return TMW_OK;
   // y = 0, r64 = bhat, r = (R) r64, rhat = r, x = p = v = 0
   CK(cudaMemsetAsync(W[3], 0, bytes64 * ncols, s));
-  CK(cudaMemsetAsync(W[6], 0, bytes64 * ncols, s));
   CK(cudaMemsetAsync(x, 0, bytesR * ncols, s));
-  CK(cudaMemsetAsync(p, 0, bytesR * ncols, s));
-  CK(cudaMemsetAsync(v, 0, bytesR * ncols, s));
   LAUNCH(launch_convert<R>(n64, W[2], rhat, act, s));
   memset(h, 0, MAXCOL * sizeof(Scalars));
   if ((rc = push_scalars(ctx))) return rc;
-  LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], r, rhat, nullptr, ctx->sc, act, s));  // r64 = bhat - 0; rho = <rhat,r>; rr = |r64|^2
+  LAUNCH(launch_resid_convert<R>(n64, W[2], nullptr, W[4], r, rhat, nullptr, ctx->sc, act, s));  // r64 = bhat - 0; rho = <rhat,r>; rr = |r64|^2
   if ((rc = fetch_scalars(ctx))) return rc;
   for (int i = 0; i < act.n; i++) {
     const int c = act.col[i];
@@ -639,7 +636,8 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
     if (cs[c].rnorm <= tol * cs[c].bnorm) cs[c].done = true;
   }
   if ((rc = push_scalars(ctx))) return rc;
-  LAUNCH(launch_update_p<R>(nR, p, r, v, ctx->sc, act, s));  // p = r (p = v = 0); later p comes out of update_xrp
+  // p = r for the first iteration; later p comes out of update_xrp (v is written by the first K2 before it is read)
+  for (int i = 0; i < act.n; i++) CK(cudaMemcpyAsync(colp(p, act.col[i], bytesR), colp(r, act.col[i], bytesR), bytesR, cudaMemcpyDeviceToDevice, s));
   const int max_iter = ctx->opt.max_iter;
   for (int k = 1; k <= max_iter; k++) {
     act.n = 0;
@@ -723,8 +721,6 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
       if ((rc = schur<double>(ctx, 0, W[3], W[6], W[5], rst))) return rc;
       for (int i = 0; i < rst.n; i++) {
         const int c = rst.col[i];
-        CK(cudaMemsetAsync(colp(p, c, bytesR), 0, bytesR, s));
-        CK(cudaMemsetAsync(colp(v, c, bytesR), 0, bytesR, s));
         memset(&h[c], 0, sizeof(Scalars));
         reset_recurrence(&h[c]);
       }
@@ -732,7 +728,8 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
       LAUNCH(launch_sub_norm(n64, W[2], W[6], W[4], ctx->red, rst, s));  // r64 = bhat - Mhat y (norm discarded)
       LAUNCH(launch_convert<R>(n64, W[4], rhat, rst, s));
       LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], r, rhat, nullptr, ctx->sc, rst, s));
-      LAUNCH(launch_update_p<R>(nR, p, r, v, ctx->sc, rst, s));  // p = r (p = v = 0, beta = 0)
+      for (int i = 0; i < rst.n; i++)  // p = r
+        CK(cudaMemcpyAsync(colp(p, rst.col[i], bytesR), colp(r, rst.col[i], bytesR), bytesR, cudaMemcpyDeviceToDevice, s));
       if ((rc = fetch_scalars(ctx))) return rc;
       for (int i = 0; i < rst.n; i++) {
         const int c = rst.col[i];

@@ -106,24 +106,6 @@ cudaError_t launch_sc_alpha(Scalars* sc, const ColMap& cm, cudaStream_t s) { sc_
 cudaError_t launch_sc_omega(Scalars* sc, const ColMap& cm, cudaStream_t s) { sc_omega_kernel<<<1, cm.n, 0, s>>>(sc, cm); return cudaGetLastError(); }
 
 // ---- vector updates ----
-template <typename R> __global__ void __launch_bounds__(BB) update_p_kernel(int64_t n, R* p, const R* r, const R* v, const Scalars* sc, ColMap cm) {
-  const int c = cm.col[blockIdx.y];
-  sc += c;
-  { const int64_t o = 4 * n * c; p += o; r += o; v += o; }
-  const R br = (R)sc->beta[0], bi = (R)sc->beta[1], wr = (R)sc->omega[0], wi = (R)sc->omega[1];
-  for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
-    R pp[4], rr[4], vv[4];
-    ldp(p, i, pp); ldp(r, i, rr); ldp(v, i, vv);
-#pragma unroll
-    for (int c = 0; c < 2; c++) {
-      const R ur = pp[2 * c] - (wr * vv[2 * c] - wi * vv[2 * c + 1]);
-      const R ui = pp[2 * c + 1] - (wr * vv[2 * c + 1] + wi * vv[2 * c]);
-      pp[2 * c] = rr[2 * c] + (br * ur - bi * ui);
-      pp[2 * c + 1] = rr[2 * c + 1] + (br * ui + bi * ur);
-    }
-    stp(p, i, pp);
-  }
-}
 template <typename R> __global__ void __launch_bounds__(BB) update_s_kernel(int64_t n, R* s, const R* r, const R* v, const Scalars* sc, ColMap cm) {
   const int c = cm.col[blockIdx.y];
   sc += c;
@@ -206,12 +188,14 @@ template <typename R> __global__ void __launch_bounds__(BB) acc_y_kernel(int64_t
 template <typename R> __global__ void __launch_bounds__(BB) resid_convert_kernel(int64_t n, int64_t Vh, const double* b, const double* w, double* r64, R* r, const R* rhat, R* p, Scalars* sc, ColMap cm) {
   const int c = cm.col[blockIdx.y];
   sc += c;
-  { const int64_t o = 4 * n * c; b += o; w += o; r64 += o; r += o; rhat += o; if (p) p += o; }
+  { const int64_t o = 4 * n * c; b += o; if (w) w += o; r64 += o; r += o; rhat += o; if (p) p += o; }
   double acc[3] = {0, 0, 0};
   for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
     double bb[4], ww[4], dd[4];
     R hh[4], rr[4];
-    ldm(b, i, Vh, bb); ldm(w, i, Vh, ww); ldm(rhat, i, Vh, hh);
+    ldm(b, i, Vh, bb); ldm(rhat, i, Vh, hh);
+    if (w) ldm(w, i, Vh, ww);
+    else ww[0] = ww[1] = ww[2] = ww[3] = 0.0;
 #pragma unroll
     for (int c = 0; c < 4; c++) { dd[c] = bb[c] - ww[c]; rr[c] = (R)dd[c]; }
     if (p) {  // p += r_new - r_old
@@ -417,11 +401,6 @@ template <typename R> __global__ void __launch_bounds__(BB) gcr_update_kernel(in
 template <typename R> static inline int64_t pairs_of(int64_t n16) { return sizeof(R) == 4 ? n16 : n16 / 2; }
 static inline dim3 grid_of(int64_t np, const ColMap& cm) { return dim3((unsigned)blas_grid(np), (unsigned)cm.n, 1); }
 
-template <typename R> cudaError_t launch_update_p(int64_t n, void* p, const void* r, const void* v, const Scalars* sc, const ColMap& cm, cudaStream_t s) {
-  const int64_t np = pairs_of<R>(n);
-  update_p_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, (R*)p, (const R*)r, (const R*)v, sc, cm);
-  return cudaGetLastError();
-}
 template <typename R> cudaError_t launch_update_s(int64_t n, void* sv, const void* r, const void* v, const Scalars* sc, const ColMap& cm, cudaStream_t s) {
   const int64_t np = pairs_of<R>(n);
   update_s_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, (R*)sv, (const R*)r, (const R*)v, sc, cm);
@@ -473,7 +452,6 @@ template cudaError_t launch_gcr_step<float>(int64_t, int, void*, void*, void*, v
 template cudaError_t launch_gcr_step<double>(int64_t, int, void*, void*, void*, void*, GcrScalars*, cudaStream_t);
 
 #define TMW_INST(R)                                                                                                          \
-  template cudaError_t launch_update_p<R>(int64_t, void*, const void*, const void*, const Scalars*, const ColMap&, cudaStream_t);           \
   template cudaError_t launch_update_s<R>(int64_t, void*, const void*, const void*, const Scalars*, const ColMap&, cudaStream_t);           \
   template cudaError_t launch_update_xrp<R>(int64_t, void*, void*, void*, const void*, const void*, const void*, Scalars*, const ColMap&, cudaStream_t); \
   template cudaError_t launch_dot_norm<R>(int64_t, const void*, const void*, double*, const ColMap&, cudaStream_t);                         \

@@ -84,7 +84,6 @@ cudaError_t launch_sc_alpha(Scalars* sc, const ColMap& cm, cudaStream_t s);     
 // beta = (rho/rho_old)(alpha/omega); zero rr
 cudaError_t launch_sc_omega(Scalars* sc, const ColMap& cm, cudaStream_t s);
 // n = number of 16-byte vectors in one column of each array
-template <typename R> cudaError_t launch_update_p(int64_t n, void* p, const void* r, const void* v, const Scalars* sc, const ColMap& cm, cudaStream_t s);      // p = r + beta (p - omega v)
 template <typename R> cudaError_t launch_update_s(int64_t n, void* sv, const void* r, const void* v, const Scalars* sc, const ColMap& cm, cudaStream_t s);     // s = r - alpha v
 // x += alpha p + omega s; r = s - omega t; p = r + beta (p - omega v); rr += <r,r>  (the end of one BiCGStab iteration and
 // the search direction of the next in one pass: 5 reads + 3 writes instead of 8 + 3 in two kernels)
@@ -93,7 +92,7 @@ template <typename R> cudaError_t launch_update_xrp(int64_t n, void* x, void* r,
 template <typename R> cudaError_t launch_dot_norm(int64_t n, const void* a, const void* b, double* out, const ColMap& cm, cudaStream_t s);
 // fp64 helpers for the reliable update
 template <typename R> cudaError_t launch_acc_y(int64_t n64, void* y64, void* x, const ColMap& cm, cudaStream_t s);  // y += x; x = 0   (n64 = number of double2 vectors per column)
-// r64 = b64 - w64; r = (R) r64; rho += <rhat, r>; rr += <r64, r64>. If p is not null (reliable update in the middle of
+// r64 = b64 - w64 (w64 may be null: zero); r = (R) r64; rho += <rhat, r>; rr += <r64, r64>. If p is not null (reliable update in the middle of
 // the recurrence): p += r_new - r_old, i.e. the search direction already built from the iterated residual is moved to
 // the true one.
 template <typename R> cudaError_t launch_resid_convert(int64_t n64, const void* b64, const void* w64, void* r64, void* r, const void* rhat, void* p, Scalars* sc, const ColMap& cm, cudaStream_t s);
