@@ -54,7 +54,7 @@ typedef struct { double re, im; } tmw_complex;
 #define TMW_ECUDA (-3)      /* a CUDA call failed; text in tmw_last_error */
 #define TMW_ESINGULAR (-4)  /* a clover block (or the twisted-mass diagonal) is not invertible */
 #define TMW_ENOCONV (-5)    /* max_iter reached: x holds the best iterate, info is filled */
-#define TMW_EBREAKDOWN (-6) /* BiCGStab breakdown (rho or <t,t> vanished / NaN) that restarts did not cure */
+#define TMW_EBREAKDOWN (-6) /* BiCGStab breakdown (rho or <t,t> vanished / NaN): 5 consecutive restarts brought no progress */
 
 /* enums */
 #define TMW_DEVICE 0

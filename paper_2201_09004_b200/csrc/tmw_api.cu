@@ -570,6 +570,9 @@ struct ColState {
   double bnorm, rnorm, maxr, rhat_norm;
   bool done;    // converged (or b = 0)
   int iters, updates, restarts;
+  double r_upd;  // true residual at the last reliable update / restart (what y stands for)
+  double best;   // smallest true residual seen at a restart
+  int stalled;   // consecutive restarts that did not improve on it
   double iter_resid, true_resid;
 };
 
@@ -613,7 +616,9 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
   const int SCD = (int)(sizeof(Scalars) / sizeof(double));
   double* red_rhat_v = (double*)((char*)ctx->sc + offsetof(Scalars, rhat_v));
   double* red_ts = (double*)((char*)ctx->sc + offsetof(Scalars, ts));
-  const double eps_break = sizeof(R) == 4 ? 1e-6 : 1e-12;
+  // restart when |rho| = |<rhat,r>| has decayed to the noise of the vectors relative to |rhat||r|: the dot products are
+  // accumulated in fp64, so for fp32 vectors that floor is ~1e-9 (rounding of r, ~6e-8/sqrt(N) per step), not 1e-6
+  const double eps_break = sizeof(R) == 4 ? 1e-8 : 1e-12;
   const bool verbose = getenv("TMW_VERBOSE") != nullptr;  // per-iteration residual log on stderr
   int rc;
   ColMap act;
@@ -631,7 +636,7 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
   for (int i = 0; i < act.n; i++) {
     const int c = act.col[i];
     reset_recurrence(&h[c]);
-    cs[c].rnorm = cs[c].maxr = cs[c].rhat_norm = sqrt(h[c].rr);
+    cs[c].rnorm = cs[c].maxr = cs[c].rhat_norm = cs[c].r_upd = cs[c].best = sqrt(h[c].rr);
     cs[c].iter_resid = cs[c].rnorm / cs[c].bnorm;
     if (cs[c].rnorm <= tol * cs[c].bnorm) cs[c].done = true;
   }
@@ -695,7 +700,7 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
         const int c = upd.col[i];
         ColState& q = cs[c];
         q.updates++;
-        q.rnorm = q.maxr = sqrt(h[c].rr);
+        q.rnorm = q.maxr = q.r_upd = sqrt(h[c].rr);
         q.iter_resid = q.rnorm / q.bnorm;
         if (verbose) fprintf(stderr, "[tmw]   col %d reliable update %d: true |r|/|b| %.3e rho (%.3e,%.3e)\n", c, q.updates, q.rnorm / q.bnorm, h[c].rho[0], h[c].rho[1]);
         if (!isfinite(q.rnorm)) return fail(ctx, TMW_EBREAKDOWN, "tmw_solve: non-finite true residual");
@@ -711,13 +716,21 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
       const double rho_abs = hypot(h[c].rho[0], h[c].rho[1]);
       if (broken[c] || !(rho_abs > eps_break * cs[c].rhat_norm * cs[c].rnorm)) {
         if (verbose) fprintf(stderr, "[tmw]   col %d breakdown: |rho| %.3e vs %.3e * %.3e * %.3e -> restart\n", c, rho_abs, eps_break, cs[c].rhat_norm, cs[c].rnorm);
-        if (++cs[c].restarts > 5) return fail(ctx, TMW_EBREAKDOWN, "tmw_solve: BiCGStab breakdown persists after 5 restarts");
+        cs[c].restarts++;
         cols_add(rst, c);
       }
     }
     if (rst.n > 0) {
-      // fold the current iterate into y first so that r is the residual of y
-      LAUNCH(launch_acc_y<R>(n64, W[3], x, rst, s));
+      // fold the current iterate into y first so that r is the residual of y - unless the recurrence has wandered off
+      // (corrupted, or its residual is above the one y already has): then the iterate is dropped
+      ColMap keep;
+      keep.n = 0;
+      for (int i = 0; i < rst.n; i++) {
+        const int c = rst.col[i];
+        if (!broken[c] && cs[c].rnorm <= cs[c].r_upd) cols_add(keep, c);
+        else CK(cudaMemsetAsync(colp(x, c, bytesR), 0, bytesR, s));
+      }
+      if (keep.n > 0) LAUNCH(launch_acc_y<R>(n64, W[3], x, keep, s));
       if ((rc = schur<double>(ctx, 0, W[3], W[6], W[5], rst))) return rc;
       for (int i = 0; i < rst.n; i++) {
         const int c = rst.col[i];
@@ -734,10 +747,14 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
       for (int i = 0; i < rst.n; i++) {
         const int c = rst.col[i];
         ColState& q = cs[c];
-        q.rnorm = q.maxr = q.rhat_norm = sqrt(h[c].rr);
+        q.rnorm = q.maxr = q.rhat_norm = q.r_upd = sqrt(h[c].rr);
         q.iter_resid = q.rnorm / q.bnorm;
         q.updates++;
-        if (q.rnorm <= tol * q.bnorm) q.done = true;
+        if (verbose) fprintf(stderr, "[tmw]   col %d restart %d: true |r|/|b| %.3e\n", c, q.restarts, q.iter_resid);
+        if (q.rnorm <= tol * q.bnorm) { q.done = true; continue; }
+        // restarts are cheap and a long solve may need many; give up only when they stop paying
+        if (q.rnorm < 0.9 * q.best) { q.best = q.rnorm; q.stalled = 0; }
+        else if (++q.stalled > 5) return fail(ctx, TMW_EBREAKDOWN, "tmw_solve: BiCGStab breakdown: no progress over 5 consecutive restarts");
       }
     }
   }

@@ -347,3 +347,23 @@ def test_create_errors(tmw):
     with pytest.raises(tmw.TmwError) as e:
         tmw.Context(4, 4, dev(synth.unit_gauge(4, 4)), -4.0, 1.0)
     assert e.value.code == tmw.ESINGULAR
+
+
+def test_solve_hard_system_with_restarts(tmw):
+    """A smooth field close to the critical mass (eps = 0.1, m = -0.2, c_sw = 1): BiCGStab needs hundreds of iterations
+    and its <rhat, r> decays to the noise several times, so the restart path (rhat := r from the fp64 true residual,
+    C11) is exercised; restarts are allowed as long as they keep paying. Checked through the oracle's operator."""
+    L, T, m, c_sw = 8, 16, -0.2 + 0.0j, 1.0
+    U = synth.gauge_field(L, T, 0.1, seed=1)
+    b = synth.gaussian_spinor(L, T, 3)
+    F = oracle.field_strength(U)
+    sols = {}
+    for precision in (tmw.MIXED, tmw.DOUBLE):
+        with tmw.Context(L, T, dev(U), m, c_sw, precision=precision, max_iter=4000) as ctx:
+            x = torch.empty((T, L, L, L, 4, 3), dtype=torch.complex128, device="cuda")
+            info = ctx.solve(dev(b), x, 1e-10)
+            assert info["true_resid"] <= 1e-10 and info["iters"] > 100 and info["restarts"] >= 1, info
+            sols[precision] = x.cpu().numpy()
+            check_solution(U, b, sols[precision], m, c_sw, F=F)
+    d = np.linalg.norm((sols[tmw.MIXED] - sols[tmw.DOUBLE]).ravel()) / np.linalg.norm(sols[tmw.DOUBLE].ravel())
+    assert d <= 1e-6, d  # both have residual 1e-10; the condition number of this system is ~1e3
