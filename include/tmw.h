@@ -131,6 +131,8 @@ int tmw_apply_schur(tmw_ctx* ctx, int op, int prec, const void* in_odd, void* ou
 /*
  * Solve D x = b to |b - D x| / |b| <= tol. b, x: canonical fp64 spinors (HOST or DEVICE per location).
  * b = 0 gives x = 0. Returns after the final fp64 true residual is known. info may be NULL.
+ * TMW_MIXED: if the fp32 BiCGStab recurrence stalls (TMW_EBREAKDOWN; only seen on near-critical systems that need
+ * ~1000 iterations) the solve is redone with fp64 recurrences before an error is returned.
  */
 int tmw_solve(tmw_ctx* ctx, const double* b, double* x, double tol, tmw_solve_info* info);
 

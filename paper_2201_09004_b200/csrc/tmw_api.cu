@@ -958,7 +958,17 @@ extern "C" int tmw_solve_multi(tmw_ctx* ctx, int nrhs, const double* b, double* 
   const size_t cdoubles = (size_t)ctx->V * 24;
   for (int c0 = 0; c0 < nrhs; c0 += chunk) {
     const int n = nrhs - c0 < chunk ? nrhs - c0 : chunk;
-    const int rc = solve_chunk(ctx, n, b + c0 * cdoubles, x + c0 * cdoubles, tol, info ? info + c0 : nullptr);
+    int rc = solve_chunk(ctx, n, b + c0 * cdoubles, x + c0 * cdoubles, tol, info ? info + c0 : nullptr);
+    if (rc == TMW_EBREAKDOWN && ctx->opt.precision == TMW_MIXED && ctx->opt.solver == TMW_BICGSTAB) {
+      // the fp32 recurrence stalled (near-critical system): redo the chunk with fp64 recurrences, which hold out longer
+      CK(cudaStreamSynchronize(ctx->stream));
+      for (int i = 0; i < 8; i++) if (ctx->w32[i]) { dev_free(ctx, ctx->w32[i]); ctx->w32[i] = nullptr; }
+      ctx->opt.precision = TMW_DOUBLE;
+      rc = solve_chunk(ctx, n, b + c0 * cdoubles, x + c0 * cdoubles, tol, info ? info + c0 : nullptr);
+      ctx->opt.precision = TMW_MIXED;
+      cudaStreamSynchronize(ctx->stream);
+      for (int i = 0; i < 8; i++) if (ctx->w32[i]) { dev_free(ctx, ctx->w32[i]); ctx->w32[i] = nullptr; }
+    }
     if (rc != TMW_OK && rc != TMW_ENOCONV) return rc;
     if (rc == TMW_ENOCONV) status = rc;
   }
