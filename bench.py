@@ -74,7 +74,7 @@ class ClockSampler(threading.Thread):
     def __init__(self, index: int, period: float = 0.05):
         super().__init__(daemon=True)
         self.index, self.period = index, period
-        self.samples, self.reason_bits, self.power = [], 0, []
+        self.samples, self.mem_samples, self.reason_bits, self.power = [], [], 0, []
         self.stop_flag = threading.Event()
         self.ok = False
         try:
@@ -94,6 +94,7 @@ class ClockSampler(threading.Thread):
         while not self.stop_flag.is_set():
             try:
                 self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                self.mem_samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_MEM))
                 self.reason_bits |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
                 self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
             except Exception:
@@ -105,6 +106,7 @@ class ClockSampler(threading.Thread):
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml unavailable: " + getattr(self, "err", "")]}
         reasons = [name for bit, name in self.REASONS.items() if self.reason_bits & bit and name != "gpu_idle"]
         return {"sm_mhz": float(np.median(self.samples)) if self.samples else None, "sm_max_mhz": float(self.max_mhz),
+                "mem_mhz": float(np.median(self.mem_samples)) if self.mem_samples else None,
                 "reasons": reasons, "samples": len(self.samples),
                 "power_w_max": float(max(self.power)) if self.power else None}
 
