@@ -365,6 +365,13 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
                  "solve_true_resid_max": max(i["true_resid"] for i in minfos),
                  "dslash_ms_per_rhs": ms_hop / n, "dslash_gflops": FLOP_PER_SITE * float(Vh) * n * world / (ms_hop * 1e-3) / 1e9,
                  "call": "tmw_solve_multi / tmw_apply_multi, columns resident in HBM"}
+        # roofline of the multi-column hop launch: per site and column 96 B in + 96 B out + 384 B of links shared by n
+        bpc = 192.0 + 384.0 / n
+        ach = bpc * Vh * n / (ms_hop * 1e-3) / 1e9
+        pk, pk_src = load_peaks()
+        multi["roofline"] = {"bound": "hbm", "kernel": "dslash_kernel<float,12,EPI_HOP,NR=2|3> (multi-column hop)", "achieved": ach,
+                             "peak": pk, "unit": "GB/s", "frac": ach / pk, "bytes_per_site_and_column": bpc, "peak_source": pk_src,
+                             "note": "not HBM-bound: the links are amortised, the 8 neighbour spinors per column are not (DESIGN.md 6b)"}
         del bm, xm, pm, pm2
         torch.cuda.empty_cache()
 
