@@ -91,7 +91,19 @@ typedef struct {
   int solver;       /* TMW_BICGSTAB (default; the paper's CPU solver) | TMW_GCR (its "standard GPU inverter with
                        GCR algorithm"): restarted GCR(nkrylov) on the same Schur system and kernels */
   int nkrylov;      /* GCR restart length, 1..16; 0 -> 8 */
+  int verbose;      /* != 0: one line per solver iteration, reliable update and restart on stderr. Setting the environment
+                       variable TMW_VERBOSE (to anything) has the same effect on every context of the process. */
+  int columns_per_thread; /* tuning of the multi-column fp32 stencil (tmw_*_multi): 1..4 right-hand-side
+                             columns per thread (links and clover blocks stay in registers for them); 0 = automatic */
+  int tile[4];      /* log2 extents (x/2, y, z, t) of the 4-D tile of 128 sites a CTA of the single-column stencil covers;
+                       all 0 (default): 128 consecutive checkerboard indices; tile[0] = -1: the largest tile that fits,
+                       preferring 8 x 4 x 2 x 2. A tile that does not divide the lattice or is not 128 sites -> 1-D. */
+  int debug;        /* bit mask of TMW_DEBUG_* (test hooks, see below); also settable later with tmw_set_debug */
 } tmw_options;
+
+/* Test hooks (tmw_options.debug / tmw_set_debug): they change which code path runs, never the result. */
+#define TMW_DEBUG_FORCE_PIVOT 1 /* tmw_create: invert the clover blocks with the pivoted Gauss-Jordan fallback kernel */
+#define TMW_DEBUG_NO_CHUNK 2    /* tmw_solve_multi: do not split the columns into chunks that fit the free memory */
 
 typedef struct {
   int iters;            /* BiCGStab iterations (each = 2 Schur-operator applications) or GCR steps (1 application each) */
@@ -184,6 +196,9 @@ int tmw_get_clover(tmw_ctx* ctx, int parity, int inverse, double* dst);
 
 /* change where the canonical-layout pointers of subsequent calls live (TMW_DEVICE | TMW_HOST) */
 int tmw_set_location(tmw_ctx* ctx, int location);
+
+/* replace the TMW_DEBUG_* mask of the context (TMW_DEBUG_FORCE_PIVOT only matters at tmw_create) */
+int tmw_set_debug(tmw_ctx* ctx, int flags);
 
 /* number of kernel launches this context has issued since creation (bench.py's gpu_launches) */
 long long tmw_launch_count(const tmw_ctx* ctx);

@@ -26,6 +26,8 @@ struct NvtxRange {
 
 using namespace tmw;
 
+enum { NW64 = 14 };
+
 struct tmw_ctx {
   Geom g;
   int64_t V;
@@ -43,7 +45,7 @@ struct tmw_ctx {
   std::vector<void*> owned;  // every device allocation
   // lazily allocated workspaces, each sized for ws_cols right-hand-side columns (column c at c * spinor bytes)
   int ws_cols;
-  void* w64[10];  // packed fp64 parity spinors
+  void* w64[NW64];  // packed fp64 parity spinors (0..7 the solver's, 8..13 only for the rare defect-correction pass)
   void* w32[8];   // packed inner-precision parity spinors (fp32 for TMW_MIXED, fp64 for TMW_DOUBLE)
   void* canon[2]; // canonical fp64 full-lattice staging (HOST location only)
   void* gcr_q;       // GCR Krylov vectors q_j, p_j: nkrylov inner-precision parity spinors each (lazily allocated)
@@ -51,6 +53,7 @@ struct tmw_ctx {
   GcrScalars* gs;       // device
   GcrScalars* gs_host;  // pinned
   int nr32;          // forced columns per thread of the fp32 stencil (1..4), 0 = automatic
+  bool verbose;
   Scalars* sc;       // MAXCOL scalar blocks
   Scalars* sc_host;  // pinned
   double* red;       // 4 * MAXCOL device doubles
@@ -174,7 +177,7 @@ static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, vo
   // columns per thread: as even a split of the columns into groups of at most nr32 as possible
   int nr = 1;
   if (sizeof(R) == 4 && cm.n > 1) {
-    if (ctx->nr32 > 0) {  // TMW_NR: as even a split into groups of at most nr32 columns as possible
+    if (ctx->nr32 > 0) {  // tmw_options.columns_per_thread
       const int groups = (cm.n + ctx->nr32 - 1) / ctx->nr32;
       nr = (cm.n + groups - 1) / groups;
     } else {  // 2 columns per thread (the fastest) unless 3 wastes fewer slots of a ragged last group
@@ -195,21 +198,18 @@ static int schur(tmw_ctx* ctx, int dagger, const void* in, void* out, void* tmp,
   return dslash<R>(ctx, EPI_A_XPAY, 1, dagger, tmp, out, in, -1.0, cm, red_mode, dotv, red, red_stride);
 }
 
-// Thread -> site mapping of the stencil kernels (Geom::tiled). Default: 1-D (CTA b = 128 consecutive cb). With
-// TMW_TILE="auto" the largest power-of-two 4-D tile of 128 sites that divides the lattice, preferring 8 (xh) x 4 (y)
-// x 2 (z) x 2 (t); with TMW_TILE="lx,ly,lz,lt" those log2 extents. Measured on B200: the tiled
-// mapping changes neither the time nor the DRAM traffic of the stencil, so it stays an opt-in tuning knob.
-static void choose_tile(Geom& g) {
+// Thread -> site mapping of the single-column stencil kernels (Geom::tiled), from tmw_options.tile: all 0 -> 1-D (CTA b =
+// 128 consecutive cb); tile[0] = -1 -> the largest power-of-two 4-D tile of 128 sites that divides the lattice,
+// preferring 8 (xh) x 4 (y) x 2 (z) x 2 (t); else those log2 extents. Measured on B200: the tiled mapping
+// changes neither the time nor the DRAM traffic of the stencil, so it stays an opt-in tuning knob.
+static void choose_tile(Geom& g, const int* tile) {
   g.tiled = 0;
   g.lx = g.ly = g.lz = g.lt = 0;
   g.ntx = g.nty = 1;
-  int l[4] = {-1, -1, -1, -1};
-  const char* e = getenv("TMW_TILE");
-  if (!e) return;
-  if (strcmp(e, "auto") != 0) {
-    if (sscanf(e, "%d,%d,%d,%d", &l[0], &l[1], &l[2], &l[3]) != 4) return;  // "0" or malformed: 1-D mapping
-  } else {
-    const int ext[4] = {g.Lh, g.L, g.L, g.T};
+  int l[4] = {tile[0], tile[1], tile[2], tile[3]};
+  if (l[0] == 0 && l[1] == 0 && l[2] == 0 && l[3] == 0) return;
+  const int ext[4] = {g.Lh, g.L, g.Lz, g.T};
+  if (l[0] < 0) {
     const int want[4] = {3, 2, 1, 1};
     int left = 7;
     for (int d = 0; d < 4; d++) {
@@ -221,7 +221,6 @@ static void choose_tile(Geom& g) {
       while (left > 0 && ext[d] % (2 << l[d]) == 0) { l[d]++; left--; }
     if (left != 0) return;
   }
-  const int ext[4] = {g.Lh, g.L, g.L, g.T};
   int sum = 0;
   for (int d = 0; d < 4; d++) {
     if (l[d] < 0 || l[d] > 7 || ext[d] % (1 << l[d]) != 0) return;
@@ -268,17 +267,19 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
   if ((o.location != TMW_DEVICE && o.location != TMW_HOST) || (o.precision != TMW_MIXED && o.precision != TMW_DOUBLE) ||
       (o.reconstruct != 12 && o.reconstruct != 18) || (o.mass_reading != TMW_TWIST_GAMMA5 && o.mass_reading != TMW_MASS_SCALAR) ||
       o.max_iter < 0 || !(o.delta > 0.0) || !(o.delta < 1.0) || (o.solver != TMW_BICGSTAB && o.solver != TMW_GCR) || o.nkrylov < 1 ||
-      o.nkrylov > GCR_KMAX)
+      o.nkrylov > GCR_KMAX || o.columns_per_thread < 0 || o.columns_per_thread > 4 ||
+      (o.debug & ~(TMW_DEBUG_FORCE_PIVOT | TMW_DEBUG_NO_CHUNK)))
     return fail(nullptr, TMW_EINVAL, "tmw_create: bad option value");
   if (!isfinite(m.re) || !isfinite(m.im) || !isfinite(c_sw)) return fail(nullptr, TMW_EINVAL, "tmw_create: non-finite parameter");
   tmw_ctx* ctx = new (std::nothrow) tmw_ctx();
   if (!ctx) return fail(nullptr, TMW_ENOMEM, "tmw_create: host allocation failed");
   ctx->g.L = L; ctx->g.T = T; ctx->g.Lh = L / 2; ctx->g.Vh = (int)(V / 2);
+  ctx->g.Lz = L; ctx->g.oz = 0; ctx->g.ot = 0; ctx->g.GT = T;
   ctx->g.sy = L / 2; ctx->g.sz = (L / 2) * L; ctx->g.st = (L / 2) * L * L;
-  choose_tile(ctx->g);
+  choose_tile(ctx->g, o.tile);
   ctx->ws_cols = 1;
-  ctx->nr32 = 0;  // 0: automatic (2 or 3 columns per thread); TMW_NR=1..4 forces the group size (tuning, tests)
-  if (const char* e = getenv("TMW_NR")) { const int v = atoi(e); if (v >= 1 && v <= 4) ctx->nr32 = v; }
+  ctx->nr32 = o.columns_per_thread;
+  ctx->verbose = o.verbose != 0 || getenv("TMW_VERBOSE") != nullptr;
   ctx->V = V;
   ctx->m_re = m.re; ctx->m_im = m.im; ctx->c_sw = c_sw;
   ctx->opt = o;
@@ -346,7 +347,7 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
     int hflag = 0;
     CKC(cudaMemcpyAsync(&hflag, flag, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
     CKC(cudaStreamSynchronize(ctx->stream));
-    if (getenv("TMW_CLOVER_PIVOT")) hflag = 1;  // tests: force the fallback
+    if (o.debug & TMW_DEBUG_FORCE_PIVOT) hflag = 1;  // tests: force the fallback
     if (hflag) {  // a tiny pivot without pivoting: redo the field with the pivoted kernel, which decides singularity
       CKC(cudaMemsetAsync(flag, 0, sizeof(int), ctx->stream));
       CKC(launch_clover_invert_pivot(ctx->g, ctx->c64[0], tw2, ctx->ci64, ctx->ci32, flag, ctx->stream));
@@ -373,6 +374,13 @@ int tmw_set_location(tmw_ctx* ctx, int location) {
   if (!ctx) return TMW_EINVAL;
   if (location != TMW_DEVICE && location != TMW_HOST) return fail(ctx, TMW_EINVAL, "tmw_set_location: bad location");
   ctx->opt.location = location;
+  return TMW_OK;
+}
+
+int tmw_set_debug(tmw_ctx* ctx, int flags) {
+  if (!ctx) return TMW_EINVAL;
+  if (flags & ~(TMW_DEBUG_FORCE_PIVOT | TMW_DEBUG_NO_CHUNK)) return fail(ctx, TMW_EINVAL, "tmw_set_debug: unknown flag");
+  ctx->opt.debug = flags;
   return TMW_OK;
 }
 
@@ -403,9 +411,11 @@ int tmw_get_clover(tmw_ctx* ctx, int parity, int inverse, double* dst) {
 
 // ---- workspaces ----
 static void release_ws(tmw_ctx* ctx) {
-  for (int i = 0; i < 10; i++) if (ctx->w64[i]) { dev_free(ctx, ctx->w64[i]); ctx->w64[i] = nullptr; }
+  for (int i = 0; i < NW64; i++) if (ctx->w64[i]) { dev_free(ctx, ctx->w64[i]); ctx->w64[i] = nullptr; }
   for (int i = 0; i < 8; i++) if (ctx->w32[i]) { dev_free(ctx, ctx->w32[i]); ctx->w32[i] = nullptr; }
   for (int i = 0; i < 2; i++) if (ctx->canon[i]) { dev_free(ctx, ctx->canon[i]); ctx->canon[i] = nullptr; }
+  if (ctx->gcr_q) { dev_free(ctx, ctx->gcr_q); ctx->gcr_q = nullptr; }
+  if (ctx->gcr_p) { dev_free(ctx, ctx->gcr_p); ctx->gcr_p = nullptr; }
 }
 // make the workspaces hold `cols` columns (existing smaller ones are released and re-made on demand)
 static int need_cols(tmw_ctx* ctx, int cols) {
@@ -619,7 +629,7 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
   // restart when |rho| = |<rhat,r>| has decayed to the noise of the vectors relative to |rhat||r|: the dot products are
   // accumulated in fp64, so for fp32 vectors that floor is ~1e-9 (rounding of r, ~6e-8/sqrt(N) per step), not 1e-6
   const double eps_break = sizeof(R) == 4 ? 1e-8 : 1e-12;
-  const bool verbose = getenv("TMW_VERBOSE") != nullptr;  // per-iteration residual log on stderr
+  const bool verbose = ctx->verbose;  // per-iteration residual log on stderr
   int rc;
   ColMap act;
   act.n = 0;
@@ -778,8 +788,8 @@ int solve_gcr(tmw_ctx* ctx, int c, double tol, ColState& q) {
   void** W = ctx->w64;
   void** X = ctx->w32;
   int rc;
-  if (!ctx->gcr_q) { if ((rc = dev_alloc(ctx, &ctx->gcr_q, bytesR * GCR_KMAX))) return rc; }
-  if (!ctx->gcr_p) { if ((rc = dev_alloc(ctx, &ctx->gcr_p, bytesR * GCR_KMAX))) return rc; }
+  if (!ctx->gcr_q) { if ((rc = ws_alloc(ctx, &ctx->gcr_q, bytesR * k))) return rc; }
+  if (!ctx->gcr_p) { if ((rc = ws_alloc(ctx, &ctx->gcr_p, bytesR * k))) return rc; }
   ColMap one;
   one.n = 0;
   cols_add(one, c);
@@ -788,7 +798,7 @@ int solve_gcr(tmw_ctx* ctx, int c, double tol, ColState& q) {
   void* tmp = colp(X[7], c, bytesR);
   Scalars* h = ctx->sc_host;
   GcrScalars* gh = ctx->gs_host;
-  const bool verbose = getenv("TMW_VERBOSE") != nullptr;
+  const bool verbose = ctx->verbose;
   const ColMap zero = cols_first(1);
   CK(cudaMemsetAsync(colp(W[3], c, (size_t)n64 * 16), 0, (size_t)n64 * 16, s));
   CK(cudaMemsetAsync(colp(W[6], c, (size_t)n64 * 16), 0, (size_t)n64 * 16, s));
@@ -831,6 +841,49 @@ int solve_gcr(tmw_ctx* ctx, int c, double tol, ColState& q) {
 
 }  // namespace
 
+// The columns of cm: from the packed fp64 source W[0] (even), W[1] (odd) to the packed solution W[7] (even), W[3] (odd).
+//   A7: bhat_o = b_o - H_oe A_ee^{-1} b_e;  Krylov iterations on Mhat y = bhat_o;  x_o = y, x_e = A_ee^{-1} (b_e - H_eo x_o)
+// cs[c].done marks the columns that are NOT to be iterated (already solved, or b = 0). Returns TMW_OK or TMW_ENOCONV.
+static int solve_packed(tmw_ctx* ctx, int nrhs, const ColMap& cm, double tol, ColState* cs) {
+  const bool dbl = ctx->opt.precision == TMW_DOUBLE;
+  cudaStream_t s = ctx->stream;
+  void** W = ctx->w64;
+  const size_t b64 = spinor_bytes(ctx, TMW_F64);
+  int rc, status = TMW_OK;
+  Diag<double> d = make_diag<double>(ctx, 0);
+  for (int i = 0; i < cm.n; i++) LAUNCH(launch_diag(d, ctx->g, 0, ctx->clover, 1, colp(W[0], cm.col[i], b64), colp(W[5], cm.col[i], b64), s));
+  if ((rc = dslash<double>(ctx, EPI_XPAY, 1, 0, W[5], W[2], W[1], -1.0, cm))) return rc;
+  {
+    NvtxRange nvtx_it("tmw_solve: Krylov iterations");
+    if (ctx->opt.solver == TMW_GCR) {
+      for (int i = 0; i < cm.n; i++) {  // GCR keeps 2 k Krylov vectors per system: the columns go one after another
+        rc = dbl ? solve_gcr<double>(ctx, cm.col[i], tol, cs[cm.col[i]]) : solve_gcr<float>(ctx, cm.col[i], tol, cs[cm.col[i]]);
+        if (rc != TMW_OK && rc != TMW_ENOCONV) return rc;
+        if (rc == TMW_ENOCONV) status = rc;
+      }
+    } else {
+      status = dbl ? solve_schur<double>(ctx, nrhs, tol, cs) : solve_schur<float>(ctx, nrhs, tol, cs);
+    }
+  }
+  if (status != TMW_OK && status != TMW_ENOCONV) return status;
+  if ((rc = dslash<double>(ctx, EPI_AINV_XPAY, 0, 0, W[3], W[7], W[0], -1.0, cm))) return rc;
+  return status;
+}
+
+// |b - D x| / |b| of the full system in fp64 for the columns of cm (b in W[0], W[1]; x in W[7], W[3]): the difference and
+// its norm are fused into the two launches of the full operator. With store_e/store_o the products D x themselves are
+// written there (both parities) instead.
+static int full_residual(tmw_ctx* ctx, const ColMap& cm, ColState* cs) {
+  void** W = ctx->w64;
+  int rc;
+  CK(cudaMemsetAsync(ctx->red, 0, 4 * MAXCOL * sizeof(double), ctx->stream));
+  if ((rc = dslash<double>(ctx, EPI_A_XPAY, 0, 0, W[3], nullptr, W[7], 1.0, cm, 3, W[0], ctx->red, 4))) return rc;
+  if ((rc = dslash<double>(ctx, EPI_A_XPAY, 1, 0, W[7], nullptr, W[3], 1.0, cm, 3, W[1], ctx->red, 4))) return rc;
+  if ((rc = fetch_red(ctx))) return rc;
+  for (int i = 0; i < cm.n; i++) cs[cm.col[i]].true_resid = sqrt(ctx->red_host[4 * cm.col[i] + 2]) / cs[cm.col[i]].bnorm;
+  return TMW_OK;
+}
+
 // nrhs columns that are known to fit in the workspaces (tmw_solve_multi below splits a call into such chunks)
 static int solve_chunk(tmw_ctx* ctx, int nrhs, const double* b, double* x, double tol, tmw_solve_info* info) {
   const bool dbl = ctx->opt.precision == TMW_DOUBLE;
@@ -854,7 +907,7 @@ static int solve_chunk(tmw_ctx* ctx, int nrhs, const double* b, double* x, doubl
   ColState cs[MAXCOL];
   memset(cs, 0, sizeof(cs));
   const ColMap all = cols_first(nrhs);
-  // A0/A7: split b, |b|, bhat_o = b_o - H_oe A_ee^{-1} b_e
+  // A0: split b into parities, |b|
   for (int c = 0; c < nrhs; c++) {
     LAUNCH(launch_pack_spinor_both(ctx->g, 1, (const double*)colp(cb, c, cbytes), colp(W[0], c, b64), colp(W[1], c, b64), s));
   }
@@ -876,35 +929,56 @@ static int solve_chunk(tmw_ctx* ctx, int nrhs, const double* b, double* x, doubl
   }
   int status = TMW_OK;
   if (nz.n > 0) {
-    Diag<double> d = make_diag<double>(ctx, 0);
-    for (int i = 0; i < nz.n; i++) LAUNCH(launch_diag(d, ctx->g, 0, ctx->clover, 1, colp(W[0], nz.col[i], b64), colp(W[5], nz.col[i], b64), s));
-    if ((rc = dslash<double>(ctx, EPI_XPAY, 1, 0, W[5], W[2], W[1], -1.0, nz))) return rc;
-    {
-    NvtxRange nvtx_it("tmw_solve: Krylov iterations");
-    if (ctx->opt.solver == TMW_GCR) {
-      for (int i = 0; i < nz.n; i++) {  // GCR keeps 2 k Krylov vectors per system: the columns go one after another
-        rc = dbl ? solve_gcr<double>(ctx, nz.col[i], tol, cs[nz.col[i]]) : solve_gcr<float>(ctx, nz.col[i], tol, cs[nz.col[i]]);
-        if (rc != TMW_OK && rc != TMW_ENOCONV) return rc;
-        if (rc == TMW_ENOCONV) status = rc;
-      }
-    } else {
-      status = dbl ? solve_schur<double>(ctx, nrhs, tol, cs) : solve_schur<float>(ctx, nrhs, tol, cs);
-    }
-    }
+    status = solve_packed(ctx, nrhs, nz, tol, cs);
     if (status != TMW_OK && status != TMW_ENOCONV) return status;
-    // A7: x_o = y, x_e = A_ee^{-1} (b_e - H_eo x_o)
-    if ((rc = dslash<double>(ctx, EPI_AINV_XPAY, 0, 0, W[3], W[7], W[0], -1.0, nz))) return rc;
+    if ((rc = full_residual(ctx, nz, cs))) return rc;
+    // The stopping rule of include/tmw.h is the residual of the FULL system, but the iteration is stopped on the odd-site
+    // Schur residual; the two agree only as far as the fp64 A_ee^{-1} is well conditioned (with near-singular clover
+    // blocks the even-site defect grows as cond(A_ee) * eps). Columns that converged on the Schur system but whose full
+    // residual is above tol get fp64 defect correction: solve D e = b - D x the same way, x += e (at most twice).
+    for (int round = 0; round < 2 && status == TMW_OK; round++) {
+      ColMap bad;
+      bad.n = 0;
+      for (int i = 0; i < nz.n; i++) if (!(cs[nz.col[i]].true_resid <= tol)) cols_add(bad, nz.col[i]);
+      if (bad.n == 0) break;
+      if (ctx->verbose) fprintf(stderr, "[tmw] defect correction %d for %d column(s): full residual %.3e > tol\n", round + 1, bad.n, cs[bad.col[0]].true_resid);
+      if ((rc = need_w64(ctx, NW64))) return rc;
+      int it0[MAXCOL], up0[MAXCOL];
+      for (int i = 0; i < bad.n; i++) {
+        const int c = bad.col[i];
+        CK(cudaMemcpyAsync(colp(W[10], c, b64), colp(W[0], c, b64), b64, cudaMemcpyDeviceToDevice, s));  // b
+        CK(cudaMemcpyAsync(colp(W[11], c, b64), colp(W[1], c, b64), b64, cudaMemcpyDeviceToDevice, s));
+        CK(cudaMemcpyAsync(colp(W[12], c, b64), colp(W[7], c, b64), b64, cudaMemcpyDeviceToDevice, s));  // x
+        CK(cudaMemcpyAsync(colp(W[13], c, b64), colp(W[3], c, b64), b64, cudaMemcpyDeviceToDevice, s));
+        it0[c] = cs[c].iters;
+        up0[c] = cs[c].updates;
+      }
+      if ((rc = full_apply64(ctx, 0, W[7], W[3], W[8], W[9], bad))) return rc;        // D x
+      LAUNCH(launch_sub_norm(n64, W[10], W[8], W[0], ctx->red, bad, s));              // b := b - D x (norm discarded)
+      LAUNCH(launch_sub_norm(n64, W[11], W[9], W[1], ctx->red, bad, s));
+      for (int c = 0; c < nrhs; c++) cs[c].done = true;
+      for (int i = 0; i < bad.n; i++) cs[bad.col[i]].done = false;
+      status = solve_packed(ctx, nrhs, bad, tol, cs);                                 // e, to the same absolute target tol |b|
+      if (status != TMW_OK && status != TMW_ENOCONV) return status;
+      LAUNCH(launch_add64(n64, W[7], W[12], bad, s));                                 // x = x + e
+      LAUNCH(launch_add64(n64, W[3], W[13], bad, s));
+      for (int i = 0; i < bad.n; i++) {
+        const int c = bad.col[i];
+        CK(cudaMemcpyAsync(colp(W[0], c, b64), colp(W[10], c, b64), b64, cudaMemcpyDeviceToDevice, s));
+        CK(cudaMemcpyAsync(colp(W[1], c, b64), colp(W[11], c, b64), b64, cudaMemcpyDeviceToDevice, s));
+        cs[c].iters += it0[c];
+        cs[c].updates += up0[c];
+      }
+      if ((rc = full_residual(ctx, bad, cs))) return rc;
+    }
     for (int i = 0; i < nz.n; i++) {
       const int c = nz.col[i];
       LAUNCH(launch_unpack_spinor_both(ctx->g, 1, colp(W[7], c, b64), colp(W[3], c, b64), (double*)colp(cx_, c, cbytes), s));
+      if (status == TMW_OK && !(cs[c].true_resid <= tol)) {
+        status = TMW_ENOCONV;
+        fail(ctx, TMW_ENOCONV, "tmw_solve: the Schur system converged but the full-lattice residual stays above tol (ill-conditioned A_ee)");
+      }
     }
-    // true residual of the full system in fp64: |b - D x|, the difference and its norm fused into the two launches of
-    // the full operator (out_p = A x_p + H x_pbar is not stored)
-    CK(cudaMemsetAsync(ctx->red, 0, 4 * MAXCOL * sizeof(double), s));
-    if ((rc = dslash<double>(ctx, EPI_A_XPAY, 0, 0, W[3], nullptr, W[7], 1.0, nz, 3, W[0], ctx->red, 4))) return rc;
-    if ((rc = dslash<double>(ctx, EPI_A_XPAY, 1, 0, W[7], nullptr, W[3], 1.0, nz, 3, W[1], ctx->red, 4))) return rc;
-    if ((rc = fetch_red(ctx))) return rc;
-    for (int i = 0; i < nz.n; i++) cs[nz.col[i]].true_resid = sqrt(ctx->red_host[4 * nz.col[i] + 2]) / cs[nz.col[i]].bnorm;
   }
   if (ctx->opt.location == TMW_HOST) CK(cudaMemcpyAsync(x, cx_, cbytes * nrhs, cudaMemcpyDeviceToHost, s));
   CK(cudaEventRecord(ctx->ev1, s));
@@ -933,20 +1007,24 @@ extern "C" int tmw_solve_multi(tmw_ctx* ctx, int nrhs, const double* b, double* 
   if (info) memset(info, 0, sizeof(*info) * nrhs);
   // How many columns fit at once: 8 fp64 + 8 inner-precision parity spinors per column (+ 2 canonical staging spinors
   // for HOST pointers) out of the free device memory plus what the workspaces already hold. More columns than that are
-  // solved chunk after chunk (as even as possible); TMW_NO_CHUNK=1 disables the split (the call then fails with
+  // solved chunk after chunk (as even as possible); TMW_DEBUG_NO_CHUNK disables the split (the call then fails with
   // TMW_ENOMEM if the columns do not fit).
   int chunk = nrhs;
-  if (nrhs > 1 && !getenv("TMW_NO_CHUNK")) {
+  if (nrhs > 1 && !(ctx->opt.debug & TMW_DEBUG_NO_CHUNK)) {
     const size_t b64 = spinor_bytes(ctx, TMW_F64), bin = spinor_bytes(ctx, ctx->opt.precision == TMW_DOUBLE ? TMW_F64 : TMW_F32);
     const size_t cbytes = (size_t)ctx->V * 24 * 8;
     const size_t per_col = 8 * b64 + 8 * bin + (ctx->opt.location == TMW_HOST ? 2 * cbytes : 0);
     size_t held = 0;
-    for (int i = 0; i < 10; i++) if (ctx->w64[i]) held += b64 * ctx->ws_cols;
+    for (int i = 0; i < NW64; i++) if (ctx->w64[i]) held += b64 * ctx->ws_cols;
     for (int i = 0; i < 8; i++) if (ctx->w32[i]) held += bin * ctx->ws_cols;
     for (int i = 0; i < 2; i++) if (ctx->canon[i]) held += cbytes * ctx->ws_cols;
     size_t free_b = 0, total_b = 0;
     CK(cudaMemGetInfo(&free_b, &total_b));
-    const size_t fit = (size_t)(0.92 * (double)(free_b + held)) / per_col;
+    // GCR: 2 nkrylov Krylov vectors of ONE column (the columns go one after another), allocated inside the solve
+    const size_t gcr = ctx->opt.solver == TMW_GCR ? 2 * (size_t)ctx->opt.nkrylov * bin : 0;
+    if (ctx->gcr_q) held += gcr;
+    const double avail = 0.92 * (double)(free_b + held) - (double)gcr;
+    const size_t fit = avail > 0 ? (size_t)avail / per_col : 0;
     if (fit < (size_t)nrhs && ctx->ws_cols < nrhs) {
       chunk = fit < 1 ? 1 : (int)fit;
       if (chunk < ctx->ws_cols) chunk = ctx->ws_cols;  // what is already allocated fits by construction

@@ -86,7 +86,10 @@ __global__ void sc_alpha_kernel(Scalars* sc0, ColMap cm) {
 }
 __global__ void sc_omega_kernel(Scalars* sc0, ColMap cm) {
   Scalars* sc = sc0 + cm.col[threadIdx.x];
-  const double wr = sc->ts[0] / sc->tt, wi = sc->ts[1] / sc->tt;
+  // <t,t> = 0: s = r - alpha v vanished, x + alpha p is exact at the half step (a source that is an eigenvector, a free
+  // field). omega = 0 then makes update_xrp do x += alpha p, r = s (= 0); beta = 0 keeps the next p finite.
+  const bool exact = sc->tt == 0.0;
+  const double wr = exact ? 0.0 : sc->ts[0] / sc->tt, wi = exact ? 0.0 : sc->ts[1] / sc->tt;
   sc->omega[0] = wr;
   sc->omega[1] = wi;
   sc->rho_old[0] = sc->rho[0];
@@ -97,8 +100,8 @@ __global__ void sc_omega_kernel(Scalars* sc0, ColMap cm) {
   double a[2], b[2];
   cdiv(sc->rho, sc->rho_old, a);
   cdiv(sc->alpha, sc->omega, b);
-  sc->beta[0] = a[0] * b[0] - a[1] * b[1];
-  sc->beta[1] = a[0] * b[1] + a[1] * b[0];
+  sc->beta[0] = exact ? 0.0 : a[0] * b[0] - a[1] * b[1];
+  sc->beta[1] = exact ? 0.0 : a[0] * b[1] + a[1] * b[0];
   sc->rr = 0.0;
 }
 cudaError_t launch_sc_begin_iter(Scalars* sc, const ColMap& cm, cudaStream_t s) { sc_begin_iter_kernel<<<1, cm.n, 0, s>>>(sc, cm); return cudaGetLastError(); }
@@ -242,6 +245,18 @@ __global__ void __launch_bounds__(BB) sub_norm_kernel(int64_t n, const double* a
   }
   double* dst[1] = {out + 2};
   reduce_atomic<1>(acc, dst);
+}
+
+// a += b (fp64, n double2-pair work items per column)
+__global__ void __launch_bounds__(BB) add64_kernel(int64_t n, double* a, const double* b, ColMap cm) {
+  { const int64_t o = 4 * n * cm.col[blockIdx.y]; a += o; b += o; }
+  for (int64_t i = (int64_t)blockIdx.x * BB + threadIdx.x; i < n; i += (int64_t)gridDim.x * BB) {
+    double aa[4], bb[4];
+    ldp(a, i, aa); ldp(b, i, bb);
+#pragma unroll
+    for (int c = 0; c < 4; c++) aa[c] += bb[c];
+    stp(a, i, aa);
+  }
 }
 
 // One step of the Clenshaw recursion for a Chebyshev series in X = scale*H + shift:
@@ -434,6 +449,12 @@ template <typename R> cudaError_t launch_convert(int64_t n64, const void* src64,
 cudaError_t launch_sub_norm(int64_t n64, const void* a, const void* b, void* d, double* out, const ColMap& cm, cudaStream_t s) {
   const int64_t np = n64 / 2;
   sub_norm_kernel<<<grid_of(np, cm), BB, 0, s>>>(np, (const double*)a, (const double*)b, (double*)d, out, cm);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_add64(int64_t n64, void* a, const void* b, const ColMap& cm, cudaStream_t s) {
+  const int64_t np = n64 / 2;
+  add64_kernel<<<grid_of(np, cm), BB, 0, s>>>(np, (double*)a, (const double*)b, cm);
   return cudaGetLastError();
 }
 

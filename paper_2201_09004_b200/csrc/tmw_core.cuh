@@ -13,8 +13,14 @@ namespace tmw {
 // ---------------------------------------------------------------------------------------------------------
 // geometry of one parity of an L^3 x T lattice; cb = (x/2) + Lh*(y + L*(z + L*t))
 // ---------------------------------------------------------------------------------------------------------
+// A Geom describes either the whole lattice or one domain of a domain-decomposed context: a sub-lattice
+// of extents L x L x Lz x T (x, y never split) whose site (x, y, z, t) is the global site (x, y, z + oz, t + ot); oz and ot
+// are even, so local and global parity agree. For the whole lattice Lz = L, oz = ot = 0.
 struct Geom {
-  int L, T, Lh;
+  int L, T, Lh;    // x, y extent; t extent; L/2
+  int Lz;          // z extent
+  int oz, ot;      // origin of the domain in the global lattice (canonical-layout conversion only)
+  int GT;          // global t extent (canonical-layout conversion only)
   int Vh;          // sites per parity (< 2^31)
   int sy, sz, st;  // cb strides of +1 in y, z, t
   // Thread -> site mapping of the stencil kernels. tiled = 0: CTA b covers cb in [b*BLOCK, (b+1)*BLOCK).
@@ -51,8 +57,8 @@ template <int BLOCK> __device__ __forceinline__ bool thread_site(const Geom& g, 
   int q = s.cb / g.Lh;
   s.y = q % g.L;
   q /= g.L;
-  s.z = q % g.L;
-  s.t = q / g.L;
+  s.z = q % g.Lz;
+  s.t = q / g.Lz;
   return s.cb < g.Vh;
 }
 
@@ -244,9 +250,12 @@ template <typename R> TMW_HD void cmadc(cx<R>& acc, cx<R> a, cx<R> b) {
 // ---------------------------------------------------------------------------------------------------------
 // SU(3) link from NG stored reals (rows 0,1 [+ row 2]); NG = 12 rebuilds row 2 = conj(row0 x row1)
 // ---------------------------------------------------------------------------------------------------------
-template <typename R, int NG> TMW_HD void load_link(const void* base, int64_t stride, int64_t idx, cx<R> (&U)[9]) {
+// STREAM: the link is read by this thread only (evict-first load, TMW_LD_STREAM); otherwise other CTAs (column groups)
+// read the same link and it should stay in L2 (plain read-only load)
+template <typename R, int NG, bool STREAM> TMW_HD void load_link(const void* base, int64_t stride, int64_t idx, cx<R> (&U)[9]) {
   R g[(NG == 12) ? 12 : 20];
-  load_reals_s<NG>(base, stride, idx, g);
+  if (STREAM) load_reals_s<NG>(base, stride, idx, g);
+  else load_reals<NG>(base, stride, idx, g);
 #pragma unroll
   for (int i = 0; i < NG / 2; i++) U[i] = mk<R>(g[2 * i], g[2 * i + 1]);
   if (NG == 12) {
@@ -485,7 +494,8 @@ template <typename R> struct DslashArgs {
 // neighbour checkerboard indices and the time-boundary sign
 struct Nbr {
   int fwd[4], bwd[4];
-  bool wrap_tf, wrap_tb;
+  bool wrap_tf, wrap_tb;  // the +t / -t hop leaves the (local) lattice
+  bool wrap_zf, wrap_zb;  // the +z / -z hop leaves the (local) lattice
 };
 TMW_HD Nbr neighbours(const Geom& g, int par, const Site& s) {
   Nbr n;
@@ -497,8 +507,10 @@ TMW_HD Nbr neighbours(const Geom& g, int par, const Site& s) {
   n.bwd[0] = cb - xh + (xb < 0 ? g.Lh - 1 : xb);
   n.fwd[1] = (y == g.L - 1) ? cb - (g.L - 1) * g.sy : cb + g.sy;
   n.bwd[1] = (y == 0) ? cb + (g.L - 1) * g.sy : cb - g.sy;
-  n.fwd[2] = (z == g.L - 1) ? cb - (g.L - 1) * g.sz : cb + g.sz;
-  n.bwd[2] = (z == 0) ? cb + (g.L - 1) * g.sz : cb - g.sz;
+  n.wrap_zf = (z == g.Lz - 1);
+  n.wrap_zb = (z == 0);
+  n.fwd[2] = n.wrap_zf ? cb - (g.Lz - 1) * g.sz : cb + g.sz;
+  n.bwd[2] = n.wrap_zb ? cb + (g.Lz - 1) * g.sz : cb - g.sz;
   n.wrap_tf = (t == g.T - 1);
   n.wrap_tb = (t == 0);
   n.fwd[3] = n.wrap_tf ? cb - (g.T - 1) * g.st : cb + g.st;
@@ -506,14 +518,14 @@ TMW_HD Nbr neighbours(const Geom& g, int par, const Site& s) {
   return n;
 }
 
-template <typename R, int NG, int MU, int NR>
+template <typename R, int NG, int MU, int NR, bool STREAM>
 __device__ __forceinline__ void hop_pair(const DslashArgs<R>& a, const Nbr& n, int cb, const int (&cofs)[NR], R (&acc)[NR][24]) {
   const int NPG = Planes<R, NG>::N;
   const int64_t Vh = a.g.Vh;
   typedef typename Vec16<R>::T V;
   {  // forward: (1 + sig g_mu) U_mu(x) psi(x+mu)
     cx<R> U[9];
-    load_link<R, NG>((const V*)a.U[a.par] + (int64_t)MU * NPG * Vh, Vh, cb, U);
+    load_link<R, NG, STREAM>((const V*)a.U[a.par] + (int64_t)MU * NPG * Vh, Vh, cb, U);
     const R bc = (MU == 3 && n.wrap_tf) ? (R)-1 : (R)1;
 #pragma unroll
     for (int j = 0; j < NR; j++) {
@@ -524,7 +536,7 @@ __device__ __forceinline__ void hop_pair(const DslashArgs<R>& a, const Nbr& n, i
   }
   {  // backward: (1 - sig g_mu) U_mu(x-mu)^dag psi(x-mu)
     cx<R> U[9];
-    load_link<R, NG>((const V*)a.U[1 - a.par] + (int64_t)MU * NPG * Vh, Vh, n.bwd[MU], U);
+    load_link<R, NG, STREAM>((const V*)a.U[1 - a.par] + (int64_t)MU * NPG * Vh, Vh, n.bwd[MU], U);
     const R bc = (MU == 3 && n.wrap_tb) ? (R)-1 : (R)1;
 #pragma unroll
     for (int j = 0; j < NR; j++) {
@@ -537,8 +549,11 @@ __device__ __forceinline__ void hop_pair(const DslashArgs<R>& a, const Nbr& n, i
 
 // One chirality b (12 reals: spins 2b, 2b+1) of the site-diagonal part, with the block held in registers so that it
 // serves several right-hand sides: w = A_b v and w = A_b^{-1} v as in apply_A / apply_Ainv above.
-template <typename R, int CLOVER> TMW_HD void load_block(const void* base, int b, int64_t Vh, int64_t cb, R* B) {
-  if (CLOVER) load_reals_s<36>((const typename Vec16<R>::T*)base + (int64_t)b * Planes<R, 36>::N * Vh, Vh, cb, B);
+template <typename R, int CLOVER, bool STREAM> TMW_HD void load_block(const void* base, int b, int64_t Vh, int64_t cb, R* B) {
+  if (CLOVER) {
+    if (STREAM) load_reals_s<36>((const typename Vec16<R>::T*)base + (int64_t)b * Planes<R, 36>::N * Vh, Vh, cb, B);
+    else load_reals<36>((const typename Vec16<R>::T*)base + (int64_t)b * Planes<R, 36>::N * Vh, Vh, cb, B);
+  }
 }
 template <typename R, int CLOVER> TMW_HD void half_A(const Diag<R>& d, int b, const R* B, const R* v, R* w) {
   if (CLOVER) {
@@ -583,7 +598,7 @@ template <int EPI, int CLOVER> __device__ __forceinline__ constexpr bool stored_
 
 // The stencil at one site for NR right-hand sides: on return acc[j] holds the output spinor of column slot j.
 // red[j] = {Re, Im <out, aux>, <out, out>} when WANT_RED2 (EPI >= 2), accumulated chirality by chirality.
-template <typename R, int NG, int EPI, int CLOVER, int NR>
+template <typename R, int NG, int EPI, int CLOVER, int NR, bool STREAM>
 __device__ __forceinline__ void dslash_site(const DslashArgs<R>& a, const Site& s, const int (&cofs)[NR], const bool (&valid)[NR], R (&acc)[NR][24], R (&red2)[NR][3]) {
   typedef typename Vec16<R>::T V;
   // cofs[j] = column * cstride: the column offset is added to the 32-bit SITE INDEX (the host checks that it fits), so
@@ -594,10 +609,10 @@ __device__ __forceinline__ void dslash_site(const DslashArgs<R>& a, const Site& 
   for (int j = 0; j < NR; j++)
 #pragma unroll
     for (int i = 0; i < 24; i++) acc[j][i] = (R)0;
-  hop_pair<R, NG, 0, NR>(a, n, cb, cofs, acc);
-  hop_pair<R, NG, 1, NR>(a, n, cb, cofs, acc);
-  hop_pair<R, NG, 2, NR>(a, n, cb, cofs, acc);
-  hop_pair<R, NG, 3, NR>(a, n, cb, cofs, acc);
+  hop_pair<R, NG, 0, NR, STREAM>(a, n, cb, cofs, acc);
+  hop_pair<R, NG, 1, NR, STREAM>(a, n, cb, cofs, acc);
+  hop_pair<R, NG, 2, NR, STREAM>(a, n, cb, cofs, acc);
+  hop_pair<R, NG, 3, NR, STREAM>(a, n, cb, cofs, acc);
   const int64_t Vh = a.g.Vh;
 #pragma unroll
   for (int j = 0; j < NR; j++) {
@@ -610,8 +625,8 @@ __device__ __forceinline__ void dslash_site(const DslashArgs<R>& a, const Site& 
 #pragma unroll
   for (int b = 0; b < 2; b++) {
     R B[CLOVER ? 36 : 1];
-    if (EPI == EPI_AINV_HOP || EPI == EPI_AINV_XPAY) load_block<R, CLOVER>(a.d.cinv[a.par], b, Vh, cb, B);
-    else if (EPI == EPI_A_XPAY) load_block<R, CLOVER>(a.d.c[a.par], b, Vh, cb, B);
+    if (EPI == EPI_AINV_HOP || EPI == EPI_AINV_XPAY) load_block<R, CLOVER, STREAM>(a.d.cinv[a.par], b, Vh, cb, B);
+    else if (EPI == EPI_A_XPAY) load_block<R, CLOVER, STREAM>(a.d.c[a.par], b, Vh, cb, B);
 #pragma unroll
     for (int j = 0; j < NR; j++) {
       R* o = acc[j] + 12 * b;
@@ -652,7 +667,7 @@ __device__ __forceinline__ void dslash_site(const DslashArgs<R>& a, const Site& 
     }
     if (CLOVER == CL_TWISTED && (EPI == EPI_AINV_HOP || EPI == EPI_AINV_XPAY)) {
       {  // (C + i tw)^{-1} = (C - i tw)(C^2 + tw^2)^{-1}: second factor, same registers
-        load_block<R, CLOVER>(a.d.c[a.par], b, Vh, cb, B);
+        load_block<R, CLOVER, STREAM>(a.d.c[a.par], b, Vh, cb, B);
 #pragma unroll
         for (int j = 0; j < NR; j++) {
           R* o = acc[j] + 12 * b;

@@ -50,7 +50,9 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<R>
   }
   R o[NR][24], r2[NR][3];
   if (active) {
-    dslash_site<R, NG, EPI, CLOVER, NR>(a, s, cofs, valid, o, r2);
+    // one column per thread: nobody else reads this thread's links and clover blocks (evict-first); with more columns the
+    // other column groups of a site block find them in L2
+    dslash_site<R, NG, EPI, CLOVER, NR, NR == 1>(a, s, cofs, valid, o, r2);
     if (!stored_in_site<EPI, CLOVER>()) {
       if (a.g5) {  // uniform across the grid
 #pragma unroll
@@ -149,7 +151,7 @@ template <typename R, int NG, int EPI, int CLOVER, int NR> static cudaError_t la
   const int B = Tune<R, NR>::BLOCK;
   a.ngroups = (a.ncol + NR - 1) / NR;
   dim3 grid;
-  if (a.g.tiled) grid = dim3((unsigned)(a.g.ntx * a.g.nty * a.ngroups), (unsigned)(a.g.L >> a.g.lz), (unsigned)(a.g.T >> a.g.lt));
+  if (a.g.tiled) grid = dim3((unsigned)(a.g.ntx * a.g.nty * a.ngroups), (unsigned)(a.g.Lz >> a.g.lz), (unsigned)(a.g.T >> a.g.lt));
   else grid = dim3((unsigned)(((a.g.Vh + B - 1) / B) * a.ngroups), 1, 1);
   dslash_kernel<R, NG, EPI, CLOVER, NR, B, Tune<R, NR>::MINB><<<grid, B, 0, s>>>(a);
   return cudaGetLastError();

@@ -101,6 +101,9 @@ template <typename R> cudaError_t launch_convert(int64_t n64, const void* src64,
 // d = a - b (fp64, n64 double2 vectors per column), out[4c+2] += <d,d>
 cudaError_t launch_sub_norm(int64_t n64, const void* a, const void* b, void* d, double* out, const ColMap& cm, cudaStream_t s);
 
+// a += b (fp64, n64 double2 vectors per column)
+cudaError_t launch_add64(int64_t n64, void* a, const void* b, const ColMap& cm, cudaStream_t s);
+
 // Clenshaw step (fp64, one column, n64 double2 vectors): out = c*psi + f*(scale*hb + shift*b1) - b2; out may alias b2
 cudaError_t launch_clenshaw(int64_t n64, void* out, const void* psi, const void* hb, const void* b1, const void* b2, double c, double f, double scale,
                             double shift, cudaStream_t s);

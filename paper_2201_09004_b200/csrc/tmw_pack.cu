@@ -5,16 +5,20 @@
 
 namespace tmw {
 
-// lexicographic site of checkerboard index cb on parity par
+// lexicographic index in the GLOBAL lattice (canonical arrays) of the site (x, y, z, t) of the (sub-)lattice g
+__device__ __forceinline__ int64_t global_lex(const Geom& g, int x, int y, int z, int t) {
+  return x + (int64_t)g.L * (y + (int64_t)g.L * ((z + g.oz) + (int64_t)g.L * (t + g.ot)));
+}
+// global lexicographic site of checkerboard index cb on parity par (origins are even: local parity = global parity)
 __device__ __forceinline__ int64_t lex_of_cb(const Geom& g, int par, int cb) {
   const int xh = cb % g.Lh;
   int q = cb / g.Lh;
   const int y = q % g.L;
   q /= g.L;
-  const int z = q % g.L;
-  const int t = q / g.L;
+  const int z = q % g.Lz;
+  const int t = q / g.Lz;
   const int x = 2 * xh + ((y + z + t + par) & 1);
-  return x + (int64_t)g.L * (y + (int64_t)g.L * (z + (int64_t)g.L * t));
+  return global_lex(g, x, y, z, t);
 }
 
 template <int NG32> __global__ void __launch_bounds__(128) pack_gauge_kernel(const Geom g, const double* __restrict__ canon, double2* g64e, double2* g64o, float4* g32e, float4* g32o) {
@@ -22,7 +26,7 @@ template <int NG32> __global__ void __launch_bounds__(128) pack_gauge_kernel(con
   const int cb = blockIdx.x * 128 + threadIdx.x;
   if (cb >= g.Vh) return;
   const int mu = blockIdx.y, par = blockIdx.z;
-  const int64_t V = 2 * (int64_t)g.Vh;
+  const int64_t V = (int64_t)g.L * g.L * g.L * g.GT;  // global volume: stride of mu in the canonical array
   const int64_t lex = lex_of_cb(g, par, cb);
   const double* u = canon + 18 * ((int64_t)mu * V + lex);
   double r[18];
@@ -69,15 +73,15 @@ template <typename R> __global__ void __launch_bounds__(128) unpack_spinor_kerne
 // with 16-byte accesses (the one-parity kernels above skip every other 192-byte site and use 8-byte accesses: 1.58 ms
 // per parity to unpack at 48^3 x 144, against 1.0 ms for both parities here). Used by tmw_apply FULL and tmw_solve.
 template <typename R> __global__ void __launch_bounds__(128) pack_spinor_both_kernel(const Geom g, const double2* __restrict__ canon, void* pe, void* po) {
-  const int64_t lex = (int64_t)blockIdx.x * 128 + threadIdx.x;
+  const int64_t lex = (int64_t)blockIdx.x * 128 + threadIdx.x;  // local lexicographic index
   if (lex >= 2 * (int64_t)g.Vh) return;
   int64_t q = lex;
   const int x = (int)(q % g.L); q /= g.L;
   const int y = (int)(q % g.L); q /= g.L;
-  const int z = (int)(q % g.L);
-  const int t = (int)(q / g.L);
+  const int z = (int)(q % g.Lz);
+  const int t = (int)(q / g.Lz);
   const int par = (x + y + z + t) & 1;
-  const double2* p = canon + 12 * lex;
+  const double2* p = canon + 12 * global_lex(g, x, y, z, t);
   R v[24];
 #pragma unroll
   for (int i = 0; i < 12; i++) {
@@ -88,17 +92,17 @@ template <typename R> __global__ void __launch_bounds__(128) pack_spinor_both_ke
   store_reals<24>(par ? po : pe, g.Vh, lex >> 1, v);
 }
 template <typename R> __global__ void __launch_bounds__(128) unpack_spinor_both_kernel(const Geom g, const void* pe, const void* po, double2* __restrict__ canon) {
-  const int64_t lex = (int64_t)blockIdx.x * 128 + threadIdx.x;
+  const int64_t lex = (int64_t)blockIdx.x * 128 + threadIdx.x;  // local lexicographic index
   if (lex >= 2 * (int64_t)g.Vh) return;
   int64_t q = lex;
   const int x = (int)(q % g.L); q /= g.L;
   const int y = (int)(q % g.L); q /= g.L;
-  const int z = (int)(q % g.L);
-  const int t = (int)(q / g.L);
+  const int z = (int)(q % g.Lz);
+  const int t = (int)(q / g.Lz);
   const int par = (x + y + z + t) & 1;
   R v[24];
   load_reals<24>(par ? po : pe, g.Vh, lex >> 1, v);
-  double2* p = canon + 12 * lex;
+  double2* p = canon + 12 * global_lex(g, x, y, z, t);
 #pragma unroll
   for (int i = 0; i < 12; i++) p[i] = make_double2((double)v[2 * i], (double)v[2 * i + 1]);
 }

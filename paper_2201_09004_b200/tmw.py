@@ -24,10 +24,11 @@ TWIST_GAMMA5, MASS_SCALAR = 0, 1
 D, DDAG, G5D = 0, 1, 2
 FULL, EVEN, ODD = 0, 1, 2
 F32, F64 = 0, 1
+DEBUG_FORCE_PIVOT, DEBUG_NO_CHUNK = 1, 2
 
 EXPORTS = ["tmw_create", "tmw_apply", "tmw_apply_schur", "tmw_solve", "tmw_apply_multi", "tmw_apply_schur_multi",
            "tmw_solve_multi", "tmw_cheb_apply", "tmw_spinor_bytes", "tmw_pack", "tmw_unpack",
-           "tmw_get_clover", "tmw_set_location", "tmw_launch_count", "tmw_destroy", "tmw_last_error"]
+           "tmw_get_clover", "tmw_set_location", "tmw_set_debug", "tmw_launch_count", "tmw_destroy", "tmw_last_error"]
 
 
 class tmw_complex(ctypes.Structure):
@@ -37,7 +38,9 @@ class tmw_complex(ctypes.Structure):
 class tmw_options(ctypes.Structure):
     _fields_ = [("location", ctypes.c_int), ("precision", ctypes.c_int), ("reconstruct", ctypes.c_int),
                 ("mass_reading", ctypes.c_int), ("max_iter", ctypes.c_int), ("delta", ctypes.c_double),
-                ("stream", ctypes.c_void_p), ("solver", ctypes.c_int), ("nkrylov", ctypes.c_int)]
+                ("stream", ctypes.c_void_p), ("solver", ctypes.c_int), ("nkrylov", ctypes.c_int),
+                ("verbose", ctypes.c_int), ("columns_per_thread", ctypes.c_int),
+                ("tile", ctypes.c_int * 4), ("debug", ctypes.c_int)]
 
 
 class tmw_solve_info(ctypes.Structure):
@@ -90,6 +93,8 @@ def load():
     lib.tmw_get_clover.restype = I
     lib.tmw_set_location.argtypes = [P, I]
     lib.tmw_set_location.restype = I
+    lib.tmw_set_debug.argtypes = [P, I]
+    lib.tmw_set_debug.restype = I
     lib.tmw_launch_count.argtypes = [P]
     lib.tmw_launch_count.restype = LL
     lib.tmw_destroy.argtypes = [P]
@@ -119,13 +124,15 @@ class Context:
 
     def __init__(self, L: int, T: int, gauge, m: complex, c_sw: float = 0.0, *, location: int = DEVICE,
                  precision: int = MIXED, reconstruct: int = 12, mass_reading: int = TWIST_GAMMA5, max_iter: int = 0,
-                 delta: float = 0.0, stream: int | None = None, solver: int = BICGSTAB, nkrylov: int = 0):
+                 delta: float = 0.0, stream: int | None = None, solver: int = BICGSTAB, nkrylov: int = 0,
+                 verbose: int = 0, columns_per_thread: int = 0, tile=(0, 0, 0, 0), debug: int = 0):
         lib = load()
         self._lib = lib
         self.L, self.T = L, T
         self.V = L * L * L * T
         self.location = location
-        opt = tmw_options(location, precision, reconstruct, mass_reading, max_iter, delta, stream, solver, nkrylov)
+        opt = tmw_options(location, precision, reconstruct, mass_reading, max_iter, delta, stream, solver, nkrylov,
+                          verbose, columns_per_thread, (ctypes.c_int * 4)(*tile), debug)
         h = ctypes.c_void_p()
         rc = lib.tmw_create(ctypes.byref(h), L, T, _ptr(gauge), tmw_complex(float(np.real(m)), float(np.imag(m))),
                             float(c_sw), ctypes.byref(opt))
@@ -183,6 +190,9 @@ class Context:
     def set_location(self, location: int):
         self._check(self._lib.tmw_set_location(self._h, location))
         self.location = location
+
+    def set_debug(self, flags: int):
+        self._check(self._lib.tmw_set_debug(self._h, flags))
 
     def launch_count(self) -> int:
         return int(self._lib.tmw_launch_count(self._h))

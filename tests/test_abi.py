@@ -49,7 +49,7 @@ def test_argument_validation_before_any_cuda_call(lib):
         assert lib.tmw_create(ctypes.byref(h), L, T, g.ctypes.data, m, 0.0, None) == tmw.EINVAL
         assert h.value is None
         assert b"even" in lib.tmw_last_error(None)
-    opt = tmw.tmw_options(0, 0, 13, 0, 0, 0.0, None)
+    opt = tmw.tmw_options(0, 0, 13, 0, 0, 0.0, None)  # reconstruct = 13
     assert lib.tmw_create(ctypes.byref(h), 4, 4, g.ctypes.data, m, 0.0, ctypes.byref(opt)) == tmw.EINVAL
     assert lib.tmw_create(ctypes.byref(h), 4, 4, g.ctypes.data, tmw.tmw_complex(float("nan"), 0.0), 0.0, None) == tmw.EINVAL
     # null context

@@ -5,11 +5,14 @@ The oracle cannot sweep these lattices many times in seconds, so:
   * operator outputs are compared with the oracle ONE SITE AT A TIME (oracle.apply_sites) on a seeded sample of
     sites plus every kind of boundary site (x, y, z wrap; the antiperiodic t wrap) — tolerance as in
     test_gpu_parity.py (fp32 1e-5, fp64 1e-12 per site);
-  * solutions are checked through a property that holds at any size: the residual b - D x, with D applied by the
-    ORACLE at sampled sites (incl. the source site and its neighbours), must satisfy |r(x)| <= tol |b| at every sampled
-    site, and the sample estimate of |r|/|b| must be <= 1e-10; on configs 1-2 the oracle also solves the full system
-    and |x_gpu - x_oracle| / |x_oracle| <= 1e-8 is checked directly.
+  * solutions: the EXACT full-lattice residual |b - D x| / |b| <= 1e-10 with D applied by the oracle over the whole
+    lattice (oracle.apply with its precomputed F; seconds at these sizes), on every config; and
+    |x_gpu - x_oracle| / |x_oracle| <= 1e-8 against the oracle's own solution (oracle.bicgstab to 1e-12): over the whole
+    lattice on configs 1-3, and on config 4 against the sample of the oracle's solution stored in
+    tests/golden/cfg4_solution_sample.txt (written by tests/golden/make_cfg4_solution_sample.py, which imports only
+    oracle/ and the input generators; the solve takes ~48 GB of host memory and tens of minutes).
 """
+import os
 import numpy as np
 import pytest
 
@@ -22,9 +25,6 @@ pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")
 
 TOL32, TOL64 = 1e-5, 1e-12
-# the sampled |r|/|b| is a statistical estimate (a few thousand of millions of sites): allow its sampling error on top
-# of the 1e-10 the library itself certifies in fp64 over ALL sites (info['true_resid'], asserted <= 1e-10 exactly)
-EST_TOL = 2e-10
 _cache = {}
 
 
@@ -44,6 +44,22 @@ def config_fields(idx):
         cfg = synth.CONFIGS[idx]
         _cache.update(idx=idx, cfg=cfg, U=synth.gauge_field(cfg["L"], cfg["T"], cfg["eps"], seed=1))
     return _cache["cfg"], _cache["U"]
+
+
+def config_F(idx):
+    """the oracle's clover-leaf field strength of configs[idx] (13.8 GB at 48^3 x 144), cached with the gauge field"""
+    cfg, U = config_fields(idx)
+    if cfg["c_sw"] == 0:
+        return None
+    if "F" not in _cache:
+        _cache["F"] = oracle.field_strength(U)
+    return _cache["F"]
+
+
+def exact_residual(U, F, b, x, m, c_sw):
+    """|b - D x| / |b| over the WHOLE lattice, D applied by the oracle (Eq. (2) + :67 Eq. (3))"""
+    r = b - oracle.apply(U, x, m, c_sw, F=F)
+    return float(np.linalg.norm(r.ravel()) / np.linalg.norm(b.ravel()))
 
 
 def lex(L, x, y, z, t):
@@ -149,23 +165,6 @@ def test_fullsize_full_operator_fp64_sampled(tmw, idx):
     torch.cuda.empty_cache()
 
 
-def sampled_residual(U, b, x, m, c_sw, sites_rand, sites_det):
-    """max_x |r(x)| and a stratified estimate of |r| (both relative to |b|) from the oracle's D: the deliberately
-    chosen sites `sites_det` (source site, its neighbours, boundary sites — where a point-source residual is
-    concentrated) count once each; the uniform random sample `sites_rand` stands for all the other sites."""
-    sites_det = np.unique(sites_det)
-    sites_rand = np.setdiff1d(np.unique(sites_rand), sites_det)
-    sites = np.concatenate([sites_det, sites_rand])
-    Dx = oracle.apply_sites(U, x, sites, m, c_sw)
-    r = b.reshape(-1, 4, 3)[sites] - Dx
-    rs2 = np.sum(np.abs(r.reshape(len(sites), -1)) ** 2, axis=1)
-    bn = np.linalg.norm(b.ravel())
-    V = b.size // 12
-    nd = len(sites_det)
-    est = np.sqrt(np.sum(rs2[:nd]) + np.sum(rs2[nd:]) * (V - nd) / len(sites_rand)) / bn
-    return float(np.sqrt(rs2.max()) / bn), float(est)
-
-
 @pytest.mark.parametrize("idx", [1, 2])
 def test_fullsize_solve_vs_oracle_solution(tmw, idx):
     cfg, U = config_fields(idx)
@@ -188,15 +187,57 @@ def test_fullsize_solve_vs_oracle_solution(tmw, idx):
     assert np.linalg.norm((xg - x_ref).ravel()) / np.linalg.norm(x_ref.ravel()) <= 1e-8
 
 
-def test_fullsize_config3_twelve_columns(tmw):
-    """configs[3]: the 12 point sources of a propagator, one after another, each checked through the oracle's D."""
-    cfg, U = config_fields(3)
+def test_fullsize_schur_fp32_sampled(tmw):
+    """The fp32 clover K1/K2 kernels (A4/A5) at full size in the launch configuration of the solver: tmw_apply_schur on
+    configs[2] (24^3 x 64, c_sw = 1.0509) against the oracle's masked pieces, Mhat p_o = A_oo p_o - H_oe A_ee^{-1} H_eo p_o
+    with A_ee^{-1} by a dense 12 x 12 solve per site (numpy) of the oracle's site term; compared per site on ALL odd
+    sites (fp32 <= 1e-5, fp64 <= 1e-12)."""
+    idx = 2
+    cfg, U = config_fields(idx)
+    F = config_F(idx)
     L, T, m, c_sw = cfg["L"], cfg["T"], complex(*cfg["m"]), cfg["c_sw"]
-    origin_nb = [lex(L, *c) for c in [(0, 0, 0, 0), (1, 0, 0, 0), (L - 1, 0, 0, 0), (0, 1, 0, 0), (0, L - 1, 0, 0),
-                                      (0, 0, 1, 0), (0, 0, L - 1, 0), (0, 0, 0, 1), (0, 0, 0, T - 1)]]
-    det = np.concatenate([boundary_sites(L, T), np.array(origin_nb, dtype=np.int64)])
-    rnd = random_sites(L, T, 4000, seed=33)
+    V = L ** 3 * T
+    psi = synth.gaussian_spinor(L, T, seed=3)
+    ev, od = H.parity_sites(L, T, 0), H.parity_sites(L, T, 1)
+    blocks = H.site_diagonal_blocks(U, c_sw, m.real)[ev]          # (Vh, 2, 6, 6) Hermitian chirality blocks on even sites
+    x_o = mask_parity_inplace(psi.copy(), L, T, 0)
+    Dx = oracle.apply(U, x_o, m, c_sw, F=F).reshape(V, 12)       # even: H_eo x_o; odd: A_oo x_o
+    t_e = np.zeros((V, 12), dtype=np.complex128)
+    rhs = Dx[ev].reshape(-1, 2, 6, 1)
+    t_e[ev] = np.linalg.solve(blocks, rhs).reshape(-1, 12)
+    Dt = oracle.apply(U, t_e.reshape(psi.shape), m, c_sw, F=F).reshape(V, 12)  # odd: H_oe t_e (+ A_oo 0)
+    ref = np.zeros((V, 12), dtype=np.complex128)
+    ref[od] = Dx[od] - Dt[od]
     dU = torch.from_numpy(U).cuda()
+    with tmw.Context(L, T, dU, m, c_sw) as ctx:
+        del dU
+        dpsi = torch.from_numpy(psi).cuda()
+        for prec, tol in ((tmw.F32, TOL32), (tmw.F64, TOL64)):
+            nb = ctx.spinor_bytes(prec)
+            pin = torch.empty(nb, dtype=torch.uint8, device="cuda")
+            pout = torch.empty(nb, dtype=torch.uint8, device="cuda")
+            out_c = torch.zeros_like(dpsi)
+            ctx.pack(prec, tmw.ODD, dpsi, pin)
+            ctx.apply_schur(tmw.D, prec, pin, pout)
+            ctx.unpack(prec, tmw.ODD, pout, out_c)
+            torch.cuda.synchronize()
+            got = out_c.cpu().numpy().reshape(V, 12)
+            assert site_err(got[od], ref[od]) <= tol, prec
+        del dpsi, out_c, pin, pout
+    torch.cuda.empty_cache()
+
+
+ORIGIN_COLS = [(0, 0), (2, 1)]  # (spin, colour) of the columns whose solution is compared with the oracle's at config 3
+
+
+def test_fullsize_config3_twelve_columns(tmw):
+    """configs[3]: the 12 point sources of a propagator, one after another. Every column: exact
+    full-lattice residual through the oracle's D. Columns (0,0) and (2,1): the solution against the oracle's."""
+    cfg, U = config_fields(3)
+    F = config_F(3)
+    L, T, m, c_sw = cfg["L"], cfg["T"], complex(*cfg["m"]), cfg["c_sw"]
+    dU = torch.from_numpy(U).cuda()
+    sols = {}
     with tmw.Context(L, T, dU, m, c_sw) as ctx:
         del dU
         x = torch.empty((T, L, L, L, 4, 3), dtype=torch.complex128, device="cuda")
@@ -205,21 +246,26 @@ def test_fullsize_config3_twelve_columns(tmw):
                 b = synth.point_source(L, T, spin, colour)
                 info = ctx.solve(torch.from_numpy(b).cuda(), x, 1e-10)
                 assert info["true_resid"] <= 1e-10
-                mx, est = sampled_residual(U, b, x.cpu().numpy(), m, c_sw, rnd, det)
-                assert mx <= 1e-10 and est <= EST_TOL, (spin, colour, mx, est)
+                xg = x.cpu().numpy()
+                assert exact_residual(U, F, b, xg, m, c_sw) <= 1e-10, (spin, colour)
+                if (spin, colour) in ORIGIN_COLS:
+                    sols[(spin, colour)] = xg
         del x
     torch.cuda.empty_cache()
+    for (spin, colour), xg in sols.items():
+        x_ref, iref = oracle.bicgstab(U, synth.point_source(L, T, spin, colour), m, c_sw, tol=1e-12, F=F)
+        assert iref["status"] == 0 and iref["true_resid"] <= 1e-11
+        assert np.linalg.norm((xg - x_ref).ravel()) / np.linalg.norm(x_ref.ravel()) <= 1e-8, (spin, colour)
+        _cache[("x3", spin, colour)] = x_ref  # reused by the batched test below
 
 
 def test_fullsize_config3_twelve_columns_batched(tmw):
-    """configs[3] again, the 12 columns in ONE tmw_solve_multi call: every column checked through the
-    oracle's D like the one-after-another solves above, and against the single-column solve of the same library."""
+    """configs[3] again, the 12 columns in ONE tmw_solve_multi call: every column's exact full-lattice
+    residual through the oracle's D, columns (0,0) and (2,1) against the oracle's solution, and one column against the
+    single-column solve of the same library."""
     cfg, U = config_fields(3)
+    F = config_F(3)
     L, T, m, c_sw = cfg["L"], cfg["T"], complex(*cfg["m"]), cfg["c_sw"]
-    origin_nb = [lex(L, *c) for c in [(0, 0, 0, 0), (1, 0, 0, 0), (L - 1, 0, 0, 0), (0, 1, 0, 0), (0, L - 1, 0, 0),
-                                      (0, 0, 1, 0), (0, 0, L - 1, 0), (0, 0, 0, 1), (0, 0, 0, T - 1)]]
-    det = np.concatenate([boundary_sites(L, T), np.array(origin_nb, dtype=np.int64)])
-    rnd = random_sites(L, T, 4000, seed=33)
     dU = torch.from_numpy(U).cuda()
     with tmw.Context(L, T, dU, m, c_sw) as ctx:
         del dU
@@ -228,41 +274,68 @@ def test_fullsize_config3_twelve_columns_batched(tmw):
             b[c, 0, 0, 0, 0, c // 3, c % 3] = 1.0
         x = torch.empty_like(b)
         infos = ctx.solve_multi(12, b, x, 1e-10)
-        for c in range(12):
-            assert infos[c]["true_resid"] <= 1e-10 and infos[c]["iters"] > 0
-            mx, est = sampled_residual(U, synth.point_source(L, T, c // 3, c % 3), x[c].cpu().numpy(), m, c_sw, rnd, det)
-            assert mx <= 1e-10 and est <= EST_TOL, (c, mx, est)
+        xs = x.cpu().numpy()
         x1 = torch.empty_like(x[0])
         ctx.solve(b[5], x1, 1e-10)
         assert float(torch.linalg.vector_norm(x1 - x[5]) / torch.linalg.vector_norm(x1)) <= 1e-8
         del b, x, x1
     torch.cuda.empty_cache()
+    for c in range(12):
+        assert infos[c]["true_resid"] <= 1e-10 and infos[c]["iters"] > 0
+        assert exact_residual(U, F, synth.point_source(L, T, c // 3, c % 3), xs[c], m, c_sw) <= 1e-10, c
+    for spin, colour in ORIGIN_COLS:
+        x_ref = _cache.get(("x3", spin, colour))
+        if x_ref is None:
+            x_ref, iref = oracle.bicgstab(U, synth.point_source(L, T, spin, colour), m, c_sw, tol=1e-12, F=F)
+            assert iref["status"] == 0
+        xg = xs[3 * spin + colour]
+        assert np.linalg.norm((xg - x_ref).ravel()) / np.linalg.norm(x_ref.ravel()) <= 1e-8, (spin, colour)
 
 
-def test_fullsize_config4_solve(tmw, monkeypatch):
+def load_solution_sample(path):
+    """tests/golden/cfg4_solution_sample.txt -> (header dict, lexicographic sites, values (n, 4, 3) complex)"""
+    hdr, sites, vals = {}, [], []
+    with open(path) as f:
+        for line in f:
+            if line.startswith("#"):
+                tok = line[1:].split()
+                for k in ("L", "T", "m_re", "m_im", "c_sw", "eps", "xnorm_full_lattice"):
+                    if k in tok:
+                        hdr[k] = float(tok[tok.index(k) + 1])
+                continue
+            t = line.split()
+            sites.append(int(t[0]))
+            vals.append([float(v) for v in t[1:]])
+    v = np.array(vals, dtype=np.float64).reshape(len(sites), 12, 2)
+    return hdr, np.array(sites, dtype=np.int64), (v[..., 0] + 1j * v[..., 1]).reshape(-1, 4, 3)
+
+
+def test_fullsize_config4_solve(tmw):
+    """configs[4] (48^3 x 144, the benchmark config): tmw_solve of the point source. (i) exact full-lattice residual
+    through the oracle's D <= 1e-10; (ii) the solution against the ORACLE's solution at the sampled sites of
+    tests/golden/cfg4_solution_sample.txt (the neighbourhood of the source, where the solution lives, corner sites
+    and random sites): relative L2 over the sample <= 1e-8, and every sampled site within 1e-8 |x| absolutely;
+    (iii) more columns than fit are solved chunk by chunk, a forced unchunked call fails cleanly with TMW_ENOMEM."""
     cfg, U = config_fields(4)
     L, T, m, c_sw = cfg["L"], cfg["T"], complex(*cfg["m"]), cfg["c_sw"]
     b = synth.point_source(L, T, 0, 0)
-    origin_nb = [lex(L, *c) for c in [(0, 0, 0, 0), (1, 0, 0, 0), (L - 1, 0, 0, 0), (0, 1, 0, 0), (0, L - 1, 0, 0),
-                                      (0, 0, 1, 0), (0, 0, L - 1, 0), (0, 0, 0, 1), (0, 0, 0, T - 1)]]
-    det = np.concatenate([boundary_sites(L, T), np.array(origin_nb, dtype=np.int64)])
-    rnd = random_sites(L, T, 20000, seed=44)
     dU = torch.from_numpy(U).cuda()
     with tmw.Context(L, T, dU, m, c_sw) as ctx:
         del dU
         x = torch.empty((T, L, L, L, 4, 3), dtype=torch.complex128, device="cuda")
         db = torch.from_numpy(b).cuda()
-        # 16 columns need 16 x 18.3 GB of workspace here: more than the GPU has. The call must fail with TMW_ENOMEM before
-        # it touches b or x (so one-column buffers are enough), release what it allocated, and leave the context usable.
-        monkeypatch.setenv("TMW_NO_CHUNK", "1")
+        # 16 columns need 16 x 18.3 GB of workspace here: more than the GPU has. With chunking disabled the call must fail
+        # with TMW_ENOMEM before it touches b or x (so one-column buffers are enough), release what it allocated, and
+        # leave the context usable.
+        ctx.set_debug(tmw.DEBUG_NO_CHUNK)
         with pytest.raises(tmw.TmwError) as e:
             ctx.solve_multi(16, db, x, 1e-10)
         assert e.value.code == tmw.ENOMEM
-        monkeypatch.delenv("TMW_NO_CHUNK")
+        ctx.set_debug(0)
         info = ctx.solve(db, x, 1e-10)
         xg = x.cpu().numpy()
         del x
-        # without TMW_NO_CHUNK more columns than fit are solved chunk after chunk: 8 columns = 147 GB of workspace
+        # with chunking, more columns than fit are solved chunk after chunk: 8 columns = 147 GB of workspace
         n = 8
         bm = torch.zeros((n, T, L, L, L, 4, 3), dtype=torch.complex128, device="cuda")
         for c in range(n):
@@ -274,9 +347,15 @@ def test_fullsize_config4_solve(tmw, monkeypatch):
         x7 = xm[7].cpu().numpy()
         del bm, xm, db
     torch.cuda.empty_cache()
-    mx7, est7 = sampled_residual(U, synth.point_source(L, T, 2, 1), x7, m, c_sw, rnd, det)
-    assert mx7 <= 1e-10 and est7 <= EST_TOL, (mx7, est7)
     assert info["true_resid"] <= 1e-10
-    mx, est = sampled_residual(U, b, xg, m, c_sw, rnd, det)
-    assert mx <= 1e-10 and est <= EST_TOL, (mx, est)
+    F = config_F(4)
+    assert exact_residual(U, F, b, xg, m, c_sw) <= 1e-10
+    assert exact_residual(U, F, synth.point_source(L, T, 2, 1), x7, m, c_sw) <= 1e-10
+    hdr, sites, ref = load_solution_sample(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "cfg4_solution_sample.txt"))
+    assert (hdr["L"], hdr["T"], hdr["m_re"], hdr["m_im"], hdr["c_sw"], hdr["eps"]) == (L, T, m.real, m.imag, c_sw, cfg["eps"])
+    got = xg.reshape(-1, 4, 3)[sites]
+    assert np.linalg.norm((got - ref).ravel()) / np.linalg.norm(ref.ravel()) <= 1e-8
+    # the sample holds the bulk of the solution (it decays fast away from the source), so its norm is the scale of x
+    assert np.linalg.norm(ref.ravel()) >= 0.99 * hdr["xnorm_full_lattice"]
+    assert np.max(np.abs(got - ref)) <= 1e-8 * hdr["xnorm_full_lattice"]
     _cache.clear()

@@ -4,8 +4,6 @@ the "12 columns" of PAPER.md:78) with the fp64 CPU oracle, column by column, on 
 The oracle has no multi-column notion: each column is an independent application / solve of the same operator, so the
 expected values are the single-column oracle results. Tolerances as in test_gpu_parity.py.
 """
-import os
-
 import numpy as np
 import pytest
 
@@ -28,17 +26,9 @@ def tmw():
     return m
 
 
-@pytest.fixture
-def nr_env():
-    """TMW_NR (columns per thread of the fp32 stencil) and TMW_TILE (thread -> site mapping) are read at tmw_create;
-    restore them afterwards"""
-    old = {k: os.environ.get(k) for k in ("TMW_NR", "TMW_TILE")}
-    yield
-    for k, v in old.items():
-        if v is None:
-            os.environ.pop(k, None)
-        else:
-            os.environ[k] = v
+TILES = {None: (0, 0, 0, 0), "auto": (-1, 0, 0, 0), "1,2,1,3": (1, 2, 1, 3)}
+# columns per thread of the fp32 stencil (tmw_options.columns_per_thread)
+SPREADS = [dict(columns_per_thread=n) for n in (1, 2, 3, 4)]
 
 
 def columns(L, T, n):
@@ -66,17 +56,15 @@ def unpack_multi(ctx, tmw, buf, n, par, prec, L, T):
     return [o.cpu().numpy() for o in out]
 
 
-@pytest.mark.parametrize("nr", [1, 2, 3, 4])
+@pytest.mark.parametrize("spread", SPREADS, ids=lambda d: "-".join(f"{k[8:]}{v}" for k, v in d.items()))
 @pytest.mark.parametrize("L,T,nrhs,tile", [(8, 16, 5, "auto"), (8, 16, 5, None), (6, 4, 12, None), (4, 8, 7, "auto"), (4, 8, 3, "1,2,1,3")])
-def test_hopping_multi_vs_oracle(tmw, nr_env, L, T, nrhs, tile, nr):
-    os.environ["TMW_NR"] = str(nr)
-    if tile:
-        os.environ["TMW_TILE"] = tile  # 4-D tiles of 128 sites instead of 128 consecutive checkerboard indices
+def test_hopping_multi_vs_oracle(tmw, L, T, nrhs, tile, spread):
+    # tile: 4-D tiles of 128 sites instead of 128 consecutive checkerboard indices
     U = synth.gauge_field(L, T, 0.4, seed=1)
     cols = columns(L, T, nrhs)
-    with tmw.Context(L, T, dev(U), 0.1) as ctx:
+    with tmw.Context(L, T, dev(U), 0.1, tile=TILES[tile], **spread) as ctx:
         for prec, tol in ((tmw.F32, TOL32), (tmw.F64, TOL64)):
-            if prec == tmw.F64 and nr > 1:
+            if prec == tmw.F64 and spread != SPREADS[0]:
                 continue  # the fp64 stencil always takes one column per thread
             for op in (tmw.D, tmw.DDAG):
                 for par in (0, 1):
@@ -90,16 +78,14 @@ def test_hopping_multi_vs_oracle(tmw, nr_env, L, T, nrhs, tile, nr):
                         assert site <= tol, (prec, op, par, c, site, glob)
 
 
-@pytest.mark.parametrize("nr", [2, 3, 4])
+@pytest.mark.parametrize("spread", SPREADS[1:], ids=lambda d: "-".join(f"{k[8:]}{v}" for k, v in d.items()))
 @pytest.mark.parametrize("case", [
     dict(L=8, T=4, eps=0.4, m=-0.0695 + 0.0j, c_sw=1.0509, nrhs=5),
     dict(L=4, T=6, eps=0.3, m=-0.044 + 0.2j, c_sw=1.0349, nrhs=4),   # twisted clover: two-factor inverse
     dict(L=6, T=4, eps=0.4, m=-0.0695 + 0.01j, c_sw=0.0, nrhs=12),
 ])
-def test_schur_multi_vs_oracle(tmw, nr_env, case, nr):
-    os.environ["TMW_NR"] = str(nr)
-    if nr == 3:
-        os.environ["TMW_TILE"] = "auto"
+def test_schur_multi_vs_oracle(tmw, case, spread):
+    tile = TILES["auto"] if spread.get("columns_per_thread") == 3 else TILES[None]
     L, T, m, c_sw, nrhs = case["L"], case["T"], case["m"], case["c_sw"], case["nrhs"]
     V = L ** 3 * T
     U = synth.gauge_field(L, T, case["eps"], seed=1)
@@ -116,7 +102,7 @@ def test_schur_multi_vs_oracle(tmw, nr_env, case, nr):
         ref = np.zeros((V, 12), dtype=np.complex128)
         ref[od] = Dx[od] - Dt[od]
         refs.append(ref.reshape(psi.shape))
-    with tmw.Context(L, T, dev(U), m, c_sw) as ctx:
+    with tmw.Context(L, T, dev(U), m, c_sw, tile=tile, **spread) as ctx:
         for prec, tol in ((tmw.F32, TOL32), (tmw.F64, TOL64)):
             inp = pack_multi(ctx, tmw, cols, 1, prec)
             out = torch.full_like(inp, 0x7f)
@@ -127,14 +113,15 @@ def test_schur_multi_vs_oracle(tmw, nr_env, case, nr):
                 assert site <= tol, (prec, c, site, glob)
 
 
-@pytest.mark.parametrize("precision", ["mixed", "double"])
-def test_solve_multi_12_columns_vs_oracle(tmw, precision):
+@pytest.mark.parametrize("precision,spread", [("mixed", {}), ("double", {}), ("mixed", dict(columns_per_thread=1)),
+                                              ("mixed", dict(columns_per_thread=3))])
+def test_solve_multi_12_columns_vs_oracle(tmw, precision, spread):
     """configs[3] shape of work on a small lattice: the 12 point sources of a propagator (C13) in ONE call."""
     L, T, m, c_sw = 4, 8, -0.0514 + 0.0j, 1.0424
     U = synth.gauge_field(L, T, 0.35, seed=1)
     F = oracle.field_strength(U)
     b = np.stack([synth.point_source(L, T, c // 3, c % 3) for c in range(12)])
-    with tmw.Context(L, T, dev(U), m, c_sw, precision=tmw.MIXED if precision == "mixed" else tmw.DOUBLE) as ctx:
+    with tmw.Context(L, T, dev(U), m, c_sw, precision=tmw.MIXED if precision == "mixed" else tmw.DOUBLE, **spread) as ctx:
         x = torch.empty(b.shape, dtype=torch.complex128, device="cuda")
         infos = ctx.solve_multi(12, dev(b), x, 1e-10)
         x = x.cpu().numpy()

@@ -313,6 +313,81 @@ def test_uniform_abelian_flux(plane, gammas):
     assert rel(diff, expect) < 1e-13
 
 
+def test_clover_sign_is_the_improving_one():
+    """Pins the SIGN and prefactor of the clover term of Eq. (3) relative to the hopping term of Eq. (2)
+     to what the term is for: "O(a) improvement". The expected values come from the continuum,
+    not from reading C7: for a Dirac operator in a uniform abelian field B in the xy-plane,
+    (gamma.D)^2 = D^2 + sum_{mu<nu} sigma_mu_nu F_mu_nu, the lowest Landau level has -D^2 = B and sigma_xy F_xy = -B on
+    one spin orientation, so gamma.D has exact zero modes. The Wilson term -(1/2) D^2 of Eq. (2) lifts them to B/2 (an
+    O(a) artefact); the clover term at c_sw = 1 must cancel exactly that Pauli term, bringing them back to O(B^2). With the
+    wrong sign it doubles the lift to B instead; with a wrong prefactor (c_sw/4, c_sw) the cancellation fails too.
+
+    Lattice: 8^3 x 2, fully periodic (antiperiodic_t=False: zero modes need p_t = 0), m = 0, one flux quantum
+    B = 2 pi / 64. Colour 2 is neutral under T3 = diag(1,-1,0) and sees a free field (exact zero modes at m = 0): the
+    vectors are restricted to colours 0, 1 (abelian links are colour-diagonal, so this sector is invariant). The operator
+    commutes with translations in z and t, so the sector of vectors constant in z and t is invariant as well; it holds
+    the lowest modes (every other (p_z, p_t) adds (1 - cos p) >= 0), and in it D is a dense 512 x 512 matrix whose
+    singular values are computed exactly. Catches: flipped sign of the clover term (or of sigma, or of F) relative to
+    the hopping term, wrong prefactor."""
+    L, T = 8, 2
+    U, B = abelian_flux_gauge(L, T, 0, 1, k=1)
+    assert abs(B - TWO_PI / 64) < 1e-15
+    F = oracle.field_strength(U)
+    n = L * L * 4 * 2
+
+    def sigma_min(c_sw):
+        M = np.empty((n, n), dtype=np.complex128)
+        j = 0
+        for y in range(L):
+            for x in range(L):
+                for s in range(4):
+                    for c in range(2):
+                        psi = np.zeros((T, L, L, L, 4, 3), dtype=np.complex128)
+                        psi[:, :, y, x, s, c] = 1.0
+                        w = oracle.apply(U, psi, 0.0, c_sw, F=F, antiperiodic_t=False)
+                        assert np.max(np.abs(w - w[:1, :1])) < 1e-14 and np.max(np.abs(w[..., 2])) == 0.0  # sector is invariant
+                        M[:, j] = w[0, 0, :, :, :, :2].ravel()
+                        j += 1
+        sv = np.sort(np.linalg.svd(M, compute_uv=False))
+        # 4 would-be zero modes: 2 colours x (flux quanta |k| = 1 each) x 2 (the lower-chirality copy): well separated from the rest
+        assert sv[4] > 3.0 * B
+        return sv[:4]
+
+    s0, sp, sm = sigma_min(0.0), sigma_min(+1.0), sigma_min(-1.0)
+    assert np.all(np.abs(s0 - B / 2) < 0.05 * B), s0    # Wilson term alone: lifted to B/2          (measured 0.04851 vs 0.04909)
+    assert np.all(np.abs(sm - B) < 0.05 * B), sm        # wrong-sign clover term: lift doubled to B  (measured 0.09752 vs 0.09817)
+    assert np.all(sp < 0.1 * s0.min()), sp              # c_sw = +1: cancelled to O(B^2)             (measured 5.0e-4)
+    assert np.all(sp < B * B), sp
+
+
+def test_table1_golden_matches_configs():
+    """tests/golden/table1_ensembles.txt holds the MILC rows of Table 1 (OCR-garbled cells read as in
+    DESIGN.md C9); synth.CONFIGS[1..4] (= BASELINE.json configs[1..4]) must carry exactly these lattice sizes, masses
+    and c_sw. Catches: a mistyped ensemble parameter in the workload table every test and bench.py use."""
+    import os
+    from conftest import GOLDEN
+    rows = {}
+    with open(os.path.join(GOLDEN, "table1_ensembles.txt")) as f:
+        for line in f:
+            line = line.strip()
+            if not line or line.startswith("#"):
+                continue
+            tag, L, T, mass, c_sw = line.split()
+            rows[tag] = (int(L), int(T), float(mass), float(c_sw))
+    assert set(rows) == {"MILC12", "MILC09", "MILC06"}
+    cfgs = synth.CONFIGS
+    # config 1 = MILC12 without clover and with a twist; config 2 = MILC12 as printed; 3 = MILC09; 4 = MILC06
+    for idx, tag in ((2, "MILC12"), (3, "MILC09"), (4, "MILC06")):
+        L, T, mass, c_sw = rows[tag]
+        c = cfgs[idx]
+        assert (c["L"], c["T"]) == (L, T), (idx, tag)
+        assert c["m"] == (mass, 0.0) and c["c_sw"] == c_sw, (idx, tag)
+    L, T, mass, _ = rows["MILC12"]
+    assert (cfgs[1]["L"], cfgs[1]["T"], cfgs[1]["m"][0], cfgs[1]["c_sw"]) == (L, T, mass, 0.0)
+    # Table 2 row 1 quotes m_cri + omega = -0.0398 for the 48^3 x 144 ensemble (PAPER.md:73): the same number as Table 1
+    assert rows["MILC06"][2] == -0.0398
+
+
 def test_clover_term_properties_on_random_field():
     """Site term is Hermitian, spin-traceless, chiral-block diagonal; c_sw = 0 reduces to the no-clover operator;
     precomputed F and on-the-fly F agree; apply_sites agrees with the full application."""
