@@ -99,6 +99,17 @@ typedef struct {
                        all 0 (default): 128 consecutive checkerboard indices; tile[0] = -1: the largest tile that fits,
                        preferring 8 x 4 x 2 x 2. A tile that does not divide the lattice or is not 128 sites -> 1-D. */
   int debug;        /* bit mask of TMW_DEBUG_* (test hooks, see below); also settable later with tmw_set_debug */
+  /* Domain decomposition (the paper's runs are all multi-GPU: PAPER.md:52, the "Nodes" columns of Tables 2-5 :71-76, and
+     "the network has much stronger impact on the performance", :315): the lattice is cut into domains_z x domains_t
+     sub-lattices (0 or 1: not cut; L / domains_z and T / domains_t must be even), each with its own packed gauge and
+     clover fields. Every stencil application then packs the (1 +- gamma_mu)-projected half spinors of the cut faces
+     (12 reals per face site), exchanges them with one copy per face, computes the interior of the domains meanwhile and
+     finishes the sites on the cuts afterwards; the antiperiodic sign stays on the physical t boundary. All calls give
+     the same results as without cuts up to rounding (the hops through a cut are added last). A packed parity spinor of
+     such a context is the domains' local packed spinors back to back, domain (iz, it) at index iz + domains_z * it. In
+     this build all domains live on the context's device (the exchange is a same-device copy); tmw_get_clover and the
+     tile / columns_per_thread tunings are not available. */
+  int domains_z, domains_t;
 } tmw_options;
 
 /* Test hooks (tmw_options.debug / tmw_set_debug): they change which code path runs, never the result. */

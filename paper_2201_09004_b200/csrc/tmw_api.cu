@@ -28,6 +28,23 @@ using namespace tmw;
 
 enum { NW64 = 14 };
 
+// One domain of a domain-decomposed context: a sub-lattice L x L x (L/Pz) x (T/Pt) with its own packed
+// gauge and clover fields and the send / receive buffers of its cuts. Domain (iz, it) has index iz + Pz * it; every
+// packed spinor of the context is the domains' local packed spinors back to back in that order.
+struct Domain {
+  Geom g;
+  int iz, it;
+  int device;        // CUDA device that holds the domain (all domains of a context share one device in this build)
+  void* g64[2];
+  void* g32[2];
+  void* c64[2];
+  void* c32[2];
+  void* ci64;
+  void* ci32;
+  void* send[2][2];  // [direction z, t][0: to the neighbour behind, 1: ahead]
+  void* recv[2][2];  // [direction][0: lo ghost (from behind), 1: hi ghost (from ahead)]
+};
+
 struct tmw_ctx {
   Geom g;
   int64_t V;
@@ -43,6 +60,14 @@ struct tmw_ctx {
   void* ci64;  // inverse blocks, even parity
   void* ci32;
   std::vector<void*> owned;  // every device allocation
+  // domain decomposition: pz * pt > 1 domains (then g64 ... ci32 above are null and the fields live in dom[])
+  int pz, pt;
+  std::vector<Domain> dom;
+  int vh_loc;        // sites per parity of one domain (= g.Vh without decomposition)
+  int ghost_cols;    // columns the send / receive buffers hold
+  void* dd_tmp;      // scratch output spinors for stencil launches that keep only a reduction
+  cudaStream_t comm; // the halo exchange runs here, beside the interior pass on `stream`
+  cudaEvent_t ev_pack, ev_comm;
   // lazily allocated workspaces, each sized for ws_cols right-hand-side columns (column c at c * spinor bytes)
   int ws_cols;
   void* w64[NW64];  // packed fp64 parity spinors (0..7 the solver's, 8..13 only for the rare defect-correction pass)
@@ -102,7 +127,7 @@ static void dev_free(tmw_ctx* ctx, void* p) {
 static size_t spinor_bytes(const tmw_ctx* c, int prec) { return (size_t)c->g.Vh * 24 * (prec == TMW_F32 ? 4 : 8); }
 
 // ---- the diagonal part for D (dagger = 0) or D^dagger ----
-template <typename R> static Diag<R> make_diag(const tmw_ctx* c, int dagger) {
+template <typename R> static Diag<R> make_diag(const tmw_ctx* c, int dagger, const Domain* dm = nullptr) {
   Diag<R> d;
   const double dg = -(4.0 + c->m_re);
   double tu, tl;
@@ -118,9 +143,15 @@ template <typename R> static Diag<R> make_diag(const tmw_ctx* c, int dagger) {
   d.inv_im_lo = (R)(-tl / den);
   d.twisted_clover = (c->clover && c->m_im != 0.0) ? 1 : 0;
   const bool f = sizeof(R) == 4;
-  d.c[0] = f ? c->c32[0] : c->c64[0];
-  d.c[1] = f ? c->c32[1] : c->c64[1];
-  d.cinv[0] = f ? c->ci32 : c->ci64;
+  if (dm) {
+    d.c[0] = f ? dm->c32[0] : dm->c64[0];
+    d.c[1] = f ? dm->c32[1] : dm->c64[1];
+    d.cinv[0] = f ? dm->ci32 : dm->ci64;
+  } else {
+    d.c[0] = f ? c->c32[0] : c->c64[0];
+    d.c[1] = f ? c->c32[1] : c->c64[1];
+    d.cinv[0] = f ? c->ci32 : c->ci64;
+  }
   d.cinv[1] = nullptr;
   return d;
 }
@@ -134,20 +165,28 @@ static ColMap cols_first(int n) {
 static void cols_add(ColMap& cm, int c) { cm.col[cm.n++] = (unsigned char)c; }
 
 template <typename R>
-static DslashArgs<R> make_args(const tmw_ctx* c, int par, int dagger, const void* in, void* out, const void* aux, double sgn, const ColMap& cm) {
+static DslashArgs<R> make_args(const tmw_ctx* c, int par, int dagger, const void* in, void* out, const void* aux, double sgn, const ColMap& cm,
+                               const Domain* dm = nullptr) {
   DslashArgs<R> a;
+  memset(&a, 0, sizeof(a));
   a.in = in;
   a.out = out;
   a.aux = aux;
   const bool f = sizeof(R) == 4;
-  a.U[0] = f ? c->g32[0] : c->g64[0];
-  a.U[1] = f ? c->g32[1] : c->g64[1];
-  a.g = c->g;
+  if (dm) {
+    a.U[0] = f ? dm->g32[0] : dm->g64[0];
+    a.U[1] = f ? dm->g32[1] : dm->g64[1];
+    a.g = dm->g;
+  } else {
+    a.U[0] = f ? c->g32[0] : c->g64[0];
+    a.U[1] = f ? c->g32[1] : c->g64[1];
+    a.g = c->g;
+  }
   a.par = par;
   a.sig = dagger ? (R)-1 : (R)1;
   a.coef = (R)(0.5 * sgn);
   a.g5 = 0;
-  a.d = make_diag<R>(c, dagger);
+  a.d = make_diag<R>(c, dagger, dm);
   a.red_mode = 0;
   a.dotv = nullptr;
   a.red = nullptr;
@@ -162,13 +201,110 @@ template <typename R> static int ng_of(const tmw_ctx* c) { return sizeof(R) == 4
 
 // out(par) = epilogue(H in) for the columns of cm (vectors of column c start c spinors after the base pointers);
 // red (if any) is the reduction target of column 0, column c's is red_stride doubles further per column.
+static inline int dom_behind(const tmw_ctx* c, const Domain& d, int dir) {
+  return dir == 0 ? ((d.iz + c->pz - 1) % c->pz) + c->pz * d.it : d.iz + c->pz * ((d.it + c->pt - 1) % c->pt);
+}
+static inline int dom_ahead(const tmw_ctx* c, const Domain& d, int dir) {
+  return dir == 0 ? ((d.iz + 1) % c->pz) + c->pz * d.it : d.iz + c->pz * ((d.it + 1) % c->pt);
+}
+
+// The stencil on a domain-decomposed context. Per application, for every domain:
+//   (a) face pack: the half spinors its neighbours need, (1 +- g_mu) projected (and U^dag-multiplied for the backward
+//       hops) BEFORE they travel: 12 reals per face site instead of 24;
+//   (b) exchange on the stream `comm`: one cudaMemcpyPeerAsync per domain, cut and side (a same-device copy when both
+//       domains share a GPU, a peer copy over NVLink otherwise);
+//   (c) interior pass on `stream`, concurrent with (b): every hop that stays inside the domain;
+//   (d) exterior pass after (b): the sites on a cut get the ghost terms, the epilogue and their share of the fused
+//       reductions. The antiperiodic sign sits on the physical t boundary only (DDArgs::bc), never on an internal cut.
+// Reductions of all domains accumulate into the same device scalars (one device; several devices would add one small
+// all-reduce per reduction here).
+template <typename R>
+static int dslash_dd(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, void* out, const void* aux, double sgn, const ColMap& cm, int red_mode,
+                     const void* dotv, double* red, int red_stride, int g5) {
+  const int nd = (int)ctx->dom.size();
+  const size_t lb = (size_t)ctx->vh_loc * 24 * sizeof(R);  // bytes of one domain's packed parity spinor
+  int cmin = MAXCOL, cmax = 0;
+  for (int i = 0; i < cm.n; i++) { cmin = cm.col[i] < cmin ? cm.col[i] : cmin; cmax = cm.col[i] > cmax ? cm.col[i] : cmax; }
+  if (cmax + 1 > ctx->ghost_cols) {  // (re)size the send / receive buffers: fp64 half spinors for cmax + 1 columns
+    CK(cudaStreamSynchronize(ctx->stream));
+    CK(cudaStreamSynchronize(ctx->comm));
+    for (Domain& d : ctx->dom)
+      for (int dir = 0; dir < 2; dir++)
+        for (int k = 0; k < 2; k++) {
+          if (d.send[dir][k]) { dev_free(ctx, d.send[dir][k]); d.send[dir][k] = nullptr; }
+          if (d.recv[dir][k]) { dev_free(ctx, d.recv[dir][k]); d.recv[dir][k] = nullptr; }
+        }
+    ctx->ghost_cols = 0;
+    for (Domain& d : ctx->dom)
+      for (int dir = 0; dir < 2; dir++) {
+        if (!(dir == 0 ? ctx->pz > 1 : ctx->pt > 1)) continue;
+        const size_t nface = (size_t)d.g.Lh * d.g.L * (dir == 0 ? d.g.T : d.g.Lz);
+        for (int k = 0; k < 2; k++) {
+          int rc = dev_alloc(ctx, &d.send[dir][k], nface * 12 * 8 * (cmax + 1));
+          if (!rc) rc = dev_alloc(ctx, &d.recv[dir][k], nface * 12 * 8 * (cmax + 1));
+          if (rc) return rc;
+        }
+      }
+    ctx->ghost_cols = cmax + 1;
+  }
+  if (!out) {  // only a reduction is wanted, but the interior pass needs somewhere to leave the raw sums of the cut sites
+    if (!ctx->dd_tmp) { int rc = dev_alloc(ctx, &ctx->dd_tmp, (size_t)ctx->g.Vh * 24 * 8 * MAXCOL); if (rc) return rc; }
+    out = ctx->dd_tmp;
+  }
+  std::vector<DslashArgs<R>> A(nd);
+  for (int k = 0; k < nd; k++) {
+    const Domain& d = ctx->dom[k];
+    DslashArgs<R>& a = A[k];
+    a = make_args<R>(ctx, par, dagger, (const char*)in + k * lb, (char*)out + k * lb, aux ? (const char*)aux + k * lb : nullptr, sgn, cm, &d);
+    a.cstride = (int)((int64_t)ctx->g.Vh * 24 * (int64_t)sizeof(R) / 16);  // a column = the packed spinor of the WHOLE lattice
+    a.g5 = g5;
+    a.red_mode = red_mode;
+    a.dotv = dotv ? (const char*)dotv + k * lb : nullptr;
+    a.red = red;
+    a.red_stride = red_stride;
+    a.dd.part[0] = ctx->pz > 1;
+    a.dd.part[1] = ctx->pt > 1;
+    for (int dir = 0; dir < 2; dir++) {
+      a.dd.nface[dir] = d.g.Lh * d.g.L * (dir == 0 ? d.g.T : d.g.Lz);
+      a.dd.gstride[dir] = a.dd.nface[dir] * (int)(12 * sizeof(R) / 16);
+      a.dd.ghost[dir][0] = d.recv[dir][0];
+      a.dd.ghost[dir][1] = d.recv[dir][1];
+      a.dd.bc[dir][0] = a.dd.bc[dir][1] = (R)1;
+    }
+    if (d.it == 0) a.dd.bc[1][0] = (R)-1;            // the backward t hop of the first time slice wraps around the lattice
+    if (d.it == ctx->pt - 1) a.dd.bc[1][1] = (R)-1;  // the forward t hop of the last one
+  }
+  const int ng = ng_of<R>(ctx);
+  const int clv = !ctx->clover ? CL_NONE : (ctx->m_im != 0.0 ? CL_TWISTED : CL_CLOVER);
+  for (int k = 0; k < nd; k++) LAUNCH(launch_face_pack(A[k], ng, ctx->dom[k].send, ctx->stream));
+  CK(cudaEventRecord(ctx->ev_pack, ctx->stream));
+  CK(cudaStreamWaitEvent(ctx->comm, ctx->ev_pack, 0));
+  for (int k = 0; k < nd; k++) {
+    const Domain& d = ctx->dom[k];
+    for (int dir = 0; dir < 2; dir++) {
+      if (!A[k].dd.part[dir]) continue;
+      const size_t colb = (size_t)A[k].dd.gstride[dir] * 16, off = colb * cmin, bytes = colb * (cmax - cmin + 1);
+      const Domain& nb = ctx->dom[dom_behind(ctx, d, dir)];
+      const Domain& na = ctx->dom[dom_ahead(ctx, d, dir)];
+      CK(cudaMemcpyPeerAsync((char*)nb.recv[dir][1] + off, nb.device, (const char*)d.send[dir][0] + off, d.device, bytes, ctx->comm));
+      CK(cudaMemcpyPeerAsync((char*)na.recv[dir][0] + off, na.device, (const char*)d.send[dir][1] + off, d.device, bytes, ctx->comm));
+    }
+  }
+  CK(cudaEventRecord(ctx->ev_comm, ctx->comm));
+  for (int k = 0; k < nd; k++) LAUNCH(launch_dslash_dd(A[k], ng, epi, clv, 0, ctx->stream));
+  CK(cudaStreamWaitEvent(ctx->stream, ctx->ev_comm, 0));
+  for (int k = 0; k < nd; k++) LAUNCH(launch_dslash_dd(A[k], ng, epi, clv, 1, ctx->stream));
+  return TMW_OK;
+}
+
 template <typename R>
 static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, void* out, const void* aux, double sgn, const ColMap& cm,
                   int red_mode = 0, const void* dotv = nullptr, double* red = nullptr, int red_stride = 0, int g5 = 0) {
-  DslashArgs<R> a = make_args<R>(ctx, par, dagger, in, out, aux, sgn, cm);
   for (int i = 0; i < cm.n; i++)  // the kernels add column * cstride to a 32-bit site index
     if (((int64_t)cm.col[i] + 1) * ((int64_t)ctx->g.Vh * 24 * (int64_t)sizeof(R) / 16) >= ((int64_t)1 << 31))
       return fail(ctx, TMW_EINVAL, "lattice too large for this many right-hand-side columns in one call");
+  if (!ctx->dom.empty()) return dslash_dd<R>(ctx, epi, par, dagger, in, out, aux, sgn, cm, red_mode, dotv, red, red_stride, g5);
+  DslashArgs<R> a = make_args<R>(ctx, par, dagger, in, out, aux, sgn, cm);
   a.g5 = g5;
   a.red_mode = red_mode;
   a.dotv = dotv;
@@ -187,6 +323,31 @@ static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, vo
   LAUNCH(launch_dslash(a, ng_of<R>(ctx), epi, !ctx->clover ? CL_NONE : (ctx->m_im != 0.0 ? CL_TWISTED : CL_CLOVER), nr, ctx->stream));
   return TMW_OK;
 }
+// out = A^{-1} in (inverse) or A in on parity par, one column, fp64 (every domain of a decomposed context)
+static int diag64(tmw_ctx* ctx, int par, int inverse, const void* in, void* out) {
+  if (ctx->dom.empty()) {
+    LAUNCH(launch_diag(make_diag<double>(ctx, 0), ctx->g, par, ctx->clover, inverse, in, out, ctx->stream));
+    return TMW_OK;
+  }
+  const size_t lb = (size_t)ctx->vh_loc * 24 * 8;
+  for (size_t k = 0; k < ctx->dom.size(); k++)
+    LAUNCH(launch_diag(make_diag<double>(ctx, 0, &ctx->dom[k]), ctx->dom[k].g, par, ctx->clover, inverse, (const char*)in + k * lb, (char*)out + k * lb, ctx->stream));
+  return TMW_OK;
+}
+// canonical fp64 spinor <-> the packed parity spinors of the context (every domain)
+static int pack_both(tmw_ctx* ctx, int prec, const double* canon, void* pe, void* po) {
+  if (ctx->dom.empty()) { LAUNCH(launch_pack_spinor_both(ctx->g, prec, canon, pe, po, ctx->stream)); return TMW_OK; }
+  const size_t lb = (size_t)ctx->vh_loc * 24 * (prec == TMW_F32 ? 4 : 8);
+  for (size_t k = 0; k < ctx->dom.size(); k++) LAUNCH(launch_pack_spinor_both(ctx->dom[k].g, prec, canon, (char*)pe + k * lb, (char*)po + k * lb, ctx->stream));
+  return TMW_OK;
+}
+static int unpack_both(tmw_ctx* ctx, int prec, const void* pe, const void* po, double* canon) {
+  if (ctx->dom.empty()) { LAUNCH(launch_unpack_spinor_both(ctx->g, prec, pe, po, canon, ctx->stream)); return TMW_OK; }
+  const size_t lb = (size_t)ctx->vh_loc * 24 * (prec == TMW_F32 ? 4 : 8);
+  for (size_t k = 0; k < ctx->dom.size(); k++) LAUNCH(launch_unpack_spinor_both(ctx->dom[k].g, prec, (const char*)pe + k * lb, (const char*)po + k * lb, canon, ctx->stream));
+  return TMW_OK;
+}
+
 // Schur operator on the odd sites: out = A_oo in - H_oe A_ee^{-1} H_eo in  (tmp: even-parity scratch)
 // The conjugate transpose is A_oo^dag in - H_eo^dag (A_ee^dag)^{-1} H_oe^dag in: the same two kernels with the
 // daggered projectors / twist, because (H_oe)^dag = the daggered hopping block from odd to even.
@@ -244,6 +405,9 @@ void tmw_destroy(tmw_ctx* ctx) {
   if (ctx->sc_host) cudaFreeHost(ctx->sc_host);
   if (ctx->red_host) cudaFreeHost(ctx->red_host);
   if (ctx->gs_host) cudaFreeHost(ctx->gs_host);
+  if (ctx->comm) { cudaStreamSynchronize(ctx->comm); cudaStreamDestroy(ctx->comm); }
+  if (ctx->ev_pack) cudaEventDestroy(ctx->ev_pack);
+  if (ctx->ev_comm) cudaEventDestroy(ctx->ev_comm);
   if (ctx->ev0) cudaEventDestroy(ctx->ev0);
   if (ctx->ev1) cudaEventDestroy(ctx->ev1);
   delete ctx;
@@ -271,6 +435,9 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
       (o.debug & ~(TMW_DEBUG_FORCE_PIVOT | TMW_DEBUG_NO_CHUNK)))
     return fail(nullptr, TMW_EINVAL, "tmw_create: bad option value");
   if (!isfinite(m.re) || !isfinite(m.im) || !isfinite(c_sw)) return fail(nullptr, TMW_EINVAL, "tmw_create: non-finite parameter");
+  const int pz = o.domains_z > 1 ? o.domains_z : 1, pt = o.domains_t > 1 ? o.domains_t : 1;
+  if (o.domains_z < 0 || o.domains_t < 0 || L % (2 * pz) != 0 || T % (2 * pt) != 0)
+    return fail(nullptr, TMW_EINVAL, "tmw_create: domains_z / domains_t must divide L / T into even local extents");
   tmw_ctx* ctx = new (std::nothrow) tmw_ctx();
   if (!ctx) return fail(nullptr, TMW_ENOMEM, "tmw_create: host allocation failed");
   ctx->g.L = L; ctx->g.T = T; ctx->g.Lh = L / 2; ctx->g.Vh = (int)(V / 2);
@@ -278,6 +445,8 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
   ctx->g.sy = L / 2; ctx->g.sz = (L / 2) * L; ctx->g.st = (L / 2) * L * L;
   choose_tile(ctx->g, o.tile);
   ctx->ws_cols = 1;
+  ctx->pz = pz; ctx->pt = pt;
+  ctx->vh_loc = ctx->g.Vh / (pz * pt);
   ctx->nr32 = o.columns_per_thread;
   ctx->verbose = o.verbose != 0 || getenv("TMW_VERBOSE") != nullptr;
   ctx->V = V;
@@ -359,6 +528,56 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
   }
   CKC(cudaStreamSynchronize(ctx->stream));
   if (staging) dev_free(ctx, staging);
+  if (pz * pt > 1) {
+    // Domain decomposition: every domain gets its own packed gauge and clover fields, cut out of the
+    // whole-lattice ones built above (the clover leaves reach across the cuts, so F is computed before the split); the
+    // whole-lattice copies are then released. Split in t first, then z (tmw_options.domains_t / domains_z).
+    CKC(cudaStreamCreateWithFlags(&ctx->comm, cudaStreamNonBlocking));
+    CKC(cudaEventCreateWithFlags(&ctx->ev_pack, cudaEventDisableTiming));
+    CKC(cudaEventCreateWithFlags(&ctx->ev_comm, cudaEventDisableTiming));
+    int device = 0;
+    CKC(cudaGetDevice(&device));
+    const int64_t gVh = ctx->g.Vh;
+    for (int it = 0; it < pt; it++)
+      for (int iz = 0; iz < pz; iz++) {
+        Domain d;
+        memset(&d, 0, sizeof(d));
+        d.g = ctx->g;
+        d.g.tiled = 0;
+        d.g.Lz = L / pz; d.g.T = T / pt;
+        d.g.oz = iz * d.g.Lz; d.g.ot = it * d.g.T;
+        d.g.Vh = ctx->vh_loc;
+        d.g.st = d.g.sz * d.g.Lz;
+        d.iz = iz; d.it = it; d.device = device;
+        const size_t lv = (size_t)d.g.Vh;
+        for (int p = 0; p < 2; p++) {
+          CKA(&d.g64[p], lv * 36 * 16);
+          CKA(&d.g32[p], lv * 4 * np32 * 16);
+          CKC(launch_extract_planes(d.g, 36, gVh, ctx->g64[p], d.g64[p], ctx->stream));
+          CKC(launch_extract_planes(d.g, 4 * np32, gVh, ctx->g32[p], d.g32[p], ctx->stream));
+          if (ctx->clover) {
+            CKA(&d.c64[p], lv * 36 * 16);
+            CKA(&d.c32[p], lv * 18 * 16);
+            CKC(launch_extract_planes(d.g, 36, gVh, ctx->c64[p], d.c64[p], ctx->stream));
+            CKC(launch_extract_planes(d.g, 18, gVh, ctx->c32[p], d.c32[p], ctx->stream));
+          }
+        }
+        if (ctx->clover) {
+          CKA(&d.ci64, lv * 36 * 16);
+          CKA(&d.ci32, lv * 18 * 16);
+          CKC(launch_extract_planes(d.g, 36, gVh, ctx->ci64, d.ci64, ctx->stream));
+          CKC(launch_extract_planes(d.g, 18, gVh, ctx->ci32, d.ci32, ctx->stream));
+        }
+        ctx->launches += ctx->clover ? 10 : 4;
+        ctx->dom.push_back(d);
+      }
+    CKC(cudaStreamSynchronize(ctx->stream));
+    for (int p = 0; p < 2; p++) {
+      dev_free(ctx, ctx->g64[p]); dev_free(ctx, ctx->g32[p]); ctx->g64[p] = ctx->g32[p] = nullptr;
+      if (ctx->clover) { dev_free(ctx, ctx->c64[p]); dev_free(ctx, ctx->c32[p]); ctx->c64[p] = ctx->c32[p] = nullptr; }
+    }
+    if (ctx->clover) { dev_free(ctx, ctx->ci64); dev_free(ctx, ctx->ci32); ctx->ci64 = ctx->ci32 = nullptr; }
+  }
   *out = ctx;
   return TMW_OK;
 #undef CKC
@@ -387,12 +606,22 @@ int tmw_set_debug(tmw_ctx* ctx, int flags) {
 int tmw_pack(tmw_ctx* ctx, int prec, int parity, const double* canonical, void* packed) {
   if (!ctx) return TMW_EINVAL;
   if (!canonical || !packed || (prec != TMW_F32 && prec != TMW_F64) || (parity != TMW_EVEN && parity != TMW_ODD)) return fail(ctx, TMW_EINVAL, "tmw_pack: bad argument");
+  if (!ctx->dom.empty()) {  // the domains' local packed spinors back to back
+    const size_t lb = (size_t)ctx->vh_loc * 24 * (prec == TMW_F32 ? 4 : 8);
+    for (size_t k = 0; k < ctx->dom.size(); k++) LAUNCH(launch_pack_spinor(ctx->dom[k].g, parity == TMW_ODD, prec, canonical, (char*)packed + k * lb, ctx->stream));
+    return TMW_OK;
+  }
   LAUNCH(launch_pack_spinor(ctx->g, parity == TMW_ODD, prec, canonical, packed, ctx->stream));
   return TMW_OK;
 }
 int tmw_unpack(tmw_ctx* ctx, int prec, int parity, const void* packed, double* canonical) {
   if (!ctx) return TMW_EINVAL;
   if (!canonical || !packed || (prec != TMW_F32 && prec != TMW_F64) || (parity != TMW_EVEN && parity != TMW_ODD)) return fail(ctx, TMW_EINVAL, "tmw_unpack: bad argument");
+  if (!ctx->dom.empty()) {
+    const size_t lb = (size_t)ctx->vh_loc * 24 * (prec == TMW_F32 ? 4 : 8);
+    for (size_t k = 0; k < ctx->dom.size(); k++) LAUNCH(launch_unpack_spinor(ctx->dom[k].g, parity == TMW_ODD, prec, (const char*)packed + k * lb, canonical, ctx->stream));
+    return TMW_OK;
+  }
   LAUNCH(launch_unpack_spinor(ctx->g, parity == TMW_ODD, prec, packed, canonical, ctx->stream));
   return TMW_OK;
 }
@@ -402,6 +631,7 @@ int tmw_get_clover(tmw_ctx* ctx, int parity, int inverse, double* dst) {
   if (!dst || (parity != TMW_EVEN && parity != TMW_ODD)) return fail(ctx, TMW_EINVAL, "tmw_get_clover: bad argument");
   if (!ctx->clover) return fail(ctx, TMW_EINVAL, "tmw_get_clover: context has no clover term (c_sw = 0)");
   if (inverse && parity != TMW_EVEN) return fail(ctx, TMW_EINVAL, "tmw_get_clover: the inverse is stored on the even parity only");
+  if (!ctx->dom.empty()) return fail(ctx, TMW_EINVAL, "tmw_get_clover: not available on a domain-decomposed context (the blocks live per domain)");
   const void* src = inverse ? ctx->ci64 : ctx->c64[parity == TMW_ODD];
   LAUNCH(launch_clover_export(ctx->g, src, dst, ctx->stream));
   return TMW_OK;
@@ -490,12 +720,12 @@ extern "C" int tmw_apply_multi(tmw_ctx* ctx, int op, int parity, int prec, int n
     cout = (double*)ctx->canon[1];
   }
   for (int c = 0; c < nrhs; c++) {
-    LAUNCH(launch_pack_spinor_both(ctx->g, 1, (const double*)colp(cin, c, cbytes), colp(ctx->w64[0], c, b64), colp(ctx->w64[1], c, b64), ctx->stream));
+    if ((rc = pack_both(ctx, 1, (const double*)colp(cin, c, cbytes), colp(ctx->w64[0], c, b64), colp(ctx->w64[1], c, b64)))) return rc;
   }
   rc = full_apply64(ctx, dagger, ctx->w64[0], ctx->w64[1], ctx->w64[2], ctx->w64[3], cm, g5);
   if (rc) return rc;
   for (int c = 0; c < nrhs; c++) {
-    LAUNCH(launch_unpack_spinor_both(ctx->g, 1, colp(ctx->w64[2], c, b64), colp(ctx->w64[3], c, b64), (double*)colp(cout, c, cbytes), ctx->stream));
+    if ((rc = unpack_both(ctx, 1, colp(ctx->w64[2], c, b64), colp(ctx->w64[3], c, b64), (double*)colp(cout, c, cbytes)))) return rc;
   }
   if (ctx->opt.location == TMW_HOST) {
     CK(cudaMemcpyAsync(out, cout, cbytes * nrhs, cudaMemcpyDeviceToHost, ctx->stream));
@@ -531,7 +761,7 @@ extern "C" int tmw_cheb_apply(tmw_ctx* ctx, int ncoef, const double* coef, doubl
   void** W = ctx->w64;
   const int64_t n64 = (int64_t)ctx->g.Vh * 12;
   const ColMap one = cols_first(1);
-  LAUNCH(launch_pack_spinor_both(ctx->g, 1, cin, W[0], W[1], s));
+  if ((rc = pack_both(ctx, 1, cin, W[0], W[1]))) return rc;
   int b1 = 2, b2 = 4;  // indices of the (even) buffers of b_{k+1}, b_{k+2}
   if (ncoef == 1) {
     for (int p = 0; p < 2; p++) LAUNCH(launch_scale(n64, W[b1 + p], W[p], coef[0], s));
@@ -547,7 +777,7 @@ extern "C" int tmw_cheb_apply(tmw_ctx* ctx, int ncoef, const double* coef, doubl
       const int t = b1; b1 = b2; b2 = t;  // the new vector was written over b_{k+2}
     }
   }
-  LAUNCH(launch_unpack_spinor_both(ctx->g, 1, W[b1], W[b1 + 1], cout, s));
+  if ((rc = unpack_both(ctx, 1, W[b1], W[b1 + 1], cout))) return rc;
   if (ctx->opt.location == TMW_HOST) {
     CK(cudaMemcpyAsync(out, cout, cbytes, cudaMemcpyDeviceToHost, s));
     CK(cudaStreamSynchronize(s));
@@ -638,10 +868,10 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
   // y = 0, r64 = bhat, r = (R) r64, rhat = r, x = p = v = 0
   CK(cudaMemsetAsync(W[3], 0, bytes64 * ncols, s));
   CK(cudaMemsetAsync(x, 0, bytesR * ncols, s));
-  LAUNCH(launch_convert<R>(n64, W[2], rhat, act, s));
+  LAUNCH(launch_convert<R>(n64, ctx->vh_loc, W[2], rhat, act, s));
   memset(h, 0, MAXCOL * sizeof(Scalars));
   if ((rc = push_scalars(ctx))) return rc;
-  LAUNCH(launch_resid_convert<R>(n64, W[2], nullptr, W[4], r, rhat, nullptr, ctx->sc, act, s));  // r64 = bhat - 0; rho = <rhat,r>; rr = |r64|^2
+  LAUNCH(launch_resid_convert<R>(n64, ctx->vh_loc, W[2], nullptr, W[4], r, rhat, nullptr, ctx->sc, act, s));  // r64 = bhat - 0; rho = <rhat,r>; rr = |r64|^2
   if ((rc = fetch_scalars(ctx))) return rc;
   for (int i = 0; i < act.n; i++) {
     const int c = act.col[i];
@@ -693,7 +923,7 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
       ColMap good;
       good.n = 0;
       for (int i = 0; i < upd.n; i++) if (!broken[upd.col[i]]) cols_add(good, upd.col[i]);
-      if (good.n > 0) LAUNCH(launch_acc_y<R>(n64, W[3], x, good, s));
+      if (good.n > 0) LAUNCH(launch_acc_y<R>(n64, ctx->vh_loc, W[3], x, good, s));
       for (int i = 0; i < brk.n; i++) CK(cudaMemsetAsync(colp(x, brk.col[i], bytesR), 0, bytesR, s));
       if ((rc = schur<double>(ctx, 0, W[3], W[6], W[5], upd))) return rc;
       for (int i = 0; i < upd.n; i++) {
@@ -704,7 +934,7 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
       }
       if ((rc = push_scalars(ctx))) return rc;
       // r := true residual; the search direction update_xrp already built from the iterated r moves with it
-      LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], r, rhat, p, ctx->sc, upd, s));
+      LAUNCH(launch_resid_convert<R>(n64, ctx->vh_loc, W[2], W[6], W[4], r, rhat, p, ctx->sc, upd, s));
       if ((rc = fetch_scalars(ctx))) return rc;
       for (int i = 0; i < upd.n; i++) {
         const int c = upd.col[i];
@@ -740,7 +970,7 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
         if (!broken[c] && cs[c].rnorm <= cs[c].r_upd) cols_add(keep, c);
         else CK(cudaMemsetAsync(colp(x, c, bytesR), 0, bytesR, s));
       }
-      if (keep.n > 0) LAUNCH(launch_acc_y<R>(n64, W[3], x, keep, s));
+      if (keep.n > 0) LAUNCH(launch_acc_y<R>(n64, ctx->vh_loc, W[3], x, keep, s));
       if ((rc = schur<double>(ctx, 0, W[3], W[6], W[5], rst))) return rc;
       for (int i = 0; i < rst.n; i++) {
         const int c = rst.col[i];
@@ -749,8 +979,8 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
       }
       if ((rc = push_scalars(ctx))) return rc;
       LAUNCH(launch_sub_norm(n64, W[2], W[6], W[4], ctx->red, rst, s));  // r64 = bhat - Mhat y (norm discarded)
-      LAUNCH(launch_convert<R>(n64, W[4], rhat, rst, s));
-      LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], r, rhat, nullptr, ctx->sc, rst, s));
+      LAUNCH(launch_convert<R>(n64, ctx->vh_loc, W[4], rhat, rst, s));
+      LAUNCH(launch_resid_convert<R>(n64, ctx->vh_loc, W[2], W[6], W[4], r, rhat, nullptr, ctx->sc, rst, s));
       for (int i = 0; i < rst.n; i++)  // p = r
         CK(cudaMemcpyAsync(colp(p, rst.col[i], bytesR), colp(r, rst.col[i], bytesR), bytesR, cudaMemcpyDeviceToDevice, s));
       if ((rc = fetch_scalars(ctx))) return rc;
@@ -808,7 +1038,7 @@ int solve_gcr(tmw_ctx* ctx, int c, double tol, ColState& q) {
     // true residual r64 = bhat - Mhat y (W[6] holds Mhat y), r = (R) r64, |r64|^2
     memset(h, 0, MAXCOL * sizeof(Scalars));
     if ((rc = push_scalars(ctx))) return rc;
-    LAUNCH(launch_resid_convert<R>(n64, W[2], W[6], W[4], X[0], X[1], nullptr, ctx->sc, one, s));
+    LAUNCH(launch_resid_convert<R>(n64, ctx->vh_loc, W[2], W[6], W[4], X[0], X[1], nullptr, ctx->sc, one, s));
     if ((rc = fetch_scalars(ctx))) return rc;
     q.rnorm = q.maxr = sqrt(h[c].rr);
     q.iter_resid = q.rnorm / q.bnorm;
@@ -833,7 +1063,7 @@ int solve_gcr(tmw_ctx* ctx, int c, double tol, ColState& q) {
       if (rn <= tol * q.bnorm || rn < ctx->opt.delta * q.maxr) break;
     }
     // restart: y += x, Mhat y in fp64
-    LAUNCH(launch_acc_y<R>(n64, W[3], X[6], one, s));
+    LAUNCH(launch_acc_y<R>(n64, ctx->vh_loc, W[3], X[6], one, s));
     if ((rc = schur<double>(ctx, 0, W[3], W[6], W[5], one))) return rc;
     q.updates++;
   }
@@ -850,8 +1080,8 @@ static int solve_packed(tmw_ctx* ctx, int nrhs, const ColMap& cm, double tol, Co
   void** W = ctx->w64;
   const size_t b64 = spinor_bytes(ctx, TMW_F64);
   int rc, status = TMW_OK;
-  Diag<double> d = make_diag<double>(ctx, 0);
-  for (int i = 0; i < cm.n; i++) LAUNCH(launch_diag(d, ctx->g, 0, ctx->clover, 1, colp(W[0], cm.col[i], b64), colp(W[5], cm.col[i], b64), s));
+  for (int i = 0; i < cm.n; i++)
+    if ((rc = diag64(ctx, 0, 1, colp(W[0], cm.col[i], b64), colp(W[5], cm.col[i], b64)))) return rc;
   if ((rc = dslash<double>(ctx, EPI_XPAY, 1, 0, W[5], W[2], W[1], -1.0, cm))) return rc;
   {
     NvtxRange nvtx_it("tmw_solve: Krylov iterations");
@@ -909,7 +1139,7 @@ static int solve_chunk(tmw_ctx* ctx, int nrhs, const double* b, double* x, doubl
   const ColMap all = cols_first(nrhs);
   // A0: split b into parities, |b|
   for (int c = 0; c < nrhs; c++) {
-    LAUNCH(launch_pack_spinor_both(ctx->g, 1, (const double*)colp(cb, c, cbytes), colp(W[0], c, b64), colp(W[1], c, b64), s));
+    if ((rc = pack_both(ctx, 1, (const double*)colp(cb, c, cbytes), colp(W[0], c, b64), colp(W[1], c, b64)))) return rc;
   }
   CK(cudaMemsetAsync(ctx->red, 0, 4 * MAXCOL * sizeof(double), s));
   LAUNCH(launch_dot_norm<double>(n64, nullptr, W[0], ctx->red, all, s));
@@ -973,7 +1203,7 @@ static int solve_chunk(tmw_ctx* ctx, int nrhs, const double* b, double* x, doubl
     }
     for (int i = 0; i < nz.n; i++) {
       const int c = nz.col[i];
-      LAUNCH(launch_unpack_spinor_both(ctx->g, 1, colp(W[7], c, b64), colp(W[3], c, b64), (double*)colp(cx_, c, cbytes), s));
+      if ((rc = unpack_both(ctx, 1, colp(W[7], c, b64), colp(W[3], c, b64), (double*)colp(cx_, c, cbytes)))) return rc;
       if (status == TMW_OK && !(cs[c].true_resid <= tol)) {
         status = TMW_ENOCONV;
         fail(ctx, TMW_ENOCONV, "tmw_solve: the Schur system converged but the full-lattice residual stays above tol (ill-conditioned A_ee)");

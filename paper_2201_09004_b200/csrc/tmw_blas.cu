@@ -26,7 +26,9 @@ __device__ __forceinline__ void stp(double* base, int64_t i, const double* v) {
 
 // Mixed-precision kernels pair an fp32 packed spinor with an fp64 packed spinor. The plane layouts differ: the
 // float4 vector (k, cb) holds reals 4k..4k+3 of site cb, which are the double2 vectors (2k, cb) and (2k+1, cb).
-// Work item i = k*Vh + cb (a float4 index); the "m" accessors address either precision by that item.
+// Work item i = k*Vh + cb (a float4 index); the "m" accessors address either precision by that item. With several
+// domains back to back in a vector (Vh = sites of ONE domain) item i = (6 d + k)*Vh + cb pairs with the double2
+// vectors (12 d + 2k [+1])*Vh + cb = (2q [+1])*Vh + cb, q = i / Vh: the same formula.
 __device__ __forceinline__ void ldm(const float* base, int64_t i, int64_t, float* v) { ldp(base, i, v); }
 __device__ __forceinline__ void stm(float* base, int64_t i, int64_t, const float* v) { stp(base, i, v); }
 __device__ __forceinline__ void ldm(const double* base, int64_t i, int64_t Vh, double* v) {
@@ -431,19 +433,19 @@ template <typename R> cudaError_t launch_dot_norm(int64_t n, const void* a, cons
   dot_norm_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, (const R*)a, (const R*)b, out, cm);
   return cudaGetLastError();
 }
-template <typename R> cudaError_t launch_acc_y(int64_t n64, void* y64, void* x, const ColMap& cm, cudaStream_t s) {
+template <typename R> cudaError_t launch_acc_y(int64_t n64, int64_t vh, void* y64, void* x, const ColMap& cm, cudaStream_t s) {
   const int64_t np = n64 / 2;
-  acc_y_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, np / 6, (double*)y64, (R*)x, cm);
+  acc_y_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, vh, (double*)y64, (R*)x, cm);
   return cudaGetLastError();
 }
-template <typename R> cudaError_t launch_resid_convert(int64_t n64, const void* b64, const void* w64, void* r64, void* r, const void* rhat, void* p, Scalars* sc, const ColMap& cm, cudaStream_t s) {
+template <typename R> cudaError_t launch_resid_convert(int64_t n64, int64_t vh, const void* b64, const void* w64, void* r64, void* r, const void* rhat, void* p, Scalars* sc, const ColMap& cm, cudaStream_t s) {
   const int64_t np = n64 / 2;
-  resid_convert_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, np / 6, (const double*)b64, (const double*)w64, (double*)r64, (R*)r, (const R*)rhat, (R*)p, sc, cm);
+  resid_convert_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, vh, (const double*)b64, (const double*)w64, (double*)r64, (R*)r, (const R*)rhat, (R*)p, sc, cm);
   return cudaGetLastError();
 }
-template <typename R> cudaError_t launch_convert(int64_t n64, const void* src64, void* dst, const ColMap& cm, cudaStream_t s) {
+template <typename R> cudaError_t launch_convert(int64_t n64, int64_t vh, const void* src64, void* dst, const ColMap& cm, cudaStream_t s) {
   const int64_t np = n64 / 2;
-  convert_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, np / 6, (const double*)src64, (R*)dst, cm);
+  convert_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, vh, (const double*)src64, (R*)dst, cm);
   return cudaGetLastError();
 }
 cudaError_t launch_sub_norm(int64_t n64, const void* a, const void* b, void* d, double* out, const ColMap& cm, cudaStream_t s) {
@@ -476,9 +478,9 @@ template cudaError_t launch_gcr_step<double>(int64_t, int, void*, void*, void*, 
   template cudaError_t launch_update_s<R>(int64_t, void*, const void*, const void*, const Scalars*, const ColMap&, cudaStream_t);           \
   template cudaError_t launch_update_xrp<R>(int64_t, void*, void*, void*, const void*, const void*, const void*, Scalars*, const ColMap&, cudaStream_t); \
   template cudaError_t launch_dot_norm<R>(int64_t, const void*, const void*, double*, const ColMap&, cudaStream_t);                         \
-  template cudaError_t launch_acc_y<R>(int64_t, void*, void*, const ColMap&, cudaStream_t);                                                 \
-  template cudaError_t launch_resid_convert<R>(int64_t, const void*, const void*, void*, void*, const void*, void*, Scalars*, const ColMap&, cudaStream_t); \
-  template cudaError_t launch_convert<R>(int64_t, const void*, void*, const ColMap&, cudaStream_t);
+  template cudaError_t launch_acc_y<R>(int64_t, int64_t, void*, void*, const ColMap&, cudaStream_t);                                        \
+  template cudaError_t launch_resid_convert<R>(int64_t, int64_t, const void*, const void*, void*, void*, const void*, void*, Scalars*, const ColMap&, cudaStream_t); \
+  template cudaError_t launch_convert<R>(int64_t, int64_t, const void*, void*, const ColMap&, cudaStream_t);
 TMW_INST(float)
 TMW_INST(double)
 

@@ -344,6 +344,82 @@ template <typename R, int MU, bool FWD> TMW_HD void hop(const R* psi, const cx<R
   }
 }
 
+// The three stages of hop<> as separate functions, for the domain-decomposed stencil, where the spin
+// projection (and, for backward hops, the colour multiply) of a hop that crosses a domain boundary happens on the
+// sending side and only the 12 reals of the half spinor travel.
+template <typename R, int MU> TMW_HD void project_half(const R* psi, R sig, cx<R> (&h)[6]) {
+#pragma unroll
+  for (int c = 0; c < 3; c++) {
+    const cx<R> p0 = mk<R>(psi[2 * c], psi[2 * c + 1]);
+    const cx<R> p1 = mk<R>(psi[6 + 2 * c], psi[6 + 2 * c + 1]);
+    const cx<R> p2 = mk<R>(psi[12 + 2 * c], psi[12 + 2 * c + 1]);
+    const cx<R> p3 = mk<R>(psi[18 + 2 * c], psi[18 + 2 * c + 1]);
+    if (MU == 0) {
+      h[c] = mk<R>(p0.re - sig * p3.im, p0.im + sig * p3.re);
+      h[3 + c] = mk<R>(p1.re - sig * p2.im, p1.im + sig * p2.re);
+    } else if (MU == 1) {
+      h[c] = mk<R>(p0.re - sig * p3.re, p0.im - sig * p3.im);
+      h[3 + c] = mk<R>(p1.re + sig * p2.re, p1.im + sig * p2.im);
+    } else if (MU == 2) {
+      h[c] = mk<R>(p0.re - sig * p2.im, p0.im + sig * p2.re);
+      h[3 + c] = mk<R>(p1.re + sig * p3.im, p1.im - sig * p3.re);
+    } else {
+      h[c] = mk<R>(p0.re + sig * p2.re, p0.im + sig * p2.im);
+      h[3 + c] = mk<R>(p1.re + sig * p3.re, p1.im + sig * p3.im);
+    }
+  }
+}
+// w = U h (FWD) or U^dagger h, for both spin rows of the half spinor
+template <typename R, bool FWD> TMW_HD void su3_mul_half(const cx<R> (&U)[9], const cx<R> (&h)[6], cx<R> (&w)[6]) {
+#pragma unroll
+  for (int s = 0; s < 2; s++)
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+      cx<R> t = mk<R>((R)0, (R)0);
+#pragma unroll
+      for (int b = 0; b < 3; b++) {
+        if (FWD) cmad(t, U[3 * a + b], h[3 * s + b]);
+        else cmadc(t, U[3 * b + a], h[3 * s + b]);
+      }
+      w[3 * s + a] = t;
+    }
+}
+// acc += the 4-spinor rebuilt from the half spinor w of the projector 1 + sig*gamma_MU (table above hop<>)
+template <typename R, int MU> TMW_HD void recon_acc(const cx<R> (&w6)[6], R sig, R* acc) {
+#pragma unroll
+  for (int s = 0; s < 2; s++)
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+      const cx<R> w = w6[3 * s + a];
+      acc[2 * (3 * s + a)] += w.re;
+      acc[2 * (3 * s + a) + 1] += w.im;
+      if (MU == 0) {
+        const int r = (s == 0) ? 3 : 2;
+        acc[2 * (3 * r + a)] += sig * w.im;
+        acc[2 * (3 * r + a) + 1] -= sig * w.re;
+      } else if (MU == 1) {
+        if (s == 0) {
+          acc[2 * (9 + a)] -= sig * w.re;
+          acc[2 * (9 + a) + 1] -= sig * w.im;
+        } else {
+          acc[2 * (6 + a)] += sig * w.re;
+          acc[2 * (6 + a) + 1] += sig * w.im;
+        }
+      } else if (MU == 2) {
+        if (s == 0) {
+          acc[2 * (6 + a)] += sig * w.im;
+          acc[2 * (6 + a) + 1] -= sig * w.re;
+        } else {
+          acc[2 * (9 + a)] -= sig * w.im;
+          acc[2 * (9 + a) + 1] += sig * w.re;
+        }
+      } else {
+        acc[2 * (3 * (s + 2) + a)] += sig * w.re;
+        acc[2 * (3 * (s + 2) + a) + 1] += sig * w.im;
+      }
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // Packed Hermitian 6x6 block (36 reals: 6 real diagonal, then 15 strictly-lower complex entries row-major,
 // entry (i,j), i>j, at 6 + 2*(i*(i-1)/2 + j)) times a 6-vector: out = B v.
@@ -463,6 +539,21 @@ enum { EPI_HOP = 0,        // out = h
        EPI_AINV_XPAY = 4   // out = A^{-1} (aux + sgn*h)          (solution reconstruction)
 };
 
+// Domain decomposition: what a stencil launch on ONE domain needs to know about its cuts. Directions
+// z (index 0) and t (index 1) may be partitioned. ghost[d][0] ("lo") holds, for the output sites at local coordinate 0,
+// the finished backward hop term (1 - sig g_mu) U_mu(x-mu)^dag psi(x-mu) as a half spinor (projected AND multiplied by
+// the neighbour, who owns that link); ghost[d][1] ("hi") holds, for the sites at the last local coordinate, the
+// projected half spinor (1 + sig g_mu) psi(x+mu) of the forward hop (this side multiplies by its own U_mu(x)).
+// 12 reals per face site: vector (k, f) of column c at index c*gstride[d] + k*nface[d] + f, k < 12/N planes,
+// face index f = xh + Lh*(y + L*t) (z cut) or xh + Lh*(y + L*z) (t cut) — the same on both sides of a cut.
+template <typename R> struct DDArgs {
+  int part[2];              // is z / t partitioned
+  const void* ghost[2][2];  // [direction][lo, hi] receive buffers
+  R bc[2][2];               // factor on the ghost term: -1 on the physical (antiperiodic) time boundary, else +1
+  int nface[2];             // face sites per parity
+  int gstride[2];           // 16-byte vectors per column in a ghost buffer
+};
+
 template <typename R> struct DslashArgs {
   const void* in;    // packed spinor, parity 1-par
   void* out;         // packed spinor, parity par
@@ -489,6 +580,7 @@ template <typename R> struct DslashArgs {
   int cstride;  // 16-byte vectors per column; (columns in the buffers) * cstride < 2^31 (checked by the host)
   int red_stride;
   unsigned char col[MAXCOL];
+  DDArgs<R> dd;      // read only by the domain-decomposition kernels (DD != 0)
 };
 
 // neighbour checkerboard indices and the time-boundary sign
@@ -518,12 +610,18 @@ TMW_HD Nbr neighbours(const Geom& g, int par, const Site& s) {
   return n;
 }
 
-template <typename R, int NG, int MU, int NR, bool STREAM>
+// DD = 1 (interior pass of a domain): hops that leave the domain through a cut are skipped, the exterior pass adds them
+template <typename R, int NG, int MU, int NR, bool STREAM, int DD>
 __device__ __forceinline__ void hop_pair(const DslashArgs<R>& a, const Nbr& n, int cb, const int (&cofs)[NR], R (&acc)[NR][24]) {
   const int NPG = Planes<R, NG>::N;
   const int64_t Vh = a.g.Vh;
   typedef typename Vec16<R>::T V;
-  {  // forward: (1 + sig g_mu) U_mu(x) psi(x+mu)
+  bool skip_f = false, skip_b = false;
+  if (DD && MU >= 2 && a.dd.part[MU - 2]) {
+    skip_f = (MU == 2) ? n.wrap_zf : n.wrap_tf;
+    skip_b = (MU == 2) ? n.wrap_zb : n.wrap_tb;
+  }
+  if (!skip_f) {  // forward: (1 + sig g_mu) U_mu(x) psi(x+mu)
     cx<R> U[9];
     load_link<R, NG, STREAM>((const V*)a.U[a.par] + (int64_t)MU * NPG * Vh, Vh, cb, U);
     const R bc = (MU == 3 && n.wrap_tf) ? (R)-1 : (R)1;
@@ -534,7 +632,7 @@ __device__ __forceinline__ void hop_pair(const DslashArgs<R>& a, const Nbr& n, i
       hop<R, MU, true>(psi, U, a.sig, bc, acc[j]);
     }
   }
-  {  // backward: (1 - sig g_mu) U_mu(x-mu)^dag psi(x-mu)
+  if (!skip_b) {  // backward: (1 - sig g_mu) U_mu(x-mu)^dag psi(x-mu)
     cx<R> U[9];
     load_link<R, NG, STREAM>((const V*)a.U[1 - a.par] + (int64_t)MU * NPG * Vh, Vh, n.bwd[MU], U);
     const R bc = (MU == 3 && n.wrap_tb) ? (R)-1 : (R)1;
@@ -598,9 +696,18 @@ template <int EPI, int CLOVER> __device__ __forceinline__ constexpr bool stored_
 
 // The stencil at one site for NR right-hand sides: on return acc[j] holds the output spinor of column slot j.
 // red[j] = {Re, Im <out, aux>, <out, out>} when WANT_RED2 (EPI >= 2), accumulated chirality by chirality.
-template <typename R, int NG, int EPI, int CLOVER, int NR, bool STREAM>
-__device__ __forceinline__ void dslash_site(const DslashArgs<R>& a, const Site& s, const int (&cofs)[NR], const bool (&valid)[NR], R (&acc)[NR][24], R (&red2)[NR][3]) {
-  typedef typename Vec16<R>::T V;
+// is this output site on a cut of its domain (some hop of it arrives through a ghost buffer)?
+template <typename R> TMW_HD bool on_cut(const DslashArgs<R>& a, const Nbr& n) {
+  return (a.dd.part[0] && (n.wrap_zf || n.wrap_zb)) || (a.dd.part[1] && (n.wrap_tf || n.wrap_tb));
+}
+
+template <typename R, int NG, int EPI, int CLOVER, int NR, bool STREAM> __device__ __forceinline__ void dslash_epilogue(const DslashArgs<R>& a, int cb, const int (&cofs)[NR], const bool (&valid)[NR], R (&acc)[NR][24], R (&red2)[NR][3]);
+
+// DD = 0: the whole lattice (or a domain without cuts). DD = 1: interior pass of a domain: returns true for a site on a
+// cut, whose hops inside the domain have then been summed and stored RAW (no 1/2, no epilogue) in `out` for the exterior
+// pass (dslash_ext_kernel) to finish; such a site takes no part in the fused reductions of this pass.
+template <typename R, int NG, int EPI, int CLOVER, int NR, bool STREAM, int DD>
+__device__ __forceinline__ bool dslash_site(const DslashArgs<R>& a, const Site& s, const int (&cofs)[NR], const bool (&valid)[NR], R (&acc)[NR][24], R (&red2)[NR][3]) {
   // cofs[j] = column * cstride: the column offset is added to the 32-bit SITE INDEX (the host checks that it fits), so
   // that every load address stays one IMAD.WIDE on a kernel-parameter base pointer, as with a single column
   const Nbr n = neighbours(a.g, a.par, s);
@@ -609,10 +716,26 @@ __device__ __forceinline__ void dslash_site(const DslashArgs<R>& a, const Site& 
   for (int j = 0; j < NR; j++)
 #pragma unroll
     for (int i = 0; i < 24; i++) acc[j][i] = (R)0;
-  hop_pair<R, NG, 0, NR, STREAM>(a, n, cb, cofs, acc);
-  hop_pair<R, NG, 1, NR, STREAM>(a, n, cb, cofs, acc);
-  hop_pair<R, NG, 2, NR, STREAM>(a, n, cb, cofs, acc);
-  hop_pair<R, NG, 3, NR, STREAM>(a, n, cb, cofs, acc);
+  hop_pair<R, NG, 0, NR, STREAM, DD>(a, n, cb, cofs, acc);
+  hop_pair<R, NG, 1, NR, STREAM, DD>(a, n, cb, cofs, acc);
+  hop_pair<R, NG, 2, NR, STREAM, DD>(a, n, cb, cofs, acc);
+  hop_pair<R, NG, 3, NR, STREAM, DD>(a, n, cb, cofs, acc);
+  if (DD && on_cut(a, n)) {
+#pragma unroll
+    for (int j = 0; j < NR; j++) {
+      if (valid[j]) store_reals<24>(a.out, a.g.Vh, cb + cofs[j], acc[j]);
+      red2[j][0] = red2[j][1] = red2[j][2] = (R)0;
+    }
+    return true;
+  }
+  dslash_epilogue<R, NG, EPI, CLOVER, NR, STREAM>(a, cb, cofs, valid, acc, red2);
+  return false;
+}
+
+// acc[j] = the summed hops of column slot j at site cb -> the output spinor (1/2, site-diagonal part, aux); see dslash_site
+template <typename R, int NG, int EPI, int CLOVER, int NR, bool STREAM>
+__device__ __forceinline__ void dslash_epilogue(const DslashArgs<R>& a, int cb, const int (&cofs)[NR], const bool (&valid)[NR], R (&acc)[NR][24], R (&red2)[NR][3]) {
+  typedef typename Vec16<R>::T V;
   const int64_t Vh = a.g.Vh;
 #pragma unroll
   for (int j = 0; j < NR; j++) {

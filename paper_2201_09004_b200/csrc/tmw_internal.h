@@ -9,6 +9,18 @@ namespace tmw {
 // nr = right-hand-side columns per thread (fp32: 1..4; fp64: always 1)
 cudaError_t launch_dslash(const DslashArgs<float>& a, int ng, int epi, int clover, int nr, cudaStream_t s);
 cudaError_t launch_dslash(const DslashArgs<double>& a, int ng, int epi, int clover, int nr, cudaStream_t s);
+// ---- domain decomposition (tmw_dd_f32.cu / tmw_dd_f64.cu) ----
+// a describes ONE domain (local geometry and fields, a.dd its cuts and receive buffers). pass 0: interior (all sites, the
+// hops through a cut skipped, sites on a cut left raw in a.out); pass 1: exterior (the sites on a cut: + ghost terms,
+// epilogue, reductions). One column per thread, a.ncol columns per launch.
+cudaError_t launch_dslash_dd(const DslashArgs<float>& a, int ng, int epi, int clover, int pass, cudaStream_t s);
+cudaError_t launch_dslash_dd(const DslashArgs<double>& a, int ng, int epi, int clover, int pass, cudaStream_t s);
+// half spinors for the neighbours of the domain from a.in: send[direction z,t][0: to the neighbour behind, 1: ahead]
+cudaError_t launch_face_pack(const DslashArgs<float>& a, int ng, void* const (&send)[2][2], cudaStream_t s);
+cudaError_t launch_face_pack(const DslashArgs<double>& a, int ng, void* const (&send)[2][2], cudaStream_t s);
+// dst (packed field of domain g, nplanes planes of 16-byte vectors) <- src (the same field of the whole lattice, gVh sites per parity)
+cudaError_t launch_extract_planes(const Geom& g, int nplanes, int64_t gVh, const void* src, void* dst, cudaStream_t s);
+
 // out = A in (inverse = 0) or A^{-1} in (inverse = 1) on parity par, site-local
 cudaError_t launch_diag(const Diag<float>& d, const Geom& g, int par, bool clover, int inverse, const void* in, void* out, cudaStream_t s);
 cudaError_t launch_diag(const Diag<double>& d, const Geom& g, int par, bool clover, int inverse, const void* in, void* out, cudaStream_t s);
@@ -91,13 +103,14 @@ template <typename R> cudaError_t launch_update_xrp(int64_t n, void* x, void* r,
 // out[4c+0..1] += <a,b>, out[4c+2] += <b,b> (a may be null: only the norm)
 template <typename R> cudaError_t launch_dot_norm(int64_t n, const void* a, const void* b, double* out, const ColMap& cm, cudaStream_t s);
 // fp64 helpers for the reliable update
-template <typename R> cudaError_t launch_acc_y(int64_t n64, void* y64, void* x, const ColMap& cm, cudaStream_t s);  // y += x; x = 0   (n64 = number of double2 vectors per column)
+// vh = sites per parity of one domain (the fp32 <-> fp64 plane correspondence works per domain block of 24 reals x vh)
+template <typename R> cudaError_t launch_acc_y(int64_t n64, int64_t vh, void* y64, void* x, const ColMap& cm, cudaStream_t s);  // y += x; x = 0   (n64 = number of double2 vectors per column)
 // r64 = b64 - w64 (w64 may be null: zero); r = (R) r64; rho += <rhat, r>; rr += <r64, r64>. If p is not null (reliable update in the middle of
 // the recurrence): p += r_new - r_old, i.e. the search direction already built from the iterated residual is moved to
 // the true one.
-template <typename R> cudaError_t launch_resid_convert(int64_t n64, const void* b64, const void* w64, void* r64, void* r, const void* rhat, void* p, Scalars* sc, const ColMap& cm, cudaStream_t s);
+template <typename R> cudaError_t launch_resid_convert(int64_t n64, int64_t vh, const void* b64, const void* w64, void* r64, void* r, const void* rhat, void* p, Scalars* sc, const ColMap& cm, cudaStream_t s);
 // dst(R) = src(double), n64 double2 vectors per column
-template <typename R> cudaError_t launch_convert(int64_t n64, const void* src64, void* dst, const ColMap& cm, cudaStream_t s);
+template <typename R> cudaError_t launch_convert(int64_t n64, int64_t vh, const void* src64, void* dst, const ColMap& cm, cudaStream_t s);
 // d = a - b (fp64, n64 double2 vectors per column), out[4c+2] += <d,d>
 cudaError_t launch_sub_norm(int64_t n64, const void* a, const void* b, void* d, double* out, const ColMap& cm, cudaStream_t s);
 
