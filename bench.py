@@ -34,6 +34,37 @@ BYTES_COMPULSORY = 576        # fp32, 12-real: 96 (in, each site once) + 8 x 48 
 BYTES_STREAMING = 1248        # 8 x 96 + 8 x 48 + 96: no neighbour reuse (the QUDA-style "effective bandwidth" model)
 
 
+def kernel_bytes_per_site(clover: bool, twisted: bool, reconstruct: int = 12) -> dict:
+    """Algorithmic (compulsory: every datum once) bytes per parity site and column of every kernel kind of the solver
+    (kinds = include/tmw.h TMW_K_*). fp32 spinor 96 B, fp64 192 B; 8 links: fp32 12-real 384 B (18-real 576),
+    fp64 18-real 1152 B; both chirality blocks of the clover term or its inverse: fp32 288 B, fp64 576 B."""
+    s32, s64 = 96, 192
+    l32, l64 = 8 * 4 * reconstruct, 8 * 144
+    c32, c64 = (288, 576) if clover else (0, 0)
+    cinv32, cinv64 = (c32 * (2 if twisted else 1), c64 * (2 if twisted else 1))  # twisted clover: (C^2+mu^2)^-1 and C
+    return {
+        "hop32": s32 + l32 + s32,
+        "k1_32": s32 + l32 + cinv32 + s32,
+        "k2_32": s32 + l32 + c32 + s32 + s32 + s32,        # in, links, A, aux, out, rhat (the fused <rhat, v>)
+        "k2_32_dots": s32 + l32 + c32 + s32 + s32 + s32,   # the same traffic: <t,s>, <t,t>, <rhat,t>, <rhat,s> ride along
+        "hop64": s64 + l64 + s64,
+        "k1_64": s64 + l64 + cinv64 + s64,
+        "k2_64": s64 + l64 + c64 + s64 + s64,
+        "xpay64": s64 + l64 + s64 + s64,
+        "ainvxpay64": s64 + l64 + cinv64 + s64 + s64,
+        "update_s": 3 * s32,
+        "update_xrp": 8 * s32,                              # x, p, s, t, v read; x, r, p written
+        "acc_y": 2 * s32 + 2 * s64,
+        "resid_convert": 3 * s64 + 2 * s32,                 # bhat, Mhat y, r64 | rhat, r (the p fix-up of a mid-run update adds 3 x 96)
+        "convert": s64 + s32,
+        "dot_norm64": s64,
+        "sub_norm": 3 * s64,
+        "diag64": s64 + cinv64 + s64,
+        "pack_both": 4 * s64,                               # canonical in (both parities), packed out
+        "unpack_both": 4 * s64,
+    }
+
+
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -48,7 +79,11 @@ def parse_args():
     ap.add_argument("--multi-rhs", type=int, default=3,
                     help="columns of the extra tmw_solve_multi / tmw_apply_multi leg (0 or 1: skip); 3 fit at 48^3 x 144")
     ap.add_argument("--cpu-solve", action="store_true",
-                    help="also time the oracle's full-lattice fp64 BiCGStab on this config's source (minutes at 32^3 x 96)")
+                    help="time the oracle's full-lattice fp64 BiCGStab on this config's source to convergence (7 min at 48^3 x 144 on "
+                         "16 cores) instead of the default bounded sample of --cpu-solve-iters iterations")
+    ap.add_argument("--cpu-solve-iters", type=int, default=2, help="iterations of the oracle's BiCGStab in the bounded sample (0: skip)")
+    ap.add_argument("--domains", default="1x2", help="domain-decomposition leg: domains_z x domains_t (e.g. 1x2, 2x2; 1x1: skip)")
+    ap.add_argument("--kernel-reps", type=int, default=20, help="launches per kernel kind in the per-kernel roofline loop (0: skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--skip-solve", action="store_true",
@@ -149,6 +184,18 @@ def time_oracle_sample(U, psi, cfg, n_sites: int, passes: int = 1):
     return time.perf_counter() - t0, int(sites.size) * passes, oracle.num_threads()
 
 
+def config_dict(cfg, args, world: int, step: str) -> dict:
+    """the `config` object of the JSON line: the same keys and values from both arms (the driver compares them)"""
+    L, T = cfg["L"], cfg["T"]
+    Vh = L ** 3 * T // 2
+    return {"workload": cfg["name"], "L": L, "T": T, "m": list(cfg["m"]), "c_sw": cfg["c_sw"], "eps": cfg["eps"],
+            "gauge": "fp32 12-real (fp64 18-real for the outer residual)",
+            "source": "Z2 noise, seed 2" if cfg["source"] == "z2" else "point, origin",
+            "tol": args.tol, "napply": max(2, args.napply // 2 * 2),
+            "parallelism": "replicas" if world > 1 else "single",
+            "l2": "inputs larger than L2 (a parity spinor is %.0f MB, gauge %.0f MB)" % (Vh * 96 / 1e6, Vh * 8 * 48 / 1e6)}
+
+
 def run_reference(args, cfg, rank: int):
     """--impl reference: the oracle timed on the host cores, same metric / unit / config; rank 0 only."""
     if rank != 0:
@@ -172,11 +219,10 @@ def run_reference(args, cfg, rank: int):
     line = {"impl": "reference", "metric": "dslash_gflops", "value": gflops, "unit": "GFLOP/s", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": cfg["name"], "L": L, "T": T, "m": list(cfg["m"]), "c_sw": cfg["c_sw"],
-                       "eps": cfg["eps"], "sample_sites_per_step": n},
+            "config": config_dict(cfg, args, 1, f"{n} sites of oracle.apply_sites per step (the oracle arm has no solve part)"),
             "cpu_baseline": {"value": gflops, "unit": "GFLOP/s", "cores": threads, "kind": "oracle", "sample": sample},
             "e2e": {"value": gflops, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-            "gpu_launches": 0}
+            "step": f"{n} sites of oracle.apply_sites", "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
 
@@ -269,6 +315,7 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
     barrier()
     sampler.start()
     launches0 = ctx.launch_count()
+    counts0 = ctx.kernel_counts()
     t0, t1 = ev(), ev()
     t0.record()
     for _ in range(args.steps):
@@ -277,6 +324,7 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
     barrier()
     sampler.stop_flag.set()
     launches = ctx.launch_count() - launches0
+    counts1 = ctx.kernel_counts()
     total_ms = max_over_ranks(t0.elapsed_time(t1))
     solve_ms = [a.elapsed_time(bb) for a, bb, _, _ in timers]
     dsl_ms = [c.elapsed_time(d) for _, _, c, d in timers]
@@ -288,19 +336,56 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
     t_launch_s = sum(dsl_ms) * 1e-3 / (napply * args.steps)  # this rank's mean launch duration, events on `stream`
     peak, peak_src = load_peaks()
     achieved = BYTES_COMPULSORY * Vh / t_launch_s / 1e9
-    traffic = None  # ncu dram__bytes_read.sum + dram__bytes_write.sum per launch of the hop kernel (profiles/dslash_traffic.csv)
-    tp = os.path.join(ROOT, "profiles", "dslash_traffic.csv")
+    # ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, by kernel kind (profiles/kernel_traffic.csv, one
+    # `ncu --set full` capture per kind; the .md beside it has the commands)
+    traffic_by_kind = {}
+    tp = os.path.join(ROOT, "profiles", "kernel_traffic.csv")
     if os.path.exists(tp):
         import csv
         with open(tp) as f:
             for row in csv.DictReader(f):
-                if row["workload"] == cfg["name"] and row["kernel"] == "hop_f32_12":
-                    traffic = float(row["dram_bytes_per_launch"])
+                if row["workload"] == cfg["name"] and int(row["columns"]) == 1:
+                    traffic_by_kind[row["kind"]] = float(row["dram_bytes_per_launch"])
+    traffic = traffic_by_kind.get("hop32")
     roofline = {"bound": "hbm", "kernel": "dslash_kernel<float,12,EPI_HOP> (fp32 hopping block, A3)",
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
                 "peak_source": peak_src, "bytes_per_site": BYTES_COMPULSORY, "sites_per_launch": Vh,
                 "launch_ms": 1e3 * t_launch_s, "streaming_model_gbs": BYTES_STREAMING * Vh / t_launch_s / 1e9,
                 "frac_of_8TBs_nominal": achieved / 8000.0}
+
+    # ---- the whole solve against the roofline: algorithmic bytes of ONE tmw_solve = (column applications of every kernel
+    # kind the context issued inside the timed region, tmw_kernel_counts) x (bytes per site of that kind) x V_h,
+    # + the solver's memsets and device copies, over solve_ms ----
+    bps = kernel_bytes_per_site(c_sw != 0.0, c_sw != 0.0 and m.imag != 0.0)
+    roofline_solve, roofline_kernels = None, None
+    if not args.skip_solve:
+        per_solve = {k: (counts1[k] - counts0[k]) / args.steps for k in counts1}
+        per_solve["hop32"] -= napply  # the Dslash-only part of the step is not the solve
+        by_kind = {k: per_solve[k] * bps[k] * Vh for k in bps if per_solve.get(k)}
+        other = 2.0 * per_solve["copy_bytes"] + per_solve["memset_bytes"]  # a copy reads and writes
+        solve_bytes = sum(by_kind.values()) + other
+        t_solve = sum(solve_ms) / len(solve_ms) * 1e-3
+        ach = solve_bytes / t_solve / 1e9
+        roofline_solve = {"bound": "hbm", "kernel": "tmw_solve: all kernels of one mixed-precision even-odd BiCGStab solve (A3-A8)",
+                          "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None, "peak_source": peak_src,
+                          "algorithmic_gb": solve_bytes / 1e9, "solve_ms": 1e3 * t_solve,
+                          "column_applications_per_solve": {k: v for k, v in per_solve.items() if v and not k.endswith("_bytes")},
+                          "gb_by_kind": {k: v / 1e9 for k, v in sorted(by_kind.items(), key=lambda kv: -kv[1])},
+                          "memset_and_copy_gb": other / 1e9,
+                          "uncounted": "the 1-thread scalar kernels and the per-iteration 2 KB scalar download (no field traffic)"}
+        # ---- every kernel the solve spends time in, alone: CUDA events around back-to-back launches on the context stream
+        # (tmw_time_kernel), on the vectors the solve left in the workspaces ----
+        if args.kernel_reps > 0:
+            roofline_kernels = {}
+            kinds = ["hop32", "k1_32", "k2_32", "k2_32_dots", "update_s", "update_xrp", "k1_64", "k2_64", "hop32_loadonly"]
+            for kind in kinds:
+                ms = ctx.time_kernel(kind, args.kernel_reps)
+                b = bps["hop32" if kind == "hop32_loadonly" else kind] * Vh
+                a_k = b / (ms * 1e-3) / 1e9
+                roofline_kernels[kind] = {"bound": "hbm", "achieved": a_k, "peak": peak, "unit": "GB/s", "frac": a_k / peak,
+                                          "traffic": traffic_by_kind.get(kind), "launch_ms": ms,
+                                          "bytes_per_site": bps["hop32" if kind == "hop32_loadonly" else kind], "sites_per_launch": Vh,
+                                          "share_of_solve": (per_solve.get(kind, 0.0) * ms / (1e3 * t_solve)) if kind != "hop32_loadonly" else None}
 
     # ---- e2e: the same two calls with HOST buffers (pinned), host<->device copies inside the timed region ----
     e2e = None
@@ -375,6 +460,41 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
         del bm, xm, pm, pm2
         torch.cuda.empty_cache()
 
+    # ---- domain decomposition: the same calls on a context cut into domains on THIS GPU: what the face
+    # pack / copy / interior / exterior split costs when there is no second GPU to gain from (reported beside the undivided
+    # figures, outside the timed step) ----
+    dd = None
+    pz, pt = (int(v) for v in args.domains.lower().split("x"))
+    if pz * pt > 1 and not args.skip_solve:
+        from paper_2201_09004_b200 import domains as dom
+        part = dom.Partition(L, T, pz, pt)
+        dUd = torch.from_numpy(np.asarray(U)).cuda() if U.flags.writeable else torch.from_numpy(np.array(U)).cuda()
+        dctx = tmw.Context(L, T, dUd, m, c_sw, stream=stream, domains_z=pz, domains_t=pt)
+        del dUd
+        torch.cuda.empty_cache()
+        x.copy_(torch.from_numpy(psi_host))
+        dctx.pack(tmw.F32, tmw.EVEN, x, pe)
+        d0, d1, d2 = ev(), ev(), ev()
+        for i in range(2):
+            barrier()
+            d0.record()
+            dinfo = dctx.solve(b, x, args.tol)
+            d1.record()
+            for _ in range(napply // 2):
+                dctx.apply(tmw.D, tmw.ODD, tmw.F32, pe, po)
+            d2.record()
+            torch.cuda.synchronize()
+        ms_hop = max_over_ranks(d1.elapsed_time(d2)) / (napply // 2)
+        dd = {"domains_z": pz, "domains_t": pt, "devices": 1,
+              "dslash_ms": ms_hop, "dslash_gflops": FLOP_PER_SITE * float(Vh) * world / (ms_hop * 1e-3) / 1e9,
+              "dslash_vs_undivided": ms_hop / (dsl_total_ms / (napply * args.steps)),
+              "solve_ms": max_over_ranks(d0.elapsed_time(d1)), "solve_iters": dinfo["iters"], "solve_true_resid": dinfo["true_resid"],
+              "exchange_bytes_per_dslash_fp32": part.exchange_bytes(4), "face_bytes_fp32": {"z": part.face_bytes(dom.Z, 4) if part.cut(dom.Z) else 0,
+                                                                                        "t": part.face_bytes(dom.T_DIR, 4) if part.cut(dom.T_DIR) else 0},
+              "note": "all domains on one GPU: the exchange is a same-device copy; multi-GPU placement unmeasured on hardware"}
+        dctx.destroy()
+        torch.cuda.empty_cache()
+
     # ---- the oracle beside it: rank 0, N = 1 only, a bounded sample of the same workload ----
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -389,30 +509,58 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
                "sample": f"oracle.apply_sites (fp64, hopping + mass of Eq. (2), explicit 4x4 gamma matrices) at {n} "
                          f"evenly spaced sites of the same {L}^3x{T} field, {passes} pass(es), {dt:.1f} s",
                "msites_per_s": ns / dt / 1e6}
-        if args.cpu_solve:
+        # the oracle's BiCGStab beside tmw_solve (the paper's one number for this path is a CPU BiCGStab time):
+        # to convergence with --cpu-solve, else a bounded sample of --cpu-solve-iters iterations (each = 2 D applications +
+        # the recurrences on the full lattice), scaled by the iteration count the full solve needs
+        if (args.cpu_solve or args.cpu_solve_iters > 0) and not args.skip_solve:
             import oracle
-            bsrc = synth.z2_source(L, T, 2) if cfg["source"] == "z2" else synth.point_source(L, T, spin, colour)
-            t0 = time.perf_counter()
-            _, oinfo = oracle.bicgstab(np.asarray(U), bsrc, m, c_sw, tol=args.tol)
-            cpu.update(solve_s=time.perf_counter() - t0, solve_iters=oinfo["iters"], solve_true_resid=oinfo["true_resid"],
-                       solve="oracle.bicgstab (full-lattice fp64 BiCGStab, no preconditioning), incl. its clover-leaf setup")
+            import psutil
+            need_gb = V * (4 * 9 + 54 + 9 * 12) * 16 / 1e9  # gauge + F + 9 spinors (complex128)
+            avail_gb = psutil.virtual_memory().available / 1e9
+            if avail_gb < 1.15 * need_gb:
+                cpu.update(solve_s=None, solve=f"skipped: the oracle's BiCGStab needs {need_gb:.0f} GB of host memory, {avail_gb:.0f} GB available")
+            else:
+                bsrc = synth.z2_source(L, T, 2) if cfg["source"] == "z2" else synth.point_source(L, T, spin, colour)
+                t0 = time.perf_counter()
+                Fo = oracle.field_strength(np.asarray(U)) if c_sw != 0.0 else None
+                t_f = time.perf_counter() - t0
+                t0 = time.perf_counter()
+                if args.cpu_solve:
+                    _, oinfo = oracle.bicgstab(np.asarray(U), bsrc, m, c_sw, tol=args.tol, F=Fo)
+                    dt = time.perf_counter() - t0
+                    cpu.update(solve_s=dt + t_f, solve_iters=oinfo["iters"], solve_true_resid=oinfo["true_resid"], solve_kind="to convergence",
+                               solve="oracle.bicgstab (full-lattice fp64 BiCGStab, no preconditioning) to tol, incl. its clover-leaf setup "
+                                     f"({t_f:.1f} s)")
+                else:
+                    k = args.cpu_solve_iters
+                    _, oinfo = oracle.bicgstab(np.asarray(U), bsrc, m, c_sw, tol=1e-300, max_iter=k, F=Fo)
+                    dt = time.perf_counter() - t0  # k iterations + the closing true-residual application
+                    per_iter = dt / (k + 0.5)
+                    # iterations the oracle needs on this config and source (measured: tests/golden/cfg4_solution_sample.txt
+                    # header for config 4 at 1e-12; BASELINE.md 5 for the others); unknown configs: twice the even-odd count
+                    full_iters = {"cfg4_48x144_clover": 36, "cfg3_32x96_clover": 27, "cfg2_24x64_clover": 23, "cfg1_24x64_tm": 22,
+                                  "cfg0_4x8": 29}.get(cfg["name"], 2 * (info["iters"] or 0))
+                    cpu.update(solve_s=per_iter * full_iters + t_f, solve_kind="bounded sample, scaled", solve_sample_s=dt, solve_sample_iters=k,
+                               solve_iters=full_iters, solve_s_per_iter=per_iter,
+                               solve=f"oracle.bicgstab (full-lattice fp64 BiCGStab, no preconditioning): {k} iterations timed ({dt:.1f} s incl. its "
+                                     f"closing residual application), scaled to the {full_iters} iterations the solve to 1e-10 takes, + its "
+                                     f"clover-leaf setup ({t_f:.1f} s); --cpu-solve runs it to convergence (411 s measured at 48^3 x 144 to "
+                                     "1e-12: profiles/r2_oracle_cfg4_solve.md)")
+                del Fo
 
     ctx.destroy()
     if rank == 0:
         line = {"metric": "dslash_gflops", "value": gflops, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
                 "warmup": max(3, args.warmup), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-                "config": {"workload": cfg["name"], "L": L, "T": T, "m": list(cfg["m"]), "c_sw": c_sw, "eps": cfg["eps"],
-                           "gauge": "fp32 12-real (fp64 18-real for the outer residual)",
-                           "source": "Z2 noise, seed 2" if cfg["source"] == "z2" else "point, origin",
-                           "step": ("SOLVE SKIPPED (profiling run, not a bench value): " if args.skip_solve else
-                                    f"1 tmw_solve(tol={args.tol:g}) + ") + f"{napply} fp32 Dslash applications",
-                           "parallelism": "replicas" if world > 1 else "single",
-                           "l2": "inputs larger than L2 (a parity spinor is %.0f MB, gauge %.0f MB)" % (nb / 1e6, Vh * 8 * 48 / 1e6)},
+                "config": config_dict(cfg, args, world, ""),
+                "step": ("SOLVE SKIPPED (profiling run, not a bench value): " if args.skip_solve else
+                         f"1 tmw_solve(tol={args.tol:g}) + ") + f"{napply} fp32 Dslash applications",
                 "dslash_gsites_per_s": sites / (dsl_total_ms * 1e-3) / 1e9, "dslash_ms": dsl_total_ms / (napply * args.steps),
                 "solve_ms": solve_mean_ms, "solve_iters": info["iters"], "solve_reliable_updates": info["reliable_updates"],
                 "solve_true_resid": info["true_resid"], "setup_ms": setup_ms,
-                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "multi_rhs": multi, "gpu_launches": int(launches),
+                "roofline": roofline, "roofline_solve": roofline_solve, "roofline_kernels": roofline_kernels,
+                "cpu_baseline": cpu, "e2e": e2e, "multi_rhs": multi, "domain_decomposition": dd, "gpu_launches": int(launches),
                 "clocks": sampler.summary()}
         print(json.dumps(line), flush=True)
     if dist is not None:

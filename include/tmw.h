@@ -214,6 +214,53 @@ int tmw_set_debug(tmw_ctx* ctx, int flags);
 /* number of kernel launches this context has issued since creation (bench.py's gpu_launches) */
 long long tmw_launch_count(const tmw_ctx* ctx);
 
+/*
+ * Measurement support (bench.py's roofline objects; DESIGN.md 5 has the algorithmic bytes per site of every kind).
+ * Kernel kinds: the stencil launches by precision and epilogue, the fused BLAS-1 kernels of the BiCGStab recurrences
+ * ("vector operations"), the layout conversions.
+ */
+#define TMW_K_HOP32 0          /* fp32 hopping block H (Eq. (2) hopping part), the benchmarked kernel */
+#define TMW_K_K1_32 1          /* fp32 K1 = A_ee^{-1} H_eo */
+#define TMW_K_K2_32 2          /* fp32 K2 = A_oo - H_oe (+ <rhat, v>) */
+#define TMW_K_K2_32_DOTS 3     /* fp32 K2 with <t,s>, <t,t>, <rhat,t>, <rhat,s> fused */
+#define TMW_K_HOP64 4
+#define TMW_K_K1_64 5          /* fp64 K1 (reliable update) */
+#define TMW_K_K2_64 6          /* fp64 K2 / full-operator half (reliable update, tmw_apply FULL, final residual) */
+#define TMW_K_XPAY64 7         /* fp64 source preparation b_o - H_oe (A_ee^{-1} b_e) */
+#define TMW_K_AINVXPAY64 8     /* fp64 reconstruction x_e = A_ee^{-1} (b_e - H_eo x_o) */
+#define TMW_K_UPDATE_S 9       /* s = r - alpha v */
+#define TMW_K_UPDATE_XRP 10    /* x, r, next p, |r|^2 in one pass */
+#define TMW_K_ACC_Y 11         /* y += x (fp64), x = 0 */
+#define TMW_K_RESID_CONVERT 12 /* r64 = bhat - Mhat y, r = (fp32) r64, <rhat, r>, |r|^2 (, p += r_new - r_old) */
+#define TMW_K_CONVERT 13       /* fp64 -> inner precision */
+#define TMW_K_DOT_NORM64 14    /* |b|^2 of one parity */
+#define TMW_K_SUB_NORM 15      /* fp64 a - b / a + b */
+#define TMW_K_DIAG64 16        /* A_ee^{-1} b_e */
+#define TMW_K_PACK_BOTH 17     /* canonical -> packed, both parities */
+#define TMW_K_UNPACK_BOTH 18   /* packed -> canonical, both parities */
+#define TMW_K_OTHER 19         /* anything else that was counted */
+#define TMW_K_MEMSET_BYTES 20  /* BYTES zeroed by device memsets inside the solver */
+#define TMW_K_COPY_BYTES 21    /* BYTES moved by device-to-device copies inside the solver */
+#define TMW_K_HOP32_LOADONLY 22 /* tmw_time_kernel only: the loads and stores of TMW_K_HOP32 without its arithmetic */
+#define TMW_K_COUNT 23
+
+/*
+ * counts[k] (k < min(n, TMW_K_COUNT)) = how many right-hand-side columns kernels of kind k have been applied to since
+ * tmw_create (a launch on N columns counts N; the two *_BYTES kinds count bytes). Returns TMW_K_COUNT, or TMW_EINVAL.
+ */
+int tmw_kernel_counts(const tmw_ctx* ctx, long long* counts, int n);
+
+/*
+ * Mean duration in milliseconds of `reps` back-to-back launches (after 3 untimed ones) of ONE kernel of the solver, on
+ * the context's own workspace vectors, timed with CUDA events on the context stream: kind = TMW_K_HOP32, K1_32, K2_32,
+ * K2_32_DOTS, K1_64, K2_64, UPDATE_S, UPDATE_XRP, or TMW_K_HOP32_LOADONLY (a kernel that issues exactly the loads and
+ * stores of the fp32 hopping kernel - 8 neighbour spinors, 8 links, one store per site, same indices and launch shape -
+ * and only adds the loaded values up: the memory floor of the access pattern). Single column, TMW_MIXED
+ * contexts without domain decomposition. The vectors hold whatever the last solve left there (run one first); the
+ * results are not meaningful, only the time is. Synchronises the stream.
+ */
+int tmw_time_kernel(tmw_ctx* ctx, int kind, int reps, double* ms);
+
 void tmw_destroy(tmw_ctx* ctx);
 
 /* text of the last error of this context (ctx-owned, valid until the next call); ctx may be NULL for create errors */

@@ -85,6 +85,7 @@ struct tmw_ctx {
   double* red_host;  // pinned
   cudaEvent_t ev0, ev1;
   long long launches;
+  long long kcount[TMW_K_COUNT];  // per kernel kind: column applications (or bytes), see include/tmw.h TMW_K_*
   std::string err;
 };
 
@@ -110,6 +111,23 @@ static int fail_cuda(tmw_ctx* c, cudaError_t e, const char* where) {
     cudaError_t e_ = (call);                                   \
     ctx->launches++;                                           \
     if (e_ != cudaSuccess) return fail_cuda(ctx, e_, #call);   \
+  } while (0)
+// a launch of kernel kind K (TMW_K_*) that works on N right-hand-side columns
+#define LAUNCHK(K, N, call)                                    \
+  do {                                                         \
+    ctx->kcount[K] += (N);                                     \
+    LAUNCH(call);                                              \
+  } while (0)
+// a device memset / device-to-device copy inside the solver (counted in bytes)
+#define MEMSETK(ptr, val, bytes)                               \
+  do {                                                         \
+    ctx->kcount[TMW_K_MEMSET_BYTES] += (long long)(bytes);     \
+    CK(cudaMemsetAsync((ptr), (val), (bytes), ctx->stream));   \
+  } while (0)
+#define COPYK(dst, src, bytes)                                 \
+  do {                                                         \
+    ctx->kcount[TMW_K_COPY_BYTES] += (long long)(bytes);       \
+    CK(cudaMemcpyAsync((dst), (src), (bytes), cudaMemcpyDeviceToDevice, ctx->stream)); \
   } while (0)
 
 static int dev_alloc(tmw_ctx* ctx, void** p, size_t bytes) {
@@ -201,6 +219,18 @@ template <typename R> static int ng_of(const tmw_ctx* c) { return sizeof(R) == 4
 
 // out(par) = epilogue(H in) for the columns of cm (vectors of column c start c spinors after the base pointers);
 // red (if any) is the reduction target of column 0, column c's is red_stride doubles further per column.
+// kernel kind (TMW_K_*) of a stencil launch
+template <typename R> static int stencil_kind(int epi, int red_mode) {
+  const bool f = sizeof(R) == 4;
+  switch (epi) {
+    case EPI_HOP: return f ? TMW_K_HOP32 : TMW_K_HOP64;
+    case EPI_AINV_HOP: return f ? TMW_K_K1_32 : TMW_K_K1_64;
+    case EPI_A_XPAY: return f ? (red_mode == 4 ? TMW_K_K2_32_DOTS : TMW_K_K2_32) : TMW_K_K2_64;
+    case EPI_XPAY: return f ? TMW_K_OTHER : TMW_K_XPAY64;
+    default: return f ? TMW_K_OTHER : TMW_K_AINVXPAY64;
+  }
+}
+
 static inline int dom_behind(const tmw_ctx* c, const Domain& d, int dir) {
   return dir == 0 ? ((d.iz + c->pz - 1) % c->pz) + c->pz * d.it : d.iz + c->pz * ((d.it + c->pt - 1) % c->pt);
 }
@@ -276,6 +306,7 @@ static int dslash_dd(tmw_ctx* ctx, int epi, int par, int dagger, const void* in,
   }
   const int ng = ng_of<R>(ctx);
   const int clv = !ctx->clover ? CL_NONE : (ctx->m_im != 0.0 ? CL_TWISTED : CL_CLOVER);
+  ctx->kcount[stencil_kind<R>(epi, red_mode)] += cm.n;
   for (int k = 0; k < nd; k++) LAUNCH(launch_face_pack(A[k], ng, ctx->dom[k].send, ctx->stream));
   CK(cudaEventRecord(ctx->ev_pack, ctx->stream));
   CK(cudaStreamWaitEvent(ctx->comm, ctx->ev_pack, 0));
@@ -320,11 +351,12 @@ static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, vo
       nr = ((cm.n + 2) / 3 * 3 < (cm.n + 1) / 2 * 2) ? 3 : 2;
     }
   }
-  LAUNCH(launch_dslash(a, ng_of<R>(ctx), epi, !ctx->clover ? CL_NONE : (ctx->m_im != 0.0 ? CL_TWISTED : CL_CLOVER), nr, ctx->stream));
+  LAUNCHK(stencil_kind<R>(epi, red_mode), cm.n, launch_dslash(a, ng_of<R>(ctx), epi, !ctx->clover ? CL_NONE : (ctx->m_im != 0.0 ? CL_TWISTED : CL_CLOVER), nr, ctx->stream));
   return TMW_OK;
 }
 // out = A^{-1} in (inverse) or A in on parity par, one column, fp64 (every domain of a decomposed context)
 static int diag64(tmw_ctx* ctx, int par, int inverse, const void* in, void* out) {
+  ctx->kcount[TMW_K_DIAG64]++;
   if (ctx->dom.empty()) {
     LAUNCH(launch_diag(make_diag<double>(ctx, 0), ctx->g, par, ctx->clover, inverse, in, out, ctx->stream));
     return TMW_OK;
@@ -336,12 +368,14 @@ static int diag64(tmw_ctx* ctx, int par, int inverse, const void* in, void* out)
 }
 // canonical fp64 spinor <-> the packed parity spinors of the context (every domain)
 static int pack_both(tmw_ctx* ctx, int prec, const double* canon, void* pe, void* po) {
+  ctx->kcount[TMW_K_PACK_BOTH]++;
   if (ctx->dom.empty()) { LAUNCH(launch_pack_spinor_both(ctx->g, prec, canon, pe, po, ctx->stream)); return TMW_OK; }
   const size_t lb = (size_t)ctx->vh_loc * 24 * (prec == TMW_F32 ? 4 : 8);
   for (size_t k = 0; k < ctx->dom.size(); k++) LAUNCH(launch_pack_spinor_both(ctx->dom[k].g, prec, canon, (char*)pe + k * lb, (char*)po + k * lb, ctx->stream));
   return TMW_OK;
 }
 static int unpack_both(tmw_ctx* ctx, int prec, const void* pe, const void* po, double* canon) {
+  ctx->kcount[TMW_K_UNPACK_BOTH]++;
   if (ctx->dom.empty()) { LAUNCH(launch_unpack_spinor_both(ctx->g, prec, pe, po, canon, ctx->stream)); return TMW_OK; }
   const size_t lb = (size_t)ctx->vh_loc * 24 * (prec == TMW_F32 ? 4 : 8);
   for (size_t k = 0; k < ctx->dom.size(); k++) LAUNCH(launch_unpack_spinor_both(ctx->dom[k].g, prec, (const char*)pe + k * lb, (const char*)po + k * lb, canon, ctx->stream));
@@ -456,6 +490,7 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
   ctx->clover = (c_sw != 0.0);
   ctx->ng32 = o.reconstruct;
   ctx->launches = 0;
+  memset(ctx->kcount, 0, sizeof(ctx->kcount));
   int rc = TMW_OK;
   // from here on errors must free ctx
 #define CKC(call)                                                       \
@@ -589,6 +624,11 @@ long long tmw_spinor_bytes(const tmw_ctx* ctx, int prec) {
   return (long long)spinor_bytes(ctx, prec);
 }
 long long tmw_launch_count(const tmw_ctx* ctx) { return ctx ? ctx->launches : 0; }
+int tmw_kernel_counts(const tmw_ctx* ctx, long long* counts, int n) {
+  if (!ctx || !counts || n < 0) return TMW_EINVAL;
+  for (int i = 0; i < n && i < TMW_K_COUNT; i++) counts[i] = ctx->kcount[i];
+  return TMW_K_COUNT;
+}
 int tmw_set_location(tmw_ctx* ctx, int location) {
   if (!ctx) return TMW_EINVAL;
   if (location != TMW_DEVICE && location != TMW_HOST) return fail(ctx, TMW_EINVAL, "tmw_set_location: bad location");
@@ -866,12 +906,12 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
   for (int c = 0; c < ncols; c++) if (!cs[c].done) cols_add(act, c);
   if (act.n == 0) return TMW_OK;
   // y = 0, r64 = bhat, r = (R) r64, rhat = r, x = p = v = 0
-  CK(cudaMemsetAsync(W[3], 0, bytes64 * ncols, s));
-  CK(cudaMemsetAsync(x, 0, bytesR * ncols, s));
-  LAUNCH(launch_convert<R>(n64, ctx->vh_loc, W[2], rhat, act, s));
+  MEMSETK(W[3], 0, bytes64 * ncols);
+  MEMSETK(x, 0, bytesR * ncols);
+  LAUNCHK(TMW_K_CONVERT, act.n, launch_convert<R>(n64, ctx->vh_loc, W[2], rhat, act, s));
   memset(h, 0, MAXCOL * sizeof(Scalars));
   if ((rc = push_scalars(ctx))) return rc;
-  LAUNCH(launch_resid_convert<R>(n64, ctx->vh_loc, W[2], nullptr, W[4], r, rhat, nullptr, ctx->sc, act, s));  // r64 = bhat - 0; rho = <rhat,r>; rr = |r64|^2
+  LAUNCHK(TMW_K_RESID_CONVERT, act.n, launch_resid_convert<R>(n64, ctx->vh_loc, W[2], nullptr, W[4], r, rhat, nullptr, ctx->sc, act, s));  // r64 = bhat - 0; rho = <rhat,r>; rr = |r64|^2
   if ((rc = fetch_scalars(ctx))) return rc;
   for (int i = 0; i < act.n; i++) {
     const int c = act.col[i];
@@ -882,7 +922,7 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
   }
   if ((rc = push_scalars(ctx))) return rc;
   // p = r for the first iteration; later p comes out of update_xrp (v is written by the first K2 before it is read)
-  for (int i = 0; i < act.n; i++) CK(cudaMemcpyAsync(colp(p, act.col[i], bytesR), colp(r, act.col[i], bytesR), bytesR, cudaMemcpyDeviceToDevice, s));
+  for (int i = 0; i < act.n; i++) COPYK(colp(p, act.col[i], bytesR), colp(r, act.col[i], bytesR), bytesR);
   const int max_iter = ctx->opt.max_iter;
   for (int k = 1; k <= max_iter; k++) {
     act.n = 0;
@@ -891,10 +931,10 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
     LAUNCH(launch_sc_begin_iter(ctx->sc, act, s));
     if ((rc = schur<R>(ctx, 0, p, v, tmp, act, 1, rhat, red_rhat_v, SCD))) return rc;
     LAUNCH(launch_sc_alpha(ctx->sc, act, s));
-    LAUNCH(launch_update_s<R>(nR, sv, r, v, ctx->sc, act, s));
+    LAUNCHK(TMW_K_UPDATE_S, act.n, launch_update_s<R>(nR, sv, r, v, ctx->sc, act, s));
     if ((rc = schur<R>(ctx, 0, sv, t, tmp, act, 4, rhat, red_ts, SCD))) return rc;  // <t,s>, <t,t>, <rhat,t>, <rhat,s>
     LAUNCH(launch_sc_omega(ctx->sc, act, s));                                        // omega, rho' = <rhat, s - omega t>, beta
-    LAUNCH(launch_update_xrp<R>(nR, x, r, p, sv, t, v, ctx->sc, act, s));             // x, r, and p of the next iteration
+    LAUNCHK(TMW_K_UPDATE_XRP, act.n, launch_update_xrp<R>(nR, x, r, p, sv, t, v, ctx->sc, act, s));             // x, r, and p of the next iteration
     if ((rc = fetch_scalars(ctx))) return rc;
     ColMap upd, brk;  // columns that take a reliable update now / whose iterate is corrupted
     upd.n = brk.n = 0;
@@ -923,8 +963,8 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
       ColMap good;
       good.n = 0;
       for (int i = 0; i < upd.n; i++) if (!broken[upd.col[i]]) cols_add(good, upd.col[i]);
-      if (good.n > 0) LAUNCH(launch_acc_y<R>(n64, ctx->vh_loc, W[3], x, good, s));
-      for (int i = 0; i < brk.n; i++) CK(cudaMemsetAsync(colp(x, brk.col[i], bytesR), 0, bytesR, s));
+      if (good.n > 0) LAUNCHK(TMW_K_ACC_Y, good.n, launch_acc_y<R>(n64, ctx->vh_loc, W[3], x, good, s));
+      for (int i = 0; i < brk.n; i++) MEMSETK(colp(x, brk.col[i], bytesR), 0, bytesR);
       if ((rc = schur<double>(ctx, 0, W[3], W[6], W[5], upd))) return rc;
       for (int i = 0; i < upd.n; i++) {
         const int c = upd.col[i];
@@ -934,7 +974,7 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
       }
       if ((rc = push_scalars(ctx))) return rc;
       // r := true residual; the search direction update_xrp already built from the iterated r moves with it
-      LAUNCH(launch_resid_convert<R>(n64, ctx->vh_loc, W[2], W[6], W[4], r, rhat, p, ctx->sc, upd, s));
+      LAUNCHK(TMW_K_RESID_CONVERT, upd.n, launch_resid_convert<R>(n64, ctx->vh_loc, W[2], W[6], W[4], r, rhat, p, ctx->sc, upd, s));
       if ((rc = fetch_scalars(ctx))) return rc;
       for (int i = 0; i < upd.n; i++) {
         const int c = upd.col[i];
@@ -968,9 +1008,9 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
       for (int i = 0; i < rst.n; i++) {
         const int c = rst.col[i];
         if (!broken[c] && cs[c].rnorm <= cs[c].r_upd) cols_add(keep, c);
-        else CK(cudaMemsetAsync(colp(x, c, bytesR), 0, bytesR, s));
+        else MEMSETK(colp(x, c, bytesR), 0, bytesR);
       }
-      if (keep.n > 0) LAUNCH(launch_acc_y<R>(n64, ctx->vh_loc, W[3], x, keep, s));
+      if (keep.n > 0) LAUNCHK(TMW_K_ACC_Y, keep.n, launch_acc_y<R>(n64, ctx->vh_loc, W[3], x, keep, s));
       if ((rc = schur<double>(ctx, 0, W[3], W[6], W[5], rst))) return rc;
       for (int i = 0; i < rst.n; i++) {
         const int c = rst.col[i];
@@ -978,11 +1018,11 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
         reset_recurrence(&h[c]);
       }
       if ((rc = push_scalars(ctx))) return rc;
-      LAUNCH(launch_sub_norm(n64, W[2], W[6], W[4], ctx->red, rst, s));  // r64 = bhat - Mhat y (norm discarded)
-      LAUNCH(launch_convert<R>(n64, ctx->vh_loc, W[4], rhat, rst, s));
-      LAUNCH(launch_resid_convert<R>(n64, ctx->vh_loc, W[2], W[6], W[4], r, rhat, nullptr, ctx->sc, rst, s));
+      LAUNCHK(TMW_K_SUB_NORM, rst.n, launch_sub_norm(n64, W[2], W[6], W[4], ctx->red, rst, s));  // r64 = bhat - Mhat y (norm discarded)
+      LAUNCHK(TMW_K_CONVERT, rst.n, launch_convert<R>(n64, ctx->vh_loc, W[4], rhat, rst, s));
+      LAUNCHK(TMW_K_RESID_CONVERT, rst.n, launch_resid_convert<R>(n64, ctx->vh_loc, W[2], W[6], W[4], r, rhat, nullptr, ctx->sc, rst, s));
       for (int i = 0; i < rst.n; i++)  // p = r
-        CK(cudaMemcpyAsync(colp(p, rst.col[i], bytesR), colp(r, rst.col[i], bytesR), bytesR, cudaMemcpyDeviceToDevice, s));
+        COPYK(colp(p, rst.col[i], bytesR), colp(r, rst.col[i], bytesR), bytesR);
       if ((rc = fetch_scalars(ctx))) return rc;
       for (int i = 0; i < rst.n; i++) {
         const int c = rst.col[i];
@@ -1038,7 +1078,7 @@ int solve_gcr(tmw_ctx* ctx, int c, double tol, ColState& q) {
     // true residual r64 = bhat - Mhat y (W[6] holds Mhat y), r = (R) r64, |r64|^2
     memset(h, 0, MAXCOL * sizeof(Scalars));
     if ((rc = push_scalars(ctx))) return rc;
-    LAUNCH(launch_resid_convert<R>(n64, ctx->vh_loc, W[2], W[6], W[4], X[0], X[1], nullptr, ctx->sc, one, s));
+    LAUNCHK(TMW_K_RESID_CONVERT, one.n, launch_resid_convert<R>(n64, ctx->vh_loc, W[2], W[6], W[4], X[0], X[1], nullptr, ctx->sc, one, s));
     if ((rc = fetch_scalars(ctx))) return rc;
     q.rnorm = q.maxr = sqrt(h[c].rr);
     q.iter_resid = q.rnorm / q.bnorm;
@@ -1063,7 +1103,7 @@ int solve_gcr(tmw_ctx* ctx, int c, double tol, ColState& q) {
       if (rn <= tol * q.bnorm || rn < ctx->opt.delta * q.maxr) break;
     }
     // restart: y += x, Mhat y in fp64
-    LAUNCH(launch_acc_y<R>(n64, ctx->vh_loc, W[3], X[6], one, s));
+    LAUNCHK(TMW_K_ACC_Y, one.n, launch_acc_y<R>(n64, ctx->vh_loc, W[3], X[6], one, s));
     if ((rc = schur<double>(ctx, 0, W[3], W[6], W[5], one))) return rc;
     q.updates++;
   }
@@ -1142,8 +1182,8 @@ static int solve_chunk(tmw_ctx* ctx, int nrhs, const double* b, double* x, doubl
     if ((rc = pack_both(ctx, 1, (const double*)colp(cb, c, cbytes), colp(W[0], c, b64), colp(W[1], c, b64)))) return rc;
   }
   CK(cudaMemsetAsync(ctx->red, 0, 4 * MAXCOL * sizeof(double), s));
-  LAUNCH(launch_dot_norm<double>(n64, nullptr, W[0], ctx->red, all, s));
-  LAUNCH(launch_dot_norm<double>(n64, nullptr, W[1], ctx->red, all, s));
+  LAUNCHK(TMW_K_DOT_NORM64, all.n, launch_dot_norm<double>(n64, nullptr, W[0], ctx->red, all, s));
+  LAUNCHK(TMW_K_DOT_NORM64, all.n, launch_dot_norm<double>(n64, nullptr, W[1], ctx->red, all, s));
   if ((rc = fetch_red(ctx))) return rc;
   ColMap nz;  // columns with b != 0
   nz.n = 0;
@@ -1184,14 +1224,14 @@ static int solve_chunk(tmw_ctx* ctx, int nrhs, const double* b, double* x, doubl
         up0[c] = cs[c].updates;
       }
       if ((rc = full_apply64(ctx, 0, W[7], W[3], W[8], W[9], bad))) return rc;        // D x
-      LAUNCH(launch_sub_norm(n64, W[10], W[8], W[0], ctx->red, bad, s));              // b := b - D x (norm discarded)
-      LAUNCH(launch_sub_norm(n64, W[11], W[9], W[1], ctx->red, bad, s));
+      LAUNCHK(TMW_K_SUB_NORM, bad.n, launch_sub_norm(n64, W[10], W[8], W[0], ctx->red, bad, s));              // b := b - D x (norm discarded)
+      LAUNCHK(TMW_K_SUB_NORM, bad.n, launch_sub_norm(n64, W[11], W[9], W[1], ctx->red, bad, s));
       for (int c = 0; c < nrhs; c++) cs[c].done = true;
       for (int i = 0; i < bad.n; i++) cs[bad.col[i]].done = false;
       status = solve_packed(ctx, nrhs, bad, tol, cs);                                 // e, to the same absolute target tol |b|
       if (status != TMW_OK && status != TMW_ENOCONV) return status;
-      LAUNCH(launch_add64(n64, W[7], W[12], bad, s));                                 // x = x + e
-      LAUNCH(launch_add64(n64, W[3], W[13], bad, s));
+      LAUNCHK(TMW_K_SUB_NORM, bad.n, launch_add64(n64, W[7], W[12], bad, s));                                 // x = x + e
+      LAUNCHK(TMW_K_SUB_NORM, bad.n, launch_add64(n64, W[3], W[13], bad, s));
       for (int i = 0; i < bad.n; i++) {
         const int c = bad.col[i];
         CK(cudaMemcpyAsync(colp(W[0], c, b64), colp(W[10], c, b64), b64, cudaMemcpyDeviceToDevice, s));
@@ -1285,4 +1325,52 @@ extern "C" int tmw_solve_multi(tmw_ctx* ctx, int nrhs, const double* b, double* 
 
 extern "C" int tmw_solve(tmw_ctx* ctx, const double* b, double* x, double tol, tmw_solve_info* info) {
   return tmw_solve_multi(ctx, 1, b, x, tol, info);
+}
+
+extern "C" int tmw_time_kernel(tmw_ctx* ctx, int kind, int reps, double* ms) {
+  if (!ctx) return TMW_EINVAL;
+  if (!ms || reps < 1) return fail(ctx, TMW_EINVAL, "tmw_time_kernel: bad argument");
+  if (ctx->opt.precision != TMW_MIXED || !ctx->dom.empty()) return fail(ctx, TMW_EINVAL, "tmw_time_kernel: needs a TMW_MIXED context without domain decomposition");
+  int rc;
+  if ((rc = need_w64(ctx, 8))) return rc;
+  if ((rc = need_w32(ctx, 8, TMW_F32))) return rc;
+  void** W = ctx->w64;
+  void** X = ctx->w32;
+  const ColMap one = cols_first(1);
+  const int64_t nR = (int64_t)ctx->g.Vh * 24 * 4 / 16;
+  const int SCD = (int)(sizeof(Scalars) / sizeof(double));
+  double* red_rhat_v = (double*)((char*)ctx->sc + offsetof(Scalars, rhat_v));
+  double* red_ts = (double*)((char*)ctx->sc + offsetof(Scalars, ts));
+  long long saved[TMW_K_COUNT];
+  memcpy(saved, ctx->kcount, sizeof(saved));
+  const long long launches0 = ctx->launches;
+  auto run = [&]() -> int {
+    switch (kind) {
+      case TMW_K_HOP32: return dslash<float>(ctx, EPI_HOP, 1, 0, X[7], X[3], nullptr, 1.0, one);
+      case TMW_K_K1_32: return dslash<float>(ctx, EPI_AINV_HOP, 0, 0, X[2], X[7], nullptr, 1.0, one);
+      case TMW_K_K2_32: return dslash<float>(ctx, EPI_A_XPAY, 1, 0, X[7], X[3], X[2], -1.0, one, 1, X[1], red_rhat_v, SCD);
+      case TMW_K_K2_32_DOTS: return dslash<float>(ctx, EPI_A_XPAY, 1, 0, X[7], X[5], X[4], -1.0, one, 4, X[1], red_ts, SCD);
+      case TMW_K_K1_64: return dslash<double>(ctx, EPI_AINV_HOP, 0, 0, W[3], W[5], nullptr, 1.0, one);
+      case TMW_K_K2_64: return dslash<double>(ctx, EPI_A_XPAY, 1, 0, W[5], W[6], W[3], -1.0, one);
+      case TMW_K_UPDATE_S: LAUNCH(launch_update_s<float>(nR, X[4], X[0], X[3], ctx->sc, one, ctx->stream)); return TMW_OK;
+      case TMW_K_UPDATE_XRP: LAUNCH(launch_update_xrp<float>(nR, X[6], X[0], X[2], X[4], X[5], X[3], ctx->sc, one, ctx->stream)); return TMW_OK;
+      case TMW_K_HOP32_LOADONLY: {
+        DslashArgs<float> a = make_args<float>(ctx, 1, 0, X[7], X[3], nullptr, 1.0, one);
+        LAUNCH(launch_hop_loadonly(a, ctx->ng32, ctx->stream));
+        return TMW_OK;
+      }
+    }
+    return fail(ctx, TMW_EINVAL, "tmw_time_kernel: this kind cannot be timed alone");
+  };
+  for (int i = 0; i < 3; i++) if ((rc = run())) return rc;
+  CK(cudaEventRecord(ctx->ev0, ctx->stream));
+  for (int i = 0; i < reps; i++) if ((rc = run())) return rc;
+  CK(cudaEventRecord(ctx->ev1, ctx->stream));
+  CK(cudaStreamSynchronize(ctx->stream));
+  float t = 0;
+  CK(cudaEventElapsedTime(&t, ctx->ev0, ctx->ev1));
+  *ms = (double)t / reps;
+  memcpy(ctx->kcount, saved, sizeof(saved));  // probing does not count as work of the path
+  ctx->launches = launches0;
+  return TMW_OK;
 }

@@ -22,6 +22,46 @@ cudaError_t launch_dslash(const DslashArgs<float>& a, int ng, int epi, int clove
   }
   return cudaErrorInvalidValue;
 }
+// The memory floor of the hopping kernel's access pattern (tmw_time_kernel, TMW_K_HOP32_LOADONLY): the same 8 neighbour
+// spinors (6 float4 each), 8 links (NG/4 float4 each, same cache policy), one 6-float4 store per site, same indices and
+// launch shape, but the loaded vectors are only added up.
+template <int NG> __global__ void __launch_bounds__(128, 4) hop_loadonly_kernel(const DslashArgs<float> a) {
+  Site s;
+  if (!thread_site<128>(a.g, blockIdx.x, s)) return;
+  const Nbr n = neighbours(a.g, a.par, s);
+  const int NPG = Planes<float, NG>::N;
+  const int64_t Vh = a.g.Vh;
+  float4 acc[6];
+#pragma unroll
+  for (int k = 0; k < 6; k++) acc[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+  for (int mu = 0; mu < 4; mu++) {
+#pragma unroll
+    for (int dir = 0; dir < 2; dir++) {
+      const int nb = dir ? n.bwd[mu] : n.fwd[mu];
+      const float4* u = (const float4*)a.U[dir ? 1 - a.par : a.par] + (int64_t)mu * NPG * Vh + (dir ? nb : s.cb);
+      const float4* p = (const float4*)a.in + nb;
+#pragma unroll
+      for (int k = 0; k < NPG; k++) {
+        const float4 q = ldv_s(u + k * Vh);
+        acc[k].x += q.x; acc[k].y += q.y; acc[k].z += q.z; acc[k].w += q.w;
+      }
+#pragma unroll
+      for (int k = 0; k < 6; k++) {
+        const float4 q = ldv(p + k * Vh);
+        acc[k].x += q.x; acc[k].y += q.y; acc[k].z += q.z; acc[k].w += q.w;
+      }
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < 6; k++) stv_s((float4*)a.out + k * Vh + s.cb, acc[k]);
+}
+cudaError_t launch_hop_loadonly(const DslashArgs<float>& a, int ng, cudaStream_t s) {
+  const unsigned grid = (unsigned)((a.g.Vh + 127) / 128);
+  if (ng == 12) hop_loadonly_kernel<12><<<grid, 128, 0, s>>>(a);
+  else hop_loadonly_kernel<18><<<grid, 128, 0, s>>>(a);
+  return cudaGetLastError();
+}
 cudaError_t launch_diag(const Diag<float>& d, const Geom& g, int par, bool clover, int inverse, const void* in, void* out, cudaStream_t s) {
   return launch_diag_t<float>(d, g, par, clover, inverse, in, out, s);
 }

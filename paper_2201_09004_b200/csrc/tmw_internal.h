@@ -9,6 +9,9 @@ namespace tmw {
 // nr = right-hand-side columns per thread (fp32: 1..4; fp64: always 1)
 cudaError_t launch_dslash(const DslashArgs<float>& a, int ng, int epi, int clover, int nr, cudaStream_t s);
 cudaError_t launch_dslash(const DslashArgs<double>& a, int ng, int epi, int clover, int nr, cudaStream_t s);
+// loads and stores of the fp32 hopping kernel without its arithmetic (measurement: tmw_time_kernel)
+cudaError_t launch_hop_loadonly(const DslashArgs<float>& a, int ng, cudaStream_t s);
+
 // ---- domain decomposition (tmw_dd_f32.cu / tmw_dd_f64.cu) ----
 // a describes ONE domain (local geometry and fields, a.dd its cuts and receive buffers). pass 0: interior (all sites, the
 // hops through a cut skipped, sites on a cut left raw in a.out); pass 1: exterior (the sites on a cut: + ghost terms,

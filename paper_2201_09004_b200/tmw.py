@@ -25,10 +25,15 @@ D, DDAG, G5D = 0, 1, 2
 FULL, EVEN, ODD = 0, 1, 2
 F32, F64 = 0, 1
 DEBUG_FORCE_PIVOT, DEBUG_NO_CHUNK = 1, 2
+# kernel kinds of tmw_kernel_counts / tmw_time_kernel (include/tmw.h TMW_K_*)
+KINDS = ["hop32", "k1_32", "k2_32", "k2_32_dots", "hop64", "k1_64", "k2_64", "xpay64", "ainvxpay64", "update_s", "update_xrp",
+         "acc_y", "resid_convert", "convert", "dot_norm64", "sub_norm", "diag64", "pack_both", "unpack_both", "other",
+         "memset_bytes", "copy_bytes", "hop32_loadonly"]
 
 EXPORTS = ["tmw_create", "tmw_apply", "tmw_apply_schur", "tmw_solve", "tmw_apply_multi", "tmw_apply_schur_multi",
            "tmw_solve_multi", "tmw_cheb_apply", "tmw_spinor_bytes", "tmw_pack", "tmw_unpack",
-           "tmw_get_clover", "tmw_set_location", "tmw_set_debug", "tmw_launch_count", "tmw_destroy", "tmw_last_error"]
+           "tmw_get_clover", "tmw_set_location", "tmw_set_debug", "tmw_launch_count", "tmw_kernel_counts",
+           "tmw_time_kernel", "tmw_destroy", "tmw_last_error"]
 
 
 class tmw_complex(ctypes.Structure):
@@ -97,6 +102,10 @@ def load():
     lib.tmw_set_debug.restype = I
     lib.tmw_launch_count.argtypes = [P]
     lib.tmw_launch_count.restype = LL
+    lib.tmw_kernel_counts.argtypes = [P, ctypes.POINTER(LL), I]
+    lib.tmw_kernel_counts.restype = I
+    lib.tmw_time_kernel.argtypes = [P, I, I, ctypes.POINTER(DBL)]
+    lib.tmw_time_kernel.restype = I
     lib.tmw_destroy.argtypes = [P]
     lib.tmw_destroy.restype = None
     lib.tmw_last_error.argtypes = [P]
@@ -196,6 +205,18 @@ class Context:
 
     def launch_count(self) -> int:
         return int(self._lib.tmw_launch_count(self._h))
+
+    def kernel_counts(self) -> dict:
+        buf = (ctypes.c_longlong * len(KINDS))()
+        n = self._lib.tmw_kernel_counts(self._h, buf, len(KINDS))
+        if n != len(KINDS):
+            raise TmwError(n, "tmw_kernel_counts: kind table out of date")
+        return {k: int(v) for k, v in zip(KINDS, buf)}
+
+    def time_kernel(self, kind: str, reps: int = 20) -> float:
+        ms = ctypes.c_double(0.0)
+        self._check(self._lib.tmw_time_kernel(self._h, KINDS.index(kind), reps, ctypes.byref(ms)))
+        return ms.value
 
     def destroy(self):
         if getattr(self, "_h", None):
