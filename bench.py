@@ -380,8 +380,8 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
             kinds = ["hop32", "k1_32", "k2_32", "k2_32_dots", "update_s", "update_xrp", "k1_64", "k2_64", "hop32_loadonly"]
             for kind in kinds:
                 ms = ctx.time_kernel(kind, args.kernel_reps)
-                b = bps["hop32" if kind == "hop32_loadonly" else kind] * Vh
-                a_k = b / (ms * 1e-3) / 1e9
+                nbytes = bps["hop32" if kind == "hop32_loadonly" else kind] * Vh
+                a_k = nbytes / (ms * 1e-3) / 1e9
                 roofline_kernels[kind] = {"bound": "hbm", "achieved": a_k, "peak": peak, "unit": "GB/s", "frac": a_k / peak,
                                           "traffic": traffic_by_kind.get(kind), "launch_ms": ms,
                                           "bytes_per_site": bps["hop32" if kind == "hop32_loadonly" else kind], "sites_per_launch": Vh,

@@ -27,6 +27,7 @@ struct NvtxRange {
 using namespace tmw;
 
 enum { NW64 = 14 };
+enum { NSLAB = 24 };  // most t-slabs of the pipelined host-pointer tmw_apply
 
 // One domain of a domain-decomposed context: a sub-lattice L x L x (L/Pz) x (T/Pt) with its own packed
 // gauge and clover fields and the send / receive buffers of its cuts. Domain (iz, it) has index iz + Pz * it; every
@@ -66,6 +67,8 @@ struct tmw_ctx {
   int vh_loc;        // sites per parity of one domain (= g.Vh without decomposition)
   int ghost_cols;    // columns the send / receive buffers hold
   void* dd_tmp;      // scratch output spinors for stencil launches that keep only a reduction
+  cudaStream_t h2d, d2h;             // copy streams of the pipelined host-pointer tmw_apply (lazily created)
+  cudaEvent_t ev_in[NSLAB], ev_out[NSLAB]; // per t-slab: input arrived / output ready
   cudaStream_t comm; // the halo exchange runs here, beside the interior pass on `stream`
   cudaEvent_t ev_pack, ev_comm;
   // lazily allocated workspaces, each sized for ws_cols right-hand-side columns (column c at c * spinor bytes)
@@ -210,6 +213,8 @@ static DslashArgs<R> make_args(const tmw_ctx* c, int par, int dagger, const void
   a.red = nullptr;
   a.ncol = cm.n;
   a.ngroups = 1;
+  a.sb0 = 0;
+  a.cb_end = a.g.Vh;
   a.cstride = (int)((int64_t)c->g.Vh * 24 * (int64_t)sizeof(R) / 16);
   a.red_stride = 0;
   for (int i = 0; i < MAXCOL; i++) a.col[i] = cm.col[i];
@@ -328,9 +333,10 @@ static int dslash_dd(tmw_ctx* ctx, int epi, int par, int dagger, const void* in,
   return TMW_OK;
 }
 
+// cb0, cb1 (optional): restrict the launch to the output sites with checkerboard index in [cb0, cb1), cb0 a multiple of 128
 template <typename R>
 static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, void* out, const void* aux, double sgn, const ColMap& cm,
-                  int red_mode = 0, const void* dotv = nullptr, double* red = nullptr, int red_stride = 0, int g5 = 0) {
+                  int red_mode = 0, const void* dotv = nullptr, double* red = nullptr, int red_stride = 0, int g5 = 0, int cb0 = 0, int cb1 = -1) {
   for (int i = 0; i < cm.n; i++)  // the kernels add column * cstride to a 32-bit site index
     if (((int64_t)cm.col[i] + 1) * ((int64_t)ctx->g.Vh * 24 * (int64_t)sizeof(R) / 16) >= ((int64_t)1 << 31))
       return fail(ctx, TMW_EINVAL, "lattice too large for this many right-hand-side columns in one call");
@@ -341,6 +347,7 @@ static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, vo
   a.dotv = dotv;
   a.red = red;
   a.red_stride = red_stride;
+  if (cb1 >= 0) { a.sb0 = cb0 / 128; a.cb_end = cb1; }
   // columns per thread: as even a split of the columns into groups of at most nr32 as possible
   int nr = 1;
   if (sizeof(R) == 4 && cm.n > 1) {
@@ -440,6 +447,12 @@ void tmw_destroy(tmw_ctx* ctx) {
   if (ctx->red_host) cudaFreeHost(ctx->red_host);
   if (ctx->gs_host) cudaFreeHost(ctx->gs_host);
   if (ctx->comm) { cudaStreamSynchronize(ctx->comm); cudaStreamDestroy(ctx->comm); }
+  if (ctx->h2d) { cudaStreamSynchronize(ctx->h2d); cudaStreamDestroy(ctx->h2d); }
+  if (ctx->d2h) { cudaStreamSynchronize(ctx->d2h); cudaStreamDestroy(ctx->d2h); }
+  for (int i = 0; i < NSLAB; i++) {
+    if (ctx->ev_in[i]) cudaEventDestroy(ctx->ev_in[i]);
+    if (ctx->ev_out[i]) cudaEventDestroy(ctx->ev_out[i]);
+  }
   if (ctx->ev_pack) cudaEventDestroy(ctx->ev_pack);
   if (ctx->ev_comm) cudaEventDestroy(ctx->ev_comm);
   if (ctx->ev0) cudaEventDestroy(ctx->ev0);
@@ -732,6 +745,71 @@ static int full_apply64(tmw_ctx* ctx, int dagger, const void* in_e, const void* 
   return dslash<double>(ctx, EPI_A_XPAY, 1, dagger, in_e, out_o, in_o, 1.0, cm, 0, nullptr, nullptr, 0, g5);
 }
 
+// tmw_apply FULL with HOST pointers, one column: the canonical spinor is cut into S t-slabs (contiguous both in the
+// canonical array and in checkerboard order) and three streams work on them at once, so that both PCIe directions are
+// busy: h2d uploads slab after slab (the LAST slab first: the periodic t-neighbour of slab 0); the context stream packs
+// every slab as it arrives and applies the operator to slab k as soon as slabs k-1, k, k+1 are there, then unpacks it;
+// d2h downloads every finished slab. Only the last two slabs cannot overlap their upload.
+static int apply_full_host_pipelined(tmw_ctx* ctx, int dagger, int g5, const double* in, double* out) {
+  const int T = ctx->g.T;
+  int S = 1;
+  for (int d = 2; d <= NSLAB && d <= T; d++) if (T % d == 0) S = d;  // as many slabs as there are events: a short tail
+  if (S < 3) S = 1;
+  const int dt = T / S;
+  if (!ctx->h2d) {
+    CK(cudaStreamCreateWithFlags(&ctx->h2d, cudaStreamNonBlocking));
+    CK(cudaStreamCreateWithFlags(&ctx->d2h, cudaStreamNonBlocking));
+    for (int i = 0; i < NSLAB; i++) {
+      CK(cudaEventCreateWithFlags(&ctx->ev_in[i], cudaEventDisableTiming));
+      CK(cudaEventCreateWithFlags(&ctx->ev_out[i], cudaEventDisableTiming));
+    }
+  }
+  int rc;
+  void** W = ctx->w64;
+  const ColMap one = cols_first(1);
+  const int64_t slice = (int64_t)ctx->g.L * ctx->g.L * ctx->g.L;  // lexicographic sites per time slice
+  const size_t slab_bytes = (size_t)slice * dt * 24 * 8;
+  const int slab_cb = ctx->g.st * dt;                            // checkerboard sites per parity and slab
+  double* cin = (double*)ctx->canon[0];
+  double* cout = (double*)ctx->canon[1];
+  // the copy streams start after whatever the context stream still has queued on the staging buffers
+  CK(cudaEventRecord(ctx->ev0, ctx->stream));
+  CK(cudaStreamWaitEvent(ctx->h2d, ctx->ev0, 0));
+  CK(cudaStreamWaitEvent(ctx->d2h, ctx->ev0, 0));
+  for (int j = 0; j < S; j++) {  // upload order: S-1, 0, 1, ..., S-2
+    const int k = (j + S - 1) % S;
+    CK(cudaMemcpyAsync((char*)cin + k * slab_bytes, (const char*)in + k * slab_bytes, slab_bytes, cudaMemcpyHostToDevice, ctx->h2d));
+    CK(cudaEventRecord(ctx->ev_in[k], ctx->h2d));
+  }
+  auto pack_slab = [&](int k) -> int {
+    CK(cudaStreamWaitEvent(ctx->stream, ctx->ev_in[k], 0));
+    ctx->kcount[TMW_K_PACK_BOTH]++;
+    LAUNCH(launch_pack_spinor_both(ctx->g, 1, cin, W[0], W[1], ctx->stream, k * slice * dt, (k + 1) * slice * dt));
+    return TMW_OK;
+  };
+  auto do_slab = [&](int k) -> int {
+    const int c0 = k * slab_cb, c1 = (k + 1) * slab_cb;
+    int r = dslash<double>(ctx, EPI_A_XPAY, 0, dagger, W[1], W[2], W[0], 1.0, one, 0, nullptr, nullptr, 0, g5, c0, c1);
+    if (!r) r = dslash<double>(ctx, EPI_A_XPAY, 1, dagger, W[0], W[3], W[1], 1.0, one, 0, nullptr, nullptr, 0, g5, c0, c1);
+    if (r) return r;
+    ctx->kcount[TMW_K_UNPACK_BOTH]++;
+    LAUNCH(launch_unpack_spinor_both(ctx->g, 1, W[2], W[3], cout, ctx->stream, k * slice * dt, (k + 1) * slice * dt));
+    CK(cudaEventRecord(ctx->ev_out[k], ctx->stream));
+    CK(cudaStreamWaitEvent(ctx->d2h, ctx->ev_out[k], 0));
+    CK(cudaMemcpyAsync((char*)out + k * slab_bytes, (const char*)cout + k * slab_bytes, slab_bytes, cudaMemcpyDeviceToHost, ctx->d2h));
+    return TMW_OK;
+  };
+  if ((rc = pack_slab(S - 1))) return rc;
+  if (S > 1 && (rc = pack_slab(0))) return rc;
+  for (int k = 0; k < S; k++) {
+    if (k + 1 < S - 1 && (rc = pack_slab(k + 1))) return rc;  // slab S-1 is already packed
+    if ((rc = do_slab(k))) return rc;
+  }
+  CK(cudaStreamSynchronize(ctx->d2h));
+  CK(cudaStreamSynchronize(ctx->stream));
+  return TMW_OK;
+}
+
 extern "C" int tmw_apply_multi(tmw_ctx* ctx, int op, int parity, int prec, int nrhs, const void* in, void* out) {
   NvtxRange nvtx("tmw_apply");
   if (!ctx) return TMW_EINVAL;
@@ -755,6 +833,7 @@ extern "C" int tmw_apply_multi(tmw_ctx* ctx, int op, int parity, int prec, int n
   if (ctx->opt.location == TMW_HOST) {
     rc = need_canon(ctx);
     if (rc) return rc;
+    if (nrhs == 1 && ctx->dom.empty() && !ctx->g.tiled && ctx->g.st % 128 == 0) return apply_full_host_pipelined(ctx, dagger, g5, (const double*)in, (double*)out);
     CK(cudaMemcpyAsync(ctx->canon[0], in, cbytes * nrhs, cudaMemcpyHostToDevice, ctx->stream));
     cin = (const double*)ctx->canon[0];
     cout = (double*)ctx->canon[1];

@@ -577,6 +577,9 @@ template <typename R> struct DslashArgs {
   // are loaded once for the NR columns); CTAs of the ngroups = ceil(ncol/NR) slot groups of one site block are
   // adjacent in blockIdx.x, so the groups after the first find the links in L2.
   int ncol, ngroups;
+  // a launch may cover only the site blocks [sb0, ...) up to checkerboard index cb_end (a t-slab of the lattice: the
+  // pipelined host-pointer path of tmw_apply); a normal launch has sb0 = 0, cb_end = Vh
+  int sb0, cb_end;
   int cstride;  // 16-byte vectors per column; (columns in the buffers) * cstride < 2^31 (checked by the host)
   int red_stride;
   unsigned char col[MAXCOL];

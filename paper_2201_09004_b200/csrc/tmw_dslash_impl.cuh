@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<R>
     grp = blockIdx.x - sblock * a.ngroups;
   }
   Site s;
-  const bool active = thread_site<BLOCK>(a.g, sblock, s);
+  const bool active = thread_site<BLOCK>(a.g, sblock + a.sb0, s) && s.cb < a.cb_end;
   int colj[NR], cofs[NR];
   bool valid[NR];
 #pragma unroll
@@ -291,7 +291,7 @@ template <typename R, int NG, int EPI, int CLOVER, int NR> static cudaError_t la
   a.ngroups = (a.ncol + NR - 1) / NR;
   dim3 grid;
   if (a.g.tiled) grid = dim3((unsigned)(a.g.ntx * a.g.nty * a.ngroups), (unsigned)(a.g.Lz >> a.g.lz), (unsigned)(a.g.T >> a.g.lt));
-  else grid = dim3((unsigned)(((a.g.Vh + B - 1) / B) * a.ngroups), 1, 1);
+  else grid = dim3((unsigned)(((a.cb_end - a.sb0 * B + B - 1) / B) * a.ngroups), 1, 1);
   dslash_kernel<R, NG, EPI, CLOVER, NR, B, Tune<R, NR>::MINB, 0><<<grid, B, 0, s>>>(a);
   return cudaGetLastError();
 }

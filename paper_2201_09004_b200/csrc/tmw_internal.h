@@ -35,9 +35,10 @@ cudaError_t launch_pack_gauge(const Geom& g, const double* canon, void* g64_even
 // canonical spinor fp64 <-> packed parity spinor (prec 0: float4 planes, 1: double2 planes)
 cudaError_t launch_pack_spinor(const Geom& g, int par, int prec, const double* canon, void* packed, cudaStream_t s);
 cudaError_t launch_unpack_spinor(const Geom& g, int par, int prec, const void* packed, double* canon, cudaStream_t s);
-// both parities in one launch (coalesced on the canonical side)
-cudaError_t launch_pack_spinor_both(const Geom& g, int prec, const double* canon, void* packed_even, void* packed_odd, cudaStream_t s);
-cudaError_t launch_unpack_spinor_both(const Geom& g, int prec, const void* packed_even, const void* packed_odd, double* canon, cudaStream_t s);
+// both parities in one launch (coalesced on the canonical side); [lex0, lex1) = the (local) lexicographic sites to convert
+// (lex1 < 0: all), e.g. one t-slab
+cudaError_t launch_pack_spinor_both(const Geom& g, int prec, const double* canon, void* packed_even, void* packed_odd, cudaStream_t s, int64_t lex0 = 0, int64_t lex1 = -1);
+cudaError_t launch_unpack_spinor_both(const Geom& g, int prec, const void* packed_even, const void* packed_odd, double* canon, cudaStream_t s, int64_t lex0 = 0, int64_t lex1 = -1);
 
 // ---- clover (tmw_clover.cu) ----
 // From the packed fp64 gauge (launch_pack_gauge's g64): packed Hermitian blocks C = (c_sw/2) sum sigma F + diag, both

@@ -72,9 +72,9 @@ template <typename R> __global__ void __launch_bounds__(128) unpack_spinor_kerne
 // Both parities at once: one thread per LEXICOGRAPHIC site, so that a warp touches 6 KB of contiguous canonical memory
 // with 16-byte accesses (the one-parity kernels above skip every other 192-byte site and use 8-byte accesses: 1.58 ms
 // per parity to unpack at 48^3 x 144, against 1.0 ms for both parities here). Used by tmw_apply FULL and tmw_solve.
-template <typename R> __global__ void __launch_bounds__(128) pack_spinor_both_kernel(const Geom g, const double2* __restrict__ canon, void* pe, void* po) {
-  const int64_t lex = (int64_t)blockIdx.x * 128 + threadIdx.x;  // local lexicographic index
-  if (lex >= 2 * (int64_t)g.Vh) return;
+template <typename R> __global__ void __launch_bounds__(128) pack_spinor_both_kernel(const Geom g, int64_t lex0, int64_t lex1, const double2* __restrict__ canon, void* pe, void* po) {
+  const int64_t lex = lex0 + (int64_t)blockIdx.x * 128 + threadIdx.x;  // local lexicographic index
+  if (lex >= lex1) return;
   int64_t q = lex;
   const int x = (int)(q % g.L); q /= g.L;
   const int y = (int)(q % g.L); q /= g.L;
@@ -91,9 +91,9 @@ template <typename R> __global__ void __launch_bounds__(128) pack_spinor_both_ke
   }
   store_reals<24>(par ? po : pe, g.Vh, lex >> 1, v);
 }
-template <typename R> __global__ void __launch_bounds__(128) unpack_spinor_both_kernel(const Geom g, const void* pe, const void* po, double2* __restrict__ canon) {
-  const int64_t lex = (int64_t)blockIdx.x * 128 + threadIdx.x;  // local lexicographic index
-  if (lex >= 2 * (int64_t)g.Vh) return;
+template <typename R> __global__ void __launch_bounds__(128) unpack_spinor_both_kernel(const Geom g, int64_t lex0, int64_t lex1, const void* pe, const void* po, double2* __restrict__ canon) {
+  const int64_t lex = lex0 + (int64_t)blockIdx.x * 128 + threadIdx.x;  // local lexicographic index
+  if (lex >= lex1) return;
   int64_t q = lex;
   const int x = (int)(q % g.L); q /= g.L;
   const int y = (int)(q % g.L); q /= g.L;
@@ -106,16 +106,18 @@ template <typename R> __global__ void __launch_bounds__(128) unpack_spinor_both_
 #pragma unroll
   for (int i = 0; i < 12; i++) p[i] = make_double2((double)v[2 * i], (double)v[2 * i + 1]);
 }
-cudaError_t launch_pack_spinor_both(const Geom& g, int prec, const double* canon, void* packed_even, void* packed_odd, cudaStream_t s) {
-  const unsigned grid = (unsigned)((2 * (int64_t)g.Vh + 127) / 128);
-  if (prec == 0) pack_spinor_both_kernel<float><<<grid, 128, 0, s>>>(g, (const double2*)canon, packed_even, packed_odd);
-  else pack_spinor_both_kernel<double><<<grid, 128, 0, s>>>(g, (const double2*)canon, packed_even, packed_odd);
+cudaError_t launch_pack_spinor_both(const Geom& g, int prec, const double* canon, void* packed_even, void* packed_odd, cudaStream_t s, int64_t lex0, int64_t lex1) {
+  if (lex1 < 0) lex1 = 2 * (int64_t)g.Vh;
+  const unsigned grid = (unsigned)((lex1 - lex0 + 127) / 128);
+  if (prec == 0) pack_spinor_both_kernel<float><<<grid, 128, 0, s>>>(g, lex0, lex1, (const double2*)canon, packed_even, packed_odd);
+  else pack_spinor_both_kernel<double><<<grid, 128, 0, s>>>(g, lex0, lex1, (const double2*)canon, packed_even, packed_odd);
   return cudaGetLastError();
 }
-cudaError_t launch_unpack_spinor_both(const Geom& g, int prec, const void* packed_even, const void* packed_odd, double* canon, cudaStream_t s) {
-  const unsigned grid = (unsigned)((2 * (int64_t)g.Vh + 127) / 128);
-  if (prec == 0) unpack_spinor_both_kernel<float><<<grid, 128, 0, s>>>(g, packed_even, packed_odd, (double2*)canon);
-  else unpack_spinor_both_kernel<double><<<grid, 128, 0, s>>>(g, packed_even, packed_odd, (double2*)canon);
+cudaError_t launch_unpack_spinor_both(const Geom& g, int prec, const void* packed_even, const void* packed_odd, double* canon, cudaStream_t s, int64_t lex0, int64_t lex1) {
+  if (lex1 < 0) lex1 = 2 * (int64_t)g.Vh;
+  const unsigned grid = (unsigned)((lex1 - lex0 + 127) / 128);
+  if (prec == 0) unpack_spinor_both_kernel<float><<<grid, 128, 0, s>>>(g, lex0, lex1, packed_even, packed_odd, (double2*)canon);
+  else unpack_spinor_both_kernel<double><<<grid, 128, 0, s>>>(g, lex0, lex1, packed_even, packed_odd, (double2*)canon);
   return cudaGetLastError();
 }
 

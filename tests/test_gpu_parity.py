@@ -178,6 +178,26 @@ def test_full_apply_vs_oracle(tmw, case):
         assert site <= TOL64
 
 
+@pytest.mark.parametrize("L,T", [(8, 6), (8, 16), (8, 4), (16, 4)])
+def test_full_apply_host_pipelined_vs_oracle(tmw, L, T):
+    """tmw_apply FULL with HOST pointers on lattices whose time slices are multiples of 128 checkerboard sites: the path that
+    cuts the spinor into t-slabs and overlaps upload, operator and download on three streams (T = 6: 6 slabs, 16: 8 slabs
+    of 2, 4: 4 slabs of 1). D, D^dag and gamma5 D, pinned and pageable host memory, twice in a row (buffer reuse)."""
+    m, c_sw = -0.0514 + 0.02j, 1.0424
+    U = synth.gauge_field(L, T, 0.35, seed=1)
+    F = oracle.field_strength(U)
+    psi = synth.gaussian_spinor(L, T, seed=3)
+    with tmw.Context(L, T, U, m, c_sw, location=tmw.HOST) as ctx:
+        for rep in range(2):
+            for op in (tmw.D, tmw.DDAG, tmw.G5D):
+                src = torch.from_numpy(psi).pin_memory() if rep else psi
+                out = np.full_like(psi, 7.0)
+                ctx.apply(op, tmw.FULL, tmw.F64, src.data_ptr() if rep else src, out)
+                ref = oracle.gamma5_apply(U, psi, m, c_sw, F=F) if op == tmw.G5D else oracle.apply(U, psi, m, c_sw, dagger=(op == tmw.DDAG), F=F)
+                site, _ = H.per_site_rel_err(out, ref)
+                assert site <= TOL64, (rep, op, site)
+
+
 # ------------------------------------------------------------------------------------------------------
 # clover blocks (A1) and their inverse (A2) against the oracle's F and sigma
 # ------------------------------------------------------------------------------------------------------
