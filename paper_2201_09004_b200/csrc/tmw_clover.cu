@@ -131,12 +131,32 @@ __device__ __forceinline__ void pack_block(const zd* E1, const zd* E2, const zd*
 // memory; warps 0 and 1 then assemble the packed block of chirality 0 / 1 of the 32 sites and store the fp64 and fp32
 // copies (one 16-byte vector per lane and plane: coalesced). The earlier one-thread-per-site version kept six field
 // strengths and both blocks in one thread (255 registers + 1.9 KB of spills) and ran 4x slower.
+//
+// Traversal. A site's six field strengths touch the links of its 2-hop neighbourhood in every plane, so the order in
+// which the CTAs sweep the lattice decides how often a link comes from DRAM. In plain checkerboard order (all of one
+// parity, then the other; the +-t neighbours a whole time slice apart) ncu counted 50.6 GB of DRAM reads at 48^3 x 144
+// for a 9.17 GB gauge field. The sweep therefore goes tile by tile: tiles of (all x) x By x Bz x Bt sites (B = the
+// largest divisor <= 8 of the extent), inside a tile first the even then the odd sites, each in (xh, y, z, t) order, so
+// that everything a tile needs (its own links plus a one-site halo in y, z, t: 1.95x its volume at B = 8) stays in L2
+// while the tile is worked on, and the y-neighbour tile comes next.
+struct CloverTiles {
+  int By, Bz, Bt;   // tile extents in y, z, t
+  int nby, nbz;     // tiles along y, z
+  int ts;           // sites of one parity in a tile = Lh * By * Bz * Bt
+};
 enum { CB_SITES = 32 };
-__global__ void __launch_bounds__(6 * CB_SITES, 2) clover_build_kernel(const Geom g, const double2* __restrict__ u64e, const double2* __restrict__ u64o, double k, double diag, double2* c64e, double2* c64o, float4* c32e, float4* c32o) {
+#ifndef TMW_CLOVER_MINB
+#define TMW_CLOVER_MINB 2
+#endif
+__global__ void __launch_bounds__(6 * CB_SITES, TMW_CLOVER_MINB) clover_build_kernel(const Geom g, const CloverTiles tl, const double2* __restrict__ u64e, const double2* __restrict__ u64o, double k, double diag, double2* c64e, double2* c64o, float4* c32e, float4* c32o) {
   __shared__ double Fs[6][9][CB_SITES];  // [plane][re(0,0) re(1,1) re(2,2) re/im(1,0) re/im(2,0) re/im(2,1)][site]
   const int lane = threadIdx.x & 31, plane = threadIdx.x >> 5;
-  const int par = blockIdx.y;
-  const int cb = blockIdx.x * CB_SITES + lane;  // 32 consecutive checkerboard sites of parity par
+  // position of this lane's site in the sweep: (tile, parity, index inside the tile's parity)
+  const int64_t pos = (int64_t)blockIdx.x * CB_SITES + lane;
+  const int tile = (int)(pos / (2 * tl.ts));
+  int r = (int)(pos - (int64_t)tile * 2 * tl.ts);
+  const int par = r / tl.ts;
+  r -= par * tl.ts;
   const double* canon = nullptr;
   Lat lt;
   lt.L = g.L;
@@ -145,14 +165,17 @@ __global__ void __launch_bounds__(6 * CB_SITES, 2) clover_build_kernel(const Geo
   lt.Vh = g.Vh;
   lt.U[0] = u64e;
   lt.U[1] = u64o;
-  const bool active = cb < g.Vh;
+  const bool active = pos < 2 * (int64_t)g.Vh;
   int c[4] = {0, 0, 0, 0};
+  int cb = 0;
   if (active) {
-    int q = cb / g.Lh;
-    c[1] = q % g.L; q /= g.L;
-    c[2] = q % g.L;
-    c[3] = q / g.L;
-    c[0] = 2 * (cb % g.Lh) + ((c[1] + c[2] + c[3] + par) & 1);
+    const int xh = r % g.Lh;
+    int q = r / g.Lh;
+    c[1] = (tile % tl.nby) * tl.By + q % tl.By; q /= tl.By;
+    c[2] = ((tile / tl.nby) % tl.nbz) * tl.Bz + q % tl.Bz; q /= tl.Bz;
+    c[3] = (tile / (tl.nby * tl.nbz)) * tl.Bt + q;
+    c[0] = 2 * xh + ((c[1] + c[2] + c[3] + par) & 1);
+    cb = xh + g.Lh * (c[1] + g.L * (c[2] + g.L * c[3]));
     zd F[9];
     // planes: xy=0 xz=1 xt=2 yz=3 yt=4 zt=5. mu, nu are RUNTIME values (one copy of the 12 unrolled 3x3 products for
     // all six warps): with one specialised copy per plane the kernel was instruction-fetch bound (ncu: stall
@@ -199,8 +222,14 @@ __global__ void __launch_bounds__(6 * CB_SITES, 2) clover_build_kernel(const Geo
 }
 
 cudaError_t launch_clover_build(const Geom& g, const void* g64_even, const void* g64_odd, double c_sw, double diag, void* c64_even, void* c64_odd, void* c32_even, void* c32_odd, cudaStream_t s) {
-  const dim3 grid((unsigned)((g.Vh + CB_SITES - 1) / CB_SITES), 2, 1);
-  clover_build_kernel<<<grid, 6 * CB_SITES, 0, s>>>(g, (const double2*)g64_even, (const double2*)g64_odd, 0.5 * c_sw, diag, (double2*)c64_even, (double2*)c64_odd, (float4*)c32_even, (float4*)c32_odd);
+  const auto tile_extent = [](int n) { int b = 1; for (int d = 2; d <= 8; d++) if (n % d == 0) b = d; return b; };
+  CloverTiles tl;
+  tl.By = tl.Bz = tile_extent(g.L);
+  tl.Bt = tile_extent(g.T);
+  tl.nby = tl.nbz = g.L / tl.By;
+  tl.ts = g.Lh * tl.By * tl.Bz * tl.Bt;
+  const dim3 grid((unsigned)((2 * (int64_t)g.Vh + CB_SITES - 1) / CB_SITES), 1, 1);
+  clover_build_kernel<<<grid, 6 * CB_SITES, 0, s>>>(g, tl, (const double2*)g64_even, (const double2*)g64_odd, 0.5 * c_sw, diag, (double2*)c64_even, (double2*)c64_odd, (float4*)c32_even, (float4*)c32_odd);
   return cudaGetLastError();
 }
 
