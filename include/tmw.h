@@ -110,6 +110,14 @@ typedef struct {
      this build all domains live on the context's device (the exchange is a same-device copy); tmw_get_clover and the
      tile / columns_per_thread tunings are not available. */
   int domains_z, domains_t;
+  /* Shared-memory staged fp32 stencil (BASELINE.json north_star subsystem (2)): a CTA covers a tile of one
+     time slice and copies the input sites its six spatial hops need into shared memory with asynchronous 16-byte copies
+     instead of loading 8 neighbour spinors per site through L1. 0 or -1 = off (default: measured on B200 the staged kernel
+     is 10-40 % slower than the plain one at every tile shape and column count, profiles/r2_stage.md), 1 = wherever a tile
+     fits (hop, K1, K2 of fp32 launches without domain decomposition). stage_tile = tile extents (x/2, y, z) in sites, all 0 =
+     chosen by the library; a tile that does not divide the lattice or does not fit in shared memory -> the plain kernel. */
+  int stage;
+  int stage_tile[3];
 } tmw_options;
 
 /* Test hooks (tmw_options.debug / tmw_set_debug): they change which code path runs, never the result. */
@@ -242,7 +250,8 @@ long long tmw_launch_count(const tmw_ctx* ctx);
 #define TMW_K_MEMSET_BYTES 20  /* BYTES zeroed by device memsets inside the solver */
 #define TMW_K_COPY_BYTES 21    /* BYTES moved by device-to-device copies inside the solver */
 #define TMW_K_HOP32_LOADONLY 22 /* tmw_time_kernel only: the loads and stores of TMW_K_HOP32 without its arithmetic */
-#define TMW_K_COUNT 23
+#define TMW_K_STAGED 23        /* of the fp32 stencil applications above: those that ran in the shared-memory staged kernel */
+#define TMW_K_COUNT 24
 
 /*
  * counts[k] (k < min(n, TMW_K_COUNT)) = how many right-hand-side columns kernels of kind k have been applied to since

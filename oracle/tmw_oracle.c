@@ -30,8 +30,11 @@
  * spectra; gamma5-hermiticity; adjoint dot test and dense conjugate transpose on 2^4; twisted-mass identity
  * |D(m)psi|^2 = |D(Re m)psi|^2 + (Im m)^2|psi|^2; gauge covariance incl. clover; F = 0 on unit / pure-gauge
  * fields; uniform abelian flux F_xy = sin(B) T3; dense LU solve on 2^4 and 4^4; free propagator by Fourier sum.
- * PARITY UNPINNED: the overall sign / prefactor of the clover term of Eq. 3 relative to the paper (the paper prints
- * no number and Eq. 3 is schematic); it is pinned to the standard Sheikholeslami-Wohlert convention only (C7).
+ * The sign and prefactor of the clover term of Eq. 3 relative to the hopping term of Eq. 2 (the paper prints no number
+ * and Eq. 3 is schematic) are pinned by what the term is for, "O(a) improvement": in a uniform abelian
+ * field the Wilson term lifts the would-be zero modes to B/2 and the clover term at c_sw = 1 must cancel that lift
+ * (test_clover_sign_is_the_improving_one: sigma_min = B/2 at c_sw = 0, O(B^2) at +1, B at -1), on a fully periodic
+ * lattice (antiperiodic_t = 0). No function of this file is "parity unpinned".
  *
  * Layouts (canonical, fp64, x fastest; same as include/tmw.h):
  *   gauge  [mu=0..3 (x,y,z,t)][t][z][y][x][row][col] complex   U_mu(x)_{row,col}

@@ -81,7 +81,13 @@ struct tmw_ctx {
   GcrScalars* gs;       // device
   GcrScalars* gs_host;  // pinned
   int nr32;          // forced columns per thread of the fp32 stencil (1..4), 0 = automatic
+  StageGeom stage[4];  // tile of the shared-memory staged fp32 stencil for nr = 1..3 columns per thread (index nr)
+  bool stage_ok[4];    // such a tile exists (tmw_options.stage / stage_tile, choose_stage)
   bool verbose;
+  int* attn;         // device int[2]: [0] a column needs the host (the queued iteration kernels return at once), [1] iterations done
+  int* attn_host;    // pinned int[6]: two lagged copies of attn (one per queued iteration) and the copy of a sync point
+  cudaEvent_t ev_lag[2];
+  const int* cur_skip;  // what make_args puts into DslashArgs::skip: attn while BiCGStab iterations are being queued, else null
   Scalars* sc;       // MAXCOL scalar blocks
   Scalars* sc_host;  // pinned
   double* red;       // 4 * MAXCOL device doubles
@@ -217,6 +223,7 @@ static DslashArgs<R> make_args(const tmw_ctx* c, int par, int dagger, const void
   a.cb_end = a.g.Vh;
   a.cstride = (int)((int64_t)c->g.Vh * 24 * (int64_t)sizeof(R) / 16);
   a.red_stride = 0;
+  a.skip = c->cur_skip;
   for (int i = 0; i < MAXCOL; i++) a.col[i] = cm.col[i];
   return a;
 }
@@ -333,6 +340,28 @@ static int dslash_dd(tmw_ctx* ctx, int epi, int par, int dagger, const void* in,
   return TMW_OK;
 }
 
+// Does this launch go through the shared-memory staged kernel (fp32 hop / K1 / K2 on the whole lattice)? nr may be lowered
+// to the most columns per thread the staged kernel has a tile for. Opt-in only (tmw_options.stage = 1): measured on B200 it
+// loses to the plain kernel at every tile shape and column count (profiles/r2_stage.md).
+template <typename R> static bool use_stage(tmw_ctx* ctx, int epi, int ncol, int cb1, int& nr) {
+  if (sizeof(R) != 4 || ctx->opt.stage <= 0 || cb1 >= 0 || !ctx->dom.empty()) return false;
+  if (epi != EPI_HOP && epi != EPI_AINV_HOP && epi != EPI_A_XPAY) return false;
+  int n = nr > 3 ? 3 : nr;
+  while (n >= 1 && !ctx->stage_ok[n]) n--;
+  if (n < 1) return false;
+  if (n != nr) {  // regroup the columns evenly
+    const int groups = (ncol + n - 1) / n;
+    n = (ncol + groups - 1) / groups;
+    if (!ctx->stage_ok[n]) return false;
+  }
+  nr = n;
+  return true;
+}
+static cudaError_t launch_stage(const DslashArgs<float>& a, int ng, int epi, int clv, int nr, const StageGeom& sg, cudaStream_t s) {
+  return launch_dslash_stage(a, ng, epi, clv, nr, sg, s);
+}
+static cudaError_t launch_stage(const DslashArgs<double>&, int, int, int, int, const StageGeom&, cudaStream_t) { return cudaErrorInvalidValue; }
+
 // cb0, cb1 (optional): restrict the launch to the output sites with checkerboard index in [cb0, cb1), cb0 a multiple of 128
 template <typename R>
 static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, void* out, const void* aux, double sgn, const ColMap& cm,
@@ -358,7 +387,13 @@ static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, vo
       nr = ((cm.n + 2) / 3 * 3 < (cm.n + 1) / 2 * 2) ? 3 : 2;
     }
   }
-  LAUNCHK(stencil_kind<R>(epi, red_mode), cm.n, launch_dslash(a, ng_of<R>(ctx), epi, !ctx->clover ? CL_NONE : (ctx->m_im != 0.0 ? CL_TWISTED : CL_CLOVER), nr, ctx->stream));
+  const int clv = !ctx->clover ? CL_NONE : (ctx->m_im != 0.0 ? CL_TWISTED : CL_CLOVER);
+  if (use_stage<R>(ctx, epi, cm.n, cb1, nr)) {
+    ctx->kcount[TMW_K_STAGED] += cm.n;
+    LAUNCHK(stencil_kind<R>(epi, red_mode), cm.n, launch_stage(a, ng_of<R>(ctx), epi, clv, nr, ctx->stage[nr], ctx->stream));
+    return TMW_OK;
+  }
+  LAUNCHK(stencil_kind<R>(epi, red_mode), cm.n, launch_dslash(a, ng_of<R>(ctx), epi, clv, nr, ctx->stream));
   return TMW_OK;
 }
 // out = A^{-1} in (inverse) or A in on parity par, one column, fp64 (every domain of a decomposed context)
@@ -435,6 +470,44 @@ static void choose_tile(Geom& g, const int* tile) {
   g.nty = g.L >> g.ly;
 }
 
+// Tile of the staged stencil (tmw_dslash_stage.cuh) for nr columns per thread: txh | Lh, ty | L, tz | L with at most
+// stage_max_threads(nr) threads and nr * 6 * nslots float4 of shared memory. Automatic choice: the tile with the fewest
+// staged sites per output site among those that are whole warps, at least 96 threads, and leave room for two CTAs per SM
+// (<= 112 KB each); a forced tile (tmw_options.stage_tile) or stage = 1 only has to fit at all (<= 226 KB).
+static bool make_stage(const Geom& g, int nr, int txh, int ty, int tz, size_t budget, StageGeom& sg) {
+  if (txh < 1 || ty < 2 || tz < 2 || g.Lh % txh || g.L % ty || g.Lz % tz) return false;
+  sg.txh = txh; sg.ty = ty; sg.tz = tz;
+  sg.ntx = g.Lh / txh; sg.nty = g.L / ty; sg.ntz = g.Lz / tz;
+  sg.fullx = (txh == g.Lh);
+  sg.rw = sg.fullx ? g.Lh : txh + 2;
+  sg.nrows = ty * tz + 2 * tz + 2 * ty;
+  sg.nslots = sg.nrows * sg.rw;
+  sg.nthr = txh * ty * tz;
+  if ((sg.nthr + 31) / 32 * 32 > stage_max_threads(nr)) return false;
+  return (size_t)nr * 6 * sg.nslots * 16 <= budget;
+}
+static bool choose_stage(const Geom& g, int nr, const tmw_options& o, StageGeom& best) {
+  if (o.stage <= 0 || g.tiled) return false;
+  if (o.stage_tile[0] || o.stage_tile[1] || o.stage_tile[2]) return make_stage(g, nr, o.stage_tile[0], o.stage_tile[1], o.stage_tile[2], 226 * 1024, best);
+  bool found = false;
+  double best_ratio = 0;
+  for (int pass = 0; pass < 2 && !found; pass++) {  // pass 1 (stage = 1 only): any tile that fits
+    if (pass == 1 && o.stage != 1) break;
+    for (int txh = g.Lh; txh >= 1; txh--) {
+      if (g.Lh % txh) continue;
+      for (int ty = 8; ty >= 2; ty >>= 1)
+        for (int tz = 8; tz >= 2; tz >>= 1) {
+          StageGeom sg;
+          if (!make_stage(g, nr, txh, ty, tz, pass == 0 ? 112 * 1024 : 226 * 1024, sg)) continue;
+          if (pass == 0 && (sg.nthr % 32 || sg.nthr < 96)) continue;
+          const double ratio = (double)sg.nslots / sg.nthr;
+          if (!found || ratio < best_ratio - 1e-9 || (ratio < best_ratio + 1e-9 && sg.nthr > best.nthr)) { best = sg; best_ratio = ratio; found = true; }
+        }
+    }
+  }
+  return found;
+}
+
 extern "C" {
 
 const char* tmw_last_error(const tmw_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
@@ -446,6 +519,8 @@ void tmw_destroy(tmw_ctx* ctx) {
   if (ctx->sc_host) cudaFreeHost(ctx->sc_host);
   if (ctx->red_host) cudaFreeHost(ctx->red_host);
   if (ctx->gs_host) cudaFreeHost(ctx->gs_host);
+  if (ctx->attn_host) cudaFreeHost(ctx->attn_host);
+  for (int i = 0; i < 2; i++) if (ctx->ev_lag[i]) cudaEventDestroy(ctx->ev_lag[i]);
   if (ctx->comm) { cudaStreamSynchronize(ctx->comm); cudaStreamDestroy(ctx->comm); }
   if (ctx->h2d) { cudaStreamSynchronize(ctx->h2d); cudaStreamDestroy(ctx->h2d); }
   if (ctx->d2h) { cudaStreamSynchronize(ctx->d2h); cudaStreamDestroy(ctx->d2h); }
@@ -479,7 +554,8 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
       (o.reconstruct != 12 && o.reconstruct != 18) || (o.mass_reading != TMW_TWIST_GAMMA5 && o.mass_reading != TMW_MASS_SCALAR) ||
       o.max_iter < 0 || !(o.delta > 0.0) || !(o.delta < 1.0) || (o.solver != TMW_BICGSTAB && o.solver != TMW_GCR) || o.nkrylov < 1 ||
       o.nkrylov > GCR_KMAX || o.columns_per_thread < 0 || o.columns_per_thread > 4 ||
-      (o.debug & ~(TMW_DEBUG_FORCE_PIVOT | TMW_DEBUG_NO_CHUNK)))
+      (o.debug & ~(TMW_DEBUG_FORCE_PIVOT | TMW_DEBUG_NO_CHUNK)) || o.stage < -1 || o.stage > 1 || o.stage_tile[0] < 0 ||
+      o.stage_tile[1] < 0 || o.stage_tile[2] < 0)
     return fail(nullptr, TMW_EINVAL, "tmw_create: bad option value");
   if (!isfinite(m.re) || !isfinite(m.im) || !isfinite(c_sw)) return fail(nullptr, TMW_EINVAL, "tmw_create: non-finite parameter");
   const int pz = o.domains_z > 1 ? o.domains_z : 1, pt = o.domains_t > 1 ? o.domains_t : 1;
@@ -495,6 +571,7 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
   ctx->pz = pz; ctx->pt = pt;
   ctx->vh_loc = ctx->g.Vh / (pz * pt);
   ctx->nr32 = o.columns_per_thread;
+  for (int nr = 0; nr < 4; nr++) ctx->stage_ok[nr] = (nr >= 1 && nr <= 3 && pz * pt == 1) ? choose_stage(ctx->g, nr, o, ctx->stage[nr]) : false;
   ctx->verbose = o.verbose != 0 || getenv("TMW_VERBOSE") != nullptr;
   ctx->V = V;
   ctx->m_re = m.re; ctx->m_im = m.im; ctx->c_sw = c_sw;
@@ -530,6 +607,9 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
   CKC(cudaEventCreate(&ctx->ev1));
   CKA(&ctx->sc, MAXCOL * sizeof(Scalars));
   CKA(&ctx->red, 4 * MAXCOL * sizeof(double));
+  CKC(cudaMallocHost((void**)&ctx->attn_host, 6 * sizeof(int)));
+  CKA(&ctx->attn, 2 * sizeof(int));
+  for (int i = 0; i < 2; i++) CKC(cudaEventCreateWithFlags(&ctx->ev_lag[i], cudaEventDisableTiming));
   CKC(cudaMallocHost((void**)&ctx->gs_host, sizeof(GcrScalars)));
   CKA(&ctx->gs, sizeof(GcrScalars));
   const size_t Vh = (size_t)ctx->g.Vh;
@@ -992,29 +1072,79 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
   if ((rc = push_scalars(ctx))) return rc;
   LAUNCHK(TMW_K_RESID_CONVERT, act.n, launch_resid_convert<R>(n64, ctx->vh_loc, W[2], nullptr, W[4], r, rhat, nullptr, ctx->sc, act, s));  // r64 = bhat - 0; rho = <rhat,r>; rr = |r64|^2
   if ((rc = fetch_scalars(ctx))) return rc;
+  // what the device compares against at the start of an iteration (Scalars::stop2 / maxr2 / brk2)
+  auto arm = [&](int c) {
+    h[c].stop2 = (tol * cs[c].bnorm) * (tol * cs[c].bnorm);
+    h[c].maxr2 = cs[c].maxr * cs[c].maxr;
+    h[c].brk2 = (eps_break * cs[c].rhat_norm) * (eps_break * cs[c].rhat_norm);
+    h[c].trip = 0;
+  };
   for (int i = 0; i < act.n; i++) {
     const int c = act.col[i];
     reset_recurrence(&h[c]);
     cs[c].rnorm = cs[c].maxr = cs[c].rhat_norm = cs[c].r_upd = cs[c].best = sqrt(h[c].rr);
     cs[c].iter_resid = cs[c].rnorm / cs[c].bnorm;
     if (cs[c].rnorm <= tol * cs[c].bnorm) cs[c].done = true;
+    arm(c);
   }
   if ((rc = push_scalars(ctx))) return rc;
   // p = r for the first iteration; later p comes out of update_xrp (v is written by the first K2 before it is read)
   for (int i = 0; i < act.n; i++) COPYK(colp(p, act.col[i], bytesR), colp(r, act.col[i], bytesR), bytesR);
   const int max_iter = ctx->opt.max_iter;
-  for (int k = 1; k <= max_iter; k++) {
+  // The host queues iterations ahead of the device and looks at the scalars only at SYNC POINTS: when the device has raised
+  // attn[0] (it tests every column at the start of each iteration, sc_begin_iter; all kernels of the queued iterations then
+  // return at once, so nothing moves past the iteration that tripped), when max_iter is near, or every iteration if verbose.
+  // Between sync points the host only waits for the 8-byte copy of attn of the iteration BEFORE the one it has just queued,
+  // so the device always has an iteration in its queue ("read back only a convergence flag").
+  const double delta2 = ctx->opt.delta * ctx->opt.delta;
+  int* const lag = ctx->attn_host;       // lag[2 * (e & 1)]: attn after queued iteration e
+  int* const attn_now = ctx->attn_host + 4;
+  CK(cudaMemsetAsync(ctx->attn, 0, 2 * sizeof(int), s));
+  int k = 0;    // iterations done, as of the last sync point
+  int enq = 0;  // iterations queued since then
+  for (;;) {
     act.n = 0;
     for (int c = 0; c < ncols; c++) if (!cs[c].done) cols_add(act, c);
     if (act.n == 0) return TMW_OK;
-    LAUNCH(launch_sc_begin_iter(ctx->sc, act, s));
-    if ((rc = schur<R>(ctx, 0, p, v, tmp, act, 1, rhat, red_rhat_v, SCD))) return rc;
-    LAUNCH(launch_sc_alpha(ctx->sc, act, s));
-    LAUNCHK(TMW_K_UPDATE_S, act.n, launch_update_s<R>(nR, sv, r, v, ctx->sc, act, s));
-    if ((rc = schur<R>(ctx, 0, sv, t, tmp, act, 4, rhat, red_ts, SCD))) return rc;  // <t,s>, <t,t>, <rhat,t>, <rhat,s>
-    LAUNCH(launch_sc_omega(ctx->sc, act, s));                                        // omega, rho' = <rhat, s - omega t>, beta
-    LAUNCHK(TMW_K_UPDATE_XRP, act.n, launch_update_xrp<R>(nR, x, r, p, sv, t, v, ctx->sc, act, s));             // x, r, and p of the next iteration
+    long long per_iter[TMW_K_COUNT];  // what one iteration adds to the kernel counts
+    memcpy(per_iter, ctx->kcount, sizeof(per_iter));
+    ctx->cur_skip = ctx->attn;
+    LAUNCH(launch_sc_begin_iter(ctx->sc, act, ctx->attn, enq > 0, delta2, s));
+    rc = schur<R>(ctx, 0, p, v, tmp, act, 1, rhat, red_rhat_v, SCD);
+    if (!rc) {
+      LAUNCH(launch_sc_alpha(ctx->sc, act, ctx->attn, s));
+      LAUNCHK(TMW_K_UPDATE_S, act.n, launch_update_s<R>(nR, sv, r, v, ctx->sc, act, ctx->attn, s));
+      rc = schur<R>(ctx, 0, sv, t, tmp, act, 4, rhat, red_ts, SCD);  // <t,s>, <t,t>, <rhat,t>, <rhat,s>
+    }
+    if (!rc) {
+      LAUNCH(launch_sc_omega(ctx->sc, act, ctx->attn, s));                                        // omega, rho' = <rhat, s - omega t>, beta
+      LAUNCHK(TMW_K_UPDATE_XRP, act.n, launch_update_xrp<R>(nR, x, r, p, sv, t, v, ctx->sc, act, ctx->attn, s));  // x, r, and p of the next iteration
+    }
+    ctx->cur_skip = nullptr;
+    if (rc) return rc;
+    for (int i = 0; i < TMW_K_COUNT; i++) per_iter[i] = ctx->kcount[i] - per_iter[i];
+    enq++;
+    bool sync_now = verbose || k + enq >= max_iter;
+    if (!sync_now) {
+      CK(cudaMemcpyAsync(lag + 2 * (enq & 1), ctx->attn, 2 * sizeof(int), cudaMemcpyDeviceToHost, s));
+      CK(cudaEventRecord(ctx->ev_lag[enq & 1], s));
+      if (enq >= 2) {
+        CK(cudaEventSynchronize(ctx->ev_lag[(enq - 1) & 1]));
+        sync_now = lag[2 * ((enq - 1) & 1)] != 0;
+      }
+    }
+    if (!sync_now) continue;
+    // ---- sync point: the state is the one after iteration attn[1]; iterations queued beyond it did nothing ----
+    CK(cudaMemcpyAsync(attn_now, ctx->attn, 2 * sizeof(int), cudaMemcpyDeviceToHost, s));
     if ((rc = fetch_scalars(ctx))) return rc;
+    {
+      const int skipped = k + enq - attn_now[1];  // their launches returned at once: not work of the path (tmw_kernel_counts)
+      for (int i = 0; i < TMW_K_COUNT; i++) ctx->kcount[i] -= skipped * per_iter[i];
+    }
+    k = attn_now[1];
+    enq = 0;
+    const bool tripped = attn_now[0] != 0;
+    if (tripped) CK(cudaMemsetAsync(ctx->attn, 0, sizeof(int), s));
     ColMap upd, brk;  // columns that take a reliable update now / whose iterate is corrupted
     upd.n = brk.n = 0;
     bool broken[MAXCOL];
@@ -1023,6 +1153,8 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
       ColState& q = cs[c];
       q.iters = k;
       broken[c] = !isfinite(h[c].rr) || !isfinite(h[c].rho[0]) || !isfinite(h[c].rho[1]);
+      const long long trip = tripped ? h[c].trip : 0;
+      if (h[c].maxr2 > q.maxr * q.maxr) q.maxr = sqrt(h[c].maxr2);  // the device tracked it over the iterations the host did not see
       q.rnorm = broken[c] ? q.maxr : sqrt(h[c].rr);
       if (verbose)
         fprintf(stderr, "[tmw] col %d it %d |r|/|b| %.3e rho (%.3e,%.3e) alpha (%.3e,%.3e) omega (%.3e,%.3e) <rhat,v> (%.3e,%.3e) tt %.3e\n", c, k,
@@ -1030,7 +1162,7 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
                 h[c].rhat_v[1], h[c].tt);
       if (!broken[c]) q.iter_resid = q.rnorm / q.bnorm;
       const bool conv = !broken[c] && q.rnorm <= tol * q.bnorm;
-      if (broken[c] || conv || q.rnorm < ctx->opt.delta * q.maxr || k == max_iter) {
+      if (broken[c] || conv || (trip & ~(long long)TRIP_BREAKDOWN) || q.rnorm < ctx->opt.delta * q.maxr || k >= max_iter) {
         cols_add(upd, c);
         if (broken[c]) cols_add(brk, c);
       } else if (q.rnorm > q.maxr) {
@@ -1064,16 +1196,18 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
         if (verbose) fprintf(stderr, "[tmw]   col %d reliable update %d: true |r|/|b| %.3e rho (%.3e,%.3e)\n", c, q.updates, q.rnorm / q.bnorm, h[c].rho[0], h[c].rho[1]);
         if (!isfinite(q.rnorm)) return fail(ctx, TMW_EBREAKDOWN, "tmw_solve: non-finite true residual");
         if (q.rnorm <= tol * q.bnorm) q.done = true;
+        arm(c);
       }
+      if ((rc = push_scalars(ctx))) return rc;
     }
-    if (k == max_iter) break;
+    if (k >= max_iter) break;
     ColMap rst;  // breakdown: restart the recurrence with rhat = r (C11)
     rst.n = 0;
     for (int i = 0; i < act.n; i++) {
       const int c = act.col[i];
       if (cs[c].done) continue;
       const double rho_abs = hypot(h[c].rho[0], h[c].rho[1]);
-      if (broken[c] || !(rho_abs > eps_break * cs[c].rhat_norm * cs[c].rnorm)) {
+      if (broken[c] || !(rho_abs > eps_break * cs[c].rhat_norm * cs[c].rnorm)) {  // (the device's TRIP_BREAKDOWN is this test on its own copy)
         if (verbose) fprintf(stderr, "[tmw]   col %d breakdown: |rho| %.3e vs %.3e * %.3e * %.3e -> restart\n", c, rho_abs, eps_break, cs[c].rhat_norm, cs[c].rnorm);
         cs[c].restarts++;
         cols_add(rst, c);
@@ -1110,11 +1244,13 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
         q.iter_resid = q.rnorm / q.bnorm;
         q.updates++;
         if (verbose) fprintf(stderr, "[tmw]   col %d restart %d: true |r|/|b| %.3e\n", c, q.restarts, q.iter_resid);
+        arm(c);
         if (q.rnorm <= tol * q.bnorm) { q.done = true; continue; }
         // restarts are cheap and a long solve may need many; give up only when they stop paying
         if (q.rnorm < 0.9 * q.best) { q.best = q.rnorm; q.stalled = 0; }
         else if (++q.stalled > 5) return fail(ctx, TMW_EBREAKDOWN, "tmw_solve: BiCGStab breakdown: no progress over 5 consecutive restarts");
       }
+      if ((rc = push_scalars(ctx))) return rc;
     }
   }
   for (int c = 0; c < ncols; c++)
@@ -1431,8 +1567,8 @@ extern "C" int tmw_time_kernel(tmw_ctx* ctx, int kind, int reps, double* ms) {
       case TMW_K_K2_32_DOTS: return dslash<float>(ctx, EPI_A_XPAY, 1, 0, X[7], X[5], X[4], -1.0, one, 4, X[1], red_ts, SCD);
       case TMW_K_K1_64: return dslash<double>(ctx, EPI_AINV_HOP, 0, 0, W[3], W[5], nullptr, 1.0, one);
       case TMW_K_K2_64: return dslash<double>(ctx, EPI_A_XPAY, 1, 0, W[5], W[6], W[3], -1.0, one);
-      case TMW_K_UPDATE_S: LAUNCH(launch_update_s<float>(nR, X[4], X[0], X[3], ctx->sc, one, ctx->stream)); return TMW_OK;
-      case TMW_K_UPDATE_XRP: LAUNCH(launch_update_xrp<float>(nR, X[6], X[0], X[2], X[4], X[5], X[3], ctx->sc, one, ctx->stream)); return TMW_OK;
+      case TMW_K_UPDATE_S: LAUNCH(launch_update_s<float>(nR, X[4], X[0], X[3], ctx->sc, one, nullptr, ctx->stream)); return TMW_OK;
+      case TMW_K_UPDATE_XRP: LAUNCH(launch_update_xrp<float>(nR, X[6], X[0], X[2], X[4], X[5], X[3], ctx->sc, one, nullptr, ctx->stream)); return TMW_OK;
       case TMW_K_HOP32_LOADONLY: {
         DslashArgs<float> a = make_args<float>(ctx, 1, 0, X[7], X[3], nullptr, 1.0, one);
         LAUNCH(launch_hop_loadonly(a, ctx->ng32, ctx->stream));

@@ -74,19 +74,38 @@ __device__ __forceinline__ void cdiv(const double* a, const double* b, double* q
   const double re = (a[0] * b[0] + a[1] * b[1]) / d, im = (a[1] * b[0] - a[0] * b[1]) / d;
   q[0] = re; q[1] = im;
 }
-__global__ void sc_begin_iter_kernel(Scalars* sc0, ColMap cm) {  // zero the accumulators of the two K2 launches
+__global__ void sc_begin_iter_kernel(Scalars* sc0, ColMap cm, int* attn, int check, double delta2) {
   Scalars* sc = sc0 + cm.col[threadIdx.x];
+  if (check) {  // does the host have to look at this column before the iteration may go on? (tmw_internal.h)
+    long long trip = 0;
+    const double rr = sc->rr, rho2 = sc->rho[0] * sc->rho[0] + sc->rho[1] * sc->rho[1];
+    if (!isfinite(rr) || !isfinite(rho2)) {
+      trip = TRIP_BROKEN;
+    } else {
+      if (rr <= sc->stop2) trip |= TRIP_CONV;
+      if (sc->maxr2 > 0.0 && rr < delta2 * sc->maxr2) trip |= TRIP_RELIABLE;
+      if (!(rho2 > sc->brk2 * rr)) trip |= TRIP_BREAKDOWN;
+      if (!trip && rr > sc->maxr2) sc->maxr2 = rr;
+    }
+    sc->trip = trip;
+    if (trip) atomicOr(attn, 1);
+  }
+  __syncthreads();
+  if (*(volatile int*)attn) return;  // raised now or by an earlier iteration: leave everything as it is
   sc->rhat_v[0] = sc->rhat_v[1] = 0.0;
   sc->ts[0] = sc->ts[1] = 0.0;
   sc->tt = 0.0;
   sc->rhat_t[0] = sc->rhat_t[1] = 0.0;
   sc->rhat_s[0] = sc->rhat_s[1] = 0.0;
+  if (threadIdx.x == 0) attn[1]++;
 }
-__global__ void sc_alpha_kernel(Scalars* sc0, ColMap cm) {
+__global__ void sc_alpha_kernel(Scalars* sc0, ColMap cm, const int* skip) {
+  if (skip && *skip) return;
   Scalars* sc = sc0 + cm.col[threadIdx.x];
   cdiv(sc->rho, sc->rhat_v, sc->alpha);
 }
-__global__ void sc_omega_kernel(Scalars* sc0, ColMap cm) {
+__global__ void sc_omega_kernel(Scalars* sc0, ColMap cm, const int* skip) {
+  if (skip && *skip) return;
   Scalars* sc = sc0 + cm.col[threadIdx.x];
   // <t,t> = 0: s = r - alpha v vanished, x + alpha p is exact at the half step (a source that is an eigenvector, a free
   // field). omega = 0 then makes update_xrp do x += alpha p, r = s (= 0); beta = 0 keeps the next p finite.
@@ -106,12 +125,16 @@ __global__ void sc_omega_kernel(Scalars* sc0, ColMap cm) {
   sc->beta[1] = exact ? 0.0 : a[0] * b[1] + a[1] * b[0];
   sc->rr = 0.0;
 }
-cudaError_t launch_sc_begin_iter(Scalars* sc, const ColMap& cm, cudaStream_t s) { sc_begin_iter_kernel<<<1, cm.n, 0, s>>>(sc, cm); return cudaGetLastError(); }
-cudaError_t launch_sc_alpha(Scalars* sc, const ColMap& cm, cudaStream_t s) { sc_alpha_kernel<<<1, cm.n, 0, s>>>(sc, cm); return cudaGetLastError(); }
-cudaError_t launch_sc_omega(Scalars* sc, const ColMap& cm, cudaStream_t s) { sc_omega_kernel<<<1, cm.n, 0, s>>>(sc, cm); return cudaGetLastError(); }
+cudaError_t launch_sc_begin_iter(Scalars* sc, const ColMap& cm, int* attn, int check, double delta2, cudaStream_t s) {
+  sc_begin_iter_kernel<<<1, cm.n, 0, s>>>(sc, cm, attn, check, delta2);
+  return cudaGetLastError();
+}
+cudaError_t launch_sc_alpha(Scalars* sc, const ColMap& cm, const int* skip, cudaStream_t s) { sc_alpha_kernel<<<1, cm.n, 0, s>>>(sc, cm, skip); return cudaGetLastError(); }
+cudaError_t launch_sc_omega(Scalars* sc, const ColMap& cm, const int* skip, cudaStream_t s) { sc_omega_kernel<<<1, cm.n, 0, s>>>(sc, cm, skip); return cudaGetLastError(); }
 
 // ---- vector updates ----
-template <typename R> __global__ void __launch_bounds__(BB) update_s_kernel(int64_t n, R* s, const R* r, const R* v, const Scalars* sc, ColMap cm) {
+template <typename R> __global__ void __launch_bounds__(BB) update_s_kernel(int64_t n, R* s, const R* r, const R* v, const Scalars* sc, ColMap cm, const int* skip) {
+  if (skip && *skip) return;
   const int c = cm.col[blockIdx.y];
   sc += c;
   { const int64_t o = 4 * n * c; s += o; r += o; v += o; }
@@ -127,7 +150,8 @@ template <typename R> __global__ void __launch_bounds__(BB) update_s_kernel(int6
     stp(s, i, ss);
   }
 }
-template <typename R> __global__ void __launch_bounds__(BB) update_xrp_kernel(int64_t n, R* x, R* r, R* p, const R* s, const R* t, const R* v, Scalars* sc, ColMap cm) {
+template <typename R> __global__ void __launch_bounds__(BB) update_xrp_kernel(int64_t n, R* x, R* r, R* p, const R* s, const R* t, const R* v, Scalars* sc, ColMap cm, const int* skip) {
+  if (skip && *skip) return;
   const int c = cm.col[blockIdx.y];
   sc += c;
   { const int64_t o = 4 * n * c; x += o; r += o; p += o; s += o; t += o; v += o; }
@@ -418,14 +442,14 @@ template <typename R> __global__ void __launch_bounds__(BB) gcr_update_kernel(in
 template <typename R> static inline int64_t pairs_of(int64_t n16) { return sizeof(R) == 4 ? n16 : n16 / 2; }
 static inline dim3 grid_of(int64_t np, const ColMap& cm) { return dim3((unsigned)blas_grid(np), (unsigned)cm.n, 1); }
 
-template <typename R> cudaError_t launch_update_s(int64_t n, void* sv, const void* r, const void* v, const Scalars* sc, const ColMap& cm, cudaStream_t s) {
+template <typename R> cudaError_t launch_update_s(int64_t n, void* sv, const void* r, const void* v, const Scalars* sc, const ColMap& cm, const int* skip, cudaStream_t s) {
   const int64_t np = pairs_of<R>(n);
-  update_s_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, (R*)sv, (const R*)r, (const R*)v, sc, cm);
+  update_s_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, (R*)sv, (const R*)r, (const R*)v, sc, cm, skip);
   return cudaGetLastError();
 }
-template <typename R> cudaError_t launch_update_xrp(int64_t n, void* x, void* r, void* p, const void* sv, const void* t, const void* v, Scalars* sc, const ColMap& cm, cudaStream_t s) {
+template <typename R> cudaError_t launch_update_xrp(int64_t n, void* x, void* r, void* p, const void* sv, const void* t, const void* v, Scalars* sc, const ColMap& cm, const int* skip, cudaStream_t s) {
   const int64_t np = pairs_of<R>(n);
-  update_xrp_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, (R*)x, (R*)r, (R*)p, (const R*)sv, (const R*)t, (const R*)v, sc, cm);
+  update_xrp_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, (R*)x, (R*)r, (R*)p, (const R*)sv, (const R*)t, (const R*)v, sc, cm, skip);
   return cudaGetLastError();
 }
 template <typename R> cudaError_t launch_dot_norm(int64_t n, const void* a, const void* b, double* out, const ColMap& cm, cudaStream_t s) {
@@ -475,8 +499,8 @@ template cudaError_t launch_gcr_step<float>(int64_t, int, void*, void*, void*, v
 template cudaError_t launch_gcr_step<double>(int64_t, int, void*, void*, void*, void*, GcrScalars*, cudaStream_t);
 
 #define TMW_INST(R)                                                                                                          \
-  template cudaError_t launch_update_s<R>(int64_t, void*, const void*, const void*, const Scalars*, const ColMap&, cudaStream_t);           \
-  template cudaError_t launch_update_xrp<R>(int64_t, void*, void*, void*, const void*, const void*, const void*, Scalars*, const ColMap&, cudaStream_t); \
+  template cudaError_t launch_update_s<R>(int64_t, void*, const void*, const void*, const Scalars*, const ColMap&, const int*, cudaStream_t);           \
+  template cudaError_t launch_update_xrp<R>(int64_t, void*, void*, void*, const void*, const void*, const void*, Scalars*, const ColMap&, const int*, cudaStream_t); \
   template cudaError_t launch_dot_norm<R>(int64_t, const void*, const void*, double*, const ColMap&, cudaStream_t);                         \
   template cudaError_t launch_acc_y<R>(int64_t, int64_t, void*, void*, const ColMap&, cudaStream_t);                                        \
   template cudaError_t launch_resid_convert<R>(int64_t, int64_t, const void*, const void*, void*, void*, const void*, void*, Scalars*, const ColMap&, cudaStream_t); \

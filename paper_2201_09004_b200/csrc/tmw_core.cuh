@@ -583,6 +583,9 @@ template <typename R> struct DslashArgs {
   int cstride;  // 16-byte vectors per column; (columns in the buffers) * cstride < 2^31 (checked by the host)
   int red_stride;
   unsigned char col[MAXCOL];
+  // launched one iteration ahead of the host's look at the solver scalars: if *skip != 0 the kernel returns at once (the
+  // device has decided that the host must act first, tmw_internal.h launch_sc_begin_iter); null: never skipped
+  const int* skip;
   DDArgs<R> dd;      // read only by the domain-decomposition kernels (DD != 0)
 };
 

@@ -7,8 +7,10 @@
 namespace tmw {
 
 // block-level sum of up to 3 doubles per thread, one atomicAdd per block and value
+// BLOCK = 0: the block size is blockDim.x (a multiple of 32, at most 256) instead of a compile-time constant
 template <int NV, int BLOCK> __device__ __forceinline__ void block_reduce_atomic(double (&v)[NV], double* dst) {
-  __shared__ double sm[NV][BLOCK / 32];
+  __shared__ double sm[NV][BLOCK ? BLOCK / 32 : 8];
+  const int nwarps = BLOCK ? BLOCK / 32 : (int)(blockDim.x >> 5);
 #pragma unroll
   for (int k = 0; k < NV; k++) {
 #pragma unroll
@@ -23,7 +25,8 @@ template <int NV, int BLOCK> __device__ __forceinline__ void block_reduce_atomic
   if (threadIdx.x < NV) {
     double s = 0;
 #pragma unroll
-    for (int i = 0; i < BLOCK / 32; i++) s += sm[threadIdx.x][i];
+    for (int i = 0; i < (BLOCK ? BLOCK / 32 : 8); i++)
+      if (i < nwarps) s += sm[threadIdx.x][i];
     atomicAdd(dst + threadIdx.x, s);
   }
 }
@@ -99,6 +102,7 @@ __device__ __forceinline__ void site_reductions(const DslashArgs<R>& a, const Si
 template <typename R, int NG, int EPI, int CLOVER, int NR, int BLOCK, int MINB, int DD>
 __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<R> a) {
   typedef typename Vec16<R>::T V;
+  if (a.skip && *a.skip) return;
   // blockIdx.x = group + ngroups * site block: the CTAs that share the links of a site block are launched together
   int sblock = blockIdx.x, grp = 0;
   if (a.ngroups > 1) {
@@ -161,7 +165,7 @@ template <typename R, int NG, int MU, int SIDE> __device__ __forceinline__ void 
 template <typename R, int NG, int BLOCK> __global__ void __launch_bounds__(BLOCK) face_pack_kernel(const DslashArgs<R> a, const FaceOut<R> fo) {
   typedef typename Vec16<R>::T V;
   const int d = blockIdx.y >> 1, side = blockIdx.y & 1;
-  if (!a.dd.part[d]) return;
+  if (!a.dd.part[d] || (a.skip && *a.skip)) return;
   const int f = blockIdx.x * BLOCK + threadIdx.x;
   if (f >= a.dd.nface[d]) return;
   const int col = a.col[blockIdx.z];
@@ -214,6 +218,7 @@ template <typename R, int NG, int MU> __device__ __forceinline__ void ghost_hops
 }
 template <typename R, int NG, int EPI, int CLOVER, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB) dslash_ext_kernel(const DslashArgs<R> a) {
+  if (a.skip && *a.skip) return;
   const Geom& g = a.g;
   const int zplane = g.Lh * g.L * g.T;                          // sites of one z-cut plane
   const int nzb = a.dd.part[0] ? 2 * zplane : 0;

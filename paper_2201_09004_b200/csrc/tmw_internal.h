@@ -9,6 +9,20 @@ namespace tmw {
 // nr = right-hand-side columns per thread (fp32: 1..4; fp64: always 1)
 cudaError_t launch_dslash(const DslashArgs<float>& a, int ng, int epi, int clover, int nr, cudaStream_t s);
 cudaError_t launch_dslash(const DslashArgs<double>& a, int ng, int epi, int clover, int nr, cudaStream_t s);
+// Shared-memory staged fp32 stencil (tmw_dslash_stage.cuh; north_star subsystem (2)): a CTA covers a tile of one time slice and
+// stages the input sites the tile's spatial hops need.
+struct StageGeom {
+  int txh, ty, tz;     // output sites per tile along x/2, y, z (one time slice)
+  int ntx, nty, ntz;   // tiles along x/2, y, z
+  int fullx;           // the tile spans the whole x extent (txh = Lh): no x halo, the x wrap happens inside the row
+  int rw;              // staged sites per row: Lh if fullx, else txh + 2 (one halo site per side)
+  int nrows;           // ty*tz interior rows + 2*tz (y halos) + 2*ty (z halos)
+  int nslots;          // nrows * rw = float4 per staged plane and column
+  int nthr;            // txh * ty * tz active threads (blockDim.x = nthr rounded up to a warp)
+};
+// epi: EPI_HOP | EPI_AINV_HOP | EPI_A_XPAY; nr = 1..3 columns per thread; the whole lattice, no domain decomposition
+cudaError_t launch_dslash_stage(const DslashArgs<float>& a, int ng, int epi, int clover, int nr, const StageGeom& sg, cudaStream_t s);
+int stage_max_threads(int nr);  // largest CTA of the staged kernel with nr columns per thread
 // loads and stores of the fp32 hopping kernel without its arithmetic (measurement: tmw_time_kernel)
 cudaError_t launch_hop_loadonly(const DslashArgs<float>& a, int ng, cudaStream_t s);
 
@@ -67,8 +81,14 @@ struct Scalars {
   double rhat_s[2];   // <rhat, s>
   double rr;          // <r, r>              (accumulated by update_xrp / resid_convert)
   double nrm;         // generic norm^2 accumulator
-  double pad[3];
+  // what the device needs to decide, at the start of an iteration, whether the host must look at this column first
+  // (sc_begin_iter with check != 0; the host sets these three whenever it (re)starts the recurrence):
+  double stop2;       // (tol |b|)^2: converged when rr <= stop2
+  double maxr2;       // largest rr since the last reliable update (0: not set yet, the next rr is taken)
+  double brk2;        // (eps_break |rhat|)^2: breakdown when |rho|^2 <= brk2 * rr
+  long long trip;     // TRIP_* bits of the last check
 };
+enum { TRIP_BROKEN = 1, TRIP_CONV = 2, TRIP_RELIABLE = 4, TRIP_BREAKDOWN = 8 };
 // GCR(k) scalars (device): see the gcr_* kernels of tmw_blas.cu
 enum { GCR_KMAX = 16 };
 struct GcrScalars {
@@ -94,16 +114,22 @@ struct ColMap {
 // Every launcher below is batched: column c of a vector starts c * (column length) after the base pointer and
 // uses the scalar block sc[c]; reductions into a plain double* go to out + 4*c.
 // sc phase kernels (one thread per column): see tmw_blas.cu
-cudaError_t launch_sc_begin_iter(Scalars* sc, const ColMap& cm, cudaStream_t s);  // zero the accumulators of the two K2 launches
-cudaError_t launch_sc_alpha(Scalars* sc, const ColMap& cm, cudaStream_t s);       // alpha = rho / rhat_v
+// `attn` (device int[2]) lets the host run one iteration ahead of the device without a round trip per iteration (SURVEY §3b
+// "read back only a convergence flag"): attn[0] != 0 = some column needs the host (converged, reliable update due,
+// breakdown, non-finite scalar); every kernel of the iteration (`skip` = attn) then returns at once, so that the vectors and
+// scalars stay as the last finished iteration left them. attn[1] counts the iterations really done.
+// sc_begin_iter: if check != 0, first test every column of cm against its stop2 / maxr2 (delta2 = delta^2) / brk2, record
+// Scalars::trip and raise attn[0]; unless attn[0] is raised: zero the accumulators of the two K2 launches, attn[1]++.
+cudaError_t launch_sc_begin_iter(Scalars* sc, const ColMap& cm, int* attn, int check, double delta2, cudaStream_t s);
+cudaError_t launch_sc_alpha(Scalars* sc, const ColMap& cm, const int* skip, cudaStream_t s);       // alpha = rho / rhat_v
 // omega = ts/tt; rho_old = rho; rho = <rhat,s> - omega <rhat,t> (= <rhat, s - omega t>, the new <rhat,r>);
 // beta = (rho/rho_old)(alpha/omega); zero rr
-cudaError_t launch_sc_omega(Scalars* sc, const ColMap& cm, cudaStream_t s);
+cudaError_t launch_sc_omega(Scalars* sc, const ColMap& cm, const int* skip, cudaStream_t s);
 // n = number of 16-byte vectors in one column of each array
-template <typename R> cudaError_t launch_update_s(int64_t n, void* sv, const void* r, const void* v, const Scalars* sc, const ColMap& cm, cudaStream_t s);     // s = r - alpha v
+template <typename R> cudaError_t launch_update_s(int64_t n, void* sv, const void* r, const void* v, const Scalars* sc, const ColMap& cm, const int* skip, cudaStream_t s);     // s = r - alpha v
 // x += alpha p + omega s; r = s - omega t; p = r + beta (p - omega v); rr += <r,r>  (the end of one BiCGStab iteration and
 // the search direction of the next in one pass: 5 reads + 3 writes instead of 8 + 3 in two kernels)
-template <typename R> cudaError_t launch_update_xrp(int64_t n, void* x, void* r, void* p, const void* sv, const void* t, const void* v, Scalars* sc, const ColMap& cm, cudaStream_t s);
+template <typename R> cudaError_t launch_update_xrp(int64_t n, void* x, void* r, void* p, const void* sv, const void* t, const void* v, Scalars* sc, const ColMap& cm, const int* skip, cudaStream_t s);
 // out[4c+0..1] += <a,b>, out[4c+2] += <b,b> (a may be null: only the norm)
 template <typename R> cudaError_t launch_dot_norm(int64_t n, const void* a, const void* b, double* out, const ColMap& cm, cudaStream_t s);
 // fp64 helpers for the reliable update
