@@ -84,6 +84,9 @@ def parse_args():
     ap.add_argument("--cpu-solve-iters", type=int, default=2, help="iterations of the oracle's BiCGStab in the bounded sample (0: skip)")
     ap.add_argument("--domains", default="1x2", help="domain-decomposition leg: domains_z x domains_t (e.g. 1x2, 2x2; 1x1: skip)")
     ap.add_argument("--kernel-reps", type=int, default=20, help="launches per kernel kind in the per-kernel roofline loop (0: skip)")
+    ap.add_argument("--stage", type=int, default=0, help="tmw_options.stage: 1 = shared-memory staged fp32 stencil wherever a tile fits (default 0: off)")
+    ap.add_argument("--stage-tile", default="0,0,0", help="tmw_options.stage_tile: tile extents x/2,y,z of the staged stencil (0,0,0: chosen by the library)")
+    ap.add_argument("--columns-per-thread", type=int, default=0, help="tmw_options.columns_per_thread of the multi-column stencil (0: automatic)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--skip-solve", action="store_true",
@@ -262,7 +265,8 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
     torch.cuda.synchronize()
     e0, e1 = ev(), ev()
     e0.record()
-    ctx = tmw.Context(L, T, dU, m, c_sw, stream=stream)
+    tuning = dict(stage=args.stage, stage_tile=tuple(int(v) for v in args.stage_tile.split(",")), columns_per_thread=args.columns_per_thread)
+    ctx = tmw.Context(L, T, dU, m, c_sw, stream=stream, **tuning)
     e1.record()
     torch.cuda.synchronize()
     setup_ms = e0.elapsed_time(e1)
@@ -433,18 +437,25 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
         pm2 = torch.empty_like(pm)
         for c in range(n):
             pm[c * nb:(c + 1) * nb].copy_(pe)
-        m0, m1, m2 = ev(), ev(), ev()
+        m0, m1, m2, m3 = ev(), ev(), ev(), ev()
+        nsch = max(2, napply // 8)
         for i in range(2):  # first pass untimed (grows the workspaces)
             barrier()
+            k0 = ctx.kernel_counts()
             m0.record()
             minfos = ctx.solve_multi(n, bm, xm, args.tol)
             m1.record()
             for _ in range(napply // 2):
                 ctx.apply_multi(tmw.D, tmw.ODD, tmw.F32, n, pm, pm2)
             m2.record()
+            for _ in range(nsch):
+                ctx.apply_schur_multi(tmw.D, tmw.F32, n, pm, pm2)
+            m3.record()
             torch.cuda.synchronize()
+            k1 = ctx.kernel_counts()
         ms_solve = max_over_ranks(m0.elapsed_time(m1))
         ms_hop = max_over_ranks(m1.elapsed_time(m2)) / (napply // 2)
+        ms_schur = max_over_ranks(m2.elapsed_time(m3)) / nsch
         multi = {"nrhs": n, "solve_ms_per_rhs": ms_solve / n, "solve_iters": [i["iters"] for i in minfos],
                  "solve_reliable_updates": [i["reliable_updates"] for i in minfos],
                  "solve_true_resid_max": max(i["true_resid"] for i in minfos),
@@ -454,9 +465,31 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
         bpc = 192.0 + 384.0 / n
         ach = bpc * Vh * n / (ms_hop * 1e-3) / 1e9
         pk, pk_src = load_peaks()
-        multi["roofline"] = {"bound": "hbm", "kernel": "dslash_kernel<float,12,EPI_HOP,NR=2|3> (multi-column hop)", "achieved": ach,
-                             "peak": pk, "unit": "GB/s", "frac": ach / pk, "bytes_per_site_and_column": bpc, "peak_source": pk_src,
+        staged = (k1["staged"] - k0["staged"]) > 0
+        multi["roofline"] = {"bound": "hbm", "kernel": ("dslash_stage_kernel" if staged else "dslash_kernel") + "<float,12,EPI_HOP,NR=2|3> (multi-column hop)",
+                             "achieved": ach, "peak": pk, "unit": "GB/s", "frac": ach / pk, "bytes_per_site_and_column": bpc, "peak_source": pk_src,
                              "note": "not HBM-bound: the links are amortised, the 8 neighbour spinors per column are not (DESIGN.md 6b)"}
+        # K1 + K2 (one Schur-operator application) on n columns: per site and column K1 96 in + 96 out, K2 96 in + 96 aux + 96 out,
+        # + the links of both launches and the two clover fields shared by the n columns
+        bps_schur = 5 * 96.0 + (bps["k1_32"] - 2 * 96.0 + bps["k2_32"] - 4 * 96.0) / n  # shared: links x 2, C^-1 (K1), C (K2)
+        ach_s = bps_schur * Vh * n / (ms_schur * 1e-3) / 1e9
+        multi["schur_ms_per_rhs"] = ms_schur / n
+        multi["roofline_schur"] = {"bound": "hbm", "kernel": "K1 + K2 on %d columns (tmw_apply_schur_multi, fp32)" % n, "achieved": ach_s, "peak": pk,
+                                   "unit": "GB/s", "frac": ach_s / pk, "bytes_per_site_and_column": bps_schur, "peak_source": pk_src}
+        multi["tuning"] = {"stage": args.stage, "stage_tile": args.stage_tile, "columns_per_thread": args.columns_per_thread, "staged_kernel_ran": staged}
+        # the fp32 ALU ceiling beside it (register-only FMA loops, tmw_time_kernel): with the links amortised the multi-column hop
+        # is as close to this ceiling as to the HBM one
+        try:
+            fmas = float(tmw.FFMA_PROBE_FMAS_PER_THREAD) * 256 * 8 * torch.cuda.get_device_properties(local_rank).multi_processor_count
+            t_f, t_f2 = ctx.time_kernel("ffma_probe", 5), ctx.time_kernel("ffma2_probe", 5)
+            peak_tf = 2 * fmas / (min(t_f, t_f2) * 1e-3) / 1e12
+            multi["alu"] = {"bound": "alu", "achieved": multi["dslash_gflops"] / world / 1e3, "peak": peak_tf, "unit": "TFLOP/s",
+                            "frac": multi["dslash_gflops"] / world / 1e3 / peak_tf, "ffma_tflops": 2 * fmas / (t_f * 1e-3) / 1e12,
+                            "ffma2_tflops": 2 * fmas / (t_f2 * 1e-3) / 1e12,
+                            "note": "achieved = 1320 flop/site of the hop at the multi-column rate; peak = measured register-only fp32 FMA rate "
+                                    "(2 flop per FMA); ~45 % of the kernel's fp32 instructions are adds and multiplies that count 1 flop"}
+        except tmw.TmwError:
+            pass
         del bm, xm, pm, pm2
         torch.cuda.empty_cache()
 

@@ -251,7 +251,10 @@ long long tmw_launch_count(const tmw_ctx* ctx);
 #define TMW_K_COPY_BYTES 21    /* BYTES moved by device-to-device copies inside the solver */
 #define TMW_K_HOP32_LOADONLY 22 /* tmw_time_kernel only: the loads and stores of TMW_K_HOP32 without its arithmetic */
 #define TMW_K_STAGED 23        /* of the fp32 stencil applications above: those that ran in the shared-memory staged kernel */
-#define TMW_K_COUNT 24
+#define TMW_K_FFMA_PROBE 24    /* tmw_time_kernel only: TMW_FFMA_PROBE_FMAS_PER_THREAD scalar fp32 FMAs (16 independent chains) per thread */
+#define TMW_K_FFMA2_PROBE 25   /* tmw_time_kernel only: the same FMAs as packed pairs (fma.rn.f32x2, 8 chains of 2) */
+#define TMW_FFMA_PROBE_FMAS_PER_THREAD (16 * 16384) /* the probe launches (SM count) x 8 CTAs of 256 threads */
+#define TMW_K_COUNT 26
 
 /*
  * counts[k] (k < min(n, TMW_K_COUNT)) = how many right-hand-side columns kernels of kind k have been applied to since
@@ -264,7 +267,9 @@ int tmw_kernel_counts(const tmw_ctx* ctx, long long* counts, int n);
  * the context's own workspace vectors, timed with CUDA events on the context stream: kind = TMW_K_HOP32, K1_32, K2_32,
  * K2_32_DOTS, K1_64, K2_64, UPDATE_S, UPDATE_XRP, or TMW_K_HOP32_LOADONLY (a kernel that issues exactly the loads and
  * stores of the fp32 hopping kernel - 8 neighbour spinors, 8 links, one store per site, same indices and launch shape -
- * and only adds the loaded values up: the memory floor of the access pattern). Single column, TMW_MIXED
+ * and only adds the loaded values up: the memory floor of the access pattern), or TMW_K_FFMA_PROBE /
+ * TMW_K_FFMA2_PROBE (register-only fp32 FMA loops: the ALU ceiling the multi-column stencil is measured against,
+ * DESIGN.md 6b; FMAs per launch = TMW_FFMA_PROBE_FMAS_PER_THREAD x 256 x 8 x SM count). Single column, TMW_MIXED
  * contexts without domain decomposition. The vectors hold whatever the last solve left there (run one first); the
  * results are not meaningful, only the time is. Synchronises the stream.
  */

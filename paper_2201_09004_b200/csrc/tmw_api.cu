@@ -1546,6 +1546,8 @@ extern "C" int tmw_time_kernel(tmw_ctx* ctx, int kind, int reps, double* ms) {
   if (!ctx) return TMW_EINVAL;
   if (!ms || reps < 1) return fail(ctx, TMW_EINVAL, "tmw_time_kernel: bad argument");
   if (ctx->opt.precision != TMW_MIXED || !ctx->dom.empty()) return fail(ctx, TMW_EINVAL, "tmw_time_kernel: needs a TMW_MIXED context without domain decomposition");
+  if ((kind == TMW_K_FFMA_PROBE || kind == TMW_K_FFMA2_PROBE) && spinor_bytes(ctx, TMW_F32) < (size_t)148 * 8 * 256 * 4)
+    return fail(ctx, TMW_EINVAL, "tmw_time_kernel: the lattice is too small to hold the probe's output");
   int rc;
   if ((rc = need_w64(ctx, 8))) return rc;
   if ((rc = need_w32(ctx, 8, TMW_F32))) return rc;
@@ -1569,6 +1571,8 @@ extern "C" int tmw_time_kernel(tmw_ctx* ctx, int kind, int reps, double* ms) {
       case TMW_K_K2_64: return dslash<double>(ctx, EPI_A_XPAY, 1, 0, W[5], W[6], W[3], -1.0, one);
       case TMW_K_UPDATE_S: LAUNCH(launch_update_s<float>(nR, X[4], X[0], X[3], ctx->sc, one, nullptr, ctx->stream)); return TMW_OK;
       case TMW_K_UPDATE_XRP: LAUNCH(launch_update_xrp<float>(nR, X[6], X[0], X[2], X[4], X[5], X[3], ctx->sc, one, nullptr, ctx->stream)); return TMW_OK;
+      case TMW_K_FFMA_PROBE:
+      case TMW_K_FFMA2_PROBE: LAUNCH(launch_ffma_probe(kind == TMW_K_FFMA2_PROBE, TMW_FFMA_PROBE_FMAS_PER_THREAD, (float*)X[7], ctx->stream)); return TMW_OK;
       case TMW_K_HOP32_LOADONLY: {
         DslashArgs<float> a = make_args<float>(ctx, 1, 0, X[7], X[3], nullptr, 1.0, one);
         LAUNCH(launch_hop_loadonly(a, ctx->ng32, ctx->stream));

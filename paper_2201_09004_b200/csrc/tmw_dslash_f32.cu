@@ -62,6 +62,44 @@ cudaError_t launch_hop_loadonly(const DslashArgs<float>& a, int ng, cudaStream_t
   else hop_loadonly_kernel<18><<<grid, 128, 0, s>>>(a);
   return cudaGetLastError();
 }
+// The fp32 ALU ceiling (tmw_time_kernel, TMW_K_FFMA_PROBE / TMW_K_FFMA2_PROBE): 16 independent FMA chains per thread in
+// registers, as scalar FFMA or as 8 packed FFMA2 pairs; enough resident warps (8 CTAs of 256 threads per SM) to fill the pipe.
+template <int PACKED> __global__ void __launch_bounds__(256) ffma_probe_kernel(float* out, float a0, float b0, int iters) {
+  float x[16];
+#pragma unroll
+  for (int i = 0; i < 16; i++) x[i] = threadIdx.x * 0.001f + i;
+  const float a = a0 + threadIdx.x * 1e-9f, b = b0 + threadIdx.x * 1e-9f;
+  if (PACKED == 0) {
+    for (int it = 0; it < iters; it++) {
+#pragma unroll
+      for (int i = 0; i < 16; i++) x[i] = fmaf(x[i], a, b);
+    }
+  } else {
+    const float2 aa = make_float2(a, a), bb = make_float2(b, b);
+    float2 y[8];
+#pragma unroll
+    for (int i = 0; i < 8; i++) y[i] = make_float2(x[2 * i], x[2 * i + 1]);
+    for (int it = 0; it < iters; it++) {
+#pragma unroll
+      for (int i = 0; i < 8; i++) y[i] = TMW_FMA2(y[i], aa, bb);
+    }
+#pragma unroll
+    for (int i = 0; i < 8; i++) { x[2 * i] = y[i].x; x[2 * i + 1] = y[i].y; }
+  }
+  float sum = 0;
+#pragma unroll
+  for (int i = 0; i < 16; i++) sum += x[i];
+  out[blockIdx.x * blockDim.x + threadIdx.x] = sum;
+}
+cudaError_t launch_ffma_probe(int packed, int fmas_per_thread, float* sink, cudaStream_t s) {
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (sms > 148) sms = 148;
+  if (packed) ffma_probe_kernel<1><<<sms * 8, 256, 0, s>>>(sink, 1.0001f, 0.5f, fmas_per_thread / 16);
+  else ffma_probe_kernel<0><<<sms * 8, 256, 0, s>>>(sink, 1.0001f, 0.5f, fmas_per_thread / 16);
+  return cudaGetLastError();
+}
 cudaError_t launch_diag(const Diag<float>& d, const Geom& g, int par, bool clover, int inverse, const void* in, void* out, cudaStream_t s) {
   return launch_diag_t<float>(d, g, par, clover, inverse, in, out, s);
 }

@@ -26,6 +26,10 @@ int stage_max_threads(int nr);  // largest CTA of the staged kernel with nr colu
 // loads and stores of the fp32 hopping kernel without its arithmetic (measurement: tmw_time_kernel)
 cudaError_t launch_hop_loadonly(const DslashArgs<float>& a, int ng, cudaStream_t s);
 
+// register-only fp32 FMA loop (packed = 0: scalar FFMA, 1: FFMA2 pairs), (SM count) x 8 CTAs of 256 threads, fmas_per_thread FMAs each;
+// sink: >= 148 * 8 * 256 floats
+cudaError_t launch_ffma_probe(int packed, int fmas_per_thread, float* sink, cudaStream_t s);
+
 // ---- domain decomposition (tmw_dd_f32.cu / tmw_dd_f64.cu) ----
 // a describes ONE domain (local geometry and fields, a.dd its cuts and receive buffers). pass 0: interior (all sites, the
 // hops through a cut skipped, sites on a cut left raw in a.out); pass 1: exterior (the sites on a cut: + ghost terms,

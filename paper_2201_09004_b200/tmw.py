@@ -28,7 +28,8 @@ DEBUG_FORCE_PIVOT, DEBUG_NO_CHUNK = 1, 2
 # kernel kinds of tmw_kernel_counts / tmw_time_kernel (include/tmw.h TMW_K_*)
 KINDS = ["hop32", "k1_32", "k2_32", "k2_32_dots", "hop64", "k1_64", "k2_64", "xpay64", "ainvxpay64", "update_s", "update_xrp",
          "acc_y", "resid_convert", "convert", "dot_norm64", "sub_norm", "diag64", "pack_both", "unpack_both", "other",
-         "memset_bytes", "copy_bytes", "hop32_loadonly", "staged"]
+         "memset_bytes", "copy_bytes", "hop32_loadonly", "staged", "ffma_probe", "ffma2_probe"]
+FFMA_PROBE_FMAS_PER_THREAD = 16 * 16384
 
 EXPORTS = ["tmw_create", "tmw_apply", "tmw_apply_schur", "tmw_solve", "tmw_apply_multi", "tmw_apply_schur_multi",
            "tmw_solve_multi", "tmw_cheb_apply", "tmw_spinor_bytes", "tmw_pack", "tmw_unpack",
