@@ -118,6 +118,11 @@ typedef struct {
      chosen by the library; a tile that does not divide the lattice or does not fit in shared memory -> the plain kernel. */
   int stage;
   int stage_tile[3];
+  /* Sweep order of the multi-column fp32 stencil launches: the lattice is cut into slabs of zchunk sites in
+     z and a launch goes through all time slices of one slab before the next, so that the +-t neighbour re-reads of all
+     columns stay in L2. 0 = automatic (the largest slab whose +-t window fits a fixed L2 budget), -1 = off (time slice
+     after time slice), > 0 = that many sites (must divide L, with L*L*zchunk/2 a multiple of 128; else off). */
+  int zchunk;
 } tmw_options;
 
 /* Test hooks (tmw_options.debug / tmw_set_debug): they change which code path runs, never the result. */

@@ -27,6 +27,7 @@ struct NvtxRange {
 using namespace tmw;
 
 enum { NW64 = 14 };
+enum { ZCHUNK_L2_BUDGET_MB = 24 };  // automatic z-slab of the multi-column sweep (tmw_options.zchunk = 0; measured)
 enum { NSLAB = 24 };  // most t-slabs of the pipelined host-pointer tmw_apply
 
 // One domain of a domain-decomposed context: a sub-lattice L x L x (L/Pz) x (T/Pt) with its own packed
@@ -377,6 +378,20 @@ static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, vo
   a.red = red;
   a.red_stride = red_stride;
   if (cb1 >= 0) { a.sb0 = cb0 / 128; a.cb_end = cb1; }
+  else if (sizeof(R) == 4 && cm.n >= 2 && !a.g.tiled) {
+    // multi-column launch: z-slab sweep order (Geom::zc) so that the +-t window of all columns fits in L2
+    int zc = 0;
+    const int64_t row = (int64_t)a.g.Lh * a.g.L;  // sites of one z of a time slice
+    if (ctx->opt.zchunk > 0) {
+      zc = ctx->opt.zchunk;
+    } else if (ctx->opt.zchunk == 0) {
+      const int64_t budget = (int64_t)ZCHUNK_L2_BUDGET_MB << 20;  // in + out spinors of all columns over the 2-slice window
+      for (int d = a.g.Lz; d >= 1; d--)
+        if (a.g.Lz % d == 0 && (row * d) % 128 == 0 && 2 * row * d * 96 * 2 * cm.n <= budget) { zc = d; break; }
+      if (zc == a.g.Lz) zc = 0;  // everything fits: keep the plain order
+    }
+    if (zc > 0 && zc < a.g.Lz && a.g.Lz % zc == 0 && (row * zc) % 128 == 0) { a.g.zc = zc; a.g.nbzt = (int)(row * zc / 128); }
+  }
   // columns per thread: as even a split of the columns into groups of at most nr32 as possible
   int nr = 1;
   if (sizeof(R) == 4 && cm.n > 1) {
@@ -555,7 +570,7 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
       o.max_iter < 0 || !(o.delta > 0.0) || !(o.delta < 1.0) || (o.solver != TMW_BICGSTAB && o.solver != TMW_GCR) || o.nkrylov < 1 ||
       o.nkrylov > GCR_KMAX || o.columns_per_thread < 0 || o.columns_per_thread > 4 ||
       (o.debug & ~(TMW_DEBUG_FORCE_PIVOT | TMW_DEBUG_NO_CHUNK)) || o.stage < -1 || o.stage > 1 || o.stage_tile[0] < 0 ||
-      o.stage_tile[1] < 0 || o.stage_tile[2] < 0)
+      o.stage_tile[1] < 0 || o.stage_tile[2] < 0 || o.zchunk < -1)
     return fail(nullptr, TMW_EINVAL, "tmw_create: bad option value");
   if (!isfinite(m.re) || !isfinite(m.im) || !isfinite(c_sw)) return fail(nullptr, TMW_EINVAL, "tmw_create: non-finite parameter");
   const int pz = o.domains_z > 1 ? o.domains_z : 1, pt = o.domains_t > 1 ? o.domains_t : 1;

@@ -30,6 +30,12 @@ struct Geom {
   int tiled;
   int lx, ly, lz, lt;
   int ntx, nty;    // tiles along xh and y
+  // Sweep order of the 1-D mapping (tiled = 0). zc = 0: site blocks in cb order, i.e. time slice after time slice. zc > 0
+  // (a divisor of Lz with Lh*L*zc a multiple of the CTA size): the lattice is cut into Lz/zc slabs in z and the blocks go
+  // through ALL time slices of one slab before the next slab, so that the -t / +t neighbours of a block are re-read
+  // after 2*Lh*L*zc sites instead of 2*Lh*L*Lz: with many right-hand-side columns per launch a whole time slice of
+  // every column no longer fits in L2 between the two reads. nbzt = CTAs per (slab, time slice).
+  int zc, nbzt;
 };
 
 // coordinates of one site of a parity: x = 2*xh + ((y + z + t + par) & 1)
@@ -51,6 +57,11 @@ template <int BLOCK> __device__ __forceinline__ bool thread_site(const Geom& g, 
     s.t = ((int)blockIdx.z << g.lt) | q;
     s.cb = s.xh + g.Lh * (s.y + g.L * (s.z + g.L * s.t));
     return true;
+  }
+  if (g.zc) {  // slab-major, then t, then the blocks of the slab's share of the time slice
+    const int q = sblock / g.nbzt, j = sblock - q * g.nbzt;
+    const int slab = q / g.T, t = q - slab * g.T;
+    sblock = (t * (g.Lz / g.zc) + slab) * g.nbzt + j;
   }
   s.cb = sblock * BLOCK + tid;
   s.xh = s.cb % g.Lh;

@@ -78,6 +78,25 @@ def test_hopping_multi_vs_oracle(tmw, L, T, nrhs, tile, spread):
                         assert site <= tol, (prec, op, par, c, site, glob)
 
 
+@pytest.mark.parametrize("L,T,nrhs,zchunk,cpt", [(8, 6, 5, 4, 2), (8, 4, 3, 4, 3), (16, 4, 2, 2, 2), (16, 4, 4, 8, 4), (8, 4, 2, 3, 2), (8, 4, 2, -1, 2)])
+def test_zchunk_sweep_vs_oracle(tmw, L, T, nrhs, zchunk, cpt):
+    """tmw_options.zchunk: the multi-column launches visit the site blocks slab by slab in z (all time slices of a slab
+    first) - a permutation of the CTAs that must not change any output site. zchunk = 3 does not divide L (ignored)."""
+    U = synth.gauge_field(L, T, 0.4, seed=1)
+    cols = columns(L, T, nrhs)
+    with tmw.Context(L, T, dev(U), 0.1, zchunk=zchunk, columns_per_thread=cpt) as ctx:
+        for op in (tmw.D, tmw.DDAG):
+            for par in (0, 1):
+                inp = pack_multi(ctx, tmw, cols, 1 - par, tmw.F32)
+                out = torch.full_like(inp, 0x7f)
+                ctx.apply_multi(op, tmw.ODD if par else tmw.EVEN, tmw.F32, nrhs, inp, out)
+                got = unpack_multi(ctx, tmw, out, nrhs, par, tmw.F32, L, T)
+                for c in range(nrhs):
+                    ref = mask_parity(oracle.apply(U, mask_parity(cols[c], 1 - par), 0.1, dagger=(op == tmw.DDAG)), par)
+                    site, glob = H.per_site_rel_err(got[c], ref)
+                    assert site <= TOL32, (op, par, c, site, glob)
+
+
 @pytest.mark.parametrize("spread", SPREADS[1:], ids=lambda d: "-".join(f"{k[8:]}{v}" for k, v in d.items()))
 @pytest.mark.parametrize("case", [
     dict(L=8, T=4, eps=0.4, m=-0.0695 + 0.0j, c_sw=1.0509, nrhs=5),
