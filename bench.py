@@ -79,7 +79,7 @@ def parse_args():
     ap.add_argument("--multi-rhs", type=int, default=3,
                     help="columns of the extra tmw_solve_multi / tmw_apply_multi leg (0 or 1: skip); 3 fit at 48^3 x 144")
     ap.add_argument("--cpu-solve", action="store_true",
-                    help="time the oracle's full-lattice fp64 BiCGStab on this config's source to convergence (7 min at 48^3 x 144 on "
+                    help="time the oracle's full-lattice fp64 BiCGStab on this config's source to convergence (6 min at 48^3 x 144 on "
                          "16 cores) instead of the default bounded sample of --cpu-solve-iters iterations")
     ap.add_argument("--cpu-solve-iters", type=int, default=2, help="iterations of the oracle's BiCGStab in the bounded sample (0: skip)")
     ap.add_argument("--domains", default="1x2", help="domain-decomposition leg: domains_z x domains_t (e.g. 1x2, 2x2; 1x1: skip)")
@@ -545,6 +545,8 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
         # the oracle's BiCGStab beside tmw_solve (the paper's one number for this path is a CPU BiCGStab time):
         # to convergence with --cpu-solve, else a bounded sample of --cpu-solve-iters iterations (each = 2 D applications +
         # the recurrences on the full lattice), scaled by the iteration count the full solve needs
+        cpu["note"] = ("not like for like: the oracle is a deliberately plain fp64 program (explicit 4x4 gamma matrices on full spinors, 18-real "
+                       "links, AoS, no even-odd, no SIMD), the GPU figure is the fp32 spin-projected 12-real kernel; the reference ships no CPU code")
         if (args.cpu_solve or args.cpu_solve_iters > 0) and not args.skip_solve:
             import oracle
             import psutil
@@ -577,8 +579,8 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
                                solve_iters=full_iters, solve_s_per_iter=per_iter,
                                solve=f"oracle.bicgstab (full-lattice fp64 BiCGStab, no preconditioning): {k} iterations timed ({dt:.1f} s incl. its "
                                      f"closing residual application), scaled to the {full_iters} iterations the solve to 1e-10 takes, + its "
-                                     f"clover-leaf setup ({t_f:.1f} s); --cpu-solve runs it to convergence (411 s measured at 48^3 x 144 to "
-                                     "1e-12: profiles/r2_oracle_cfg4_solve.md)")
+                                     f"clover-leaf setup ({t_f:.1f} s); --cpu-solve runs it to convergence (340 s measured at 48^3 x 144 to "
+                                     "1e-10: profiles/r2_oracle_cfg4_solve.md)")
                 del Fo
 
     ctx.destroy()

@@ -625,8 +625,8 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
   CKC(cudaMallocHost((void**)&ctx->attn_host, 6 * sizeof(int)));
   CKA(&ctx->attn, 2 * sizeof(int));
   for (int i = 0; i < 2; i++) CKC(cudaEventCreateWithFlags(&ctx->ev_lag[i], cudaEventDisableTiming));
-  CKC(cudaMallocHost((void**)&ctx->gs_host, sizeof(GcrScalars)));
-  CKA(&ctx->gs, sizeof(GcrScalars));
+  CKC(cudaMallocHost((void**)&ctx->gs_host, MAXCOL * sizeof(GcrScalars)));
+  CKA(&ctx->gs, MAXCOL * sizeof(GcrScalars));
   const size_t Vh = (size_t)ctx->g.Vh;
   const int np32 = (ctx->ng32 == 12) ? 3 : 5;
   for (int p = 0; p < 2; p++) {
@@ -1274,69 +1274,93 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
 }
 
 
-// Restarted GCR(k) (the paper's GPU solver) on the Schur system of column c, inner
-// precision R, restarted from the fp64 true residual (the same reliable update as in solve_schur): per step one Mhat
-// application (K1, K2) and the five launches of launch_gcr_step.
+// Restarted GCR(k) (the paper's GPU solver) on the Schur systems of the columns c with
+// !cs[c].done, inner precision R, restarted from the fp64 true residual (the same reliable update as in solve_schur). The
+// columns run in lockstep like BiCGStab's: per step one Mhat application (K1, K2) over the columns still stepping, so that
+// links and clover blocks are read once for all of them, and the five launches of launch_gcr_step; a column leaves the
+// steps of a cycle when it has converged or its residual has dropped by delta, and all columns of the cycle restart together.
 //   w64 as in solve_schur; w32: 0 r, 1 zero (the rhat slot of resid_convert), 6 x, 7 tmp_e
+//   gcr_q, gcr_p: nkrylov x ws_cols inner-precision spinors, vector j of column c at (j * ws_cols + c)
 template <typename R>
-int solve_gcr(tmw_ctx* ctx, int c, double tol, ColState& q) {
+int solve_gcr(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
   cudaStream_t s = ctx->stream;
   const int64_t n64 = (int64_t)ctx->g.Vh * 12;
   const int64_t nR = (int64_t)ctx->g.Vh * 24 * (int64_t)sizeof(R) / 16;
-  const size_t bytesR = (size_t)nR * 16;
-  const int k = ctx->opt.nkrylov;
+  const size_t bytesR = (size_t)nR * 16, bytes64 = (size_t)n64 * 16;
+  const int k = ctx->opt.nkrylov, ncw = ctx->ws_cols;
   void** W = ctx->w64;
   void** X = ctx->w32;
   int rc;
-  if (!ctx->gcr_q) { if ((rc = ws_alloc(ctx, &ctx->gcr_q, bytesR * k))) return rc; }
-  if (!ctx->gcr_p) { if ((rc = ws_alloc(ctx, &ctx->gcr_p, bytesR * k))) return rc; }
-  ColMap one;
-  one.n = 0;
-  cols_add(one, c);
-  void* r = colp(X[0], c, bytesR);
-  void* x = colp(X[6], c, bytesR);
-  void* tmp = colp(X[7], c, bytesR);
+  if (!ctx->gcr_q) { if ((rc = ws_alloc(ctx, &ctx->gcr_q, bytesR * k * ncw))) return rc; }
+  if (!ctx->gcr_p) { if ((rc = ws_alloc(ctx, &ctx->gcr_p, bytesR * k * ncw))) return rc; }
+  void *r = X[0], *x = X[6], *tmp = X[7];
   Scalars* h = ctx->sc_host;
   GcrScalars* gh = ctx->gs_host;
   const bool verbose = ctx->verbose;
-  const ColMap zero = cols_first(1);
-  CK(cudaMemsetAsync(colp(W[3], c, (size_t)n64 * 16), 0, (size_t)n64 * 16, s));
-  CK(cudaMemsetAsync(colp(W[6], c, (size_t)n64 * 16), 0, (size_t)n64 * 16, s));
-  CK(cudaMemsetAsync(colp(X[1], c, bytesR), 0, bytesR, s));
   const int max_iter = ctx->opt.max_iter;
+  bool given_up[MAXCOL] = {false};  // max_iter reached
+  for (int c = 0; c < ncols; c++) {
+    if (cs[c].done) continue;
+    CK(cudaMemsetAsync(colp(W[3], c, bytes64), 0, bytes64, s));
+    CK(cudaMemsetAsync(colp(W[6], c, bytes64), 0, bytes64, s));
+    CK(cudaMemsetAsync(colp(X[1], c, bytesR), 0, bytesR, s));
+  }
   for (;;) {
-    // true residual r64 = bhat - Mhat y (W[6] holds Mhat y), r = (R) r64, |r64|^2
+    ColMap cyc;  // the columns of this cycle
+    cyc.n = 0;
+    for (int c = 0; c < ncols; c++) if (!cs[c].done && !given_up[c]) cols_add(cyc, c);
+    if (cyc.n == 0) break;
+    // true residuals r64 = bhat - Mhat y (W[6] holds Mhat y), r = (R) r64, |r64|^2
     memset(h, 0, MAXCOL * sizeof(Scalars));
     if ((rc = push_scalars(ctx))) return rc;
-    LAUNCHK(TMW_K_RESID_CONVERT, one.n, launch_resid_convert<R>(n64, ctx->vh_loc, W[2], W[6], W[4], X[0], X[1], nullptr, ctx->sc, one, s));
+    LAUNCHK(TMW_K_RESID_CONVERT, cyc.n, launch_resid_convert<R>(n64, ctx->vh_loc, W[2], W[6], W[4], r, X[1], nullptr, ctx->sc, cyc, s));
     if ((rc = fetch_scalars(ctx))) return rc;
-    q.rnorm = q.maxr = sqrt(h[c].rr);
-    q.iter_resid = q.rnorm / q.bnorm;
-    if (verbose) fprintf(stderr, "[tmw] gcr col %d cycle %d it %d true |r|/|b| %.3e\n", c, q.updates, q.iters, q.iter_resid);
-    if (!isfinite(q.rnorm)) return fail(ctx, TMW_EBREAKDOWN, "tmw_solve: non-finite true residual");
-    if (q.rnorm <= tol * q.bnorm) { q.done = true; return TMW_OK; }
-    if (q.iters >= max_iter) return fail(ctx, TMW_ENOCONV, "tmw_solve: max_iter reached");
-    CK(cudaMemsetAsync(x, 0, bytesR, s));
-    CK(cudaMemsetAsync(ctx->gs, 0, sizeof(GcrScalars), s));
-    for (int i = 0; i < k && q.iters < max_iter; i++) {
+    ColMap step;  // the columns still stepping
+    step.n = 0;
+    for (int i = 0; i < cyc.n; i++) {
+      const int c = cyc.col[i];
+      ColState& q = cs[c];
+      q.rnorm = q.maxr = sqrt(h[c].rr);
+      q.iter_resid = q.rnorm / q.bnorm;
+      if (verbose) fprintf(stderr, "[tmw] gcr col %d cycle %d it %d true |r|/|b| %.3e\n", c, q.updates, q.iters, q.iter_resid);
+      if (!isfinite(q.rnorm)) return fail(ctx, TMW_EBREAKDOWN, "tmw_solve: non-finite true residual");
+      if (q.rnorm <= tol * q.bnorm) q.done = true;
+      else if (q.iters >= max_iter) given_up[c] = true;
+      else cols_add(step, c);
+    }
+    if (step.n == 0) continue;
+    cyc = step;
+    for (int i = 0; i < cyc.n; i++) CK(cudaMemsetAsync(colp(x, cyc.col[i], bytesR), 0, bytesR, s));
+    CK(cudaMemsetAsync(ctx->gs, 0, MAXCOL * sizeof(GcrScalars), s));
+    for (int i = 0; i < k && step.n > 0; i++) {
       // q_i = Mhat r (orthogonalised in launch_gcr_step), p_i = r - ...
-      if ((rc = schur<R>(ctx, 0, r, colp(ctx->gcr_q, i, bytesR), tmp, zero))) return rc;
-      LAUNCH(launch_gcr_step<R>(nR, i, ctx->gcr_q, ctx->gcr_p, x, r, ctx->gs, s));
+      if ((rc = schur<R>(ctx, 0, r, (char*)ctx->gcr_q + (size_t)i * ncw * bytesR, tmp, step))) return rc;
+      LAUNCH(launch_gcr_step<R>(nR, i, ncw, ctx->gcr_q, ctx->gcr_p, x, r, ctx->gs, step, s));
       ctx->launches += (i > 0) ? 4 : 3;  // launch_gcr_step is 5 launches (4 for the first vector)
-      CK(cudaMemcpyAsync(gh, ctx->gs, sizeof(GcrScalars), cudaMemcpyDeviceToHost, s));
+      CK(cudaMemcpyAsync(gh, ctx->gs, MAXCOL * sizeof(GcrScalars), cudaMemcpyDeviceToHost, s));
       CK(cudaStreamSynchronize(s));
-      q.iters++;
-      if (!isfinite(gh->rr) || !(gh->nw > 0.0)) return fail(ctx, TMW_EBREAKDOWN, "tmw_solve: GCR breakdown (Mhat p vanished or non-finite)");
-      const double rn = sqrt(gh->rr);
-      q.iter_resid = rn / q.bnorm;
-      if (verbose) fprintf(stderr, "[tmw] gcr col %d it %d |r|/|b| %.3e\n", c, q.iters, q.iter_resid);
-      if (rn <= tol * q.bnorm || rn < ctx->opt.delta * q.maxr) break;
+      ColMap next;
+      next.n = 0;
+      for (int j = 0; j < step.n; j++) {
+        const int c = step.col[j];
+        ColState& q = cs[c];
+        q.iters++;
+        if (!isfinite(gh[c].rr) || !(gh[c].nw > 0.0)) return fail(ctx, TMW_EBREAKDOWN, "tmw_solve: GCR breakdown (Mhat p vanished or non-finite)");
+        const double rn = sqrt(gh[c].rr);
+        q.iter_resid = rn / q.bnorm;
+        if (verbose) fprintf(stderr, "[tmw] gcr col %d it %d |r|/|b| %.3e\n", c, q.iters, q.iter_resid);
+        if (!(rn <= tol * q.bnorm || rn < ctx->opt.delta * q.maxr || q.iters >= max_iter)) cols_add(next, c);
+      }
+      step = next;
     }
     // restart: y += x, Mhat y in fp64
-    LAUNCHK(TMW_K_ACC_Y, one.n, launch_acc_y<R>(n64, ctx->vh_loc, W[3], X[6], one, s));
-    if ((rc = schur<double>(ctx, 0, W[3], W[6], W[5], one))) return rc;
-    q.updates++;
+    LAUNCHK(TMW_K_ACC_Y, cyc.n, launch_acc_y<R>(n64, ctx->vh_loc, W[3], x, cyc, s));
+    if ((rc = schur<double>(ctx, 0, W[3], W[6], W[5], cyc))) return rc;
+    for (int i = 0; i < cyc.n; i++) cs[cyc.col[i]].updates++;
   }
+  for (int c = 0; c < ncols; c++)
+    if (given_up[c]) return fail(ctx, TMW_ENOCONV, "tmw_solve: max_iter reached");
+  return TMW_OK;
 }
 
 }  // namespace
@@ -1356,11 +1380,7 @@ static int solve_packed(tmw_ctx* ctx, int nrhs, const ColMap& cm, double tol, Co
   {
     NvtxRange nvtx_it("tmw_solve: Krylov iterations");
     if (ctx->opt.solver == TMW_GCR) {
-      for (int i = 0; i < cm.n; i++) {  // GCR keeps 2 k Krylov vectors per system: the columns go one after another
-        rc = dbl ? solve_gcr<double>(ctx, cm.col[i], tol, cs[cm.col[i]]) : solve_gcr<float>(ctx, cm.col[i], tol, cs[cm.col[i]]);
-        if (rc != TMW_OK && rc != TMW_ENOCONV) return rc;
-        if (rc == TMW_ENOCONV) status = rc;
-      }
+      status = dbl ? solve_gcr<double>(ctx, nrhs, tol, cs) : solve_gcr<float>(ctx, nrhs, tol, cs);
     } else {
       status = dbl ? solve_schur<double>(ctx, nrhs, tol, cs) : solve_schur<float>(ctx, nrhs, tol, cs);
     }
@@ -1513,17 +1533,17 @@ extern "C" int tmw_solve_multi(tmw_ctx* ctx, int nrhs, const double* b, double* 
   if (nrhs > 1 && !(ctx->opt.debug & TMW_DEBUG_NO_CHUNK)) {
     const size_t b64 = spinor_bytes(ctx, TMW_F64), bin = spinor_bytes(ctx, ctx->opt.precision == TMW_DOUBLE ? TMW_F64 : TMW_F32);
     const size_t cbytes = (size_t)ctx->V * 24 * 8;
-    const size_t per_col = 8 * b64 + 8 * bin + (ctx->opt.location == TMW_HOST ? 2 * cbytes : 0);
+    // GCR: 2 nkrylov Krylov vectors per column on top (the columns step together)
+    const size_t gcr = ctx->opt.solver == TMW_GCR ? 2 * (size_t)ctx->opt.nkrylov * bin : 0;
+    const size_t per_col = 8 * b64 + 8 * bin + gcr + (ctx->opt.location == TMW_HOST ? 2 * cbytes : 0);
     size_t held = 0;
     for (int i = 0; i < NW64; i++) if (ctx->w64[i]) held += b64 * ctx->ws_cols;
     for (int i = 0; i < 8; i++) if (ctx->w32[i]) held += bin * ctx->ws_cols;
     for (int i = 0; i < 2; i++) if (ctx->canon[i]) held += cbytes * ctx->ws_cols;
     size_t free_b = 0, total_b = 0;
     CK(cudaMemGetInfo(&free_b, &total_b));
-    // GCR: 2 nkrylov Krylov vectors of ONE column (the columns go one after another), allocated inside the solve
-    const size_t gcr = ctx->opt.solver == TMW_GCR ? 2 * (size_t)ctx->opt.nkrylov * bin : 0;
-    if (ctx->gcr_q) held += gcr;
-    const double avail = 0.92 * (double)(free_b + held) - (double)gcr;
+    if (ctx->gcr_q) held += gcr * ctx->ws_cols;
+    const double avail = 0.92 * (double)(free_b + held);
     const size_t fit = avail > 0 ? (size_t)avail / per_col : 0;
     if (fit < (size_t)nrhs && ctx->ws_cols < nrhs) {
       chunk = fit < 1 ? 1 : (int)fit;

@@ -320,11 +320,18 @@ cudaError_t launch_scale(int64_t n64, void* dst, const void* src, double c, cuda
 }
 
 // ---- GCR(k) kernels (the paper's "standard GPU inverter with GCR algorithm") ----
-// Krylov vectors q_j (= Mhat p_j, orthogonal, NOT normalised: nq[j] = <q_j,q_j>) and p_j, j < KMAX, are stored back to
-// back: vector j starts j*n work items after the base pointer. All scalars stay in a GcrScalars block on the device.
+// Batched over right-hand-side columns like the BiCGStab kernels: blockIdx.y (vector kernels) or blockIdx.x / threadIdx.x
+// (scalar kernels) = slot, column c = cm.col[slot] with its own GcrScalars block gs[c]. Krylov vectors q_j (= Mhat p_j,
+// orthogonal, NOT normalised: nq[j] = <q_j,q_j>) and p_j, j < KMAX: vector j of column c starts (j*ncw + c)*n work items
+// after the base pointer (ncw = columns the workspace holds), so that the vectors j of all columns are one multi-column
+// spinor the stencil can write. x and r of column c start c*n work items after their base pointers.
 
-// dots[2j..2j+1] += <q_j, w> for j < i: one pass over w and the i vectors q_j
-template <typename R> __global__ void __launch_bounds__(BB) gcr_dots_kernel(int64_t n, int i, const R* Q, const R* w, GcrScalars* gs) {
+// dots[2j..2j+1] += <q_j, w> for j < i (w = q_i before orthogonalisation): one pass over w and the i vectors q_j
+template <typename R> __global__ void __launch_bounds__(BB) gcr_dots_kernel(int64_t n, int i, int ncw, const R* Q, GcrScalars* gs0, ColMap cm) {
+  const int c = cm.col[blockIdx.y];
+  GcrScalars* gs = gs0 + c;
+  Q += 4 * n * c;
+  const R* w = Q + 4 * n * ncw * i;
   double acc[2 * GCR_KMAX];
 #pragma unroll
   for (int j = 0; j < 2 * GCR_KMAX; j++) acc[j] = 0.0;
@@ -335,7 +342,7 @@ template <typename R> __global__ void __launch_bounds__(BB) gcr_dots_kernel(int6
     for (int j = 0; j < GCR_KMAX; j++) {
       if (j < i) {
         R qq[4];
-        ldp(Q + 4 * n * j, e, qq);
+        ldp(Q + 4 * n * ncw * j, e, qq);
         acc[2 * j] += (double)(qq[0] * ww[0] + qq[1] * ww[1] + qq[2] * ww[2] + qq[3] * ww[3]);
         acc[2 * j + 1] += (double)(qq[0] * ww[1] - qq[1] * ww[0] + qq[2] * ww[3] - qq[3] * ww[2]);
       }
@@ -358,8 +365,9 @@ template <typename R> __global__ void __launch_bounds__(BB) gcr_dots_kernel(int6
     __syncthreads();
   }
 }
-// coef_j = dots_j / nq_j (j < i); zero the accumulators of the next two kernels
-__global__ void gcr_coef_kernel(int i, GcrScalars* gs) {
+// coef_j = dots_j / nq_j (j < i); zero the accumulators of the next two kernels. blockIdx.x = slot, threadIdx.x = j
+__global__ void gcr_coef_kernel(int i, GcrScalars* gs0, ColMap cm) {
+  GcrScalars* gs = gs0 + cm.col[blockIdx.x];
   const int j = threadIdx.x;
   if (j < i) {
     gs->coef[2 * j] = gs->dots[2 * j] / gs->nq[j];
@@ -369,7 +377,12 @@ __global__ void gcr_coef_kernel(int i, GcrScalars* gs) {
   if (j == 0) { gs->nw = 0.0; gs->g[0] = gs->g[1] = 0.0; gs->rr = 0.0; }
 }
 // w -= sum_j coef_j q_j (stored as q_i);  p_i = r - sum_j coef_j p_j;  nw += <w,w>;  g += <w,r>
-template <typename R> __global__ void __launch_bounds__(BB) gcr_orth_kernel(int64_t n, int i, R* Q, R* P, const R* r, GcrScalars* gs) {
+template <typename R> __global__ void __launch_bounds__(BB) gcr_orth_kernel(int64_t n, int i, int ncw, R* Q, R* P, const R* r, GcrScalars* gs0, ColMap cm) {
+  const int col = cm.col[blockIdx.y];
+  GcrScalars* gs = gs0 + col;
+  Q += 4 * n * col;
+  P += 4 * n * col;
+  r += 4 * n * col;
   R cr[GCR_KMAX], ci[GCR_KMAX];
 #pragma unroll
   for (int j = 0; j < GCR_KMAX; j++) {
@@ -377,8 +390,8 @@ template <typename R> __global__ void __launch_bounds__(BB) gcr_orth_kernel(int6
     ci[j] = j < i ? (R)gs->coef[2 * j + 1] : (R)0;
   }
   double acc[3] = {0, 0, 0};
-  R* w = Q + 4 * n * i;
-  R* p = P + 4 * n * i;
+  R* w = Q + 4 * n * ncw * i;
+  R* p = P + 4 * n * ncw * i;
   for (int64_t e = (int64_t)blockIdx.x * BB + threadIdx.x; e < n; e += (int64_t)gridDim.x * BB) {
     R ww[4], pp[4], rr[4];
     ldp(w, e, ww); ldp(r, e, rr);
@@ -388,7 +401,7 @@ template <typename R> __global__ void __launch_bounds__(BB) gcr_orth_kernel(int6
     for (int j = 0; j < GCR_KMAX; j++) {
       if (j < i) {
         R qq[4], pj[4];
-        ldp(Q + 4 * n * j, e, qq); ldp(P + 4 * n * j, e, pj);
+        ldp(Q + 4 * n * ncw * j, e, qq); ldp(P + 4 * n * ncw * j, e, pj);
 #pragma unroll
         for (int c = 0; c < 2; c++) {
           ww[2 * c] -= cr[j] * qq[2 * c] - ci[j] * qq[2 * c + 1];
@@ -409,17 +422,22 @@ template <typename R> __global__ void __launch_bounds__(BB) gcr_orth_kernel(int6
   double* dst[3] = {&gs->nw, &gs->g[0], &gs->g[1]};
   reduce_atomic<3>(acc, dst);
 }
-// a = g / nw; nq[i] = nw
-__global__ void gcr_alpha_kernel(int i, GcrScalars* gs) {
+// a = g / nw; nq[i] = nw. threadIdx.x = slot
+__global__ void gcr_alpha_kernel(int i, GcrScalars* gs0, ColMap cm) {
+  GcrScalars* gs = gs0 + cm.col[threadIdx.x];
   gs->nq[i] = gs->nw;
   gs->a[0] = gs->g[0] / gs->nw;
   gs->a[1] = gs->g[1] / gs->nw;
 }
 // x += a p_i;  r -= a q_i;  rr += <r,r>
-template <typename R> __global__ void __launch_bounds__(BB) gcr_update_kernel(int64_t n, int i, R* x, R* r, const R* Q, const R* P, GcrScalars* gs) {
+template <typename R> __global__ void __launch_bounds__(BB) gcr_update_kernel(int64_t n, int i, int ncw, R* x, R* r, const R* Q, const R* P, GcrScalars* gs0, ColMap cm) {
+  const int col = cm.col[blockIdx.y];
+  GcrScalars* gs = gs0 + col;
+  x += 4 * n * col;
+  r += 4 * n * col;
   const R ar = (R)gs->a[0], ai = (R)gs->a[1];
-  const R* w = Q + 4 * n * i;
-  const R* p = P + 4 * n * i;
+  const R* w = Q + 4 * n * (ncw * i + col);
+  const R* p = P + 4 * n * (ncw * i + col);
   double acc[1] = {0};
   for (int64_t e = (int64_t)blockIdx.x * BB + threadIdx.x; e < n; e += (int64_t)gridDim.x * BB) {
     R xx[4], rr[4], ww[4], pp[4];
@@ -484,19 +502,17 @@ cudaError_t launch_add64(int64_t n64, void* a, const void* b, const ColMap& cm, 
   return cudaGetLastError();
 }
 
-template <typename R> cudaError_t launch_gcr_step(int64_t n16, int i, void* Q, void* P, void* x, void* r, GcrScalars* gs, cudaStream_t s) {
+template <typename R> cudaError_t launch_gcr_step(int64_t n16, int i, int ncw, void* Q, void* P, void* x, void* r, GcrScalars* gs, const ColMap& cm, cudaStream_t s) {
   const int64_t np = pairs_of<R>(n16);
-  if (i > 0) {
-    gcr_dots_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, i, (const R*)Q, (const R*)Q + 4 * np * i, gs);
-  }
-  gcr_coef_kernel<<<1, GCR_KMAX, 0, s>>>(i, gs);
-  gcr_orth_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, i, (R*)Q, (R*)P, (const R*)r, gs);
-  gcr_alpha_kernel<<<1, 1, 0, s>>>(i, gs);
-  gcr_update_kernel<R><<<blas_grid(np), BB, 0, s>>>(np, i, (R*)x, (R*)r, (const R*)Q, (const R*)P, gs);
+  if (i > 0) gcr_dots_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, i, ncw, (const R*)Q, gs, cm);
+  gcr_coef_kernel<<<cm.n, GCR_KMAX, 0, s>>>(i, gs, cm);
+  gcr_orth_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, i, ncw, (R*)Q, (R*)P, (const R*)r, gs, cm);
+  gcr_alpha_kernel<<<1, cm.n, 0, s>>>(i, gs, cm);
+  gcr_update_kernel<R><<<grid_of(np, cm), BB, 0, s>>>(np, i, ncw, (R*)x, (R*)r, (const R*)Q, (const R*)P, gs, cm);
   return cudaGetLastError();
 }
-template cudaError_t launch_gcr_step<float>(int64_t, int, void*, void*, void*, void*, GcrScalars*, cudaStream_t);
-template cudaError_t launch_gcr_step<double>(int64_t, int, void*, void*, void*, void*, GcrScalars*, cudaStream_t);
+template cudaError_t launch_gcr_step<float>(int64_t, int, int, void*, void*, void*, void*, GcrScalars*, const ColMap&, cudaStream_t);
+template cudaError_t launch_gcr_step<double>(int64_t, int, int, void*, void*, void*, void*, GcrScalars*, const ColMap&, cudaStream_t);
 
 #define TMW_INST(R)                                                                                                          \
   template cudaError_t launch_update_s<R>(int64_t, void*, const void*, const void*, const Scalars*, const ColMap&, const int*, cudaStream_t);           \

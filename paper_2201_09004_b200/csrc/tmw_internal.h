@@ -105,10 +105,12 @@ struct GcrScalars {
   double rr;                  // <r, r> after the update
   double pad[2];
 };
-// One GCR step after q_i = Mhat p_i(= Mhat r) has been stored as vector i of Q: orthogonalise it against q_0..q_{i-1}
-// (classical Gram-Schmidt, one pass for the dot products and one for the updates), build p_i alongside, then
-// x += a p_i, r -= a q_i with a = <q_i, r>/<q_i, q_i>; gs->rr = |r|^2. n16 = 16-byte vectors per spinor; 5 launches.
-template <typename R> cudaError_t launch_gcr_step(int64_t n16, int i, void* Q, void* P, void* x, void* r, GcrScalars* gs, cudaStream_t s);
+// One GCR step for the columns of cm after q_i = Mhat r has been stored as vector i of Q: orthogonalise it against
+// q_0..q_{i-1} (classical Gram-Schmidt, one pass for the dot products and one for the updates), build p_i alongside, then
+// x += a p_i, r -= a q_i with a = <q_i, r>/<q_i, q_i>; gs[c].rr = |r|^2. n16 = 16-byte vectors per spinor; vector j of
+// column c of Q / P starts (j*ncw + c) spinors after the base pointer; 5 launches (4 for i = 0).
+struct ColMap;
+template <typename R> cudaError_t launch_gcr_step(int64_t n16, int i, int ncw, void* Q, void* P, void* x, void* r, GcrScalars* gs, const ColMap& cm, cudaStream_t s);
 
 // The right-hand-side columns a batched launch works on: slot j -> column col[j].
 struct ColMap {

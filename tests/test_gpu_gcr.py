@@ -39,6 +39,36 @@ def test_gcr_solve_vs_oracle(tmw, case, precision, nkrylov):
         check_solution(U, b, x.cpu().numpy(), m, c_sw, x_ref, mass_scalar=scalar)
 
 
+@pytest.mark.parametrize("precision,nkrylov,c_sw", [("mixed", 4, 1.0509), ("mixed", 0, 0.0), ("double", 3, 1.0509)])
+def test_gcr_columns_in_lockstep_vs_oracle(tmw, precision, nkrylov, c_sw):
+    """tmw_solve_multi with TMW_GCR steps all columns together (one multi-column Schur application per step); columns of
+    different kind leave the steps of a cycle, and the solve, at different times: every column against the oracle."""
+    L, T, m = 8, 4, -0.0695 + 0.0j
+    U = synth.gauge_field(L, T, 0.4, seed=1)
+    F = oracle.field_strength(U) if c_sw else None
+    g = synth.gaussian_spinor(L, T, 3)
+    b = np.stack([synth.point_source(L, T, 0, 0), synth.z2_source(L, T, 2), g, 1e-4 * g, synth.point_source(L, T, 2, 1),
+                  np.zeros_like(g), synth.gaussian_spinor(L, T, 5)])
+    n = b.shape[0]
+    with tmw.Context(L, T, dev(U), m, c_sw, precision=tmw.MIXED if precision == "mixed" else tmw.DOUBLE, solver=tmw.GCR, nkrylov=nkrylov) as ctx:
+        x = torch.empty(b.shape, dtype=torch.complex128, device="cuda")
+        k0 = ctx.kernel_counts()
+        infos = ctx.solve_multi(n, dev(b), x, 1e-10)
+        k1 = ctx.kernel_counts()
+        x = x.cpu().numpy()
+        assert infos[5]["iters"] == 0 and np.count_nonzero(x[5]) == 0
+        steps = 0
+        for c in range(n):
+            if c == 5:
+                continue
+            assert infos[c]["true_resid"] <= 1e-10 and infos[c]["iters"] > 0 and infos[c]["reliable_updates"] >= 1
+            steps += infos[c]["iters"]
+            x_ref, _ = oracle.bicgstab(U, b[c], m, c_sw, tol=1e-12, F=F)
+            check_solution(U, b[c], x[c], m, c_sw, x_ref, F=F)
+        if precision == "mixed":  # one K1 column application per step and column, issued by multi-column launches
+            assert k1["k1_32"] - k0["k1_32"] == steps
+
+
 def test_gcr_columns_host_and_edge_cases(tmw):
     L, T, m, c_sw = 4, 6, -0.0514 + 0.0j, 1.0424
     U = synth.gauge_field(L, T, 0.35, seed=1)
