@@ -86,6 +86,7 @@ def parse_args():
     ap.add_argument("--kernel-reps", type=int, default=20, help="launches per kernel kind in the per-kernel roofline loop (0: skip)")
     ap.add_argument("--stage", type=int, default=0, help="tmw_options.stage: 1 = shared-memory staged fp32 stencil wherever a tile fits (default 0: off)")
     ap.add_argument("--stage-tile", default="0,0,0", help="tmw_options.stage_tile: tile extents x/2,y,z of the staged stencil (0,0,0: chosen by the library)")
+    ap.add_argument("--ring", type=int, default=0, help="tmw_options.ring: 1 = persistent stencil with the links prefetched through a shared-memory ring (default 0: off)")
     ap.add_argument("--columns-per-thread", type=int, default=0, help="tmw_options.columns_per_thread of the multi-column stencil (0: automatic)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -265,7 +266,7 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
     torch.cuda.synchronize()
     e0, e1 = ev(), ev()
     e0.record()
-    tuning = dict(stage=args.stage, stage_tile=tuple(int(v) for v in args.stage_tile.split(",")), columns_per_thread=args.columns_per_thread)
+    tuning = dict(stage=args.stage, stage_tile=tuple(int(v) for v in args.stage_tile.split(",")), columns_per_thread=args.columns_per_thread, ring=args.ring)
     ctx = tmw.Context(L, T, dU, m, c_sw, stream=stream, **tuning)
     e1.record()
     torch.cuda.synchronize()
@@ -466,7 +467,8 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
         ach = bpc * Vh * n / (ms_hop * 1e-3) / 1e9
         pk, pk_src = load_peaks()
         staged = (k1["staged"] - k0["staged"]) > 0
-        multi["roofline"] = {"bound": "hbm", "kernel": ("dslash_stage_kernel" if staged else "dslash_kernel") + "<float,12,EPI_HOP,NR=2|3> (multi-column hop)",
+        ringed = (k1["ring"] - k0["ring"]) > 0
+        multi["roofline"] = {"bound": "hbm", "kernel": ("dslash_stage_kernel" if staged else "dslash_ring_kernel" if ringed else "dslash_kernel") + "<float,12,EPI_HOP,NR=2|3> (multi-column hop)",
                              "achieved": ach, "peak": pk, "unit": "GB/s", "frac": ach / pk, "bytes_per_site_and_column": bpc, "peak_source": pk_src,
                              "note": "not HBM-bound: the links are amortised, the 8 neighbour spinors per column are not (DESIGN.md 6b)"}
         # K1 + K2 (one Schur-operator application) on n columns: per site and column K1 96 in + 96 out, K2 96 in + 96 aux + 96 out,
@@ -476,7 +478,8 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
         multi["schur_ms_per_rhs"] = ms_schur / n
         multi["roofline_schur"] = {"bound": "hbm", "kernel": "K1 + K2 on %d columns (tmw_apply_schur_multi, fp32)" % n, "achieved": ach_s, "peak": pk,
                                    "unit": "GB/s", "frac": ach_s / pk, "bytes_per_site_and_column": bps_schur, "peak_source": pk_src}
-        multi["tuning"] = {"stage": args.stage, "stage_tile": args.stage_tile, "columns_per_thread": args.columns_per_thread, "staged_kernel_ran": staged}
+        multi["tuning"] = {"stage": args.stage, "stage_tile": args.stage_tile, "columns_per_thread": args.columns_per_thread, "ring": args.ring,
+                           "staged_kernel_ran": staged, "ring_kernel_ran": ringed}
         # the fp32 ALU ceiling beside it (register-only FMA loops, tmw_time_kernel): with the links amortised the multi-column hop
         # is as close to this ceiling as to the HBM one
         try:

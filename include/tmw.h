@@ -123,6 +123,12 @@ typedef struct {
      columns stay in L2. 0 = automatic (the largest slab whose +-t window fits a fixed L2 budget), -1 = off (time slice
      after time slice), > 0 = that many sites (must divide L, with L*L*zchunk/2 a multiple of 128; else off). */
   int zchunk;
+  /* Persistent fp32 stencil with link prefetch: CTAs walk over the site blocks and every thread has the 8
+     links of its next site in flight through a private ring in shared memory (cp.async), so that the loads that always
+     miss to DRAM are off the critical path. 12-real links, hop / K1 / K2, no domain decomposition, 1-D site mapping.
+     0 or -1 = off (default: measured on B200 it is 20-120 % slower than the plain kernel, the extra LDGSTS + LDS traffic
+     saturates the L1/shared-memory pipe; profiles/r2_stage.md), 1 = wherever it applies. */
+  int ring;
 } tmw_options;
 
 /* Test hooks (tmw_options.debug / tmw_set_debug): they change which code path runs, never the result. */
@@ -259,7 +265,8 @@ long long tmw_launch_count(const tmw_ctx* ctx);
 #define TMW_K_FFMA_PROBE 24    /* tmw_time_kernel only: TMW_FFMA_PROBE_FMAS_PER_THREAD scalar fp32 FMAs (16 independent chains) per thread */
 #define TMW_K_FFMA2_PROBE 25   /* tmw_time_kernel only: the same FMAs as packed pairs (fma.rn.f32x2, 8 chains of 2) */
 #define TMW_FFMA_PROBE_FMAS_PER_THREAD (16 * 16384) /* the probe launches (SM count) x 8 CTAs of 256 threads */
-#define TMW_K_COUNT 26
+#define TMW_K_RING 26          /* of the fp32 stencil applications above: those that ran in the persistent link-ring kernel */
+#define TMW_K_COUNT 27
 
 /*
  * counts[k] (k < min(n, TMW_K_COUNT)) = how many right-hand-side columns kernels of kind k have been applied to since

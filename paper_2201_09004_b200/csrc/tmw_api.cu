@@ -362,6 +362,14 @@ static cudaError_t launch_stage(const DslashArgs<float>& a, int ng, int epi, int
   return launch_dslash_stage(a, ng, epi, clv, nr, sg, s);
 }
 static cudaError_t launch_stage(const DslashArgs<double>&, int, int, int, int, const StageGeom&, cudaStream_t) { return cudaErrorInvalidValue; }
+// the persistent link-ring kernel (tmw_dslash_ring.cuh): fp32, 12-real links, hop / K1 / K2 on the whole lattice, 1-D mapping
+template <typename R> static bool use_ring(tmw_ctx* ctx, int epi, int ncol, int cb1) {
+  (void)ncol;
+  if (sizeof(R) != 4 || ctx->opt.ring <= 0 || ctx->ng32 != 12 || cb1 >= 0 || !ctx->dom.empty() || ctx->g.tiled || ctx->opt.stage > 0) return false;
+  return epi == EPI_HOP || epi == EPI_AINV_HOP || epi == EPI_A_XPAY;
+}
+static cudaError_t launch_ring(const DslashArgs<float>& a, int epi, int clv, int nr, cudaStream_t s) { return launch_dslash_ring(a, epi, clv, nr, s); }
+static cudaError_t launch_ring(const DslashArgs<double>&, int, int, int, cudaStream_t) { return cudaErrorInvalidValue; }
 
 // cb0, cb1 (optional): restrict the launch to the output sites with checkerboard index in [cb0, cb1), cb0 a multiple of 128
 template <typename R>
@@ -403,6 +411,11 @@ static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, vo
     }
   }
   const int clv = !ctx->clover ? CL_NONE : (ctx->m_im != 0.0 ? CL_TWISTED : CL_CLOVER);
+  if (use_ring<R>(ctx, epi, cm.n, cb1)) {
+    ctx->kcount[TMW_K_RING] += cm.n;
+    LAUNCHK(stencil_kind<R>(epi, red_mode), cm.n, launch_ring(a, epi, clv, nr, ctx->stream));
+    return TMW_OK;
+  }
   if (use_stage<R>(ctx, epi, cm.n, cb1, nr)) {
     ctx->kcount[TMW_K_STAGED] += cm.n;
     LAUNCHK(stencil_kind<R>(epi, red_mode), cm.n, launch_stage(a, ng_of<R>(ctx), epi, clv, nr, ctx->stage[nr], ctx->stream));
@@ -570,7 +583,7 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
       o.max_iter < 0 || !(o.delta > 0.0) || !(o.delta < 1.0) || (o.solver != TMW_BICGSTAB && o.solver != TMW_GCR) || o.nkrylov < 1 ||
       o.nkrylov > GCR_KMAX || o.columns_per_thread < 0 || o.columns_per_thread > 4 ||
       (o.debug & ~(TMW_DEBUG_FORCE_PIVOT | TMW_DEBUG_NO_CHUNK)) || o.stage < -1 || o.stage > 1 || o.stage_tile[0] < 0 ||
-      o.stage_tile[1] < 0 || o.stage_tile[2] < 0 || o.zchunk < -1)
+      o.stage_tile[1] < 0 || o.stage_tile[2] < 0 || o.zchunk < -1 || o.ring < -1 || o.ring > 1)
     return fail(nullptr, TMW_EINVAL, "tmw_create: bad option value");
   if (!isfinite(m.re) || !isfinite(m.im) || !isfinite(c_sw)) return fail(nullptr, TMW_EINVAL, "tmw_create: non-finite parameter");
   const int pz = o.domains_z > 1 ? o.domains_z : 1, pt = o.domains_t > 1 ? o.domains_t : 1;
