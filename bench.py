@@ -86,6 +86,7 @@ def parse_args():
     ap.add_argument("--kernel-reps", type=int, default=20, help="launches per kernel kind in the per-kernel roofline loop (0: skip)")
     ap.add_argument("--stage", type=int, default=0, help="tmw_options.stage: 1 = shared-memory staged fp32 stencil wherever a tile fits (default 0: off)")
     ap.add_argument("--stage-tile", default="0,0,0", help="tmw_options.stage_tile: tile extents x/2,y,z of the staged stencil (0,0,0: chosen by the library)")
+    ap.add_argument("--delta", type=float, default=0.0, help="tmw_options.delta: reliable-update threshold (0: the library default 1e-5)")
     ap.add_argument("--ring", type=int, default=0, help="tmw_options.ring: 1 = persistent stencil with the links prefetched through a shared-memory ring (default 0: off)")
     ap.add_argument("--columns-per-thread", type=int, default=0, help="tmw_options.columns_per_thread of the multi-column stencil (0: automatic)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -266,7 +267,8 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
     torch.cuda.synchronize()
     e0, e1 = ev(), ev()
     e0.record()
-    tuning = dict(stage=args.stage, stage_tile=tuple(int(v) for v in args.stage_tile.split(",")), columns_per_thread=args.columns_per_thread, ring=args.ring)
+    tuning = dict(stage=args.stage, stage_tile=tuple(int(v) for v in args.stage_tile.split(",")), columns_per_thread=args.columns_per_thread, ring=args.ring,
+                  delta=args.delta)
     ctx = tmw.Context(L, T, dU, m, c_sw, stream=stream, **tuning)
     e1.record()
     torch.cuda.synchronize()

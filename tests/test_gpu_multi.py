@@ -97,6 +97,23 @@ def test_zchunk_sweep_vs_oracle(tmw, L, T, nrhs, zchunk, cpt):
                     assert site <= TOL32, (op, par, c, site, glob)
 
 
+@pytest.mark.parametrize("zchunk,cpt", [(4, 2), (4, 3), (-1, 4)])
+def test_zchunk_solve_vs_oracle(tmw, zchunk, cpt):
+    """the z-slab sweep under K1, K2 and their fused dot products: 8^3 x 4 clover, six columns through tmw_solve_multi"""
+    L, T, m, c_sw = 8, 4, -0.0514 + 0.0j, 1.0424
+    U = synth.gauge_field(L, T, 0.35, seed=1)
+    F = oracle.field_strength(U)
+    b = np.stack([synth.point_source(L, T, c // 3, c % 3) for c in (0, 2, 5, 7, 9, 11)])
+    with tmw.Context(L, T, dev(U), m, c_sw, zchunk=zchunk, columns_per_thread=cpt) as ctx:
+        x = torch.empty(b.shape, dtype=torch.complex128, device="cuda")
+        infos = ctx.solve_multi(6, dev(b), x, 1e-10)
+        x = x.cpu().numpy()
+        for c in range(6):
+            assert infos[c]["true_resid"] <= 1e-10 and infos[c]["iters"] > 0
+            x_ref, _ = oracle.bicgstab(U, b[c], m, c_sw, tol=1e-12, F=F)
+            check_solution(U, b[c], x[c], m, c_sw, x_ref, F=F)
+
+
 @pytest.mark.parametrize("spread", SPREADS[1:], ids=lambda d: "-".join(f"{k[8:]}{v}" for k, v in d.items()))
 @pytest.mark.parametrize("case", [
     dict(L=8, T=4, eps=0.4, m=-0.0695 + 0.0j, c_sw=1.0509, nrhs=5),
