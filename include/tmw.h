@@ -129,6 +129,12 @@ typedef struct {
      0 or -1 = off (default: measured on B200 it is 20-120 % slower than the plain kernel, the extra LDGSTS + LDS traffic
      saturates the L1/shared-memory pipe; profiles/r2_stage.md), 1 = wherever it applies. */
   int ring;
+  /* L2 prefetch of the links: a CTA of the plain stencil also issues prefetch.global.L2 for the links of the
+     site block `prefetch` blocks ahead of its own (the links are the loads that always miss to DRAM). 0 = automatic: one
+     block ahead in the multi-column fp32 hop launches (measured: -7..10 % at 12 columns 32^3 x 96, -3 % at 3 columns
+     48^3 x 144; no gain for K1 / K2 and for one column, where it stays off), -1 = off, > 0 = that distance in site blocks
+     of 128 sites for every stencil launch. */
+  int prefetch;
 } tmw_options;
 
 /* Test hooks (tmw_options.debug / tmw_set_debug): they change which code path runs, never the result. */

@@ -225,6 +225,7 @@ static DslashArgs<R> make_args(const tmw_ctx* c, int par, int dagger, const void
   a.cstride = (int)((int64_t)c->g.Vh * 24 * (int64_t)sizeof(R) / 16);
   a.red_stride = 0;
   a.skip = c->cur_skip;
+  a.pf_blocks = c->opt.prefetch > 0 ? c->opt.prefetch : 0;  // automatic (0): set per launch in dslash<R>()
   for (int i = 0; i < MAXCOL; i++) a.col[i] = cm.col[i];
   return a;
 }
@@ -385,6 +386,8 @@ static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, vo
   a.dotv = dotv;
   a.red = red;
   a.red_stride = red_stride;
+  // automatic link prefetch: one site block ahead in the multi-column hop launches, the one case where it was measured to pay
+  if (ctx->opt.prefetch == 0 && sizeof(R) == 4 && epi == EPI_HOP && cm.n >= 2) a.pf_blocks = 1;
   if (cb1 >= 0) { a.sb0 = cb0 / 128; a.cb_end = cb1; }
   else if (sizeof(R) == 4 && cm.n >= 2 && !a.g.tiled) {
     // multi-column launch: z-slab sweep order (Geom::zc) so that the +-t window of all columns fits in L2
@@ -583,7 +586,7 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
       o.max_iter < 0 || !(o.delta > 0.0) || !(o.delta < 1.0) || (o.solver != TMW_BICGSTAB && o.solver != TMW_GCR) || o.nkrylov < 1 ||
       o.nkrylov > GCR_KMAX || o.columns_per_thread < 0 || o.columns_per_thread > 4 ||
       (o.debug & ~(TMW_DEBUG_FORCE_PIVOT | TMW_DEBUG_NO_CHUNK)) || o.stage < -1 || o.stage > 1 || o.stage_tile[0] < 0 ||
-      o.stage_tile[1] < 0 || o.stage_tile[2] < 0 || o.zchunk < -1 || o.ring < -1 || o.ring > 1)
+      o.stage_tile[1] < 0 || o.stage_tile[2] < 0 || o.zchunk < -1 || o.ring < -1 || o.ring > 1 || o.prefetch < -1)
     return fail(nullptr, TMW_EINVAL, "tmw_create: bad option value");
   if (!isfinite(m.re) || !isfinite(m.im) || !isfinite(c_sw)) return fail(nullptr, TMW_EINVAL, "tmw_create: non-finite parameter");
   const int pz = o.domains_z > 1 ? o.domains_z : 1, pt = o.domains_t > 1 ? o.domains_t : 1;

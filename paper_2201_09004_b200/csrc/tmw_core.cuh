@@ -691,6 +691,10 @@ template <typename R> struct DslashArgs {
   // launched one iteration ahead of the host's look at the solver scalars: if *skip != 0 the kernel returns at once (the
   // device has decided that the host must act first, tmw_internal.h launch_sc_begin_iter); null: never skipped
   const int* skip;
+  // L2 prefetch distance in site blocks (0: off): a thread also issues prefetch.global.L2 for the 8 links of its lane's site in
+  // block sblock + pf_blocks, so that the links - the loads of the stencil that always miss to DRAM - are L2 hits when that
+  // block's CTA runs (tmw_options.prefetch)
+  int pf_blocks;
   DDArgs<R> dd;      // read only by the domain-decomposition kernels (DD != 0)
 };
 

@@ -120,6 +120,23 @@ __global__ void __launch_bounds__(BLOCK, MINB) dslash_kernel(const DslashArgs<R>
     colj[j] = a.col[valid[j] ? slot : a.ncol - 1];
     cofs[j] = colj[j] * a.cstride;
   }
+  if (DD == 0 && a.pf_blocks > 0 && grp == 0 && !a.g.tiled) {  // the first column group of a site block prefetches for a later block
+    Site sp;
+    if (thread_site<BLOCK>(a.g, sblock + a.sb0 + a.pf_blocks, sp) && sp.cb < a.cb_end) {
+      const Nbr np = neighbours(a.g, a.par, sp);
+      const int NPG = Planes<R, NG>::N;
+#pragma unroll
+      for (int mu = 0; mu < 4; mu++) {
+        const V* uf = (const V*)a.U[a.par] + (int64_t)mu * NPG * a.g.Vh + sp.cb;
+        const V* ub = (const V*)a.U[1 - a.par] + (int64_t)mu * NPG * a.g.Vh + np.bwd[mu];
+#pragma unroll
+        for (int k = 0; k < NPG; k++) {
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(uf + (int64_t)k * a.g.Vh));
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(ub + (int64_t)k * a.g.Vh));
+        }
+      }
+    }
+  }
   R o[NR][24], r2[NR][3];
   bool raw = false;
   if (active) {

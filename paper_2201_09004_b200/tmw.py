@@ -47,7 +47,7 @@ class tmw_options(ctypes.Structure):
                 ("stream", ctypes.c_void_p), ("solver", ctypes.c_int), ("nkrylov", ctypes.c_int),
                 ("verbose", ctypes.c_int), ("columns_per_thread", ctypes.c_int),
                 ("tile", ctypes.c_int * 4), ("debug", ctypes.c_int), ("domains_z", ctypes.c_int), ("domains_t", ctypes.c_int),
-                ("stage", ctypes.c_int), ("stage_tile", ctypes.c_int * 3), ("zchunk", ctypes.c_int), ("ring", ctypes.c_int)]
+                ("stage", ctypes.c_int), ("stage_tile", ctypes.c_int * 3), ("zchunk", ctypes.c_int), ("ring", ctypes.c_int), ("prefetch", ctypes.c_int)]
 
 
 class tmw_solve_info(ctypes.Structure):
@@ -137,14 +137,14 @@ class Context:
                  precision: int = MIXED, reconstruct: int = 12, mass_reading: int = TWIST_GAMMA5, max_iter: int = 0,
                  delta: float = 0.0, stream: int | None = None, solver: int = BICGSTAB, nkrylov: int = 0,
                  verbose: int = 0, columns_per_thread: int = 0, tile=(0, 0, 0, 0), debug: int = 0, domains_z: int = 0, domains_t: int = 0,
-                 stage: int = 0, stage_tile=(0, 0, 0), zchunk: int = 0, ring: int = 0):
+                 stage: int = 0, stage_tile=(0, 0, 0), zchunk: int = 0, ring: int = 0, prefetch: int = 0):
         lib = load()
         self._lib = lib
         self.L, self.T = L, T
         self.V = L * L * L * T
         self.location = location
         opt = tmw_options(location, precision, reconstruct, mass_reading, max_iter, delta, stream, solver, nkrylov,
-                          verbose, columns_per_thread, (ctypes.c_int * 4)(*tile), debug, domains_z, domains_t, stage, (ctypes.c_int * 3)(*stage_tile), zchunk, ring)
+                          verbose, columns_per_thread, (ctypes.c_int * 4)(*tile), debug, domains_z, domains_t, stage, (ctypes.c_int * 3)(*stage_tile), zchunk, ring, prefetch)
         h = ctypes.c_void_p()
         rc = lib.tmw_create(ctypes.byref(h), L, T, _ptr(gauge), tmw_complex(float(np.real(m)), float(np.imag(m))),
                             float(c_sw), ctypes.byref(opt))

@@ -97,6 +97,32 @@ def test_zchunk_sweep_vs_oracle(tmw, L, T, nrhs, zchunk, cpt):
                     assert site <= TOL32, (op, par, c, site, glob)
 
 
+@pytest.mark.parametrize("prefetch,nrhs,zchunk", [(1, 4, 0), (5, 3, 4), (1000, 2, 0), (3, 1, 0), (-1, 4, 0)])
+def test_link_prefetch_changes_nothing(tmw, prefetch, nrhs, zchunk):
+    """tmw_options.prefetch: prefetch.global.L2 of the links of a later site block (also past the end of the lattice) is a
+    hint: hop and K1 / K2 outputs against the oracle as without it"""
+    L, T, m, c_sw = 8, 4, -0.0695 + 0.0j, 1.0509
+    U = synth.gauge_field(L, T, 0.4, seed=1)
+    cols = columns(L, T, nrhs)
+    F = oracle.field_strength(U)
+    with tmw.Context(L, T, dev(U), m, c_sw, prefetch=prefetch, zchunk=zchunk) as ctx:
+        inp = pack_multi(ctx, tmw, cols, 0, tmw.F32)
+        out = torch.full_like(inp, 0x7f)
+        ctx.apply_multi(tmw.D, tmw.ODD, tmw.F32, nrhs, inp, out)
+        got = unpack_multi(ctx, tmw, out, nrhs, 1, tmw.F32, L, T)
+        for c in range(nrhs):
+            ref = mask_parity(oracle.apply(U, mask_parity(cols[c], 0), m, 0.0), 1)
+            assert H.per_site_rel_err(got[c], ref)[0] <= TOL32, c
+        b = np.stack([synth.point_source(L, T, c % 4, c % 3) for c in range(nrhs)])
+        x = torch.empty(b.shape, dtype=torch.complex128, device="cuda")
+        infos = ctx.solve_multi(nrhs, dev(b), x, 1e-10)
+        x = x.cpu().numpy()
+        for c in range(nrhs):
+            assert infos[c]["true_resid"] <= 1e-10
+            x_ref, _ = oracle.bicgstab(U, b[c], m, c_sw, tol=1e-12, F=F)
+            check_solution(U, b[c], x[c], m, c_sw, x_ref, F=F)
+
+
 @pytest.mark.parametrize("zchunk,cpt", [(4, 2), (4, 3), (-1, 4)])
 def test_zchunk_solve_vs_oracle(tmw, zchunk, cpt):
     """the z-slab sweep under K1, K2 and their fused dot products: 8^3 x 4 clover, six columns through tmw_solve_multi"""
