@@ -144,6 +144,37 @@ def test_fullsize_hopping_fp32_sampled(tmw, idx):
     torch.cuda.empty_cache()
 
 
+@pytest.mark.parametrize("idx,ncol", [(3, 12), (4, 3)])
+def test_fullsize_hopping_multi_column_fp32_sampled(tmw, idx, ncol):
+    """the multi-column hop launches of bench.py's `multi_rhs` leg (tmw_apply_multi; automatic columns per thread, packed
+    fp32 pairs, z-slab sweep, link prefetch): every column at sampled sites incl. all boundary kinds against the oracle"""
+    cfg, U = config_fields(idx)
+    L, T, m = cfg["L"], cfg["T"], complex(*cfg["m"])
+    dU = torch.from_numpy(U).cuda()
+    with tmw.Context(L, T, dU, m, cfg["c_sw"]) as ctx:
+        del dU
+        nb = ctx.spinor_bytes(tmw.F32)
+        pin = torch.empty(nb * ncol, dtype=torch.uint8, device="cuda")
+        pout = torch.full_like(pin, 0x7f)
+        tmp = torch.empty((T, L, L, L, 4, 3), dtype=torch.complex128, device="cuda")
+        seeds = [20 + c for c in range(ncol)]
+        for c in range(ncol):
+            tmp.copy_(torch.from_numpy(synth.gaussian_spinor(L, T, seed=seeds[c])))
+            ctx.pack(tmw.F32, tmw.EVEN, tmp, pin[c * nb:(c + 1) * nb])
+        ctx.apply_multi(tmw.D, tmw.ODD, tmw.F32, ncol, pin, pout)
+        sites = sample_sites(L, T, 4000, seed=31 + idx, parity=1)
+        for c in range(ncol):
+            tmp.zero_()
+            ctx.unpack(tmw.F32, tmw.ODD, pout[c * nb:(c + 1) * nb], tmp)
+            got = tmp.cpu().numpy().reshape(-1, 4, 3)[sites]
+            psi = synth.gaussian_spinor(L, T, seed=seeds[c])
+            mask_parity_inplace(psi, L, T, 1)  # the input lives on the even sites
+            ref = oracle.apply_sites(U, psi, sites, m, 0.0)  # at odd sites of an even-only input: the hopping block alone
+            assert site_err(got, ref) <= TOL32, c
+        del pin, pout, tmp
+    torch.cuda.empty_cache()
+
+
 @pytest.mark.parametrize("idx", [2, 4])
 def test_fullsize_full_operator_fp64_sampled(tmw, idx):
     cfg, U = config_fields(idx)
