@@ -155,7 +155,10 @@ __global__ void __launch_bounds__(RING_BLOCK, MINB) dslash_ring_kernel(const Dsl
           if (valid[j] && a.out) store_reals_s<24>(a.out, a.g.Vh, s.cb + cofs[j], o[j]);
       }
     }
-    if (a.red_mode != 0) site_reductions<float, NR, RING_BLOCK>(a, s, active, cofs, colj, valid, o, r2);  // uniform across the grid
+    if (a.red_mode != 0) {  // uniform across the grid
+      site_reductions<float, NR, RING_BLOCK>(a, s, active, cofs, colj, valid, o, r2);
+      __syncthreads();  // the reduction's shared scratch is written again by the next site block of this CTA
+    }
     if (!have_next) break;
     w = wn;
     s = sn;
@@ -173,17 +176,25 @@ template <> struct RingTune<4> { enum { MINB = 2 }; };
 template <int EPI, int CLOVER, int NR> static cudaError_t launch_ring_one(DslashArgs<float> a, cudaStream_t s) {
   const size_t smem = (size_t)8 * 3 * RING_BLOCK * sizeof(float4);
   auto kern = dslash_ring_kernel<EPI, CLOVER, NR, RingTune<NR>::MINB>;
-  static int ctas_per_sm = 0, sms = 0;  // per instantiation
-  if (!ctas_per_sm) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  // resident CTAs per SM and the SM count, per device (the shared-memory attribute belongs to (function, device) as well)
+  enum { MAXDEV = 64 };
+  static int ctas_cache[MAXDEV] = {0}, sms_cache[MAXDEV] = {0};
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= MAXDEV) return cudaErrorInvalidDevice;
+  if (!ctas_cache[dev]) {
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, kern, RING_BLOCK, smem);
+    int n = 0, m = 0;
+    e = cudaDeviceGetAttribute(&m, cudaDevAttrMultiProcessorCount, dev);
     if (e != cudaSuccess) return e;
-    if (ctas_per_sm < 1) ctas_per_sm = 1;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, RING_BLOCK, smem);
+    if (e != cudaSuccess) return e;
+    sms_cache[dev] = m;
+    ctas_cache[dev] = n < 1 ? 1 : n;
   }
+  const int ctas_per_sm = ctas_cache[dev], sms = sms_cache[dev];
   a.ngroups = (a.ncol + NR - 1) / NR;
   const int nwork = ((a.g.Vh + RING_BLOCK - 1) / RING_BLOCK) * a.ngroups;
   const int grid = nwork < sms * ctas_per_sm ? nwork : sms * ctas_per_sm;

@@ -200,12 +200,9 @@ template <int NG, int EPI, int CLOVER, int NR> static cudaError_t launch_stage_o
   if (block > TN::MAXT) return cudaErrorInvalidConfiguration;
   const size_t smem = (size_t)NR * 6 * sg.nslots * sizeof(float4);
   auto kern = dslash_stage_kernel<NG, EPI, CLOVER, NR, TN::MAXT, TN::MINB>;
-  static size_t smem_set = 0;  // per instantiation
-  if (smem > smem_set) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    smem_set = smem;
-  }
+  // the attribute belongs to (function, device): set it on every launch rather than cache it across devices
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
   a.ngroups = (a.ncol + NR - 1) / NR;
   const unsigned grid = (unsigned)((int64_t)sg.ntx * sg.nty * sg.ntz * a.g.T * a.ngroups);
   kern<<<grid, block, smem, s>>>(a, sg);
