@@ -665,7 +665,7 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
     }
     CKA(&ctx->ci64, Vh * 36 * 16);
     CKA(&ctx->ci32, Vh * 18 * 16);
-    CKC(launch_clover_build(ctx->g, ctx->g64[0], ctx->g64[1], c_sw, -(4.0 + m.re), ctx->c64[0], ctx->c64[1], ctx->c32[0], ctx->c32[1], ctx->stream));
+    CKC(launch_clover_build(ctx->g, ctx->g64[0], ctx->g64[1], c_sw, -(4.0 + m.re), ctx->c64[0], ctx->c64[1], ctx->c32[0], ctx->c32[1], ctx->ng32 == 12, ctx->stream));
     ctx->launches++;
     int* flag = (int*)ctx->red;
     CKC(cudaMemsetAsync(flag, 0, sizeof(int), ctx->stream));

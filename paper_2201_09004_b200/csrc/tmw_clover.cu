@@ -61,22 +61,53 @@ __device__ __forceinline__ void ld_link(const Lat& g, const double* __restrict__
   }
 }
 
-// Q += A op B op C op D with the daggers given; all four links loaded here
-template <bool D0, bool D1, bool D2, bool D3>
+// Q += op(A) op(B) op(C) op(D) with the daggers given; all four links loaded here. The product is built row by row:
+// v = the first NROW rows of op(A), then v <- v op(B), v <- v op(C), v <- v op(D) (3 x NROW x 9 complex multiply-adds).
+// That keeps NROW x 3 + 9 complex numbers live per step instead of three full matrices, so that the next link is in
+// flight while the current one is multiplied. NROW = 2 (links known to be SU(3): the context stores 12-real fp32 links):
+// the third row of the SU(3) product is conj(row0 x row1), a third fewer multiply-adds.
+template <int NROW, bool DAG> __device__ __forceinline__ void vmul(zd (&v)[NROW][3], const zd* M) {
+#pragma unroll
+  for (int r = 0; r < NROW; r++) {
+    zd w[3];
+#pragma unroll
+    for (int j = 0; j < 3; j++) {
+      zd s = mk<double>(0.0, 0.0);
+#pragma unroll
+      for (int k = 0; k < 3; k++) cmad(s, v[r][k], DAG ? conj(M[3 * j + k]) : M[3 * k + j]);
+      w[j] = s;
+    }
+#pragma unroll
+    for (int j = 0; j < 3; j++) v[r][j] = w[j];
+  }
+}
+template <int NROW, bool D0, bool D1, bool D2, bool D3>
 __device__ __forceinline__ void leaf(const Lat& g, const double* canon, int m0, int64_t s0, int m1, int64_t s1, int m2, int64_t s2, int m3, int64_t s3, zd* Q) {
-  zd A[9], B[9], P[9], R2[9];
+  zd A[9], B[9];
+  zd v[NROW][3];
   ld_link(g, canon, m0, s0, A);
   ld_link(g, canon, m1, s1, B);
-  mm<D0, D1>(A, B, P);
-  ld_link(g, canon, m2, s2, A);
-  mm<false, D2>(P, A, R2);
-  ld_link(g, canon, m3, s3, B);
-  mm<false, D3>(R2, B, P);
 #pragma unroll
-  for (int i = 0; i < 9; i++) Q[i] = Q[i] + P[i];
+  for (int r = 0; r < NROW; r++)
+#pragma unroll
+    for (int k = 0; k < 3; k++) v[r][k] = D0 ? conj(A[3 * k + r]) : A[3 * r + k];
+  ld_link(g, canon, m2, s2, A);
+  vmul<NROW, D1>(v, B);
+  ld_link(g, canon, m3, s3, B);
+  vmul<NROW, D2>(v, A);
+  vmul<NROW, D3>(v, B);
+#pragma unroll
+  for (int r = 0; r < NROW; r++)
+#pragma unroll
+    for (int k = 0; k < 3; k++) Q[3 * r + k] = Q[3 * r + k] + v[r][k];
+  if (NROW == 2) {
+    Q[6] = Q[6] + conj(v[0][1] * v[1][2] - v[0][2] * v[1][1]);
+    Q[7] = Q[7] + conj(v[0][2] * v[1][0] - v[0][0] * v[1][2]);
+    Q[8] = Q[8] + conj(v[0][0] * v[1][1] - v[0][1] * v[1][0]);
+  }
 }
 
-__device__ __noinline__ void field_strength(const Lat& g, const double* canon, const int* c, int mu, int nu, zd* F) {
+template <int NROW> __device__ __noinline__ void field_strength(const Lat& g, const double* canon, const int* c, int mu, int nu, zd* F) {
   zd Q[9];
 #pragma unroll
   for (int i = 0; i < 9; i++) Q[i] = mk<double>(0.0, 0.0);
@@ -85,13 +116,13 @@ __device__ __noinline__ void field_strength(const Lat& g, const double* canon, c
   const int64_t xmm = shifted(g, c, mu, -1, nu, 0), xmn = shifted(g, c, mu, 0, nu, -1);
   const int64_t xmmpn = shifted(g, c, mu, -1, nu, +1), xmmmn = shifted(g, c, mu, -1, nu, -1), xpmmn = shifted(g, c, mu, +1, nu, -1);
   // U_mu(x) U_nu(x+mu) U_mu(x+nu)^dag U_nu(x)^dag
-  leaf<false, false, true, true>(g, canon, mu, x, nu, xpm, mu, xpn, nu, x, Q);
+  leaf<NROW, false, false, true, true>(g, canon, mu, x, nu, xpm, mu, xpn, nu, x, Q);
   // U_nu(x) U_mu(x-mu+nu)^dag U_nu(x-mu)^dag U_mu(x-mu)
-  leaf<false, true, true, false>(g, canon, nu, x, mu, xmmpn, nu, xmm, mu, xmm, Q);
+  leaf<NROW, false, true, true, false>(g, canon, nu, x, mu, xmmpn, nu, xmm, mu, xmm, Q);
   // U_mu(x-mu)^dag U_nu(x-mu-nu)^dag U_mu(x-mu-nu) U_nu(x-nu)
-  leaf<true, true, false, false>(g, canon, mu, xmm, nu, xmmmn, mu, xmmmn, nu, xmn, Q);
+  leaf<NROW, true, true, false, false>(g, canon, mu, xmm, nu, xmmmn, mu, xmmmn, nu, xmn, Q);
   // U_nu(x-nu)^dag U_mu(x-nu) U_nu(x+mu-nu) U_mu(x)^dag
-  leaf<true, false, false, true>(g, canon, nu, xmn, mu, xmn, nu, xpmmn, mu, x, Q);
+  leaf<NROW, true, false, false, true>(g, canon, nu, xmn, mu, xmn, nu, xpmmn, mu, x, Q);
   // (Q - Q^dag)/(8i):  z/(8i) = (z.im, -z.re)/8
 #pragma unroll
   for (int i = 0; i < 3; i++)
@@ -148,7 +179,7 @@ enum { CB_SITES = 32 };
 #ifndef TMW_CLOVER_MINB
 #define TMW_CLOVER_MINB 2
 #endif
-__global__ void __launch_bounds__(6 * CB_SITES, TMW_CLOVER_MINB) clover_build_kernel(const Geom g, const CloverTiles tl, const double2* __restrict__ u64e, const double2* __restrict__ u64o, double k, double diag, double2* c64e, double2* c64o, float4* c32e, float4* c32o) {
+template <int NROW> __global__ void __launch_bounds__(6 * CB_SITES, TMW_CLOVER_MINB) clover_build_kernel(const Geom g, const CloverTiles tl, const double2* __restrict__ u64e, const double2* __restrict__ u64o, double k, double diag, double2* c64e, double2* c64o, float4* c32e, float4* c32o) {
   __shared__ double Fs[6][9][CB_SITES];  // [plane][re(0,0) re(1,1) re(2,2) re/im(1,0) re/im(2,0) re/im(2,1)][site]
   const int lane = threadIdx.x & 31, plane = threadIdx.x >> 5;
   // position of this lane's site in the sweep: (tile, parity, index inside the tile's parity)
@@ -182,7 +213,7 @@ __global__ void __launch_bounds__(6 * CB_SITES, TMW_CLOVER_MINB) clover_build_ke
     // no_instruction 8.9 per issue, fp64 pipe 24 %).
     const int mu = (plane < 3) ? 0 : (plane < 5 ? 1 : 2);
     const int nu = (plane < 3) ? plane + 1 : (plane < 5 ? plane - 1 : 3);
-    field_strength(lt, canon, c, mu, nu, F);
+    field_strength<NROW>(lt, canon, c, mu, nu, F);
     Fs[plane][0][lane] = F[0].re;
     Fs[plane][1][lane] = F[4].re;
     Fs[plane][2][lane] = F[8].re;
@@ -221,7 +252,7 @@ __global__ void __launch_bounds__(6 * CB_SITES, TMW_CLOVER_MINB) clover_build_ke
   store_reals<36>(d32, g.Vh, cb, Bf);
 }
 
-cudaError_t launch_clover_build(const Geom& g, const void* g64_even, const void* g64_odd, double c_sw, double diag, void* c64_even, void* c64_odd, void* c32_even, void* c32_odd, cudaStream_t s) {
+cudaError_t launch_clover_build(const Geom& g, const void* g64_even, const void* g64_odd, double c_sw, double diag, void* c64_even, void* c64_odd, void* c32_even, void* c32_odd, bool su3, cudaStream_t s) {
   const auto tile_extent = [](int n) { int b = 1; for (int d = 2; d <= 8; d++) if (n % d == 0) b = d; return b; };
   CloverTiles tl;
   tl.By = tl.Bz = tile_extent(g.L);
@@ -229,7 +260,8 @@ cudaError_t launch_clover_build(const Geom& g, const void* g64_even, const void*
   tl.nby = tl.nbz = g.L / tl.By;
   tl.ts = g.Lh * tl.By * tl.Bz * tl.Bt;
   const dim3 grid((unsigned)((2 * (int64_t)g.Vh + CB_SITES - 1) / CB_SITES), 1, 1);
-  clover_build_kernel<<<grid, 6 * CB_SITES, 0, s>>>(g, tl, (const double2*)g64_even, (const double2*)g64_odd, 0.5 * c_sw, diag, (double2*)c64_even, (double2*)c64_odd, (float4*)c32_even, (float4*)c32_odd);
+  if (su3) clover_build_kernel<2><<<grid, 6 * CB_SITES, 0, s>>>(g, tl, (const double2*)g64_even, (const double2*)g64_odd, 0.5 * c_sw, diag, (double2*)c64_even, (double2*)c64_odd, (float4*)c32_even, (float4*)c32_odd);
+  else clover_build_kernel<3><<<grid, 6 * CB_SITES, 0, s>>>(g, tl, (const double2*)g64_even, (const double2*)g64_odd, 0.5 * c_sw, diag, (double2*)c64_even, (double2*)c64_odd, (float4*)c32_even, (float4*)c32_odd);
   return cudaGetLastError();
 }
 

@@ -64,7 +64,9 @@ cudaError_t launch_unpack_spinor_both(const Geom& g, int prec, const void* packe
 // ---- clover (tmw_clover.cu) ----
 // From the packed fp64 gauge (launch_pack_gauge's g64): packed Hermitian blocks C = (c_sw/2) sum sigma F + diag, both
 // parities, fp64 [36 planes][Vh] double2 and fp32 [18 planes][Vh] float4.
-cudaError_t launch_clover_build(const Geom& g, const void* g64_even, const void* g64_odd, double c_sw, double diag, void* c64_even, void* c64_odd, void* c32_even, void* c32_odd, cudaStream_t s);
+// su3: the links are SU(3) (the context stores 12-real fp32 links, which requires it): the third row of every plaquette
+// product is rebuilt from the first two instead of multiplied out
+cudaError_t launch_clover_build(const Geom& g, const void* g64_even, const void* g64_odd, double c_sw, double diag, void* c64_even, void* c64_odd, void* c32_even, void* c32_odd, bool su3, cudaStream_t s);
 // inverse blocks of one parity: (C^2 + tw2)^{-1} if tw2 != 0 else C^{-1}. launch_clover_invert: unpivoted LDL^dag in
 // registers; *flag (device int) is set if any block met a tiny pivot (its output is then not written) and the caller
 // reruns the field with launch_clover_invert_pivot (Gauss-Jordan with pivoting), whose *singular is set on failure.

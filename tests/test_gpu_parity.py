@@ -201,15 +201,17 @@ def test_full_apply_host_pipelined_vs_oracle(tmw, L, T):
 # ------------------------------------------------------------------------------------------------------
 # clover blocks (A1) and their inverse (A2) against the oracle's F and sigma
 # ------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("pivot", [False, True])
+@pytest.mark.parametrize("pivot,reconstruct", [(False, 12), (True, 12), (False, 18)])
 @pytest.mark.parametrize("L,T,m,c_sw", [(4, 6, -0.0695 + 0.0j, 1.0509), (6, 4, -0.044 + 0.2j, 1.0349), (8, 4, -3.9 + 0.0j, 2.5)])
-def test_clover_blocks_and_inverse(tmw, L, T, m, c_sw, pivot):
+def test_clover_blocks_and_inverse(tmw, L, T, m, c_sw, pivot, reconstruct):
     """the third case makes the blocks indefinite (diagonal -(4+m) = -0.1, clover term of order 1): the unpivoted
-    L D L^dag still has to invert them; pivot = True forces the Gauss-Jordan fallback kernel (TMW_DEBUG_FORCE_PIVOT)."""
+    L D L^dag still has to invert them; pivot = True forces the Gauss-Jordan fallback kernel (TMW_DEBUG_FORCE_PIVOT).
+    reconstruct = 12: the plaquette products rebuild their third row from the first two (SU(3) links); 18: all three rows
+    are multiplied out."""
     U = synth.gauge_field(L, T, 0.4, seed=1)
     blocks = H.site_diagonal_blocks(U, c_sw, m.real)  # (V,2,6,6)
     Vh = L ** 3 * T // 2
-    with tmw.Context(L, T, dev(U), m, c_sw, debug=tmw.DEBUG_FORCE_PIVOT if pivot else 0) as ctx:
+    with tmw.Context(L, T, dev(U), m, c_sw, debug=tmw.DEBUG_FORCE_PIVOT if pivot else 0, reconstruct=reconstruct) as ctx:
         for par in (0, 1):
             dst = torch.empty((Vh, 2, 36), dtype=torch.float64, device="cuda")
             ctx.get_clover(tmw.ODD if par else tmw.EVEN, 0, dst)
