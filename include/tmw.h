@@ -185,6 +185,44 @@ int tmw_apply_schur(tmw_ctx* ctx, int op, int prec, const void* in_odd, void* ou
 int tmw_solve(tmw_ctx* ctx, const double* b, double* x, double tol, tmw_solve_info* info);
 
 /*
+ * tmw_apply_schur for callers that must not allocate device memory: same operator (Eq. (2), :67 Eq. (3) on
+ * the even-odd Schur complement), same kernels, same arguments and result as tmw_apply_schur, but the call itself never
+ * allocates or frees anything - no cudaMalloc, no cudaFree, no library routine that allocates.
+ *
+ * Who needs this. tmw_apply_schur keeps its even-parity intermediate A_ee^{-1} H_eo in_o in a workspace that it
+ * cudaMallocs on first use (and again whenever a multi-column call has resized the workspaces). Some programs cannot
+ * afford that inside their steady state: a process that, once start-up is over, has handed the rest of the card to a
+ * pooling allocator (a PyTorch or RAPIDS job: a raw cudaMalloc then fails although the pool has room, or it fragments
+ * the pool's address space); a job that runs under a fixed device-memory quota; and a latency-critical loop that shares
+ * the GPU with other streams, because cudaMalloc and cudaFree stall the whole device until every stream has drained.
+ * Such a caller creates the context at start-up, while allocating is still allowed (tmw_create allocates the gauge and
+ * clover fields), and from then on applies the operator through this entry point.
+ *
+ * Where the intermediate lives. In one array of TMW_STATIC_SCRATCH_BYTES (8 MiB) that is compiled into libtmw.so as
+ * a device global. Every GPU on which the library's kernels are loaded sets these 8 MiB aside until the process exits,
+ * whether or not this call is ever used. A lattice whose packed parity spinor (tmw_spinor_bytes(ctx, prec): 96 bytes
+ * per site and parity in fp32, 192 in fp64) is larger than the array is refused with TMW_EINVAL and an error text that
+ * names both sizes; nothing is launched then. 16^3 x 32 in fp32 and 16^3 x 16 in fp64 still fit.
+ *
+ * First call on a device. The first call on each device looks up the device address of the array (a CUDA runtime
+ * query, no allocation) with the context's device current, and remembers it; make that first call during set-up,
+ * before any stream capture is begun. The context's device must be the calling thread's current device in every call,
+ * as for all other calls of this library (checked here: TMW_EINVAL otherwise).
+ *
+ * Sharing. There is ONE array per device for all contexts, streams and threads of the process, and it still holds
+ * whatever the previous call left in it. Nothing in it has to start at zero: the first kernel writes the intermediate
+ * of every even site before the second kernel reads it, so stale contents are never read. But two calls whose kernels
+ * can be on the GPU at the same time (different streams, or different contexts with different streams) overwrite each
+ * other's intermediate: that is a data race with wrong results and no error. Keep all calls of this entry point on one
+ * stream per device, or order them with events. It does not disturb, and is not disturbed by, any other call.
+ *
+ * One column, packed DEVICE spinors as for tmw_apply_schur, contexts without domain decomposition (a decomposed context
+ * grows its exchange buffers on demand; TMW_EINVAL). Asynchronous on the context stream.
+ */
+#define TMW_STATIC_SCRATCH_BYTES (8u << 20)
+int tmw_apply_schur_static(tmw_ctx* ctx, int op, int prec, const void* in_odd, void* out_odd);
+
+/*
  * Several right-hand sides at once (the "12 columns" of a propagator, Table 2 caption).
  * The columns are independent problems with the same operator; doing them in one call lets every link and clover
  * block be read once for all columns. nrhs in 1..16. Column c of every spinor argument follows column c-1 directly:

@@ -4,10 +4,12 @@
 // the CUDA kernels of this directory.
 #include <math.h>
 #include <stddef.h>
+#include <stdint.h>
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
 
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1031,6 +1033,64 @@ extern "C" int tmw_apply_schur_multi(tmw_ctx* ctx, int op, int prec, int nrhs, c
 }
 extern "C" int tmw_apply_schur(tmw_ctx* ctx, int op, int prec, const void* in_odd, void* out_odd) {
   return tmw_apply_schur_multi(ctx, op, prec, 1, in_odd, out_odd);
+}
+
+// ---- tmw_apply_schur_static (include/tmw.h): the Schur operator for callers that must not allocate ----
+// The even-parity intermediate of K1 -> K2 lives in this array instead of the cudaMalloc'ed workspace w64[0]. It is part of
+// the library image: every device that loads libtmw.so's kernels holds these bytes until the process ends.
+// In HOST code the name g_static_scratch is only a handle for the runtime, not a device address (a kernel given
+// `g_static_scratch` itself would fault, or scribble over host memory where the GPU can reach it): the device address
+// comes from cudaGetSymbolAddress, asked in this translation unit, once per device, with that device current.
+static __device__ __align__(256) unsigned char g_static_scratch[TMW_STATIC_SCRATCH_BYTES];
+
+namespace {
+enum { STATIC_MAX_DEVICES = 64 };
+void* g_static_ptr[STATIC_MAX_DEVICES];  // device address of g_static_scratch on device d, null until first asked
+std::mutex g_static_mutex;
+}  // namespace
+
+// Device address of the static scratch array on the current device (which must be the context's). No allocation.
+static int static_scratch_ptr(tmw_ctx* ctx, void** out) {
+  int dev = -1;
+  CK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= STATIC_MAX_DEVICES) return fail(ctx, TMW_EINVAL, "tmw_apply_schur_static: device ordinal out of range");
+  cudaPointerAttributes attr;
+  CK(cudaPointerGetAttributes(&attr, ctx->g64[1]));  // the context's own gauge field tells which device it lives on
+  if (attr.type != cudaMemoryTypeDevice || attr.device != dev)
+    return fail(ctx, TMW_EINVAL, "tmw_apply_schur_static: the context's device is not the calling thread's current device");
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  if (!g_static_ptr[dev]) {
+    void* p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+    if (e != cudaSuccess) return fail_cuda(ctx, e, "cudaGetSymbolAddress(g_static_scratch)");
+    if (!p || ((uintptr_t)p & 255)) return fail(ctx, TMW_ECUDA, "tmw_apply_schur_static: bad address for the static scratch array");
+    g_static_ptr[dev] = p;
+  }
+  *out = g_static_ptr[dev];
+  return TMW_OK;
+}
+
+extern "C" int tmw_apply_schur_static(tmw_ctx* ctx, int op, int prec, const void* in_odd, void* out_odd) {
+  if (!ctx) return TMW_EINVAL;
+  if (!in_odd || !out_odd || in_odd == out_odd) return fail(ctx, TMW_EINVAL, "tmw_apply_schur_static: null or aliased pointers");
+  if ((op != TMW_D && op != TMW_DDAG) || (prec != TMW_F32 && prec != TMW_F64)) return fail(ctx, TMW_EINVAL, "tmw_apply_schur_static: bad op or precision");
+  if (!ctx->dom.empty())
+    return fail(ctx, TMW_EINVAL, "tmw_apply_schur_static: not available on a domain-decomposed context (its exchange buffers are allocated on demand)");
+  const size_t need = spinor_bytes(ctx, prec);
+  if (need > (size_t)TMW_STATIC_SCRATCH_BYTES) {
+    char buf[256];
+    snprintf(buf, sizeof(buf), "tmw_apply_schur_static: a packed parity spinor of this lattice takes %zu bytes, the static scratch array holds %zu (TMW_STATIC_SCRATCH_BYTES); use tmw_apply_schur",
+             need, (size_t)TMW_STATIC_SCRATCH_BYTES);
+    return fail(ctx, TMW_EINVAL, buf);
+  }
+  void* tmp = nullptr;
+  int rc = static_scratch_ptr(ctx, &tmp);
+  if (rc) return rc;
+  // K1 writes the intermediate of every even site, K2 reads only those: nothing in the array has to be cleared first
+  const int dagger = (op == TMW_DDAG);
+  const ColMap cm = cols_first(1);
+  if (prec == TMW_F64) return schur<double>(ctx, dagger, in_odd, out_odd, tmp, cm);
+  return schur<float>(ctx, dagger, in_odd, out_odd, tmp, cm);
 }
 
 // ---- the solver ----

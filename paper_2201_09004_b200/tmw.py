@@ -25,13 +25,14 @@ D, DDAG, G5D = 0, 1, 2
 FULL, EVEN, ODD = 0, 1, 2
 F32, F64 = 0, 1
 DEBUG_FORCE_PIVOT, DEBUG_NO_CHUNK = 1, 2
+STATIC_SCRATCH_BYTES = 8 << 20  # TMW_STATIC_SCRATCH_BYTES
 # kernel kinds of tmw_kernel_counts / tmw_time_kernel (include/tmw.h TMW_K_*)
 KINDS = ["hop32", "k1_32", "k2_32", "k2_32_dots", "hop64", "k1_64", "k2_64", "xpay64", "ainvxpay64", "update_s", "update_xrp",
          "acc_y", "resid_convert", "convert", "dot_norm64", "sub_norm", "diag64", "pack_both", "unpack_both", "other",
          "memset_bytes", "copy_bytes", "hop32_loadonly", "staged", "ffma_probe", "ffma2_probe", "ring"]
 FFMA_PROBE_FMAS_PER_THREAD = 16 * 16384
 
-EXPORTS = ["tmw_create", "tmw_apply", "tmw_apply_schur", "tmw_solve", "tmw_apply_multi", "tmw_apply_schur_multi",
+EXPORTS = ["tmw_create", "tmw_apply", "tmw_apply_schur", "tmw_apply_schur_static", "tmw_solve", "tmw_apply_multi", "tmw_apply_schur_multi",
            "tmw_solve_multi", "tmw_cheb_apply", "tmw_spinor_bytes", "tmw_pack", "tmw_unpack",
            "tmw_get_clover", "tmw_set_location", "tmw_set_debug", "tmw_launch_count", "tmw_kernel_counts",
            "tmw_time_kernel", "tmw_destroy", "tmw_last_error"]
@@ -80,6 +81,8 @@ def load():
     lib.tmw_apply.restype = I
     lib.tmw_apply_schur.argtypes = [P, I, I, P, P]
     lib.tmw_apply_schur.restype = I
+    lib.tmw_apply_schur_static.argtypes = [P, I, I, P, P]
+    lib.tmw_apply_schur_static.restype = I
     lib.tmw_solve.argtypes = [P, P, P, DBL, ctypes.POINTER(tmw_solve_info)]
     lib.tmw_solve.restype = I
     lib.tmw_apply_multi.argtypes = [P, I, I, I, I, P, P]
@@ -162,6 +165,13 @@ class Context:
 
     def apply_schur(self, op: int, prec: int, src, dst):
         self._check(self._lib.tmw_apply_schur(self._h, op, prec, _ptr(src), _ptr(dst)))
+
+    def apply_schur_static(self, op: int, prec: int, src, dst):
+        """tmw_apply_schur_static: apply_schur for callers that must not allocate device memory (a pool allocator owns
+        the card, a memory quota, a loop that cannot take cudaMalloc's device-wide stall). The intermediate lives in the
+        8 MiB array built into libtmw.so (STATIC_SCRATCH_BYTES); larger parity spinors raise TmwError(EINVAL). All
+        calls on a device share that array, so keep them on one stream; see include/tmw.h."""
+        self._check(self._lib.tmw_apply_schur_static(self._h, op, prec, _ptr(src), _ptr(dst)))
 
     def solve(self, b, x, tol: float, allow_noconv: bool = False) -> dict:
         info = tmw_solve_info()
