@@ -140,6 +140,8 @@ typedef struct {
 /* Test hooks (tmw_options.debug / tmw_set_debug): they change which code path runs, never the result. */
 #define TMW_DEBUG_FORCE_PIVOT 1 /* tmw_create: invert the clover blocks with the pivoted Gauss-Jordan fallback kernel */
 #define TMW_DEBUG_NO_CHUNK 2    /* tmw_solve_multi: do not split the columns into chunks that fit the free memory */
+#define TMW_DEBUG_FORCE_DEFECT 4 /* tmw_solve_multi: send the odd-numbered columns through one fp64 defect-correction pass as if
+                                   their full-lattice residual had missed tol (the other columns must come out untouched) */
 
 typedef struct {
   int iters;            /* BiCGStab iterations (each = 2 Schur-operator applications) or GCR steps (1 application each) */

@@ -70,6 +70,7 @@ struct tmw_ctx {
   int vh_loc;        // sites per parity of one domain (= g.Vh without decomposition)
   int ghost_cols;    // columns the send / receive buffers hold
   void* dd_tmp;      // scratch output spinors for stencil launches that keep only a reduction
+  size_t dd_tmp_bytes; // its size: grows with the highest column a reduction-only launch has used
   cudaStream_t h2d, d2h;             // copy streams of the pipelined host-pointer tmw_apply (lazily created)
   cudaEvent_t ev_in[NSLAB], ev_out[NSLAB]; // per t-slab: input arrived / output ready
   cudaStream_t comm; // the halo exchange runs here, beside the interior pass on `stream`
@@ -99,6 +100,16 @@ struct tmw_ctx {
   long long launches;
   long long kcount[TMW_K_COUNT];  // per kernel kind: column applications (or bytes), see include/tmw.h TMW_K_*
   std::string err;
+};
+
+// Sets tmw_ctx::cur_skip for the lifetime of the guard: the LAUNCH / CK macros return from the middle of a block, and a
+// skip pointer left behind would make every later stencil launch of the context return without writing.
+struct SkipGuard {
+  tmw_ctx* c;
+  SkipGuard(tmw_ctx* ctx, const int* skip) : c(ctx) { c->cur_skip = skip; }
+  ~SkipGuard() { c->cur_skip = nullptr; }
+  SkipGuard(const SkipGuard&) = delete;
+  SkipGuard& operator=(const SkipGuard&) = delete;
 };
 
 static thread_local std::string g_create_err;
@@ -294,7 +305,15 @@ static int dslash_dd(tmw_ctx* ctx, int epi, int par, int dagger, const void* in,
     ctx->ghost_cols = cmax + 1;
   }
   if (!out) {  // only a reduction is wanted, but the interior pass needs somewhere to leave the raw sums of the cut sites
-    if (!ctx->dd_tmp) { int rc = dev_alloc(ctx, &ctx->dd_tmp, (size_t)ctx->g.Vh * 24 * 8 * MAXCOL); if (rc) return rc; }
+    // column c is written at c whole-lattice packed spinors of precision R: room for columns 0..cmax, no more
+    const size_t need = (size_t)ctx->g.Vh * 24 * sizeof(R) * (cmax + 1);
+    if (need > ctx->dd_tmp_bytes) {
+      CK(cudaStreamSynchronize(ctx->stream));
+      if (ctx->dd_tmp) { dev_free(ctx, ctx->dd_tmp); ctx->dd_tmp = nullptr; ctx->dd_tmp_bytes = 0; }
+      int rc = dev_alloc(ctx, &ctx->dd_tmp, need);
+      if (rc) return rc;
+      ctx->dd_tmp_bytes = need;
+    }
     out = ctx->dd_tmp;
   }
   std::vector<DslashArgs<R>> A(nd);
@@ -587,7 +606,7 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
       (o.reconstruct != 12 && o.reconstruct != 18) || (o.mass_reading != TMW_TWIST_GAMMA5 && o.mass_reading != TMW_MASS_SCALAR) ||
       o.max_iter < 0 || !(o.delta > 0.0) || !(o.delta < 1.0) || (o.solver != TMW_BICGSTAB && o.solver != TMW_GCR) || o.nkrylov < 1 ||
       o.nkrylov > GCR_KMAX || o.columns_per_thread < 0 || o.columns_per_thread > 4 ||
-      (o.debug & ~(TMW_DEBUG_FORCE_PIVOT | TMW_DEBUG_NO_CHUNK)) || o.stage < -1 || o.stage > 1 || o.stage_tile[0] < 0 ||
+      (o.debug & ~(TMW_DEBUG_FORCE_PIVOT | TMW_DEBUG_NO_CHUNK | TMW_DEBUG_FORCE_DEFECT)) || o.stage < -1 || o.stage > 1 || o.stage_tile[0] < 0 ||
       o.stage_tile[1] < 0 || o.stage_tile[2] < 0 || o.zchunk < -1 || o.ring < -1 || o.ring > 1 || o.prefetch < -1)
     return fail(nullptr, TMW_EINVAL, "tmw_create: bad option value");
   if (!isfinite(m.re) || !isfinite(m.im) || !isfinite(c_sw)) return fail(nullptr, TMW_EINVAL, "tmw_create: non-finite parameter");
@@ -764,7 +783,7 @@ int tmw_set_location(tmw_ctx* ctx, int location) {
 
 int tmw_set_debug(tmw_ctx* ctx, int flags) {
   if (!ctx) return TMW_EINVAL;
-  if (flags & ~(TMW_DEBUG_FORCE_PIVOT | TMW_DEBUG_NO_CHUNK)) return fail(ctx, TMW_EINVAL, "tmw_set_debug: unknown flag");
+  if (flags & ~(TMW_DEBUG_FORCE_PIVOT | TMW_DEBUG_NO_CHUNK | TMW_DEBUG_FORCE_DEFECT)) return fail(ctx, TMW_EINVAL, "tmw_set_debug: unknown flag");
   ctx->opt.debug = flags;
   return TMW_OK;
 }
@@ -1156,8 +1175,11 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
   for (int c = 0; c < ncols; c++) if (!cs[c].done) cols_add(act, c);
   if (act.n == 0) return TMW_OK;
   // y = 0, r64 = bhat, r = (R) r64, rhat = r, x = p = v = 0
-  MEMSETK(W[3], 0, bytes64 * ncols);
-  MEMSETK(x, 0, bytesR * ncols);
+  // only the columns that are iterated: W[3] of the others holds their finished solution (defect-correction pass)
+  for (int i = 0; i < act.n; i++) {
+    MEMSETK(colp(W[3], act.col[i], bytes64), 0, bytes64);
+    MEMSETK(colp(x, act.col[i], bytesR), 0, bytesR);
+  }
   LAUNCHK(TMW_K_CONVERT, act.n, launch_convert<R>(n64, ctx->vh_loc, W[2], rhat, act, s));
   memset(h, 0, MAXCOL * sizeof(Scalars));
   if ((rc = push_scalars(ctx))) return rc;
@@ -1199,19 +1221,20 @@ int solve_schur(tmw_ctx* ctx, int ncols, double tol, ColState* cs) {
     if (act.n == 0) return TMW_OK;
     long long per_iter[TMW_K_COUNT];  // what one iteration adds to the kernel counts
     memcpy(per_iter, ctx->kcount, sizeof(per_iter));
-    ctx->cur_skip = ctx->attn;
-    LAUNCH(launch_sc_begin_iter(ctx->sc, act, ctx->attn, enq > 0, delta2, s));
-    rc = schur<R>(ctx, 0, p, v, tmp, act, 1, rhat, red_rhat_v, SCD);
-    if (!rc) {
-      LAUNCH(launch_sc_alpha(ctx->sc, act, ctx->attn, s));
-      LAUNCHK(TMW_K_UPDATE_S, act.n, launch_update_s<R>(nR, sv, r, v, ctx->sc, act, ctx->attn, s));
-      rc = schur<R>(ctx, 0, sv, t, tmp, act, 4, rhat, red_ts, SCD);  // <t,s>, <t,t>, <rhat,t>, <rhat,s>
+    {
+      SkipGuard skip_guard(ctx, ctx->attn);  // cur_skip = attn until the end of this block, on every way out of it
+      LAUNCH(launch_sc_begin_iter(ctx->sc, act, ctx->attn, enq > 0, delta2, s));
+      rc = schur<R>(ctx, 0, p, v, tmp, act, 1, rhat, red_rhat_v, SCD);
+      if (!rc) {
+        LAUNCH(launch_sc_alpha(ctx->sc, act, ctx->attn, s));
+        LAUNCHK(TMW_K_UPDATE_S, act.n, launch_update_s<R>(nR, sv, r, v, ctx->sc, act, ctx->attn, s));
+        rc = schur<R>(ctx, 0, sv, t, tmp, act, 4, rhat, red_ts, SCD);  // <t,s>, <t,t>, <rhat,t>, <rhat,s>
+      }
+      if (!rc) {
+        LAUNCH(launch_sc_omega(ctx->sc, act, ctx->attn, s));                                        // omega, rho' = <rhat, s - omega t>, beta
+        LAUNCHK(TMW_K_UPDATE_XRP, act.n, launch_update_xrp<R>(nR, x, r, p, sv, t, v, ctx->sc, act, ctx->attn, s));  // x, r, and p of the next iteration
+      }
     }
-    if (!rc) {
-      LAUNCH(launch_sc_omega(ctx->sc, act, ctx->attn, s));                                        // omega, rho' = <rhat, s - omega t>, beta
-      LAUNCHK(TMW_K_UPDATE_XRP, act.n, launch_update_xrp<R>(nR, x, r, p, sv, t, v, ctx->sc, act, ctx->attn, s));  // x, r, and p of the next iteration
-    }
-    ctx->cur_skip = nullptr;
     if (rc) return rc;
     for (int i = 0; i < TMW_K_COUNT; i++) per_iter[i] = ctx->kcount[i] - per_iter[i];
     enq++;
@@ -1535,7 +1558,11 @@ static int solve_chunk(tmw_ctx* ctx, int nrhs, const double* b, double* x, doubl
     for (int round = 0; round < 2 && status == TMW_OK; round++) {
       ColMap bad;
       bad.n = 0;
-      for (int i = 0; i < nz.n; i++) if (!(cs[nz.col[i]].true_resid <= tol)) cols_add(bad, nz.col[i]);
+      for (int i = 0; i < nz.n; i++) {
+        const int c = nz.col[i];
+        const bool forced = round == 0 && (ctx->opt.debug & TMW_DEBUG_FORCE_DEFECT) && (c & 1);  // test hook: a strict subset
+        if (!(cs[c].true_resid <= tol) || forced) cols_add(bad, c);
+      }
       if (bad.n == 0) break;
       if (ctx->verbose) fprintf(stderr, "[tmw] defect correction %d for %d column(s): full residual %.3e > tol\n", round + 1, bad.n, cs[bad.col[0]].true_resid);
       if ((rc = need_w64(ctx, NW64))) return rc;
@@ -1611,7 +1638,8 @@ extern "C" int tmw_solve_multi(tmw_ctx* ctx, int nrhs, const double* b, double* 
     const size_t cbytes = (size_t)ctx->V * 24 * 8;
     // GCR: 2 nkrylov Krylov vectors per column on top (the columns step together)
     const size_t gcr = ctx->opt.solver == TMW_GCR ? 2 * (size_t)ctx->opt.nkrylov * bin : 0;
-    const size_t per_col = 8 * b64 + 8 * bin + gcr + (ctx->opt.location == TMW_HOST ? 2 * cbytes : 0);
+    // decomposed contexts: one more fp64 parity spinor per column for the reduction-only launches of the final residual (dd_tmp)
+    const size_t per_col = 8 * b64 + 8 * bin + gcr + (ctx->opt.location == TMW_HOST ? 2 * cbytes : 0) + (ctx->dom.empty() ? 0 : b64);
     size_t held = 0;
     for (int i = 0; i < NW64; i++) if (ctx->w64[i]) held += b64 * ctx->ws_cols;
     for (int i = 0; i < 8; i++) if (ctx->w32[i]) held += bin * ctx->ws_cols;

@@ -24,7 +24,7 @@ TWIST_GAMMA5, MASS_SCALAR = 0, 1
 D, DDAG, G5D = 0, 1, 2
 FULL, EVEN, ODD = 0, 1, 2
 F32, F64 = 0, 1
-DEBUG_FORCE_PIVOT, DEBUG_NO_CHUNK = 1, 2
+DEBUG_FORCE_PIVOT, DEBUG_NO_CHUNK, DEBUG_FORCE_DEFECT = 1, 2, 4
 STATIC_SCRATCH_BYTES = 8 << 20  # TMW_STATIC_SCRATCH_BYTES
 # kernel kinds of tmw_kernel_counts / tmw_time_kernel (include/tmw.h TMW_K_*)
 KINDS = ["hop32", "k1_32", "k2_32", "k2_32_dots", "hop64", "k1_64", "k2_64", "xpay64", "ainvxpay64", "update_s", "update_xrp",

@@ -218,6 +218,28 @@ def test_solve_multi_mixed_columns_host(tmw):
         assert np.linalg.norm((x0 - x[0]).ravel()) <= 1e-9 * np.linalg.norm(x[0].ravel())
 
 
+@pytest.mark.parametrize("solver", ["bicgstab", "gcr"])
+def test_defect_correction_of_a_subset_leaves_the_other_columns_alone(tmw, solver):
+    """The fp64 defect-correction pass (full-lattice residual above tol although the Schur system converged) re-solves only
+    the columns that missed; TMW_DEBUG_FORCE_DEFECT sends columns 1 and 3 of 5 through it. Every column, corrected or not,
+    must still be the oracle's solution (the pass once zeroed the odd-site solution of the columns it did not re-solve)."""
+    L, T, m, c_sw = 4, 8, -0.0514 + 0.003j, 1.0424
+    U = synth.gauge_field(L, T, 0.35, seed=1)
+    F = oracle.field_strength(U)
+    b = np.stack([synth.point_source(L, T, 0, 0), synth.gaussian_spinor(L, T, 3), synth.z2_source(L, T, 2),
+                  synth.point_source(L, T, 2, 1), synth.gaussian_spinor(L, T, 4)])
+    n = b.shape[0]
+    with tmw.Context(L, T, dev(U), m, c_sw, solver=tmw.GCR if solver == "gcr" else tmw.BICGSTAB, debug=tmw.DEBUG_FORCE_DEFECT) as ctx:
+        x = torch.full(b.shape, 7.0, dtype=torch.complex128, device="cuda")
+        infos = ctx.solve_multi(n, dev(b), x, 1e-10)
+        assert ctx.kernel_counts()["sub_norm"] >= 2 * 2 * 2  # b - D x and x + e, two parities, two columns
+        x = x.cpu().numpy()
+        for c in range(n):
+            assert infos[c]["true_resid"] <= 1e-10 and infos[c]["iters"] > 0, (c, infos[c])
+            x_ref, _ = oracle.bicgstab(U, b[c], m, c_sw, tol=1e-12, F=F)
+            check_solution(U, b[c], x[c], m, c_sw, x_ref, F=F)
+
+
 def test_solve_multi_edge_cases(tmw):
     L, T = 4, 4
     U = synth.gauge_field(L, T, 0.3, seed=1)
