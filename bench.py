@@ -87,7 +87,6 @@ def parse_args():
     ap.add_argument("--stage", type=int, default=0, help="tmw_options.stage: 1 = shared-memory staged fp32 stencil wherever a tile fits (default 0: off)")
     ap.add_argument("--stage-tile", default="0,0,0", help="tmw_options.stage_tile: tile extents x/2,y,z of the staged stencil (0,0,0: chosen by the library)")
     ap.add_argument("--delta", type=float, default=0.0, help="tmw_options.delta: reliable-update threshold (0: the library default 1e-5)")
-    ap.add_argument("--ring", type=int, default=0, help="tmw_options.ring: 1 = persistent stencil with the links prefetched through a shared-memory ring (default 0: off)")
     ap.add_argument("--columns-per-thread", type=int, default=0, help="tmw_options.columns_per_thread of the multi-column stencil (0: automatic)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -111,10 +110,11 @@ class ClockSampler(threading.Thread):
                0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
                0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
 
-    def __init__(self, index: int, period: float = 0.05):
+    def __init__(self, index: int, period: float = 0.02):
         super().__init__(daemon=True)
         self.index, self.period = index, period
         self.samples, self.mem_samples, self.reason_bits, self.power = [], [], 0, []
+        self.timeline = []  # (host perf_counter, SM MHz, reason bits) of every sample
         self.stop_flag = threading.Event()
         self.ok = False
         try:
@@ -133,13 +133,23 @@ class ClockSampler(threading.Thread):
         nv = self.nv
         while not self.stop_flag.is_set():
             try:
-                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                mhz = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                bits = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                self.samples.append(mhz)
                 self.mem_samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_MEM))
-                self.reason_bits |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                self.reason_bits |= bits
+                self.timeline.append((time.perf_counter(), mhz, bits))
                 self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
             except Exception:
                 pass
             self.stop_flag.wait(self.period)
+
+    def window(self, t_lo: float, t_hi: float):
+        """(median SM MHz, share of the samples with sw_power_cap set, samples) over the host-time window [t_lo, t_hi]"""
+        w = [(mhz, bits) for (t, mhz, bits) in self.timeline if t_lo <= t <= t_hi]
+        if not w:
+            return None, None, 0
+        return float(np.median([a for a, _ in w])), float(np.mean([1.0 if b & 0x4 else 0.0 for _, b in w])), len(w)
 
     def summary(self):
         if not self.ok:
@@ -267,7 +277,7 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
     torch.cuda.synchronize()
     e0, e1 = ev(), ev()
     e0.record()
-    tuning = dict(stage=args.stage, stage_tile=tuple(int(v) for v in args.stage_tile.split(",")), columns_per_thread=args.columns_per_thread, ring=args.ring,
+    tuning = dict(stage=args.stage, stage_tile=tuple(int(v) for v in args.stage_tile.split(",")), columns_per_thread=args.columns_per_thread,
                   delta=args.delta)
     ctx = tmw.Context(L, T, dU, m, c_sw, stream=stream, **tuning)
     e1.record()
@@ -324,6 +334,8 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
     launches0 = ctx.launch_count()
     counts0 = ctx.kernel_counts()
     t0, t1 = ev(), ev()
+    torch.cuda.synchronize()
+    host_t0 = time.perf_counter()  # the device is idle: t0 fires now, so device offsets from t0 map onto the host clock
     t0.record()
     for _ in range(args.steps):
         step(timers)
@@ -340,7 +352,18 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
     info = infos[-1] or {"iters": None, "reliable_updates": None, "true_resid": None}
     sites = float(Vh) * napply * args.steps * world
     gflops = FLOP_PER_SITE * sites / (dsl_total_ms * 1e-3) / 1e9
-    t_launch_s = sum(dsl_ms) * 1e-3 / (napply * args.steps)  # this rank's mean launch duration, events on `stream`
+    # SURVEY 8(d) protocol: the Dslash part of every step is one repeat of `napply` back-to-back launches; the roofline
+    # figure is the MEDIAN repeat (min and every repeat with the SM clock it ran at are printed beside it)
+    per_launch_ms = [v / napply for v in dsl_ms]
+    repeats = []
+    for (_, _, d0, d1), v in zip(timers, per_launch_ms):
+        lo, hi = host_t0 + t0.elapsed_time(d0) * 1e-3, host_t0 + t0.elapsed_time(d1) * 1e-3
+        mhz, capped, nsamp = sampler.window(lo, hi) if sampler.ok else (None, None, 0)
+        repeats.append({"ms_per_launch": v, "sm_mhz": mhz, "power_capped_share": capped, "clock_samples": nsamp})
+    dsl_median_ms, dsl_min_ms = float(np.median(per_launch_ms)), float(min(per_launch_ms))
+    capped = [r["power_capped_share"] for r in repeats if r["power_capped_share"] is not None]
+    regime = None if not capped else ("power-capped" if float(np.median(capped)) >= 0.5 else "burst")
+    t_launch_s = dsl_median_ms * 1e-3  # this rank's median-repeat launch duration, events on `stream`
     peak, peak_src = load_peaks()
     achieved = BYTES_COMPULSORY * Vh / t_launch_s / 1e9
     # ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, by kernel kind (profiles/kernel_traffic.csv, one
@@ -358,7 +381,10 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
                 "peak_source": peak_src, "bytes_per_site": BYTES_COMPULSORY, "sites_per_launch": Vh,
                 "launch_ms": 1e3 * t_launch_s, "streaming_model_gbs": BYTES_STREAMING * Vh / t_launch_s / 1e9,
-                "frac_of_8TBs_nominal": achieved / 8000.0}
+                "frac_of_8TBs_nominal": achieved / 8000.0,
+                "statistic": f"median of {len(per_launch_ms)} repeats of {napply} launches", "regime": regime,
+                "frac_min_repeat": BYTES_COMPULSORY * Vh / (dsl_min_ms * 1e-3) / 1e9 / peak,
+                "frac_mean": BYTES_COMPULSORY * Vh / (sum(dsl_ms) * 1e-3 / (napply * args.steps)) / 1e9 / peak}
 
     # ---- the whole solve against the roofline: algorithmic bytes of ONE tmw_solve = (column applications of every kernel
     # kind the context issued inside the timed region, tmw_kernel_counts) x (bytes per site of that kind) x V_h,
@@ -469,8 +495,7 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
         ach = bpc * Vh * n / (ms_hop * 1e-3) / 1e9
         pk, pk_src = load_peaks()
         staged = (k1["staged"] - k0["staged"]) > 0
-        ringed = (k1["ring"] - k0["ring"]) > 0
-        multi["roofline"] = {"bound": "hbm", "kernel": ("dslash_stage_kernel" if staged else "dslash_ring_kernel" if ringed else "dslash_kernel") + "<float,12,EPI_HOP,NR=2|3> (multi-column hop)",
+        multi["roofline"] = {"bound": "hbm", "kernel": ("dslash_stage_kernel" if staged else "dslash_kernel") + "<float,12,EPI_HOP,NR=2|3> (multi-column hop)",
                              "achieved": ach, "peak": pk, "unit": "GB/s", "frac": ach / pk, "bytes_per_site_and_column": bpc, "peak_source": pk_src,
                              "note": "not HBM-bound: the links are amortised, the 8 neighbour spinors per column are not (DESIGN.md 6b)"}
         # K1 + K2 (one Schur-operator application) on n columns: per site and column K1 96 in + 96 out, K2 96 in + 96 aux + 96 out,
@@ -480,8 +505,8 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
         multi["schur_ms_per_rhs"] = ms_schur / n
         multi["roofline_schur"] = {"bound": "hbm", "kernel": "K1 + K2 on %d columns (tmw_apply_schur_multi, fp32)" % n, "achieved": ach_s, "peak": pk,
                                    "unit": "GB/s", "frac": ach_s / pk, "bytes_per_site_and_column": bps_schur, "peak_source": pk_src}
-        multi["tuning"] = {"stage": args.stage, "stage_tile": args.stage_tile, "columns_per_thread": args.columns_per_thread, "ring": args.ring,
-                           "staged_kernel_ran": staged, "ring_kernel_ran": ringed}
+        multi["tuning"] = {"stage": args.stage, "stage_tile": args.stage_tile, "columns_per_thread": args.columns_per_thread,
+                           "staged_kernel_ran": staged}
         # the fp32 ALU ceiling beside it (register-only FMA loops, tmw_time_kernel): with the links amortised the multi-column hop
         # is as close to this ceiling as to the HBM one
         try:
@@ -548,8 +573,8 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
                          f"evenly spaced sites of the same {L}^3x{T} field, {passes} pass(es), {dt:.1f} s",
                "msites_per_s": ns / dt / 1e6}
         # the oracle's BiCGStab beside tmw_solve (the paper's one number for this path is a CPU BiCGStab time):
-        # to convergence with --cpu-solve, else a bounded sample of --cpu-solve-iters iterations (each = 2 D applications +
-        # the recurrences on the full lattice), scaled by the iteration count the full solve needs
+        # to convergence with --cpu-solve, else a bounded sample: runs of --cpu-solve-iters - 1 and --cpu-solve-iters iterations
+        # (each = 2 D applications + the recurrences on the full lattice), reported per iteration
         cpu["note"] = ("not like for like: the oracle is a deliberately plain fp64 program (explicit 4x4 gamma matrices on full spinors, 18-real "
                        "links, AoS, no even-odd, no SIMD), the GPU figure is the fp32 spin-projected 12-real kernel; the reference ships no CPU code")
         if (args.cpu_solve or args.cpu_solve_iters > 0) and not args.skip_solve:
@@ -572,20 +597,25 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
                                solve="oracle.bicgstab (full-lattice fp64 BiCGStab, no preconditioning) to tol, incl. its clover-leaf setup "
                                      f"({t_f:.1f} s)")
                 else:
-                    k = args.cpu_solve_iters
-                    _, oinfo = oracle.bicgstab(np.asarray(U), bsrc, m, c_sw, tol=1e-300, max_iter=k, F=Fo)
-                    dt = time.perf_counter() - t0  # k iterations + the closing true-residual application
-                    per_iter = dt / (k + 0.5)
-                    # iterations the oracle needs on this config and source (measured: tests/golden/cfg4_solution_sample.txt
-                    # header for config 4 at 1e-12; BASELINE.md 5 for the others); unknown configs: twice the even-odd count
-                    full_iters = {"cfg4_48x144_clover": 36, "cfg3_32x96_clover": 27, "cfg2_24x64_clover": 23, "cfg1_24x64_tm": 22,
-                                  "cfg0_4x8": 29}.get(cfg["name"], 2 * (info["iters"] or 0))
-                    cpu.update(solve_s=per_iter * full_iters + t_f, solve_kind="bounded sample, scaled", solve_sample_s=dt, solve_sample_iters=k,
-                               solve_iters=full_iters, solve_s_per_iter=per_iter,
-                               solve=f"oracle.bicgstab (full-lattice fp64 BiCGStab, no preconditioning): {k} iterations timed ({dt:.1f} s incl. its "
-                                     f"closing residual application), scaled to the {full_iters} iterations the solve to 1e-10 takes, + its "
-                                     f"clover-leaf setup ({t_f:.1f} s); --cpu-solve runs it to convergence (340 s measured at 48^3 x 144 to "
-                                     "1e-10: profiles/r2_oracle_cfg4_solve.md)")
+                    # two bounded runs of k1 < k2 iterations; their difference is the cost of k2 - k1 iterations with the
+                    # start-up and the closing true-residual application cancelled. Nothing is extrapolated: the line carries
+                    # the measured seconds per iteration, not a product with an iteration count taken from elsewhere.
+                    k2 = max(2, args.cpu_solve_iters)
+                    k1 = k2 - 1
+                    t0 = time.perf_counter()
+                    oracle.bicgstab(np.asarray(U), bsrc, m, c_sw, tol=1e-300, max_iter=k1, F=Fo)
+                    dt1 = time.perf_counter() - t0
+                    t0 = time.perf_counter()
+                    oracle.bicgstab(np.asarray(U), bsrc, m, c_sw, tol=1e-300, max_iter=k2, F=Fo)
+                    dt2 = time.perf_counter() - t0
+                    per_iter = (dt2 - dt1) / (k2 - k1)
+                    cpu.update(solve_s=None, solve_kind="bounded sample, per iteration", solve_sample_s=dt1 + dt2, solve_sample_iters=[k1, k2],
+                               solve_s_per_iter=per_iter, solve_fixed_s=dt1 - k1 * per_iter, solve_setup_s=t_f,
+                               solve=f"oracle.bicgstab (full-lattice fp64 BiCGStab, no preconditioning): runs of {k1} and {k2} iterations timed "
+                                     f"({dt1:.1f} s, {dt2:.1f} s); solve_s_per_iter = their difference, solve_fixed_s = start-up + closing "
+                                     f"residual, solve_setup_s = its clover-leaf setup; no whole-solve figure is derived (solve_s null). "
+                                     "--cpu-solve runs it to convergence (340 s measured at 48^3 x 144 to 1e-10: "
+                                     "profiles/r2_oracle_cfg4_solve.md)")
                 del Fo
 
     ctx.destroy()
@@ -597,6 +627,7 @@ def run_tmw(args, cfg, rank: int, world: int, local_rank: int):
                 "step": ("SOLVE SKIPPED (profiling run, not a bench value): " if args.skip_solve else
                          f"1 tmw_solve(tol={args.tol:g}) + ") + f"{napply} fp32 Dslash applications",
                 "dslash_gsites_per_s": sites / (dsl_total_ms * 1e-3) / 1e9, "dslash_ms": dsl_total_ms / (napply * args.steps),
+                "dslash_ms_median": dsl_median_ms, "dslash_ms_min": dsl_min_ms, "dslash_repeats": repeats,
                 "solve_ms": solve_mean_ms, "solve_iters": info["iters"], "solve_reliable_updates": info["reliable_updates"],
                 "solve_true_resid": info["true_resid"], "setup_ms": setup_ms,
                 "roofline": roofline, "roofline_solve": roofline_solve, "roofline_kernels": roofline_kernels,

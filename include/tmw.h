@@ -39,6 +39,8 @@
 #ifndef TMW_H
 #define TMW_H
 
+#include <stddef.h>
+
 #ifdef __cplusplus
 extern "C" {
 #endif
@@ -81,6 +83,9 @@ typedef struct { double re, im; } tmw_complex;
 #define TMW_F64 1
 
 typedef struct {
+  size_t struct_size; /* = sizeof(tmw_options) of the header the caller was compiled against (TMW_OPTIONS_INIT sets it).
+                         tmw_create refuses (TMW_EINVAL) a size it does not know instead of misreading a struct laid out by
+                         another version of this header; every other member may be 0 = default. */
   int location;     /* TMW_DEVICE (default) | TMW_HOST: where canonical-layout pointers live */
   int precision;    /* TMW_MIXED (default) | TMW_DOUBLE: solver arithmetic */
   int reconstruct;  /* fp32 gauge storage: 12 (default; third row rebuilt in-kernel, links must be SU(3)) | 18 */
@@ -91,8 +96,7 @@ typedef struct {
   int solver;       /* TMW_BICGSTAB (default; the paper's CPU solver) | TMW_GCR (its "standard GPU inverter with
                        GCR algorithm"): restarted GCR(nkrylov) on the same Schur system and kernels */
   int nkrylov;      /* GCR restart length, 1..16; 0 -> 8 */
-  int verbose;      /* != 0: one line per solver iteration, reliable update and restart on stderr. Setting the environment
-                       variable TMW_VERBOSE (to anything) has the same effect on every context of the process. */
+  int verbose;      /* != 0: one line per solver iteration, reliable update and restart on stderr */
   int columns_per_thread; /* tuning of the multi-column fp32 stencil (tmw_*_multi): 1..4 right-hand-side
                              columns per thread (links and clover blocks stay in registers for them); 0 = automatic */
   int tile[4];      /* log2 extents (x/2, y, z, t) of the 4-D tile of 128 sites a CTA of the single-column stencil covers;
@@ -123,12 +127,6 @@ typedef struct {
      columns stay in L2. 0 = automatic (the largest slab whose +-t window fits a fixed L2 budget), -1 = off (time slice
      after time slice), > 0 = that many sites (must divide L, with L*L*zchunk/2 a multiple of 128; else off). */
   int zchunk;
-  /* Persistent fp32 stencil with link prefetch: CTAs walk over the site blocks and every thread has the 8
-     links of its next site in flight through a private ring in shared memory (cp.async), so that the loads that always
-     miss to DRAM are off the critical path. 12-real links, hop / K1 / K2, no domain decomposition, 1-D site mapping.
-     0 or -1 = off (default: measured on B200 it is 20-120 % slower than the plain kernel, the extra LDGSTS + LDS traffic
-     saturates the L1/shared-memory pipe; profiles/r2_stage.md), 1 = wherever it applies. */
-  int ring;
   /* L2 prefetch of the links: a CTA of the plain stencil also issues prefetch.global.L2 for the links of the
      site block `prefetch` blocks ahead of its own (the links are the loads that always miss to DRAM). 0 = automatic: one
      block ahead in the multi-column fp32 hop launches (measured: -7..10 % at 12 columns 32^3 x 96, -3 % at 3 columns
@@ -136,6 +134,7 @@ typedef struct {
      of 128 sites for every stencil launch. */
   int prefetch;
 } tmw_options;
+#define TMW_OPTIONS_INIT {sizeof(tmw_options)} /* tmw_options o = TMW_OPTIONS_INIT; : all defaults, struct_size set */
 
 /* Test hooks (tmw_options.debug / tmw_set_debug): they change which code path runs, never the result. */
 #define TMW_DEBUG_FORCE_PIVOT 1 /* tmw_create: invert the clover blocks with the pivoted Gauss-Jordan fallback kernel */
@@ -311,8 +310,7 @@ long long tmw_launch_count(const tmw_ctx* ctx);
 #define TMW_K_FFMA_PROBE 24    /* tmw_time_kernel only: TMW_FFMA_PROBE_FMAS_PER_THREAD scalar fp32 FMAs (16 independent chains) per thread */
 #define TMW_K_FFMA2_PROBE 25   /* tmw_time_kernel only: the same FMAs as packed pairs (fma.rn.f32x2, 8 chains of 2) */
 #define TMW_FFMA_PROBE_FMAS_PER_THREAD (16 * 16384) /* the probe launches (SM count) x 8 CTAs of 256 threads */
-#define TMW_K_RING 26          /* of the fp32 stencil applications above: those that ran in the persistent link-ring kernel */
-#define TMW_K_COUNT 27
+#define TMW_K_COUNT 26
 
 /*
  * counts[k] (k < min(n, TMW_K_COUNT)) = how many right-hand-side columns kernels of kind k have been applied to since

@@ -16,7 +16,7 @@ CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libtmw.so")
 OBJDIR = os.path.join(_HERE, "build")
 SOURCES = ["tmw_api.cu", "tmw_dslash_f32.cu", "tmw_dslash_f32_nr2.cu", "tmw_dslash_f32_nr3.cu", "tmw_dslash_f32_nr4.cu",
-           "tmw_dslash_f64.cu", "tmw_dslash_stage_nr1.cu", "tmw_dslash_stage_nr2.cu", "tmw_dslash_stage_nr3.cu", "tmw_dslash_ring_nr1.cu", "tmw_dslash_ring_nr2.cu", "tmw_dslash_ring_nr3.cu", "tmw_dslash_ring_nr4.cu", "tmw_dd_f32.cu", "tmw_dd_f64.cu", "tmw_pack.cu", "tmw_clover.cu", "tmw_blas.cu"]
+           "tmw_dslash_f64.cu", "tmw_dslash_stage_nr1.cu", "tmw_dslash_stage_nr2.cu", "tmw_dslash_stage_nr3.cu", "tmw_dd_f32.cu", "tmw_dd_f64.cu", "tmw_pack.cu", "tmw_clover.cu", "tmw_blas.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
 
 

@@ -29,7 +29,9 @@ struct NvtxRange {
 using namespace tmw;
 
 enum { NW64 = 14 };
-enum { ZCHUNK_L2_BUDGET_MB = 24 };  // automatic z-slab of the multi-column sweep (tmw_options.zchunk = 0; measured)
+// automatic z-slab of the multi-column sweep (tmw_options.zchunk = 0): the +-t window may take this share of the L2 the
+// device reports (3/16 of B200's 126 MB = the 24 MB found best by the sweep of DESIGN.md 5a)
+enum { ZCHUNK_L2_SHARE_NUM = 3, ZCHUNK_L2_SHARE_DEN = 16, ZCHUNK_L2_FALLBACK_MB = 126 };
 enum { NSLAB = 24 };  // most t-slabs of the pipelined host-pointer tmw_apply
 
 // One domain of a domain-decomposed context: a sub-lattice L x L x (L/Pz) x (T/Pt) with its own packed
@@ -97,6 +99,8 @@ struct tmw_ctx {
   double* red;       // 4 * MAXCOL device doubles
   double* red_host;  // pinned
   cudaEvent_t ev0, ev1;
+  int sms;           // SM count and L2 size of the context's device (asked once in tmw_create)
+  int64_t l2_bytes;
   long long launches;
   long long kcount[TMW_K_COUNT];  // per kernel kind: column applications (or bytes), see include/tmw.h TMW_K_*
   std::string err;
@@ -384,14 +388,6 @@ static cudaError_t launch_stage(const DslashArgs<float>& a, int ng, int epi, int
   return launch_dslash_stage(a, ng, epi, clv, nr, sg, s);
 }
 static cudaError_t launch_stage(const DslashArgs<double>&, int, int, int, int, const StageGeom&, cudaStream_t) { return cudaErrorInvalidValue; }
-// the persistent link-ring kernel (tmw_dslash_ring.cuh): fp32, 12-real links, hop / K1 / K2 on the whole lattice, 1-D mapping
-template <typename R> static bool use_ring(tmw_ctx* ctx, int epi, int ncol, int cb1) {
-  (void)ncol;
-  if (sizeof(R) != 4 || ctx->opt.ring <= 0 || ctx->ng32 != 12 || cb1 >= 0 || !ctx->dom.empty() || ctx->g.tiled || ctx->opt.stage > 0) return false;
-  return epi == EPI_HOP || epi == EPI_AINV_HOP || epi == EPI_A_XPAY;
-}
-static cudaError_t launch_ring(const DslashArgs<float>& a, int epi, int clv, int nr, cudaStream_t s) { return launch_dslash_ring(a, epi, clv, nr, s); }
-static cudaError_t launch_ring(const DslashArgs<double>&, int, int, int, cudaStream_t) { return cudaErrorInvalidValue; }
 
 // cb0, cb1 (optional): restrict the launch to the output sites with checkerboard index in [cb0, cb1), cb0 a multiple of 128
 template <typename R>
@@ -417,7 +413,7 @@ static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, vo
     if (ctx->opt.zchunk > 0) {
       zc = ctx->opt.zchunk;
     } else if (ctx->opt.zchunk == 0) {
-      const int64_t budget = (int64_t)ZCHUNK_L2_BUDGET_MB << 20;  // in + out spinors of all columns over the 2-slice window
+      const int64_t budget = ctx->l2_bytes / ZCHUNK_L2_SHARE_DEN * ZCHUNK_L2_SHARE_NUM;  // in + out spinors of all columns over the 2-slice window
       for (int d = a.g.Lz; d >= 1; d--)
         if (a.g.Lz % d == 0 && (row * d) % 128 == 0 && 2 * row * d * 96 * 2 * cm.n <= budget) { zc = d; break; }
       if (zc == a.g.Lz) zc = 0;  // everything fits: keep the plain order
@@ -435,11 +431,6 @@ static int dslash(tmw_ctx* ctx, int epi, int par, int dagger, const void* in, vo
     }
   }
   const int clv = !ctx->clover ? CL_NONE : (ctx->m_im != 0.0 ? CL_TWISTED : CL_CLOVER);
-  if (use_ring<R>(ctx, epi, cm.n, cb1)) {
-    ctx->kcount[TMW_K_RING] += cm.n;
-    LAUNCHK(stencil_kind<R>(epi, red_mode), cm.n, launch_ring(a, epi, clv, nr, ctx->stream));
-    return TMW_OK;
-  }
   if (use_stage<R>(ctx, epi, cm.n, cb1, nr)) {
     ctx->kcount[TMW_K_STAGED] += cm.n;
     LAUNCHK(stencil_kind<R>(epi, red_mode), cm.n, launch_stage(a, ng_of<R>(ctx), epi, clv, nr, ctx->stage[nr], ctx->stream));
@@ -597,7 +588,11 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
   if (V / 2 >= (int64_t)1 << 31) return fail(nullptr, TMW_EINVAL, "tmw_create: lattice too large");
   tmw_options o;
   memset(&o, 0, sizeof(o));
-  if (opt) o = *opt;
+  if (opt) {
+    if (opt->struct_size != sizeof(tmw_options))
+      return fail(nullptr, TMW_EINVAL, "tmw_create: tmw_options.struct_size is not sizeof(tmw_options) of this library (set it, e.g. with TMW_OPTIONS_INIT; a header of another version?)");
+    o = *opt;
+  }
   if (o.reconstruct == 0) o.reconstruct = 12;
   if (o.max_iter == 0) o.max_iter = 10000;
   if (o.nkrylov == 0) o.nkrylov = 8;  // GCR(8) beats GCR(16) on every config (orthogonalisation traffic)
@@ -607,7 +602,7 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
       o.max_iter < 0 || !(o.delta > 0.0) || !(o.delta < 1.0) || (o.solver != TMW_BICGSTAB && o.solver != TMW_GCR) || o.nkrylov < 1 ||
       o.nkrylov > GCR_KMAX || o.columns_per_thread < 0 || o.columns_per_thread > 4 ||
       (o.debug & ~(TMW_DEBUG_FORCE_PIVOT | TMW_DEBUG_NO_CHUNK | TMW_DEBUG_FORCE_DEFECT)) || o.stage < -1 || o.stage > 1 || o.stage_tile[0] < 0 ||
-      o.stage_tile[1] < 0 || o.stage_tile[2] < 0 || o.zchunk < -1 || o.ring < -1 || o.ring > 1 || o.prefetch < -1)
+      o.stage_tile[1] < 0 || o.stage_tile[2] < 0 || o.zchunk < -1 || o.prefetch < -1)
     return fail(nullptr, TMW_EINVAL, "tmw_create: bad option value");
   if (!isfinite(m.re) || !isfinite(m.im) || !isfinite(c_sw)) return fail(nullptr, TMW_EINVAL, "tmw_create: non-finite parameter");
   const int pz = o.domains_z > 1 ? o.domains_z : 1, pt = o.domains_t > 1 ? o.domains_t : 1;
@@ -624,7 +619,20 @@ int tmw_create(tmw_ctx** out, int L, int T, const double* gauge, tmw_complex m, 
   ctx->vh_loc = ctx->g.Vh / (pz * pt);
   ctx->nr32 = o.columns_per_thread;
   for (int nr = 0; nr < 4; nr++) ctx->stage_ok[nr] = (nr >= 1 && nr <= 3 && pz * pt == 1) ? choose_stage(ctx->g, nr, o, ctx->stage[nr]) : false;
-  ctx->verbose = o.verbose != 0 || getenv("TMW_VERBOSE") != nullptr;
+  ctx->verbose = o.verbose != 0;
+  {
+    int dev = 0, sms = 0, l2 = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev);
+    if (e != cudaSuccess) {
+      const int rc = fail_cuda(nullptr, e, "tmw_create: device attributes");
+      delete ctx;
+      return rc;
+    }
+    ctx->sms = sms > 0 ? sms : 148;
+    ctx->l2_bytes = l2 > 0 ? (int64_t)l2 : (int64_t)ZCHUNK_L2_FALLBACK_MB << 20;
+  }
   ctx->V = V;
   ctx->m_re = m.re; ctx->m_im = m.im; ctx->c_sw = c_sw;
   ctx->opt = o;
@@ -1685,7 +1693,7 @@ extern "C" int tmw_time_kernel(tmw_ctx* ctx, int kind, int reps, double* ms) {
   if (!ctx) return TMW_EINVAL;
   if (!ms || reps < 1) return fail(ctx, TMW_EINVAL, "tmw_time_kernel: bad argument");
   if (ctx->opt.precision != TMW_MIXED || !ctx->dom.empty()) return fail(ctx, TMW_EINVAL, "tmw_time_kernel: needs a TMW_MIXED context without domain decomposition");
-  if ((kind == TMW_K_FFMA_PROBE || kind == TMW_K_FFMA2_PROBE) && spinor_bytes(ctx, TMW_F32) < (size_t)148 * 8 * 256 * 4)
+  if ((kind == TMW_K_FFMA_PROBE || kind == TMW_K_FFMA2_PROBE) && spinor_bytes(ctx, TMW_F32) < (size_t)ctx->sms * 8 * 256 * 4)
     return fail(ctx, TMW_EINVAL, "tmw_time_kernel: the lattice is too small to hold the probe's output");
   int rc;
   if ((rc = need_w64(ctx, 8))) return rc;
@@ -1711,7 +1719,7 @@ extern "C" int tmw_time_kernel(tmw_ctx* ctx, int kind, int reps, double* ms) {
       case TMW_K_UPDATE_S: LAUNCH(launch_update_s<float>(nR, X[4], X[0], X[3], ctx->sc, one, nullptr, ctx->stream)); return TMW_OK;
       case TMW_K_UPDATE_XRP: LAUNCH(launch_update_xrp<float>(nR, X[6], X[0], X[2], X[4], X[5], X[3], ctx->sc, one, nullptr, ctx->stream)); return TMW_OK;
       case TMW_K_FFMA_PROBE:
-      case TMW_K_FFMA2_PROBE: LAUNCH(launch_ffma_probe(kind == TMW_K_FFMA2_PROBE, TMW_FFMA_PROBE_FMAS_PER_THREAD, (float*)X[7], ctx->stream)); return TMW_OK;
+      case TMW_K_FFMA2_PROBE: LAUNCH(launch_ffma_probe(kind == TMW_K_FFMA2_PROBE, TMW_FFMA_PROBE_FMAS_PER_THREAD, ctx->sms, (float*)X[7], ctx->stream)); return TMW_OK;
       case TMW_K_HOP32_LOADONLY: {
         DslashArgs<float> a = make_args<float>(ctx, 1, 0, X[7], X[3], nullptr, 1.0, one);
         LAUNCH(launch_hop_loadonly(a, ctx->ng32, ctx->stream));

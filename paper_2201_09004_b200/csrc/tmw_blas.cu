@@ -6,6 +6,8 @@
 // Every kernel is batched over right-hand-side columns: blockIdx.y = slot, column c = cm.col[slot];
 // column c of a vector starts c*cs work items after its base pointer and uses the scalar block sc[c]. A single
 // solve is the batch {0}.
+#include <atomic>
+
 #include "tmw_internal.h"
 
 namespace tmw {
@@ -43,9 +45,23 @@ __device__ __forceinline__ void stm(double* base, int64_t i, int64_t Vh, const d
 }
 
 enum { BB = 256 };
+// SM count of the current device (asked once per device; 148 = B200 if the query fails)
+static int sm_count() {
+  enum { MAXDEV = 64 };
+  static std::atomic<int> cache[MAXDEV];
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAXDEV) return 148;
+  int n = cache[dev].load(std::memory_order_relaxed);
+  if (n == 0) {
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) n = 148;
+    cache[dev].store(n, std::memory_order_relaxed);
+  }
+  return n;
+}
+// grid-stride launches: at most 8 CTAs of 256 threads per SM
 static inline int blas_grid(int64_t n) {
   int64_t g = (n + BB - 1) / BB;
-  const int64_t cap = 148 * 8;
+  const int64_t cap = (int64_t)sm_count() * 8;
   return (int)(g < cap ? (g > 0 ? g : 1) : cap);
 }
 

@@ -91,11 +91,7 @@ template <int PACKED> __global__ void __launch_bounds__(256) ffma_probe_kernel(f
   for (int i = 0; i < 16; i++) sum += x[i];
   out[blockIdx.x * blockDim.x + threadIdx.x] = sum;
 }
-cudaError_t launch_ffma_probe(int packed, int fmas_per_thread, float* sink, cudaStream_t s) {
-  int dev = 0, sms = 148;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  if (sms > 148) sms = 148;
+cudaError_t launch_ffma_probe(int packed, int fmas_per_thread, int sms, float* sink, cudaStream_t s) {
   if (packed) ffma_probe_kernel<1><<<sms * 8, 256, 0, s>>>(sink, 1.0001f, 0.5f, fmas_per_thread / 16);
   else ffma_probe_kernel<0><<<sms * 8, 256, 0, s>>>(sink, 1.0001f, 0.5f, fmas_per_thread / 16);
   return cudaGetLastError();

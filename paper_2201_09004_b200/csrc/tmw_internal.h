@@ -23,15 +23,12 @@ struct StageGeom {
 // epi: EPI_HOP | EPI_AINV_HOP | EPI_A_XPAY; nr = 1..3 columns per thread; the whole lattice, no domain decomposition
 cudaError_t launch_dslash_stage(const DslashArgs<float>& a, int ng, int epi, int clover, int nr, const StageGeom& sg, cudaStream_t s);
 int stage_max_threads(int nr);  // largest CTA of the staged kernel with nr columns per thread
-// Persistent fp32 stencil with the links prefetched through a per-thread shared-memory ring (tmw_dslash_ring.cuh): 12-real
-// links, epi EPI_HOP | EPI_AINV_HOP | EPI_A_XPAY, nr = 1..4 columns per thread, the whole lattice in the 1-D site mapping
-cudaError_t launch_dslash_ring(const DslashArgs<float>& a, int epi, int clover, int nr, cudaStream_t s);
 // loads and stores of the fp32 hopping kernel without its arithmetic (measurement: tmw_time_kernel)
 cudaError_t launch_hop_loadonly(const DslashArgs<float>& a, int ng, cudaStream_t s);
 
 // register-only fp32 FMA loop (packed = 0: scalar FFMA, 1: FFMA2 pairs), (SM count) x 8 CTAs of 256 threads, fmas_per_thread FMAs each;
-// sink: >= 148 * 8 * 256 floats
-cudaError_t launch_ffma_probe(int packed, int fmas_per_thread, float* sink, cudaStream_t s);
+// sink: >= sms * 8 * 256 floats (sms = the device's SM count)
+cudaError_t launch_ffma_probe(int packed, int fmas_per_thread, int sms, float* sink, cudaStream_t s);
 
 // ---- domain decomposition (tmw_dd_f32.cu / tmw_dd_f64.cu) ----
 // a describes ONE domain (local geometry and fields, a.dd its cuts and receive buffers). pass 0: interior (all sites, the

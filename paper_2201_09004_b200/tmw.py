@@ -29,7 +29,7 @@ STATIC_SCRATCH_BYTES = 8 << 20  # TMW_STATIC_SCRATCH_BYTES
 # kernel kinds of tmw_kernel_counts / tmw_time_kernel (include/tmw.h TMW_K_*)
 KINDS = ["hop32", "k1_32", "k2_32", "k2_32_dots", "hop64", "k1_64", "k2_64", "xpay64", "ainvxpay64", "update_s", "update_xrp",
          "acc_y", "resid_convert", "convert", "dot_norm64", "sub_norm", "diag64", "pack_both", "unpack_both", "other",
-         "memset_bytes", "copy_bytes", "hop32_loadonly", "staged", "ffma_probe", "ffma2_probe", "ring"]
+         "memset_bytes", "copy_bytes", "hop32_loadonly", "staged", "ffma_probe", "ffma2_probe"]
 FFMA_PROBE_FMAS_PER_THREAD = 16 * 16384
 
 EXPORTS = ["tmw_create", "tmw_apply", "tmw_apply_schur", "tmw_apply_schur_static", "tmw_solve", "tmw_apply_multi", "tmw_apply_schur_multi",
@@ -43,12 +43,23 @@ class tmw_complex(ctypes.Structure):
 
 
 class tmw_options(ctypes.Structure):
-    _fields_ = [("location", ctypes.c_int), ("precision", ctypes.c_int), ("reconstruct", ctypes.c_int),
+    _fields_ = [("struct_size", ctypes.c_size_t), ("location", ctypes.c_int), ("precision", ctypes.c_int), ("reconstruct", ctypes.c_int),
                 ("mass_reading", ctypes.c_int), ("max_iter", ctypes.c_int), ("delta", ctypes.c_double),
                 ("stream", ctypes.c_void_p), ("solver", ctypes.c_int), ("nkrylov", ctypes.c_int),
                 ("verbose", ctypes.c_int), ("columns_per_thread", ctypes.c_int),
                 ("tile", ctypes.c_int * 4), ("debug", ctypes.c_int), ("domains_z", ctypes.c_int), ("domains_t", ctypes.c_int),
-                ("stage", ctypes.c_int), ("stage_tile", ctypes.c_int * 3), ("zchunk", ctypes.c_int), ("ring", ctypes.c_int), ("prefetch", ctypes.c_int)]
+                ("stage", ctypes.c_int), ("stage_tile", ctypes.c_int * 3), ("zchunk", ctypes.c_int), ("prefetch", ctypes.c_int)]
+
+
+def make_options(**fields) -> tmw_options:
+    """tmw_options with struct_size set (what TMW_OPTIONS_INIT does in C) and the given members; the rest stay 0 = default."""
+    opt = tmw_options()
+    opt.struct_size = ctypes.sizeof(tmw_options)
+    for k, v in fields.items():
+        if k not in {f[0] for f in tmw_options._fields_} or k == "struct_size":
+            raise TypeError(f"tmw_options has no member {k!r}")
+        setattr(opt, k, v)
+    return opt
 
 
 class tmw_solve_info(ctypes.Structure):
@@ -140,14 +151,17 @@ class Context:
                  precision: int = MIXED, reconstruct: int = 12, mass_reading: int = TWIST_GAMMA5, max_iter: int = 0,
                  delta: float = 0.0, stream: int | None = None, solver: int = BICGSTAB, nkrylov: int = 0,
                  verbose: int = 0, columns_per_thread: int = 0, tile=(0, 0, 0, 0), debug: int = 0, domains_z: int = 0, domains_t: int = 0,
-                 stage: int = 0, stage_tile=(0, 0, 0), zchunk: int = 0, ring: int = 0, prefetch: int = 0):
+                 stage: int = 0, stage_tile=(0, 0, 0), zchunk: int = 0, prefetch: int = 0):
         lib = load()
         self._lib = lib
         self.L, self.T = L, T
         self.V = L * L * L * T
         self.location = location
-        opt = tmw_options(location, precision, reconstruct, mass_reading, max_iter, delta, stream, solver, nkrylov,
-                          verbose, columns_per_thread, (ctypes.c_int * 4)(*tile), debug, domains_z, domains_t, stage, (ctypes.c_int * 3)(*stage_tile), zchunk, ring, prefetch)
+        opt = make_options(location=location, precision=precision, reconstruct=reconstruct, mass_reading=mass_reading,
+                           max_iter=max_iter, delta=delta, stream=stream, solver=solver, nkrylov=nkrylov, verbose=verbose,
+                           columns_per_thread=columns_per_thread, tile=(ctypes.c_int * 4)(*tile), debug=debug,
+                           domains_z=domains_z, domains_t=domains_t, stage=stage,
+                           stage_tile=(ctypes.c_int * 3)(*stage_tile), zchunk=zchunk, prefetch=prefetch)
         h = ctypes.c_void_p()
         rc = lib.tmw_create(ctypes.byref(h), L, T, _ptr(gauge), tmw_complex(float(np.real(m)), float(np.imag(m))),
                             float(c_sw), ctypes.byref(opt))

@@ -6,6 +6,7 @@ from __future__ import annotations
 import numpy as np
 
 import oracle
+from paper_2201_09004_b200 import synth
 
 
 def parity_sites(L: int, T: int, par: int) -> np.ndarray:
@@ -102,3 +103,16 @@ def per_site_rel_err(got: np.ndarray, ref: np.ndarray):
     site = float(np.max(dn[~zero] / rn[~zero])) if np.any(~zero) else 0.0
     glob = float(np.linalg.norm(g - r) / max(np.linalg.norm(r), 1e-300))
     return site, glob
+
+
+def exact_eigenvector_case(L=4, T=8):
+    """A system on which BiCGStab is exact at its first half step, IN FLOATING POINT: unit links except U_t = -1 on the last
+    time slice (which undoes the antiperiodic wrap of C6, so a constant spinor is an eigenvector), m = -2, a constant source
+    with entries in {0, +-1/2, +-1, +-2}. Every hop term is then +-psi or +-i psi times 1/2, summed to 4 psi; the site term is
+    -(4 + m) psi = -2 psi; so D b = 2 b, alpha = 1/2, s = r - alpha v = 0, <t,t> = 0, all without a rounding error.
+    Returns (U, b); the solution is b / 2."""
+    U = synth.unit_gauge(L, T).copy()
+    U[3, T - 1] *= -1.0
+    u = np.array([[1, -2, 0.5], [0.5j, 1 + 1j, -1], [2j, 0, -0.5 + 1j], [-1, 0.5, 2 - 0.5j]], dtype=np.complex128)
+    b = np.ascontiguousarray(np.broadcast_to(u, (T, L, L, L, 4, 3))).copy()
+    return U, b

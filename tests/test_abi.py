@@ -49,7 +49,7 @@ def test_argument_validation_before_any_cuda_call(lib):
         assert lib.tmw_create(ctypes.byref(h), L, T, g.ctypes.data, m, 0.0, None) == tmw.EINVAL
         assert h.value is None
         assert b"even" in lib.tmw_last_error(None)
-    opt = tmw.tmw_options(0, 0, 13, 0, 0, 0.0, None)  # reconstruct = 13
+    opt = tmw.make_options(reconstruct=13)
     assert lib.tmw_create(ctypes.byref(h), 4, 4, g.ctypes.data, m, 0.0, ctypes.byref(opt)) == tmw.EINVAL
     assert lib.tmw_create(ctypes.byref(h), 4, 4, g.ctypes.data, tmw.tmw_complex(float("nan"), 0.0), 0.0, None) == tmw.EINVAL
     # null context
@@ -59,8 +59,14 @@ def test_argument_validation_before_any_cuda_call(lib):
     assert lib.tmw_apply_schur_multi(None, 0, 0, 2, None, None) == tmw.EINVAL
     assert lib.tmw_solve_multi(None, 2, None, None, 1e-10, None) == tmw.EINVAL
     assert lib.tmw_cheb_apply(None, 1, (ctypes.c_double * 1)(1.0), 1.0, 0.0, None, None) == tmw.EINVAL
-    bad = tmw.tmw_options(0, 0, 12, 0, 0, 0.0, None, 7, 0)  # unknown solver
+    bad = tmw.make_options(reconstruct=12, solver=7)  # unknown solver
     assert lib.tmw_create(ctypes.byref(h), 4, 4, g.ctypes.data, m, 0.0, ctypes.byref(bad)) == tmw.EINVAL
+    # an options struct laid out by another version of the header: refused by its size, before anything is read from it
+    for size in (0, ctypes.sizeof(tmw.tmw_options) - 4, ctypes.sizeof(tmw.tmw_options) + 8):
+        other = tmw.make_options()
+        other.struct_size = size
+        assert lib.tmw_create(ctypes.byref(h), 4, 4, g.ctypes.data, m, 0.0, ctypes.byref(other)) == tmw.EINVAL
+        assert b"struct_size" in lib.tmw_last_error(None)
     assert lib.tmw_spinor_bytes(None, 0) == 0
     assert lib.tmw_launch_count(None) == 0
     lib.tmw_destroy(None)

@@ -258,6 +258,118 @@ def test_fullsize_schur_fp32_sampled(tmw):
     torch.cuda.empty_cache()
 
 
+def neighbours(L, T, sites):
+    """the 8 nearest neighbours (periodic index arithmetic; the antiperiodic sign is the operator's business) of each site"""
+    x, y, z, t = sites % L, (sites // L) % L, (sites // (L * L)) % L, sites // (L ** 3)
+    out = []
+    for d in (1, -1):
+        out += [lex(L, (x + d) % L, y, z, t), lex(L, x, (y + d) % L, z, t), lex(L, x, y, (z + d) % L, t), lex(L, x, y, z, (t + d) % T)]
+    return np.unique(np.concatenate(out)).astype(np.int64)
+
+
+class SchurSampledRef:
+    """Mhat p_o = A_oo p_o - H_oe A_ee^{-1} H_eo p_o at a list S of odd sites, from the oracle's per-site routine only
+    (oracle.apply_sites; no full-lattice sweep, so it works at 48^3 x 144): with N = the even neighbours of S,
+      h_N = (D p_o)(N)  (p_o lives on odd sites, so at an even site this is the hopping block alone),
+      A(x) for x in N column by column from D applied to unit vectors placed on N (even sites do not see one another),
+      t_N = A^{-1} h_N by a dense 12 x 12 solve per site (numpy), t = 0 elsewhere,
+      ref(S) = (D p_o)(S) - (D t)(S)  (at an odd site: A_oo p_o, and the hopping block of the even field t).
+    The site matrices depend on the fields only and are shared by all columns."""
+
+    def __init__(self, U, m, c_sw, S, dagger=False):
+        self.U, self.m, self.c_sw, self.S, self.dagger = U, m, c_sw, S, dagger
+        T, L = U.shape[1], U.shape[2]
+        self.L, self.T = L, T
+        self.N = neighbours(L, T, S)
+        xs = self.N % L + (self.N // L) % L + (self.N // (L * L)) % L + self.N // (L ** 3)
+        assert np.all(xs % 2 == 0), "S must hold odd sites only"
+        self.work = np.zeros((T, L, L, L, 4, 3), dtype=np.complex128)
+        flat = self.work.reshape(-1, 12)
+        A = np.empty((self.N.size, 12, 12), dtype=np.complex128)
+        for k in range(12):
+            flat[self.N, k] = 1.0
+            A[:, :, k] = oracle.apply_sites(U, self.work, self.N, m, c_sw, dagger=dagger).reshape(-1, 12)
+            flat[self.N, k] = 0.0
+        self.A = A
+
+    def __call__(self, p_o):
+        """p_o: canonical spinor that vanishes on the even sites -> (len(S), 4, 3)"""
+        h = oracle.apply_sites(self.U, p_o, self.N, self.m, self.c_sw, dagger=self.dagger).reshape(-1, 12)
+        flat = self.work.reshape(-1, 12)
+        flat[self.N] = np.linalg.solve(self.A, h[..., None])[..., 0]
+        ref = oracle.apply_sites(self.U, p_o, self.S, self.m, self.c_sw, dagger=self.dagger) - \
+            oracle.apply_sites(self.U, self.work, self.S, self.m, self.c_sw, dagger=self.dagger)
+        flat[self.N] = 0.0
+        return ref
+
+
+def test_schur_sampled_reference_agrees_with_the_full_lattice_one():
+    """the sampled reference above against the whole-lattice construction of test_fullsize_schur_fp32_sampled on a small
+    lattice (both from the oracle; this checks the test's own bookkeeping, not the product)"""
+    L, T, m, c_sw = 4, 6, -0.044 + 0.2j, 1.0349
+    U = synth.gauge_field(L, T, 0.4, seed=1)
+    V = L ** 3 * T
+    psi = mask_parity_inplace(synth.gaussian_spinor(L, T, seed=3), L, T, 0)
+    ev, od = H.parity_sites(L, T, 0), H.parity_sites(L, T, 1)
+    Dx = oracle.apply(U, psi, m, c_sw).reshape(V, 12)
+    A = np.empty((V, 12, 12), dtype=np.complex128)
+    e = np.zeros((V, 12), dtype=np.complex128)
+    for k in range(12):
+        e[ev, k] = 1.0
+        A[:, :, k] = oracle.apply(U, e.reshape(psi.shape), m, c_sw).reshape(V, 12)
+        e[ev, k] = 0.0
+    t_e = np.zeros((V, 12), dtype=np.complex128)
+    t_e[ev] = np.linalg.solve(A[ev], Dx[ev][..., None])[..., 0]
+    ref = Dx - oracle.apply(U, t_e.reshape(psi.shape), m, c_sw).reshape(V, 12)
+    S = od[::7]
+    got = SchurSampledRef(U, m, c_sw, S)(psi).reshape(-1, 12)
+    assert np.max(np.abs(got - ref[S])) <= 1e-13 * np.max(np.abs(ref))
+
+
+@pytest.mark.parametrize("idx,ncol", [(3, 12), (4, 3)])
+def test_fullsize_schur_single_and_multi_column_sampled(tmw, idx, ncol):
+    """K1/K2 at the sizes and in the launch shapes bench.py times, against the oracle site by site (not through a converging
+    solve): tmw_apply_schur_multi on `ncol` columns (fp32: columns per thread, packed pairs, z-slab sweep) and
+    tmw_apply_schur on one column in fp32 and fp64, at 1500 seeded odd sites plus the odd boundary sites of every kind."""
+    cfg, U = config_fields(idx)
+    L, T, m, c_sw = cfg["L"], cfg["T"], complex(*cfg["m"]), cfg["c_sw"]
+    S = sample_sites(L, T, 3000, seed=41 + idx, parity=1)
+    ref_of = SchurSampledRef(U, m, c_sw, S)
+    seeds = [50 + c for c in range(ncol)]
+    dU = torch.from_numpy(U).cuda()
+    with tmw.Context(L, T, dU, m, c_sw) as ctx:
+        del dU
+        tmp = torch.empty((T, L, L, L, 4, 3), dtype=torch.complex128, device="cuda")
+        nb = ctx.spinor_bytes(tmw.F32)
+        pin = torch.empty(nb * ncol, dtype=torch.uint8, device="cuda")
+        pout = torch.full_like(pin, 0x7f)
+        for c in range(ncol):
+            tmp.copy_(torch.from_numpy(synth.gaussian_spinor(L, T, seed=seeds[c])))
+            ctx.pack(tmw.F32, tmw.ODD, tmp, pin[c * nb:(c + 1) * nb])
+        ctx.apply_schur_multi(tmw.D, tmw.F32, ncol, pin, pout)
+        for c in range(ncol):
+            tmp.zero_()
+            ctx.unpack(tmw.F32, tmw.ODD, pout[c * nb:(c + 1) * nb], tmp)
+            got = tmp.cpu().numpy().reshape(-1, 4, 3)[S]
+            psi = mask_parity_inplace(synth.gaussian_spinor(L, T, seed=seeds[c]), L, T, 0)
+            ref = ref_of(psi)
+            assert site_err(got, ref) <= TOL32, ("multi", c)
+            if c == 0:  # the single-column launches on the same input, fp32 and fp64
+                for prec, tol in ((tmw.F32, TOL32), (tmw.F64, TOL64)):
+                    n1 = ctx.spinor_bytes(prec)
+                    a = torch.empty(n1, dtype=torch.uint8, device="cuda")
+                    o = torch.full_like(a, 0x7f)
+                    tmp.copy_(torch.from_numpy(psi))
+                    ctx.pack(prec, tmw.ODD, tmp, a)
+                    ctx.apply_schur(tmw.D, prec, a, o)
+                    tmp.zero_()
+                    ctx.unpack(prec, tmw.ODD, o, tmp)
+                    assert site_err(tmp.cpu().numpy().reshape(-1, 4, 3)[S], ref) <= tol, ("single", prec)
+                    del a, o
+        del pin, pout, tmp
+    torch.cuda.empty_cache()
+
+
 ORIGIN_COLS = [(0, 0), (2, 1)]  # (spin, colour) of the columns whose solution is compared with the oracle's at config 3
 
 

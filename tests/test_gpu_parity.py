@@ -280,6 +280,24 @@ def check_solution(U, b, x, m, c_sw, x_ref=None, mass_scalar=False, F=None):
     return resid
 
 
+@pytest.mark.parametrize("precision", ["mixed", "double"])
+def test_solve_exact_at_the_half_step(tmw, precision):
+    """A source that is an eigenvector of D, set up so that no rounding error occurs (helpers.exact_eigenvector_case; the
+    oracle's side of it is pinned in test_oracle_pins.py): s = r - alpha v vanishes identically, <t,t> = 0, and the guard in
+    sc_omega_kernel (omega = beta = 0 instead of 0/0) has to carry the solve to x = b / 2. Links with det = -1: 18-real."""
+    L, T, m = 4, 8, -2.0 + 0.0j
+    U, b = H.exact_eigenvector_case(L, T)
+    x_ref, oinfo = oracle.bicgstab(U, b, m, tol=1e-12)
+    assert oinfo["status"] == 0 and oinfo["iters"] == 1
+    with tmw.Context(L, T, dev(U), m, 0.0, reconstruct=18, precision=tmw.MIXED if precision == "mixed" else tmw.DOUBLE) as ctx:
+        x = torch.full(b.shape, float("nan"), dtype=torch.complex128, device="cuda")
+        info = ctx.solve(dev(b), x, 1e-10)
+        x = x.cpu().numpy()
+    assert np.all(np.isfinite(x)), info
+    assert info["iters"] <= 2 and info["true_resid"] <= 1e-10, info
+    check_solution(U, b, x, m, 0.0, x_ref)
+
+
 SOLVE_CASES = [
     dict(L=4, T=8, eps=0.3, m=0.1 + 0.0j, c_sw=0.0, src="point"),           # BASELINE.json configs[0]
     dict(L=6, T=4, eps=0.4, m=-0.0695 + 0.01j, c_sw=0.0, src="z2"),         # configs[1] parameters, small

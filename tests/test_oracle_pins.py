@@ -8,6 +8,7 @@ import itertools
 import numpy as np
 import pytest
 
+import helpers as H
 import oracle
 from paper_2201_09004_b200 import synth
 
@@ -481,6 +482,17 @@ def test_zero_source_gives_zero_solution():
     U = synth.gauge_field(2, 2, 0.3, seed=1)
     x, info = oracle.bicgstab(U, np.zeros((2, 2, 2, 2, 4, 3), dtype=np.complex128), 0.1)
     assert info["status"] == 0 and np.all(x == 0)
+
+
+def test_bicgstab_exact_at_the_half_step():
+    """The <t,t> = 0 exit of the oracle's BiCGStab (s = r - alpha v vanished: x + alpha p is the solution). Without that exit
+    omega = 0/0 poisons x; an exit that forgets x += alpha p returns 0. Closed form: D b = 2 b, so x = b / 2 after ONE
+    iteration with a residual of exactly 0."""
+    U, b = H.exact_eigenvector_case()
+    assert np.array_equal(oracle.apply(U, b, -2.0), 2.0 * b)  # the premise, bit for bit
+    x, info = oracle.bicgstab(U, b, -2.0, tol=1e-12)
+    assert info["status"] == 0 and info["iters"] == 1 and info["true_resid"] == 0.0
+    assert np.array_equal(x, 0.5 * b)
 
 
 # ----------------------------------------------------------------------------------------------------------
