@@ -370,6 +370,88 @@ def test_fullsize_schur_single_and_multi_column_sampled(tmw, idx, ncol):
     torch.cuda.empty_cache()
 
 
+def cut_plane_sites(L, T, pz, pt):
+    """every site next to a domain cut: z in {0, lz-1, lz, ...} for domains_z > 1, t likewise (lexicographic indices)"""
+    zs = sorted({(k * (L // pz) + d) % L for k in range(pz) for d in (-1, 0)}) if pz > 1 else []
+    ts = sorted({(k * (T // pt) + d) % T for k in range(pt) for d in (-1, 0)}) if pt > 1 else []
+    ax, ay = np.arange(L), np.arange(L)
+    out = []
+    for z in zs:
+        t, y, x = np.meshgrid(np.arange(T), ay, ax, indexing="ij")
+        out.append(lex(L, x, y, z, t).ravel())
+    for t in ts:
+        z, y, x = np.meshgrid(np.arange(L), ay, ax, indexing="ij")
+        out.append(lex(L, x, y, z, t).ravel())
+    return np.unique(np.concatenate(out)).astype(np.int64)
+
+
+def of_parity(L, sites, par):
+    return sites[((sites % L) + (sites // L) % L + (sites // (L * L)) % L + sites // (L ** 3)) % 2 == par]
+
+
+@pytest.mark.parametrize("idx,pz,pt", [(3, 2, 2), (4, 1, 2)])
+def test_fullsize_decomposed_context_sampled(tmw, idx, pz, pt):
+    """Domain-decomposed contexts at full size - 2 x 2 domains at configs[3], the 1 x 2 split bench.py times
+    at configs[4] - where the local site mapping, the vh_loc-strided buffers and the face indices span many CTAs: the fp32
+    hopping block and the fp64 FULL operator at EVERY site next to a cut plus 5000 seeded sites and the lattice-boundary
+    sites; K1/K2 (tmw_apply_schur, fp32 and fp64) at a seeded sample of those; one solve with the exact residual through the
+    oracle's D. All against the oracle site by site (oracle.apply_sites)."""
+    cfg, U = config_fields(idx)
+    L, T, m, c_sw = cfg["L"], cfg["T"], complex(*cfg["m"]), cfg["c_sw"]
+    cuts = cut_plane_sites(L, T, pz, pt)
+    sites = np.unique(np.concatenate([cuts, sample_sites(L, T, 5000, seed=61 + idx)]))
+    rng = np.random.default_rng(71 + idx)
+    S = np.unique(np.concatenate([rng.choice(of_parity(L, cuts, 1), size=2000, replace=False),
+                                  sample_sites(L, T, 2000, seed=81 + idx, parity=1)]))
+    psi = synth.gaussian_spinor(L, T, seed=3)
+    psi_o = mask_parity_inplace(psi.copy(), L, T, 0)
+    ref_schur = SchurSampledRef(U, m, c_sw, S)(psi_o)
+    dU = torch.from_numpy(U).cuda()
+    with tmw.Context(L, T, dU, m, c_sw, domains_z=pz, domains_t=pt) as ctx:
+        del dU
+        dpsi = torch.from_numpy(psi).cuda()
+        out_c = torch.zeros_like(dpsi)
+        # fp32 hopping block, both parities
+        nb = ctx.spinor_bytes(tmw.F32)
+        pin = torch.empty(nb, dtype=torch.uint8, device="cuda")
+        pout = torch.full_like(pin, 0x7f)
+        for par in (0, 1):
+            ctx.pack(tmw.F32, tmw.EVEN if par else tmw.ODD, dpsi, pin)
+            ctx.apply(tmw.D, tmw.ODD if par else tmw.EVEN, tmw.F32, pin, pout)
+            ctx.unpack(tmw.F32, tmw.ODD if par else tmw.EVEN, pout, out_c)
+        torch.cuda.synchronize()
+        got = out_c.cpu().numpy().reshape(-1, 4, 3)[sites]
+        p = psi.reshape(-1, 4, 3)[sites]
+        g5 = np.array([1, 1, -1, -1])[None, :, None]
+        ref = oracle.apply_sites(U, psi, sites, m, 0.0) - (-(4.0 + m.real) * p - 1j * m.imag * g5 * p)  # D (c_sw = 0) minus its site term
+        assert site_err(got, ref) <= TOL32
+        # K1 / K2
+        for prec, tol in ((tmw.F32, TOL32), (tmw.F64, TOL64)):
+            n1 = ctx.spinor_bytes(prec)
+            a = torch.empty(n1, dtype=torch.uint8, device="cuda")
+            o = torch.full_like(a, 0x7f)
+            ctx.pack(prec, tmw.ODD, dpsi, a)
+            ctx.apply_schur(tmw.D, prec, a, o)
+            out_c.zero_()
+            ctx.unpack(prec, tmw.ODD, o, out_c)
+            assert site_err(out_c.cpu().numpy().reshape(-1, 4, 3)[S], ref_schur) <= tol, prec
+            del a, o
+        del pin, pout
+        # fp64 FULL operator
+        ctx.apply(tmw.D, tmw.FULL, tmw.F64, dpsi, out_c)
+        torch.cuda.synchronize()
+        assert site_err(out_c.cpu().numpy().reshape(-1, 4, 3)[sites], oracle.apply_sites(U, psi, sites, m, c_sw)) <= TOL64
+        # one solve, residual by the oracle's operator over the whole lattice
+        b = synth.point_source(L, T, 0, 0)
+        dpsi.copy_(torch.from_numpy(b))
+        info = ctx.solve(dpsi, out_c, 1e-10)
+        xg = out_c.cpu().numpy()
+        del dpsi, out_c
+    torch.cuda.empty_cache()
+    assert info["true_resid"] <= 1e-10
+    assert exact_residual(U, config_F(idx), b, xg, m, c_sw) <= 1e-10
+
+
 ORIGIN_COLS = [(0, 0), (2, 1)]  # (spin, colour) of the columns whose solution is compared with the oracle's at config 3
 
 
