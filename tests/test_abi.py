@@ -57,6 +57,7 @@ def test_argument_validation_before_any_cuda_call(lib):
     assert lib.tmw_solve(None, None, None, 1e-10, None) == tmw.EINVAL
     assert lib.tmw_apply_multi(None, 0, 0, 0, 2, None, None) == tmw.EINVAL
     assert lib.tmw_apply_schur_multi(None, 0, 0, 2, None, None) == tmw.EINVAL
+    assert lib.tmw_apply_schur_static(None, 0, 0, None, None) == tmw.EINVAL
     assert lib.tmw_solve_multi(None, 2, None, None, 1e-10, None) == tmw.EINVAL
     assert lib.tmw_cheb_apply(None, 1, (ctypes.c_double * 1)(1.0), 1.0, 0.0, None, None) == tmw.EINVAL
     bad = tmw.make_options(reconstruct=12, solver=7)  # unknown solver
